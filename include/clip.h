@@ -1,0 +1,90 @@
+/*
+ * clip.h -- C ABI of libclip: the per-timestep update of the two D3Q19 population sets (Allen-Cahn `g`,
+ * velocity/pressure `f`) of the conservative phase-field lattice Boltzmann method of arxiv 2505.12205,
+ * hand-written CUDA for sm_100a (B200).  Citations are PAPER.md line numbers / equation numbers.
+ *
+ * Problem statement (PAPER.md:341 Fig. 4a, :541 Alg. 3 "Ensure"): initial phi and u in; after n time steps
+ * phi, p, u out.  One step = collision (Alg. 1, :351-429) -> streaming (Alg. 2, :432-459) -> boundary conditions
+ * (App. B, :963-1129) -> macroscopic variables (Alg. 3, :461-541).
+ *
+ * Conventions
+ *   - Lattice units dx = dt = c = 1, c_s^2 = 1/3 (:172, :193).  Paper tau: nu = tau/3 (Eq. 23), rate 1/(tau+1/2).
+ *   - Field layout: scalar fields [nz][ny][nx] with x fastest (Fig. 4b, :343); vectors SoA [3][nz][ny][nx].
+ *   - Every `d_*` pointer is a DEVICE pointer; element type is float (precision 32) or double (precision 64),
+ *     for the workspace and for all user I/O alike.  Pointers must be aligned to 16 bytes.
+ *   - Ownership: the caller owns every device buffer, including the workspace, and keeps the workspace alive
+ *     until clip_destroy.  The library never allocates device memory.  clip_init / clip_get read / write their
+ *     arguments asynchronously on the handle's stream and do not retain them.
+ *   - The handle is a host heap object owned by the library.  One handle = one stream; not thread-safe.
+ *   - Errors: every int-returning call returns CLIP_OK (0) or a negative code; no exceptions, no aborts, no
+ *     host synchronisation inside clip_step.  Text via clip_last_error.
+ */
+#ifndef CLIP_H_
+#define CLIP_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { CLIP_OK = 0, CLIP_EINVAL = -1, CLIP_ENOMEM = -2, CLIP_ESTATE = -3, CLIP_ECUDA = -4 };
+
+/* Boundary type of one lattice face.  PERIODIC: App. B.1 (:971-1003).  WALL: halfway bounce-back, App. B.3
+ * (:1028-1038).  INLET: velocity inlet, App. B.4 (:1042-1088), only on the -z face.  OUTLET: convective outlet,
+ * App. B.5 (:1094-1129), only on the +z face. */
+enum { CLIP_BC_PERIODIC = 0, CLIP_BC_WALL = 1, CLIP_BC_INLET = 2, CLIP_BC_OUTLET = 3 };
+
+typedef struct clip_params {
+  int precision;           /* 32 or 64: element type of every device array incl. user I/O */
+  double rho_h, rho_l;     /* densities of the phi=1 (heavy) and phi=0 (light) fluid, Eq. 39 (:301) */
+  double tau_h, tau_l;     /* paper relaxation times, nu = tau/3, Eq. 23-24 (:209-213) */
+  double sigma, W, M;      /* surface tension, interface width xi, mobility: Eq. 12 (:154), 34 (:277), 37 (:293) */
+  double g[3], rho_ref;    /* body force F_b = (rho - rho_ref) g  (Eq. 58 :825; rho_ref = 0 gives rho g, :649) */
+  int bc[6];               /* faces -x,+x,-y,+y,-z,+z : CLIP_BC_* ; PERIODIC faces must come in pairs */
+  double inlet_u[3];       /* plug inflow velocity u_in, B.12 (:1048) */
+  double inlet_phi;        /* phi_in, B.16 (:1069) */
+  double inlet_c[2];       /* nozzle disc centre (x, y) in node coordinates */
+  double inlet_r;          /* nozzle radius; nodes of the -z face outside the disc are WALL */
+  int outlet_u_mode;       /* 0 = U_local of B.22 (:1104); 1 (U_ave) and 2 (U_max) are not implemented */
+  int visc_interp;         /* 0 = linear tau, Eq. 24 (paper); 1 = harmonic (1/tau linear in phi; non-paper) */
+} clip_params;
+
+typedef struct clip_handle clip_t;
+
+/* Bytes of device workspace clip_create needs for this lattice; 0 if the arguments are invalid. */
+size_t clip_workspace_bytes(int nx, int ny, int nz, const clip_params* params);
+
+/* Validate, carve `d_workspace` (device, >= clip_workspace_bytes, 256-byte aligned) and bind to `cuda_stream`
+ * (a cudaStream_t / CUstream passed as void*; NULL = default stream).  Copies *params.  Host only apart from
+ * one small asynchronous upload (the inlet mask).  On failure *out = NULL and the reason is available from
+ * clip_last_error(NULL). */
+int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params, void* d_workspace, size_t bytes,
+                void* cuda_stream);
+
+/* Set t = 0 from phi0 [nz][ny][nx] and u0 [3][nz][ny][nx] (device): p* = 0, populations at the barred
+ * equilibria g = phi Gamma - F^phi/2, f = (Gamma - w) - F_a/2 with F = F_s + F_b (Eq. 16-19, 34-36; the paper
+ * only says "Initialization", :341 -- DESIGN.md reading R8). */
+int clip_init(clip_t* h, const void* d_phi0, const void* d_u0);
+
+/* Advance n >= 0 time steps (Eq. 13, 33 with all of App. B); asynchronous on the stream. */
+int clip_step(clip_t* h, int n);
+
+/* Write phi, the physical pressure p = p* rho c_s^2 (:189) and u at the current time into caller buffers
+ * (device; any may be NULL); asynchronous on the stream. */
+int clip_get(clip_t* h, void* d_phi, void* d_p, void* d_u);
+
+/* Free the handle (not the workspace). */
+int clip_destroy(clip_t* h);
+
+/* Last error text of the handle, or of the last failed clip_create / clip_workspace_bytes when h == NULL.
+ * The string is owned by the library and valid until the next call on that handle. */
+const char* clip_last_error(const clip_t* h);
+
+/* Number of kernel launches the handle has enqueued so far (instrumentation for bench.py's gpu_launches). */
+long long clip_launch_count(const clip_t* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CLIP_H_ */

@@ -1,0 +1,245 @@
+// clip.cu -- host side of libclip: the C ABI of include/clip.h.  No device allocation happens here: the caller's
+// workspace is carved into the arrays listed at the top of clip_kernels.cuh.
+#include "../../include/clip.h"
+#include "clip_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+namespace {
+
+char g_create_error[256] = "";
+
+void set_err(char* dst, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(dst, 256, fmt, ap);
+  va_end(ap);
+}
+
+constexpr size_t ALIGN = 256;
+size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Layout {
+  size_t word;  // 4 or 8
+  size_t off_f[2], off_g[2], off_phi, off_u, off_obf, off_obg, off_lam, off_mask, total;
+};
+
+Layout make_layout(int nx, int ny, int nz, const clip_params* p) {
+  Layout L{};
+  L.word = p->precision == 32 ? 4 : 8;
+  const size_t n = (size_t)nx * ny * nz, nxy = (size_t)nx * ny;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o += align_up(bytes); return r; };
+  L.off_f[0] = take(19 * n * L.word); L.off_f[1] = take(19 * n * L.word);
+  L.off_g[0] = take(19 * n * L.word); L.off_g[1] = take(19 * n * L.word);
+  L.off_phi = take(n * L.word);
+  L.off_u = take(3 * n * L.word);
+  const bool outlet = p->bc[5] == CLIP_BC_OUTLET, inlet = p->bc[4] == CLIP_BC_INLET;
+  L.off_obf = take(outlet ? 19 * nxy * L.word : 0);
+  L.off_obg = take(outlet ? 19 * nxy * L.word : 0);
+  L.off_lam = take(outlet ? nxy * L.word : 0);
+  L.off_mask = take(inlet ? nxy : 0);
+  L.total = o;
+  return L;
+}
+
+// returns nullptr if valid, else a reason
+const char* validate(int nx, int ny, int nz, const clip_params* p) {
+  if (!p) return "params is NULL";
+  if (nx < 1 || ny < 1 || nz < 1) return "nx, ny, nz must be >= 1";
+  if ((double)nx * ny * nz > 2.0e9) return "lattice too large (nx*ny*nz must stay below 2e9)";
+  if (p->precision != 32 && p->precision != 64) return "precision must be 32 or 64";
+  if (!(p->rho_h > 0.0) || !(p->rho_l > 0.0)) return "densities must be positive";
+  if (!(p->tau_h + 0.5 > 0.0) || !(p->tau_l + 0.5 > 0.0)) return "tau + 1/2 must be positive";
+  if (p->visc_interp == 1 && (!(p->tau_h > 0.0) || !(p->tau_l > 0.0))) return "harmonic interpolation needs tau > 0";
+  if (p->visc_interp != 0 && p->visc_interp != 1) return "visc_interp must be 0 or 1";
+  if (!(3.0 * p->M + 0.5 > 0.0)) return "tau_phi + 1/2 must be positive";
+  if (!(p->W > 0.0)) return "W must be positive";
+  if (!std::isfinite(p->sigma)) return "sigma must be finite";
+  for (int d = 0; d < 3; ++d) {
+    const int lo = p->bc[2 * d], hi = p->bc[2 * d + 1];
+    if (lo < 0 || lo > 3 || hi < 0 || hi > 3) return "unknown boundary type";
+    if ((lo == CLIP_BC_PERIODIC) != (hi == CLIP_BC_PERIODIC)) return "PERIODIC faces must come in pairs";
+    if (d < 2 && (lo >= CLIP_BC_INLET || hi >= CLIP_BC_INLET)) return "INLET / OUTLET are only supported on the z faces";
+  }
+  if (p->bc[4] == CLIP_BC_OUTLET) return "OUTLET is only supported on the +z face";
+  if (p->bc[5] == CLIP_BC_INLET) return "INLET is only supported on the -z face";
+  if (p->bc[5] == CLIP_BC_OUTLET && nz < 2) return "OUTLET needs nz >= 2";
+  if (p->bc[4] == CLIP_BC_INLET && !(p->inlet_r >= 0.0)) return "inlet_r must be >= 0";
+  if (p->outlet_u_mode != 0) return "outlet_u_mode 1 (U_ave) and 2 (U_max) are not implemented";
+  return nullptr;
+}
+
+}  // namespace
+
+struct clip_handle {
+  int nx, ny, nz;
+  clip_params p;
+  Layout L;
+  char* ws;
+  cudaStream_t stream;
+  int cur;      // which of the A/B population buffers holds the current post-collision state
+  bool inited;
+  long long launches;
+  long long t;
+  std::vector<uint8_t> mask_host;
+  char err[256];
+};
+
+namespace {
+
+template <typename T> clip::KP<T> make_kp(const clip_handle* h) {
+  clip::KP<T> P{};
+  const clip_params& p = h->p;
+  P.nx = h->nx; P.ny = h->ny; P.nz = h->nz;
+  P.n = (long long)h->nx * h->ny * h->nz;
+  P.nxy = (long long)h->nx * h->ny;
+  P.any_nonperiodic = 0;
+  for (int k = 0; k < 6; ++k) { P.bc[k] = p.bc[k]; if (p.bc[k] != CLIP_BC_PERIODIC) P.any_nonperiodic = 1; }
+  P.has_inlet = p.bc[4] == CLIP_BC_INLET;
+  P.has_outlet = p.bc[5] == CLIP_BC_OUTLET;
+  P.visc_interp = p.visc_interp;
+  P.rho_h = (T)p.rho_h; P.rho_l = (T)p.rho_l; P.drho = (T)(p.rho_h - p.rho_l);
+  P.tau_h = (T)p.tau_h; P.tau_l = (T)p.tau_l;
+  P.itau_h = (T)(p.tau_h != 0.0 ? 1.0 / p.tau_h : 0.0); P.itau_l = (T)(p.tau_l != 0.0 ? 1.0 / p.tau_l : 0.0);
+  P.beta4 = (T)(4.0 * 12.0 * p.sigma / p.W);  // 4 beta, Eq. 12
+  P.kappa = (T)(1.5 * p.sigma * p.W);
+  P.inv_W = (T)(1.0 / p.W);
+  P.om_phi = (T)(1.0 / (3.0 * p.M + 0.5));    // Eq. 33, 37
+  P.gx = (T)p.g[0]; P.gy = (T)p.g[1]; P.gz = (T)p.g[2]; P.rho_ref = (T)p.rho_ref;
+  for (int k = 0; k < 3; ++k) P.uin[k] = (T)p.inlet_u[k];
+  P.phi_in = (T)p.inlet_phi;
+  char* ws = h->ws;
+  P.f_src = (const T*)(ws + h->L.off_f[h->cur]); P.g_src = (const T*)(ws + h->L.off_g[h->cur]);
+  P.f_dst = (T*)(ws + h->L.off_f[h->cur ^ 1]); P.g_dst = (T*)(ws + h->L.off_g[h->cur ^ 1]);
+  P.phi = (T*)(ws + h->L.off_phi); P.u = (T*)(ws + h->L.off_u);
+  P.ob_f = (T*)(ws + h->L.off_obf); P.ob_g = (T*)(ws + h->L.off_obg); P.lam = (T*)(ws + h->L.off_lam);
+  P.mask = (const uint8_t*)(ws + h->L.off_mask);
+  return P;
+}
+
+int check_cuda(clip_handle* h, const char* what) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    set_err(h->err, "%s: %s", what, cudaGetErrorString(e));
+    return CLIP_ECUDA;
+  }
+  return CLIP_OK;
+}
+
+unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / block); }
+
+template <typename T> int do_init(clip_handle* h, const void* phi0, const void* u0) {
+  h->cur = 1;  // k_init writes into "dst"; flip afterwards so that it becomes the current state
+  clip::KP<T> P = make_kp<T>(h);
+  clip::k_init<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P, (const T*)phi0, (const T*)u0);
+  h->launches += 1;
+  h->cur = 0;
+  return check_cuda(h, "k_init");
+}
+
+template <typename T> int do_step(clip_handle* h, int nsteps) {
+  for (int s = 0; s < nsteps; ++s) {
+    clip::KP<T> P = make_kp<T>(h);
+    clip::k_phi<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
+    clip::k_step<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
+    h->launches += 2;
+    h->cur ^= 1;
+    h->t += 1;
+  }
+  return check_cuda(h, "k_step");
+}
+
+template <typename T> int do_get(clip_handle* h, void* phi, void* p, void* u) {
+  clip::KP<T> P = make_kp<T>(h);
+  clip::k_get<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P, (T*)phi, (T*)p, (T*)u);
+  h->launches += 1;
+  return check_cuda(h, "k_get");
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t clip_workspace_bytes(int nx, int ny, int nz, const clip_params* params) {
+  const char* why = validate(nx, ny, nz, params);
+  if (why) { set_err(g_create_error, "clip_workspace_bytes: %s", why); return 0; }
+  return make_layout(nx, ny, nz, params).total;
+}
+
+int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params, void* d_workspace, size_t bytes,
+                void* cuda_stream) {
+  if (!out) { set_err(g_create_error, "clip_create: out is NULL"); return CLIP_EINVAL; }
+  *out = nullptr;
+  const char* why = validate(nx, ny, nz, params);
+  if (why) { set_err(g_create_error, "clip_create: %s", why); return CLIP_EINVAL; }
+  if (!d_workspace) { set_err(g_create_error, "clip_create: workspace is NULL"); return CLIP_EINVAL; }
+  if (((uintptr_t)d_workspace) % ALIGN) { set_err(g_create_error, "clip_create: workspace must be 256-byte aligned"); return CLIP_EINVAL; }
+  Layout L = make_layout(nx, ny, nz, params);
+  if (bytes < L.total) {
+    set_err(g_create_error, "clip_create: workspace too small (%zu < %zu bytes)", bytes, L.total);
+    return CLIP_ENOMEM;
+  }
+  clip_handle* h = new (std::nothrow) clip_handle();
+  if (!h) { set_err(g_create_error, "clip_create: out of host memory"); return CLIP_ENOMEM; }
+  h->nx = nx; h->ny = ny; h->nz = nz; h->p = *params; h->L = L; h->ws = (char*)d_workspace;
+  h->stream = (cudaStream_t)cuda_stream; h->cur = 0; h->inited = false; h->launches = 0; h->t = 0; h->err[0] = 0;
+  if (params->bc[4] == CLIP_BC_INLET) {  // disc mask, decided in double on the host
+    h->mask_host.resize((size_t)nx * ny);
+    for (int y = 0; y < ny; ++y)
+      for (int x = 0; x < nx; ++x) {
+        const double dx = x - params->inlet_c[0], dy = y - params->inlet_c[1];
+        h->mask_host[(size_t)y * nx + x] = (dx * dx + dy * dy <= params->inlet_r * params->inlet_r) ? 1 : 0;
+      }
+    cudaError_t e = cudaMemcpyAsync(h->ws + L.off_mask, h->mask_host.data(), h->mask_host.size(), cudaMemcpyHostToDevice, h->stream);
+    if (e != cudaSuccess) {
+      set_err(g_create_error, "clip_create: mask upload: %s", cudaGetErrorString(e));
+      delete h;
+      return CLIP_ECUDA;
+    }
+  }
+  *out = h;
+  return CLIP_OK;
+}
+
+int clip_init(clip_t* h, const void* d_phi0, const void* d_u0) {
+  if (!h) return CLIP_EINVAL;
+  if (!d_phi0 || !d_u0) { set_err(h->err, "clip_init: NULL input"); return CLIP_EINVAL; }
+  if (((uintptr_t)d_phi0) % 16 || ((uintptr_t)d_u0) % 16) { set_err(h->err, "clip_init: inputs must be 16-byte aligned"); return CLIP_EINVAL; }
+  int rc = h->p.precision == 32 ? do_init<float>(h, d_phi0, d_u0) : do_init<double>(h, d_phi0, d_u0);
+  if (rc == CLIP_OK) { h->inited = true; h->t = 0; }
+  return rc;
+}
+
+int clip_step(clip_t* h, int n) {
+  if (!h) return CLIP_EINVAL;
+  if (!h->inited) { set_err(h->err, "clip_step: clip_init has not been called"); return CLIP_ESTATE; }
+  if (n < 0) { set_err(h->err, "clip_step: n must be >= 0"); return CLIP_EINVAL; }
+  return h->p.precision == 32 ? do_step<float>(h, n) : do_step<double>(h, n);
+}
+
+int clip_get(clip_t* h, void* d_phi, void* d_p, void* d_u) {
+  if (!h) return CLIP_EINVAL;
+  if (!h->inited) { set_err(h->err, "clip_get: clip_init has not been called"); return CLIP_ESTATE; }
+  if (((uintptr_t)d_phi) % 16 || ((uintptr_t)d_p) % 16 || ((uintptr_t)d_u) % 16) { set_err(h->err, "clip_get: outputs must be 16-byte aligned"); return CLIP_EINVAL; }
+  if (!d_phi && !d_p && !d_u) return CLIP_OK;
+  return h->p.precision == 32 ? do_get<float>(h, d_phi, d_p, d_u) : do_get<double>(h, d_phi, d_p, d_u);
+}
+
+int clip_destroy(clip_t* h) {
+  if (!h) return CLIP_EINVAL;
+  if (!h->mask_host.empty()) cudaStreamSynchronize(h->stream);  // the mask upload reads host memory we own
+  delete h;
+  return CLIP_OK;
+}
+
+const char* clip_last_error(const clip_t* h) { return h ? h->err : g_create_error; }
+
+long long clip_launch_count(const clip_t* h) { return h ? h->launches : 0; }
+
+}  // extern "C"

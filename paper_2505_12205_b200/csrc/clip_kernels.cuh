@@ -1,0 +1,465 @@
+// clip_kernels.cuh -- device code of libclip (sm_100a).  See DESIGN.md for the kernel designs and the roofline.
+//
+// State kept in HBM between steps (SoA, x fastest; T = float or double):
+//   f[cur], g[cur]  POST-collision populations f+(x,t), g+(x,t)            [19][nz][ny][nx]   (A/B buffered)
+//   phi             phi(x,t)                                                    [nz][ny][nx]
+//   u               u(x,t)                                                   [3][nz][ny][nx]   (node-local update)
+//   ob_f, ob_g      PRE-collision populations of the outlet layer z = nz-1 at t   [19][ny][nx] (outlet only)
+//   lam             lambda = max(0, u_z(x,y,nz-2,t)) of B.25                         [ny][nx]  (outlet only)
+//   mask            inlet disc mask of the -z face (uint8)                           [ny][nx]  (inlet only)
+//
+// One step t -> t+1:
+//   k_phi : pull g+ (streaming B.4 + all of App. B for g)  ->  phi(t+1) = sum_a g_a   (Eq. 38)
+//   k_step: pull f+, g+ (Alg. 2 + App. B) -> macros (Alg. 3) -> both collisions (Alg. 1) -> store f+, g+, u
+//
+// The arithmetic is the "lean" form of the paper's equations:
+//   M^-1 S M = I - (1 - s_nu) P with P_ab = w_a/(2 c_s^4) Q_a : dev(Q_b)   (Eq. 27-28 as read in G2)
+//   => f+_a = w_a [p* + 3 e.u + 4.5 (e.u)^2 - 1.5 u.u] + 1.5 w_a (e_a.F)/rho + 4.5 (1 - s_nu) w_a e_a^T D e_a
+//      with D = dev(Pi^neq), Pi^neq = sum_a e_a e_a f_a - (p*/3 I + u u)      (Eq. 13, 16, 17, 19)
+//   => F_mu = -tau (rho_h - rho_l) [s_nu D + tr(Pi^neq)/3 I] . grad phi          (Eq. 30, 32)
+//      g+_a = (1 - w_phi) g_a + w_phi phi Gamma_a + (1 - w_phi/2) F^phi_a        (Eq. 33-36)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace clip {
+
+enum { BC_PERIODIC = 0, BC_WALL = 1, BC_INLET = 2, BC_OUTLET = 3 };
+constexpr int Q = 19;
+
+// D3Q19 velocity set, Eq. 14; ordering chosen so that the +x set is {1,7,9,11,13}
+// and opposite directions are adjacent (a odd -> a+1).
+__host__ __device__ constexpr int cx(int a) {
+  return (a == 1 || a == 7 || a == 9 || a == 11 || a == 13) ? 1 : ((a == 2 || a == 8 || a == 10 || a == 12 || a == 14) ? -1 : 0);
+}
+__host__ __device__ constexpr int cy(int a) {
+  return (a == 3 || a == 7 || a == 10 || a == 15 || a == 17) ? 1 : ((a == 4 || a == 8 || a == 9 || a == 16 || a == 18) ? -1 : 0);
+}
+__host__ __device__ constexpr int cz(int a) {
+  return (a == 5 || a == 11 || a == 14 || a == 15 || a == 18) ? 1 : ((a == 6 || a == 12 || a == 13 || a == 16 || a == 17) ? -1 : 0);
+}
+__host__ __device__ constexpr int copp(int a) { return a == 0 ? 0 : ((a & 1) ? a + 1 : a - 1); }
+// Eq. 15
+template <typename T> __host__ __device__ constexpr T cw(int a) {
+  return a == 0 ? T(1.0 / 3.0) : (a < 7 ? T(1.0 / 18.0) : T(1.0 / 36.0));
+}
+
+template <typename T> struct KP {
+  int nx, ny, nz;
+  long long n;    // nodes
+  long long nxy;  // nodes per z layer
+  int bc[6];
+  int has_inlet, has_outlet, any_nonperiodic, visc_interp;
+  T rho_h, rho_l, drho;
+  T tau_h, tau_l, itau_h, itau_l;
+  T beta4, kappa, inv_W, om_phi;
+  T gx, gy, gz, rho_ref;
+  T uin[3], phi_in;
+  // arrays
+  const T* f_src; const T* g_src;  // post-collision at t
+  T* f_dst; T* g_dst;              // post-collision at t+1
+  T* phi; T* u;
+  T* ob_f; T* ob_g; T* lam;
+  const uint8_t* mask;
+};
+
+template <typename T> __device__ __forceinline__ T rsqrt_(T x);
+template <> __device__ __forceinline__ float rsqrt_<float>(float x) { return rsqrtf(x); }
+template <> __device__ __forceinline__ double rsqrt_<double>(double x) { return rsqrt(x); }
+template <typename T> __device__ __forceinline__ T sqrt_(T x);
+template <> __device__ __forceinline__ float sqrt_<float>(float x) { return sqrtf(x); }
+template <> __device__ __forceinline__ double sqrt_<double>(double x) { return sqrt(x); }
+
+// ------------------------------------------------------------------------------------------------ geometry
+struct Nbr {
+  // element offsets to the x-1 / x+1 / y-1 / y+1 / z-1 / z+1 neighbour (periodic wrap applied)
+  long long xm, xp, ym, yp, zm, zp;
+  // the link towards that side crosses a non-periodic face and bounces back (B.10-B.11)
+  bool bxm, bxp, bym, byp, bzm, bzp;
+  // the link crosses the inlet disc (unknown, B.4) / the outlet face (layer overwritten, B.5)
+  bool ozm, ozp;
+  bool any;
+};
+
+template <typename T>
+__device__ __forceinline__ Nbr make_nbr(const KP<T>& P, int x, int y, int z) {
+  Nbr b;
+  b.xm = (x == 0) ? (long long)(P.nx - 1) : -1LL;
+  b.xp = (x == P.nx - 1) ? -(long long)(P.nx - 1) : 1LL;
+  b.ym = ((y == 0) ? (long long)(P.ny - 1) : -1LL) * P.nx;
+  b.yp = ((y == P.ny - 1) ? -(long long)(P.ny - 1) : 1LL) * P.nx;
+  b.zm = ((z == 0) ? (long long)(P.nz - 1) : -1LL) * P.nxy;
+  b.zp = ((z == P.nz - 1) ? -(long long)(P.nz - 1) : 1LL) * P.nxy;
+  b.bxm = b.bxp = b.bym = b.byp = b.bzm = b.bzp = b.ozm = b.ozp = false;
+  if (P.any_nonperiodic) {
+    b.bxm = (x == 0) && P.bc[0] != BC_PERIODIC;
+    b.bxp = (x == P.nx - 1) && P.bc[1] != BC_PERIODIC;
+    b.bym = (y == 0) && P.bc[2] != BC_PERIODIC;
+    b.byp = (y == P.ny - 1) && P.bc[3] != BC_PERIODIC;
+    if (z == 0 && P.bc[4] != BC_PERIODIC) {
+      const bool disc = (P.bc[4] == BC_INLET) && P.mask[(long long)y * P.nx + x];
+      b.bzm = !disc;
+      b.ozm = disc;
+    }
+    if (z == P.nz - 1 && P.bc[5] != BC_PERIODIC) {
+      b.bzp = (P.bc[5] == BC_WALL);
+      b.ozp = (P.bc[5] == BC_OUTLET);
+    }
+  }
+  b.any = b.bxm | b.bxp | b.bym | b.byp | b.bzm | b.bzp | b.ozm | b.ozp;
+  return b;
+}
+
+template <int a> __device__ __forceinline__ long long src_off(const Nbr& b) {
+  long long o = 0;
+  if (cx(a) == 1) o += b.xm; else if (cx(a) == -1) o += b.xp;
+  if (cy(a) == 1) o += b.ym; else if (cy(a) == -1) o += b.yp;
+  if (cz(a) == 1) o += b.zm; else if (cz(a) == -1) o += b.zp;
+  return o;
+}
+template <int a> __device__ __forceinline__ bool src_bounce(const Nbr& b) {
+  return (cx(a) == 1 && b.bxm) || (cx(a) == -1 && b.bxp) || (cy(a) == 1 && b.bym) || (cy(a) == -1 && b.byp) ||
+         (cz(a) == 1 && b.bzm) || (cz(a) == -1 && b.bzp);
+}
+template <int a> __device__ __forceinline__ bool src_open(const Nbr& b) {
+  return (cz(a) == 1 && b.ozm) || (cz(a) == -1 && b.ozp);
+}
+
+// Streaming (pull) of one population set at node i: Alg. 2 / B.3-B.4 with periodic wrap (B.5-B.6) and halfway
+// bounce-back (B.10-B.11; a wall crossing wins at edges and corners, R11).  Open links (inlet disc / outlet
+// face) get 0 and are filled by the caller.
+template <typename T, int a>
+__device__ __forceinline__ T pull_one(const T* __restrict__ src, long long n, long long i, const Nbr& b, bool slow) {
+  if (!slow) return __ldg(src + (long long)a * n + i + src_off<a>(b));
+  if (src_bounce<a>(b)) return __ldg(src + (long long)copp(a) * n + i);
+  if (src_open<a>(b)) return T(0);
+  return __ldg(src + (long long)a * n + i + src_off<a>(b));
+}
+
+template <typename T, int a = 0> struct PullAll {
+  static __device__ __forceinline__ void run(const T* __restrict__ src, long long n, long long i, const Nbr& b, bool slow,
+                                              T (&v)[Q]) {
+    v[a] = pull_one<T, a>(src, n, i, b, slow);
+    PullAll<T, a + 1>::run(src, n, i, b, slow, v);
+  }
+};
+template <typename T> struct PullAll<T, Q> {
+  static __device__ __forceinline__ void run(const T* __restrict__, long long, long long, const Nbr&, bool, T (&)[Q]) {}
+};
+
+// Gamma_a / w_a, Eq. 18
+template <typename T, int a> __device__ __forceinline__ T gamma_over_w(T ux, T uy, T uz, T usq15) {
+  const T eu = T(cx(a)) * ux + T(cy(a)) * uy + T(cz(a)) * uz;
+  return T(1) + T(3) * eu + T(4.5) * eu * eu - usq15;
+}
+
+// Velocity inlet for g on a disc node (B.16-B.20 as read in G6): unknown set e_z = +1.
+template <typename T> __device__ __forceinline__ void inlet_g(const KP<T>& P, T (&g)[Q]) {
+  const T ux = P.uin[0], uy = P.uin[1], uz = P.uin[2];
+  const T usq15 = T(1.5) * (ux * ux + uy * uy + uz * uz);
+  T geq[Q];
+#pragma unroll
+  for (int a = 0; a < Q; ++a) {
+    const T eu = T(cx(a)) * ux + T(cy(a)) * uy + T(cz(a)) * uz;
+    geq[a] = P.phi_in * cw<T>(a) * (T(1) + T(3) * eu + T(4.5) * eu * eu - usq15);
+  }
+  T theta = 0;
+#pragma unroll
+  for (int a = 0; a < Q; ++a) if (cz(a) == 0) theta += g[a] - geq[a];
+#pragma unroll
+  for (int a = 0; a < Q; ++a) if (cz(a) == 1) {
+    const int b = copp(a);
+    g[a] = geq[a] - (g[b] - geq[b]) - ((cx(a) != 0 || cy(a) != 0) ? theta * T(0.25) : T(0));
+  }
+}
+// Velocity inlet for f (B.12-B.15 as read in G6; F = 0 at the inlet so f' = f).
+template <typename T> __device__ __forceinline__ void inlet_f(const KP<T>& P, T (&f)[Q]) {
+  const T ux = P.uin[0], uy = P.uin[1], uz = P.uin[2];
+  T Mx = 0, My = 0;
+#pragma unroll
+  for (int a = 0; a < Q; ++a) if (cz(a) == 0) { Mx += T(cx(a)) * f[a]; My += T(cy(a)) * f[a]; }
+  Mx -= T(2.0 / 3.0) * ux; My -= T(2.0 / 3.0) * uy;
+#pragma unroll
+  for (int a = 0; a < Q; ++a) if (cz(a) == 1) {
+    const T eu = T(cx(a)) * ux + T(cy(a)) * uy + T(cz(a)) * uz;
+    f[a] = f[copp(a)] + T(6) * cw<T>(a) * eu - T(0.5) * (T(cx(a)) * Mx + T(cy(a)) * My);
+  }
+}
+
+// Post-stream, post-BC populations of node (x,y,z) at t+1 (steps 7-9 of DESIGN.md): pull, inlet, outlet.
+// lam_out (may be null): where the outlet lambda of this column is stored when it is computed from u(t).
+template <typename T, bool WITH_F, bool LAM_FROM_U>
+__device__ __forceinline__ void load_node(const KP<T>& P, int x, int y, int z, T (&f)[Q], T (&g)[Q]) {
+  const bool outlet_layer = P.has_outlet && (z == P.nz - 1);
+  const int zs = outlet_layer ? z - 1 : z;  // B.26-B.27 need the post-stream values of layer N-1
+  const long long i = (long long)zs * P.nxy + (long long)y * P.nx + x;
+  const Nbr b = make_nbr(P, x, y, zs);
+  const bool slow = P.any_nonperiodic && b.any;
+  PullAll<T>::run(P.g_src, P.n, i, b, slow, g);
+  if (WITH_F) PullAll<T>::run(P.f_src, P.n, i, b, slow, f);
+  if (P.has_inlet && b.ozm) {
+    inlet_g(P, g);
+    if (WITH_F) inlet_f(P, f);
+  }
+  if (outlet_layer) {
+    const long long c = (long long)y * P.nx + x;
+    T lam;
+    if (LAM_FROM_U) {  // U_local of B.22 from the stored u(t) of layer N-1, clamped at 0 (R12)
+      lam = P.u[2 * P.n + i];
+      lam = lam > T(0) ? lam : T(0);
+      P.lam[c] = lam;
+    } else {
+      lam = P.lam[c];
+    }
+    const T inv = T(1) / (T(1) + lam);
+#pragma unroll
+    for (int a = 0; a < Q; ++a) {
+      g[a] = (P.ob_g[a * P.nxy + c] + lam * g[a]) * inv;
+      if (WITH_F) f[a] = (P.ob_f[a * P.nxy + c] + lam * f[a]) * inv;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ stencils
+// Eq. 40a/b on differences d_a = phi(x+e_a) - phi(x); ghost rule: periodic wrap (B.7) or
+// clamp at non-periodic faces (R9).
+template <typename T>
+__device__ __forceinline__ void phi_stencil(const KP<T>& P, const T* __restrict__ phi, int x, int y, int z, T pc,
+                                            T (&G)[3], T& L) {
+  const long long i = (long long)z * P.nxy + (long long)y * P.nx + x;
+  long long oxm = (x == 0) ? ((P.bc[0] == BC_PERIODIC) ? (long long)(P.nx - 1) : 0LL) : -1LL;
+  long long oxp = (x == P.nx - 1) ? ((P.bc[1] == BC_PERIODIC) ? -(long long)(P.nx - 1) : 0LL) : 1LL;
+  long long oym = ((y == 0) ? ((P.bc[2] == BC_PERIODIC) ? (long long)(P.ny - 1) : 0LL) : -1LL) * P.nx;
+  long long oyp = ((y == P.ny - 1) ? ((P.bc[3] == BC_PERIODIC) ? -(long long)(P.ny - 1) : 0LL) : 1LL) * P.nx;
+  long long ozm = ((z == 0) ? ((P.bc[4] == BC_PERIODIC) ? (long long)(P.nz - 1) : 0LL) : -1LL) * P.nxy;
+  long long ozp = ((z == P.nz - 1) ? ((P.bc[5] == BC_PERIODIC) ? -(long long)(P.nz - 1) : 0LL) : 1LL) * P.nxy;
+  T d[Q];
+#pragma unroll
+  for (int a = 1; a < Q; ++a) {
+    long long o = 0;
+    if (cx(a) == 1) o += oxp; else if (cx(a) == -1) o += oxm;
+    if (cy(a) == 1) o += oyp; else if (cy(a) == -1) o += oym;
+    if (cz(a) == 1) o += ozp; else if (cz(a) == -1) o += ozm;
+    d[a] = phi[i + o] - pc;
+  }
+  const T s1 = ((d[1] + d[2]) + (d[3] + d[4])) + (d[5] + d[6]);
+  const T s2 = (((d[7] + d[8]) + (d[9] + d[10])) + ((d[11] + d[12]) + (d[13] + d[14]))) + ((d[15] + d[16]) + (d[17] + d[18]));
+  L = T(6) * (T(1.0 / 18.0) * s1 + T(1.0 / 36.0) * s2);
+  G[0] = T(3) * (T(1.0 / 18.0) * (d[1] - d[2]) + T(1.0 / 36.0) * (((d[7] - d[8]) + (d[9] - d[10])) + ((d[11] - d[12]) + (d[13] - d[14]))));
+  G[1] = T(3) * (T(1.0 / 18.0) * (d[3] - d[4]) + T(1.0 / 36.0) * (((d[7] - d[8]) - (d[9] - d[10])) + ((d[15] - d[16]) + (d[17] - d[18]))));
+  G[2] = T(3) * (T(1.0 / 18.0) * (d[5] - d[6]) + T(1.0 / 36.0) * (((d[11] - d[12]) - (d[13] - d[14])) + ((d[15] - d[16]) - (d[17] - d[18]))));
+}
+
+// ------------------------------------------------------------------------------------------------ physics
+template <typename T> struct Mat {  // material state of a node from phi and its stencils
+  T rho, inv_rho, tau, s_nu, mu;
+};
+template <typename T> __device__ __forceinline__ Mat<T> materials(const KP<T>& P, T phi, T L) {
+  Mat<T> m;
+  m.rho = P.rho_l + phi * P.drho;                                              // Eq. 39
+  m.inv_rho = T(1) / m.rho;
+  if (P.visc_interp == 1) m.tau = T(1) / (P.itau_l + phi * (P.itau_h - P.itau_l));
+  else m.tau = P.tau_l + phi * (P.tau_h - P.tau_l);                            // Eq. 24
+  m.s_nu = T(1) / (m.tau + T(0.5));                                            // G3
+  m.mu = P.beta4 * phi * (phi - T(1)) * (phi - T(0.5)) - P.kappa * L;          // Eq. 11 (sign corrected, G4)
+  return m;
+}
+
+template <typename T> struct Mom {  // p* = sum f, m = sum f e, Pi = sum f e e
+  T p, mx, my, mz, xx, yy, zz, xy, yz, xz;
+};
+template <typename T> __device__ __forceinline__ Mom<T> moments(const T (&f)[Q]) {
+  Mom<T> m;
+  // pairwise sums / differences of opposite directions
+  const T s12 = f[1] + f[2], s34 = f[3] + f[4], s56 = f[5] + f[6];
+  const T s78 = f[7] + f[8], s910 = f[9] + f[10], s1112 = f[11] + f[12], s1314 = f[13] + f[14];
+  const T s1516 = f[15] + f[16], s1718 = f[17] + f[18];
+  const T d12 = f[1] - f[2], d34 = f[3] - f[4], d56 = f[5] - f[6];
+  const T d78 = f[7] - f[8], d910 = f[9] - f[10], d1112 = f[11] - f[12], d1314 = f[13] - f[14];
+  const T d1516 = f[15] - f[16], d1718 = f[17] - f[18];
+  const T sxy = s78 + s910, sxz = s1112 + s1314, syz = s1516 + s1718;
+  m.p = (f[0] + (s12 + s34 + s56)) + (sxy + sxz + syz);
+  m.mx = d12 + (d78 + d910) + (d1112 + d1314);
+  m.my = d34 + (d78 - d910) + (d1516 + d1718);
+  m.mz = d56 + (d1112 - d1314) + (d1516 - d1718);
+  m.xx = s12 + sxy + sxz;
+  m.yy = s34 + sxy + syz;
+  m.zz = s56 + sxz + syz;
+  m.xy = s78 - s910;
+  m.xz = s1112 - s1314;
+  m.yz = s1516 - s1718;
+  return m;
+}
+
+// Total force, Eq. 20: F_s (Eq. 10) + F_b (G16) + F_p (Eq. 21) + F_mu (Eq. 30 in closed form).  Also returns
+// D = dev(Pi^neq) for the collision.
+template <typename T>
+__device__ __forceinline__ void total_force(const KP<T>& P, const Mom<T>& m, const Mat<T>& mat, T ux, T uy, T uz,
+                                            const T (&G)[3], T (&F)[3], T (&D)[6]) {
+  const T p3 = m.p * T(1.0 / 3.0);
+  const T nxx = m.xx - (p3 + ux * ux), nyy = m.yy - (p3 + uy * uy), nzz = m.zz - (p3 + uz * uz);
+  const T nxy = m.xy - ux * uy, nyz = m.yz - uy * uz, nxz = m.xz - ux * uz;
+  const T tr3 = (nxx + nyy + nzz) * T(1.0 / 3.0);
+  D[0] = nxx - tr3; D[1] = nyy - tr3; D[2] = nzz - tr3; D[3] = nxy; D[4] = nyz; D[5] = nxz;
+  const T s = mat.s_nu;
+  const T Sxx = s * D[0] + tr3, Syy = s * D[1] + tr3, Szz = s * D[2] + tr3;
+  const T Sxy = s * D[3], Syz = s * D[4], Sxz = s * D[5];
+  const T cmu = -mat.tau * P.drho;
+  const T cs = mat.mu - p3 * P.drho;  // F_s + F_p = (mu_phi - p* c_s^2 (rho_h - rho_l)) grad phi
+  const T rb = mat.rho - P.rho_ref;
+  F[0] = cs * G[0] + rb * P.gx + cmu * (Sxx * G[0] + Sxy * G[1] + Sxz * G[2]);
+  F[1] = cs * G[1] + rb * P.gy + cmu * (Sxy * G[0] + Syy * G[1] + Syz * G[2]);
+  F[2] = cs * G[2] + rb * P.gz + cmu * (Sxz * G[0] + Syz * G[1] + Szz * G[2]);
+}
+
+// Both collisions of one node (Alg. 1): in f, g pre-collision; out post-collision in place.
+template <typename T>
+__device__ __forceinline__ void collide(const KP<T>& P, const Mom<T>& m, const Mat<T>& mat, T phi, const T (&G)[3], T ux,
+                                        T uy, T uz, T (&f)[Q], T (&g)[Q]) {
+  T F[3], D[6];
+  total_force(P, m, mat, ux, uy, uz, G, F, D);
+  const T usq15 = T(1.5) * (ux * ux + uy * uy + uz * uz);
+  const T hx = T(1.5) * F[0] * mat.inv_rho, hy = T(1.5) * F[1] * mat.inv_rho, hz = T(1.5) * F[2] * mat.inv_rho;
+  const T k = T(4.5) * (T(1) - mat.s_nu);
+  // interface normal (R10) and F^phi prefactor, Eq. 34
+  const T gn = sqrt_(G[0] * G[0] + G[1] * G[1] + G[2] * G[2]) + T(1e-32);
+  const T ign = T(1) / gn;
+  const T pref = (T(1) - T(4) * (phi - T(0.5)) * (phi - T(0.5))) * P.inv_W;
+  const T om = P.om_phi;
+  const T cphi = (T(1) - T(0.5) * om) * pref;
+  const T nx_ = G[0] * ign * cphi, ny_ = G[1] * ign * cphi, nz_ = G[2] * ign * cphi;
+  const T omphi = om * phi, om1 = T(1) - om;
+#pragma unroll
+  for (int a = 0; a < Q; ++a) {
+    const T ex = T(cx(a)), ey = T(cy(a)), ez = T(cz(a));
+    const T eu = ex * ux + ey * uy + ez * uz;
+    const T gam = T(3) * eu + T(4.5) * eu * eu - usq15;  // Gamma_a / w_a - 1
+    const T eDe = ex * ex * D[0] + ey * ey * D[1] + ez * ez * D[2] + T(2) * (ex * ey * D[3] + ey * ez * D[4] + ex * ez * D[5]);
+    f[a] = cw<T>(a) * ((m.p + gam) + (ex * hx + ey * hy + ez * hz) + k * eDe);
+    g[a] = om1 * g[a] + cw<T>(a) * (omphi * (T(1) + gam) + (ex * nx_ + ey * ny_ + ez * nz_));
+  }
+}
+
+template <typename T, int a = 0> struct StoreAll {
+  static __device__ __forceinline__ void run(T* __restrict__ dst, long long n, long long i, const T (&v)[Q]) {
+    dst[(long long)a * n + i] = v[a];
+    StoreAll<T, a + 1>::run(dst, n, i, v);
+  }
+};
+template <typename T> struct StoreAll<T, Q> {
+  static __device__ __forceinline__ void run(T* __restrict__, long long, long long, const T (&)[Q]) {}
+};
+
+// ------------------------------------------------------------------------------------------------ kernels
+// k_phi: phi(t+1) = sum_a g_a(x,t+1)  (Eq. 38) from the post-collision g+(t); inlet nodes get phi_in.
+template <typename T> __global__ void __launch_bounds__(256) k_phi(const __grid_constant__ KP<T> P) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= P.n) return;
+  const int x = (int)(i % P.nx);
+  const long long r = i / P.nx;
+  const int y = (int)(r % P.ny), z = (int)(r / P.ny);
+  T f[Q], g[Q];
+  load_node<T, false, true>(P, x, y, z, f, g);
+  T s = ((g[0] + (g[1] + g[2])) + ((g[3] + g[4]) + (g[5] + g[6]))) +
+        (((g[7] + g[8]) + (g[9] + g[10])) + ((g[11] + g[12]) + (g[13] + g[14])) + ((g[15] + g[16]) + (g[17] + g[18])));
+  if (P.has_inlet && z == 0 && P.mask[(long long)y * P.nx + x]) s = P.phi_in;
+  P.phi[i] = s;
+}
+
+// k_step: the fused stream -> BC -> macro -> collide kernel.
+template <typename T> __global__ void __launch_bounds__(256) k_step(const __grid_constant__ KP<T> P) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= P.n) return;
+  const int x = (int)(i % P.nx);
+  const long long r = i / P.nx;
+  const int y = (int)(r % P.ny), z = (int)(r / P.ny);
+  T f[Q], g[Q];
+  load_node<T, true, false>(P, x, y, z, f, g);
+  if (P.has_outlet && z == P.nz - 1) {  // keep chi(N, t+1) for the next step's B.26-B.27
+    const long long c = (long long)y * P.nx + x;
+#pragma unroll
+    for (int a = 0; a < Q; ++a) { P.ob_f[a * P.nxy + c] = f[a]; P.ob_g[a * P.nxy + c] = g[a]; }
+  }
+  const T phi = P.phi[i];
+  T G[3], L;
+  phi_stencil(P, P.phi, x, y, z, phi, G, L);
+  const Mat<T> mat = materials(P, phi, L);
+  const Mom<T> m = moments(f);
+  // macros, Alg. 3: F from (new p*, new phi, lagged u), then Eq. 31b
+  T ux = P.u[i], uy = P.u[P.n + i], uz = P.u[2 * P.n + i];
+  {
+    T F[3], D[6];
+    total_force(P, m, mat, ux, uy, uz, G, F, D);
+    const T h = T(0.5) * mat.inv_rho;
+    ux = m.mx + h * F[0]; uy = m.my + h * F[1]; uz = m.mz + h * F[2];
+  }
+  if (P.has_inlet && z == 0 && P.mask[(long long)y * P.nx + x]) { ux = P.uin[0]; uy = P.uin[1]; uz = P.uin[2]; }
+  P.u[i] = ux; P.u[P.n + i] = uy; P.u[2 * P.n + i] = uz;
+  collide(P, m, mat, phi, G, ux, uy, uz, f, g);
+  StoreAll<T>::run(P.f_dst, P.n, i, f);
+  StoreAll<T>::run(P.g_dst, P.n, i, g);
+}
+
+// k_init: I1-I4 of DESIGN.md (R8), then the first collision; phi0/u0 are caller buffers.
+template <typename T>
+__global__ void __launch_bounds__(256) k_init(const __grid_constant__ KP<T> P, const T* __restrict__ phi0,
+                                              const T* __restrict__ u0) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= P.n) return;
+  const int x = (int)(i % P.nx);
+  const long long r = i / P.nx;
+  const int y = (int)(r % P.ny), z = (int)(r / P.ny);
+  const T phi = phi0[i];
+  const T ux = u0[i], uy = u0[P.n + i], uz = u0[2 * P.n + i];
+  T G[3], L;
+  phi_stencil(P, phi0, x, y, z, phi, G, L);
+  const Mat<T> mat = materials(P, phi, L);
+  // I3: F = F_s + F_b (p* = 0 => F_p = 0; F_mu = 0)
+  const T rb = mat.rho - P.rho_ref;
+  const T F0 = mat.mu * G[0] + rb * P.gx, F1 = mat.mu * G[1] + rb * P.gy, F2 = mat.mu * G[2] + rb * P.gz;
+  const T usq15 = T(1.5) * (ux * ux + uy * uy + uz * uz);
+  const T gn = sqrt_(G[0] * G[0] + G[1] * G[1] + G[2] * G[2]) + T(1e-32);
+  const T pref = (T(1) - T(4) * (phi - T(0.5)) * (phi - T(0.5))) * P.inv_W / gn;
+  T f[Q], g[Q];
+#pragma unroll
+  for (int a = 0; a < Q; ++a) {
+    const T ex = T(cx(a)), ey = T(cy(a)), ez = T(cz(a));
+    const T eu = ex * ux + ey * uy + ez * uz;
+    const T gam = T(3) * eu + T(4.5) * eu * eu - usq15;
+    const T Fa = T(3) * (ex * F0 + ey * F1 + ez * F2) * mat.inv_rho;  // Eq. 19 / w_a
+    const T Fp = pref * (ex * G[0] + ey * G[1] + ez * G[2]);          // Eq. 34 / w_a
+    f[a] = cw<T>(a) * (gam - T(0.5) * Fa);                            // I4
+    g[a] = cw<T>(a) * (phi * (T(1) + gam) - T(0.5) * Fp);
+  }
+  if (P.has_outlet && z == P.nz - 1) {
+    const long long c = (long long)y * P.nx + x;
+#pragma unroll
+    for (int a = 0; a < Q; ++a) { P.ob_f[a * P.nxy + c] = f[a]; P.ob_g[a * P.nxy + c] = g[a]; }
+  }
+  P.phi[i] = phi;
+  P.u[i] = ux; P.u[P.n + i] = uy; P.u[2 * P.n + i] = uz;
+  const Mom<T> m = moments(f);
+  collide(P, m, mat, phi, G, ux, uy, uz, f, g);
+  StoreAll<T>::run(P.f_dst, P.n, i, f);
+  StoreAll<T>::run(P.g_dst, P.n, i, g);
+}
+
+// k_get: phi, p = p* rho c_s^2 with p* = sum_a f+_a (the collision conserves sum f), u.
+template <typename T>
+__global__ void __launch_bounds__(256) k_get(const __grid_constant__ KP<T> P, T* __restrict__ phi_out, T* __restrict__ p_out,
+                                             T* __restrict__ u_out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= P.n) return;
+  const T phi = P.phi[i];
+  if (phi_out) phi_out[i] = phi;
+  if (u_out) { u_out[i] = P.u[i]; u_out[P.n + i] = P.u[P.n + i]; u_out[2 * P.n + i] = P.u[2 * P.n + i]; }
+  if (p_out) {
+    T f[Q];
+#pragma unroll
+    for (int a = 0; a < Q; ++a) f[a] = P.f_src[(long long)a * P.n + i];
+    const Mom<T> m = moments(f);
+    p_out[i] = m.p * (P.rho_l + phi * P.drho) * T(1.0 / 3.0);
+  }
+}
+
+}  // namespace clip

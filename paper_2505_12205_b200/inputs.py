@@ -1,0 +1,161 @@
+"""Seeded synthetic inputs for the CLIP hot path (shared by the oracle tests, the GPU tests and bench.py).
+
+This module holds *no* arithmetic of the method: it only builds initial fields phi0 / u0 and parameter
+dictionaries.  Recipes are the ones stated in DESIGN.md ("Input recipe") and SURVEY.md section 8(d); the initial
+interface profile is the paper's equilibrium kernel, PAPER.md:118 (Eq. 5), and the Rayleigh-Taylor perturbation
+is PAPER.md:729 (Eq. 53) as restated by BASELINE.json configs[2].
+
+Layout everywhere: phi0[z, y, x] (x fastest), u0[c, z, y, x].  Node j sits at coordinate j (cell index); walls
+(halfway bounce-back) sit half a cell outside the first / last node.
+
+Parameter dictionary keys (both the oracle binding and the CUDA binding marshal these into their own structs):
+  precision (32|64), rho_h, rho_l, tau_h, tau_l, sigma, W, M, g (3), rho_ref, bc (6: -x,+x,-y,+y,-z,+z),
+  inlet_u (3), inlet_phi, inlet_c (2), inlet_r, outlet_u_mode, visc_interp
+"""
+from __future__ import annotations
+
+import numpy as np
+
+PERIODIC, WALL, INLET, OUTLET = 0, 1, 2, 3
+
+
+def default_params(**kw) -> dict:
+    p = dict(
+        precision=64,
+        rho_h=1.0, rho_l=1.0e-3,
+        tau_h=0.8, tau_l=0.8,
+        sigma=0.01, W=4.0, M=0.1,
+        g=(0.0, 0.0, 0.0), rho_ref=0.0,
+        bc=(PERIODIC,) * 6,
+        inlet_u=(0.0, 0.0, 0.0), inlet_phi=1.0,
+        inlet_c=(0.0, 0.0), inlet_r=0.0,
+        outlet_u_mode=0, visc_interp=0,
+    )
+    p.update(kw)
+    return p
+
+
+def _grid(nx, ny, nz):
+    z, y, x = np.meshgrid(np.arange(nz, dtype=np.float64), np.arange(ny, dtype=np.float64),
+                          np.arange(nx, dtype=np.float64), indexing="ij")
+    return x, y, z
+
+
+def _case(nx, ny, nz, params, phi0, u0, name):
+    return dict(name=name, nx=int(nx), ny=int(ny), nz=int(nz), params=params,
+                phi0=np.ascontiguousarray(phi0, dtype=np.float64),
+                u0=np.ascontiguousarray(u0, dtype=np.float64))
+
+
+def drop(n=32, R=8.0, W=4.0, sigma=0.01, rho_ratio=1000.0, tau=0.8, M=0.1, precision=64):
+    """BASELINE.json configs[0]: stationary drop in a periodic cube, centred at ((n-1)/2,)*3, u0 = 0."""
+    x, y, z = _grid(n, n, n)
+    c = 0.5 * (n - 1)
+    r = np.sqrt((x - c) ** 2 + (y - c) ** 2 + (z - c) ** 2)
+    phi0 = 0.5 + 0.5 * np.tanh(2.0 * (R - r) / W)
+    u0 = np.zeros((3, n, n, n))
+    p = default_params(precision=precision, rho_h=1.0, rho_l=1.0 / rho_ratio, tau_h=tau, tau_l=tau,
+                       sigma=sigma, W=W, M=M)
+    return _case(n, n, n, p, phi0, u0, f"drop{n}")
+
+
+def poiseuille(nx=4, ny=128, nz=4, tau_a=1.0, tau_b=0.1, rho_a=1.0, rho_b=1.0, gx=1.0e-6, W=4.0, M=0.1,
+               visc_interp=0, precision=64):
+    """BASELINE.json configs[1]: layered two-phase Poiseuille; fluid A (phi=1) below y = ny/2, walls in y."""
+    x, y, z = _grid(nx, ny, nz)
+    yc = y + 0.5
+    phi0 = 0.5 - 0.5 * np.tanh(2.0 * (yc - 0.5 * ny) / W)
+    u0 = np.zeros((3, nz, ny, nx))
+    p = default_params(precision=precision, rho_h=rho_a, rho_l=rho_b, tau_h=tau_a, tau_l=tau_b, sigma=0.0,
+                       W=W, M=M, g=(gx, 0.0, 0.0), rho_ref=0.0,
+                       bc=(PERIODIC, PERIODIC, WALL, WALL, PERIODIC, PERIODIC), visc_interp=visc_interp)
+    return _case(nx, ny, nz, p, phi0, u0, f"poiseuille{nx}x{ny}x{nz}")
+
+
+def rayleigh_taylor(L=128, W=5.0, precision=32):
+    """BASELINE.json configs[2] at scale L (L=128 is the named lattice L x 4L x L; L=16 the parity replica).
+
+    At = 0.5 (rho_h=3, rho_l=1); U0 = sqrt(g L) = 0.04; Re = 3000; mu ratio 1; Pe = 1000; Ca = 0.26
+    (Table 5; Eq. 54-57).  Heavy fluid on top, gravity along -y, walls in y.
+    """
+    nx, ny, nz = L, 4 * L, L
+    x, y, z = _grid(nx, ny, nz)
+    y0 = 2.0 * L + 0.05 * L * (np.cos(2 * np.pi * x / L) + np.cos(2 * np.pi * z / L))
+    phi0 = 0.5 + 0.5 * np.tanh(2.0 * (y - y0) / W)
+    u0 = np.zeros((3, nz, ny, nx))
+    U0 = 0.04
+    gy = U0 * U0 / L
+    rho_h, rho_l = 3.0, 1.0
+    nu_h = U0 * L / 3000.0
+    tau_h = 3.0 * nu_h
+    tau_l = tau_h * rho_h / rho_l          # equal dynamic viscosity
+    Mob = U0 * L / 1000.0
+    sigma = rho_h * nu_h * U0 / 0.26
+    p = default_params(precision=precision, rho_h=rho_h, rho_l=rho_l, tau_h=tau_h, tau_l=tau_l, sigma=sigma,
+                       W=W, M=Mob, g=(0.0, -gy, 0.0), rho_ref=0.5 * (rho_h + rho_l),
+                       bc=(PERIODIC, PERIODIC, WALL, WALL, PERIODIC, PERIODIC))
+    return _case(nx, ny, nz, p, phi0, u0, f"rt{L}")
+
+
+def jet(nxy=192, nz=1536, r_nozzle=12.0, We=2.2, W=4.0, U=0.05, precision=32):
+    """BASELINE.json configs[3] (nxy=192, nz=1536, r=12) or its parity replica (24, 96, 4).
+
+    -z face: INLET disc (plug inflow U along +z, phi_in = 1; wall outside the disc); +z face: convective OUTLET;
+    x and y faces: no-slip walls.  Re = 200, mu ratio 100, rho ratio 1000 (Table 6).
+    """
+    nx = ny = nxy
+    x, y, z = _grid(nx, ny, nz)
+    c = 0.5 * (nxy - 1)
+    rxy = np.sqrt((x - c) ** 2 + (y - c) ** 2)
+    d = np.minimum(r_nozzle - rxy, r_nozzle - z)
+    phi0 = 0.5 + 0.5 * np.tanh(2.0 * d / W)
+    u0 = np.zeros((3, nz, ny, nx))
+    D = 2.0 * r_nozzle
+    rho_h, rho_l = 1.0, 1.0e-3
+    nu_h = U * D / 200.0
+    nu_l = nu_h * (rho_h / rho_l) / 100.0
+    sigma = rho_h * U * U * D / We
+    p = default_params(precision=precision, rho_h=rho_h, rho_l=rho_l, tau_h=3 * nu_h, tau_l=3 * nu_l,
+                       sigma=sigma, W=W, M=0.1,
+                       bc=(WALL, WALL, WALL, WALL, INLET, OUTLET),
+                       inlet_u=(0.0, 0.0, U), inlet_phi=1.0, inlet_c=(c, c), inlet_r=r_nozzle)
+    return _case(nx, ny, nz, p, phi0, u0, f"jet{nxy}x{nz}")
+
+
+def sweep_drops(n=64, seed=2505, ndrops=20, rmin=6.0, rmax=20.0, W=4.0, u_amp=0.01, precision=32,
+                shape=None):
+    """BASELINE.json configs[4]: periodic box with `ndrops` seeded spherical drops and i.i.d. uniform u0.
+
+    phi0 = max_k [0.5 + 0.5 tanh(2 (R_k - d_k)/W)] with d_k the periodic minimum-image distance.
+    `shape=(nx,ny,nz)` gives a non-cubic box (used by the odd-size parity case).
+    """
+    nx, ny, nz = (n, n, n) if shape is None else shape
+    rng = np.random.Generator(np.random.PCG64(seed))
+    cen = rng.uniform(0.0, 1.0, size=(ndrops, 3)) * np.array([nx, ny, nz], dtype=np.float64)
+    rad = rng.uniform(rmin, rmax, size=ndrops)
+    x = np.arange(nx, dtype=np.float64)[None, None, :]
+    y = np.arange(ny, dtype=np.float64)[None, :, None]
+    z = np.arange(nz, dtype=np.float64)[:, None, None]
+    phi0 = np.zeros((nz, ny, nx))
+    for k in range(ndrops):
+        dx = np.abs(x - cen[k, 0]); dx = np.minimum(dx, nx - dx)
+        dy = np.abs(y - cen[k, 1]); dy = np.minimum(dy, ny - dy)
+        dz = np.abs(z - cen[k, 2]); dz = np.minimum(dz, nz - dz)
+        d = np.sqrt(dx * dx + dy * dy + dz * dz)
+        np.maximum(phi0, 0.5 + 0.5 * np.tanh(2.0 * (rad[k] - d) / W), out=phi0)
+    u0 = rng.uniform(-u_amp, u_amp, size=(3, nz, ny, nx))
+    p = default_params(precision=precision, rho_h=1.0, rho_l=1.0e-3, tau_h=0.8, tau_l=0.8, sigma=0.01,
+                       W=W, M=0.1)
+    return _case(nx, ny, nz, p, phi0, u0, f"sweep{nx}x{ny}x{nz}")
+
+
+def walled_box(nx=12, ny=10, nz=14, seed=7, precision=64):
+    """A small all-walls box with one off-centre drop and a random u0 (exercises edges and corners, R11)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    x, y, z = _grid(nx, ny, nz)
+    r = np.sqrt((x - 0.45 * nx) ** 2 + (y - 0.5 * ny) ** 2 + (z - 0.4 * nz) ** 2)
+    phi0 = 0.5 + 0.5 * np.tanh(2.0 * (0.28 * min(nx, ny, nz) - r) / 3.0)
+    u0 = rng.uniform(-0.005, 0.005, size=(3, nz, ny, nx))
+    p = default_params(precision=precision, rho_h=1.0, rho_l=0.1, tau_h=0.6, tau_l=0.3, sigma=0.005, W=3.0,
+                       M=0.05, g=(0.0, 0.0, -1.0e-5), bc=(WALL,) * 6)
+    return _case(nx, ny, nz, p, phi0, u0, f"walled{nx}x{ny}x{nz}")

@@ -1,0 +1,141 @@
+"""GPU parity: libclip (CUDA, through the C ABI) vs the CPU oracle, element by element on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): after 100 steps, fp64 max-abs difference <= 1e-10 on phi, p, u; fp32 max
+relative difference (of field scale, reading G20) <= 1e-4 on phi and <= 1e-3 on u.
+"""
+import numpy as np
+import pytest
+
+from paper_2505_12205_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FP64_ABS = 1e-10
+FP32_PHI, FP32_U = 1e-4, 1e-3
+
+
+def _oracle(case, steps):
+    from oracle.clip_oracle import Oracle
+    o = Oracle.from_case(case)
+    o.step(steps)
+    return o.get()
+
+
+def _gpu(case, steps, precision, chunks=(None,)):
+    import torch
+    from paper_2505_12205_b200 import clip
+    sim = clip.Clip.from_case(case, precision=precision)
+    if chunks == (None,):
+        sim.step(steps)
+    else:
+        done = 0
+        for c in chunks:
+            sim.step(c); done += c
+        assert done == steps
+    phi, p, u = sim.get()
+    torch.cuda.synchronize()
+    out = tuple(t.double().cpu().numpy() for t in (phi, p, u))
+    sim.close()
+    return out
+
+
+def _compare(case, steps, precision, ref=None):
+    rphi, rp, ru = ref if ref is not None else _oracle(case, steps)
+    phi, p, u = _gpu(case, steps, precision)
+    assert np.isfinite(phi).all() and np.isfinite(p).all() and np.isfinite(u).all()
+    if precision == 64:
+        ephi, ep, eu = np.abs(phi - rphi).max(), np.abs(p - rp).max(), np.abs(u - ru).max()
+        print(f"{case['name']} fp64 {steps} steps: max-abs phi {ephi:.2e} p {ep:.2e} u {eu:.2e}")
+        assert ephi <= FP64_ABS and ep <= FP64_ABS and eu <= FP64_ABS
+    else:
+        ephi = np.abs(phi - rphi).max() / np.abs(rphi).max()
+        eu = np.abs(u - ru).max() / max(np.abs(ru).max(), 1e-30)
+        ep = np.abs(p - rp).max() / max(np.abs(rp).max(), 1e-30)
+        print(f"{case['name']} fp32 {steps} steps: field-rel phi {ephi:.2e} u {eu:.2e} p {ep:.2e} (p not gated)")
+        assert ephi <= FP32_PHI and eu <= FP32_U
+
+
+CASES = {
+    "drop32": (lambda: inputs.drop(), 100),                                              # BASELINE configs[0]
+    "sweep64": (lambda: inputs.sweep_drops(n=64), 100),                                 # configs[4] at 64^3
+    "poiseuille_replica": (lambda: inputs.poiseuille(nx=4, ny=32, nz=4), 1000),         # configs[1] replica
+    "rt_replica": (lambda: inputs.rayleigh_taylor(L=16, W=3.0), 100),                   # configs[2] replica
+    "jet_replica": (lambda: inputs.jet(nxy=24, nz=96, r_nozzle=4.0), 200),              # configs[3] replica
+    "odd_box": (lambda: inputs.sweep_drops(shape=(20, 12, 36), ndrops=4, rmin=3, rmax=5), 100),
+    "walled_box": (lambda: inputs.walled_box(), 100),
+}
+
+_ref_cache = {}
+
+
+def _ref(name):
+    if name not in _ref_cache:
+        mk, steps = CASES[name]
+        case = mk()
+        _ref_cache[name] = (case, steps, _oracle(case, steps))
+    return _ref_cache[name]
+
+
+@pytest.mark.parametrize("name", list(CASES))
+@pytest.mark.parametrize("precision", [64, 32])
+def test_parity(name, precision):
+    case, steps, ref = _ref(name)
+    _compare(case, steps, precision, ref)
+
+
+def test_time_zero_roundtrip():
+    """After clip_init, clip_get returns (phi0, p = 0, u0) as the oracle defines them."""
+    case = inputs.sweep_drops(n=16, ndrops=3, rmin=3.0, rmax=5.0, W=3.0)
+    rphi, rp, ru = _oracle(case, 0)
+    phi, p, u = _gpu(case, 0, 64)
+    assert np.abs(phi - rphi).max() == 0.0 and np.abs(u - ru).max() == 0.0
+    assert np.abs(p - rp).max() < 1e-16
+
+
+def test_step_chunking_is_exact():
+    """clip_step(100) == clip_step(30); clip_step(70) bit for bit (time semantics of the C ABI)."""
+    case = inputs.sweep_drops(n=16, ndrops=3, rmin=3.0, rmax=5.0, W=3.0)
+    a = _gpu(case, 100, 64)
+    b = _gpu(case, 100, 64, chunks=(30, 70))
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+
+
+def test_uniform_rest_gpu():
+    """P1 on the GPU: phi == 1 (and 0), u = 0: f stays 0 bitwise -> p = 0, u = 0 exactly."""
+    for val in (1.0, 0.0):
+        case = inputs.drop(n=16)
+        case["phi0"][...] = val
+        phi, p, u = _gpu(case, 200, 64)
+        assert np.abs(u).max() == 0.0 and np.abs(p).max() == 0.0
+        assert np.abs(phi - val).max() <= 1e-13
+
+
+def test_phi_conservation_gpu():
+    """P2 on the GPU (fp64): relative drift of sum(phi) < 1e-12 over 1000 steps."""
+    case = inputs.drop(n=32)
+    phi, p, u = _gpu(case, 1000, 64)
+    s0 = case["phi0"].sum()
+    assert abs(phi.sum() - s0) / s0 < 1e-12
+
+
+def test_error_paths():
+    import torch
+    from paper_2505_12205_b200 import clip
+    p = inputs.default_params()
+    bad = dict(p); bad["precision"] = 16
+    assert clip.clip_workspace_bytes(8, 8, 8, clip.make_params(bad)) == 0
+    bad = dict(p); bad["bc"] = (0, 1, 0, 0, 0, 0)
+    assert clip.clip_workspace_bytes(8, 8, 8, clip.make_params(bad)) == 0
+    assert "PERIODIC" in clip.clip_last_error(None)
+    cp = clip.make_params(p)
+    n = clip.clip_workspace_bytes(8, 8, 8, cp)
+    ws = torch.empty(n + 256, dtype=torch.uint8, device="cuda")
+    ptr = (ws.data_ptr() + 255) // 256 * 256
+    rc, h = clip.clip_create(8, 8, 8, cp, ptr, n - 1, 0)
+    assert rc == clip.CLIP_ENOMEM
+    rc, h = clip.clip_create(8, 8, 8, cp, ptr, n, 0)
+    assert rc == clip.CLIP_OK
+    assert clip.clip_step(h, 1) == clip.CLIP_ESTATE
+    assert clip.clip_get(h, 0, 0, 0) == clip.CLIP_ESTATE
+    assert clip.clip_destroy(h) == clip.CLIP_OK
