@@ -1,0 +1,258 @@
+#!/usr/bin/env python
+"""bench.py -- MLUPS / HBM roofline of the fused CLIP step on B200 (contract: see DESIGN.md "Measurement").
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n 256] [--precision 32|64]
+
+One "step" = one pass of the whole hot path (rows a1-a10 of SURVEY.md 8(a)) over the lattice = one LBM time step.
+Workload at N=1: BASELINE.json configs[4] (throughput sweep) at 256^3, fp32, periodic, 20 seeded drops, density
+ratio 1000 -- the lattice BASELINE.json's `north_star` quotes its target on.  State is 2.7 GB (>> 126 MB L2), so
+no L2 flush is needed between timed steps.  Prints ONE JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+B_MIN_WORDS = 84  # f 19R+19W, g 19R+19W, phi 1R+1W, u 3R+3W
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index = index
+        self.samples = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            parts = [x.strip() for x in s.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_baseline(n_sample, steps, warmup, seed=2505):
+    """Time the oracle as it stands on the host (single thread) on a bounded sample of the same workload."""
+    from oracle.clip_oracle import Oracle
+    from paper_2505_12205_b200 import inputs
+    case = inputs.sweep_drops(n=n_sample, seed=seed, precision=64)
+    o = Oracle.from_case(case)
+    o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    mlups = n_sample ** 3 * steps / dt / 1e6
+    return mlups, dt / steps * 1e3, f"configs[4] at {n_sample}^3 (same recipe, seed {seed}), fp64, {warmup} warm-up + {steps} timed steps"
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import __graft_entry__ as g
+    from oracle import clip_oracle
+    clip_oracle.build()
+    n_sample = 64 if (args.steps + args.warmup) <= 40 else (48 if (args.steps + args.warmup) <= 120 else 32)
+    mlups, ms, sample = oracle_baseline(n_sample, args.steps, args.warmup)
+    line = {
+        "impl": "reference", "metric": "MLUPS", "value": mlups, "unit": "MLUPS", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"BASELINE configs[4] sweep, periodic two-phase, bounded sample {n_sample}^3 of the 256^3 lattice",
+                   "l2": "n/a (CPU)"},
+        "cpu_baseline": {"value": mlups, "unit": "MLUPS", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": mlups, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as g
+    g.build()
+    from paper_2505_12205_b200 import clip, inputs
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    n = args.n
+    prec = args.precision
+    dtype = torch.float32 if prec == 32 else torch.float64
+    word = 4 if prec == 32 else 8
+    # one independent lattice per rank (replicas): seed differs per rank
+    case = inputs.sweep_drops(n=n, seed=2505 + rank, precision=prec)
+    nodes = n ** 3
+    sim = clip.Clip(n, n, n, case["params"], device=dev)
+    phi0_h = torch.as_tensor(case["phi0"]).to(dtype).pin_memory()
+    u0_h = torch.as_tensor(case["u0"]).to(dtype).pin_memory()
+    sim.init(phi0_h, u0_h)
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps
+    sim.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = sim.launches
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(sim.stream)
+    sim.step(args.steps)
+    e1.record(sim.stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = sim.launches - l0
+    clocks = sampler.stop() if rank == 0 else None
+    phi, p, u = sim.get()
+    finite = bool(torch.isfinite(phi).all() and torch.isfinite(u).all() and torch.isfinite(p).all())
+
+    # ---- per-kernel durations (CUDA events on the launch stream around every launch)
+    prof = sim.step_profiled(args.steps)
+    step_ms_prof = sum(v[0] for v in prof.values()) / args.steps
+    dom = max(prof, key=lambda k: prof[k][0])
+
+    # ---- end to end through the host-buffer call: H2D(phi0,u0) -> init -> K steps -> get -> D2H(phi,p,u)
+    out_phi = torch.empty((n, n, n), dtype=dtype).pin_memory()
+    out_p = torch.empty((n, n, n), dtype=dtype).pin_memory()
+    out_u = torch.empty((3, n, n, n), dtype=dtype).pin_memory()
+    bufs = (torch.empty_like(phi0_h, device=dev), torch.empty_like(u0_h, device=dev), torch.empty_like(out_phi, device=dev),
+            torch.empty_like(out_p, device=dev), torch.empty_like(out_u, device=dev))
+    clip.run_host(sim, phi0_h, u0_h, 2, out_phi, out_p, out_u, bufs)  # warm-up job
+    barrier()
+    t0 = time.perf_counter()
+    h2d, d2h = clip.run_host(sim, phi0_h, u0_h, args.steps, out_phi, out_p, out_u, bufs)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+
+    if world > 1:
+        t = torch.tensor([ms, e2e_s], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_s = float(t[0]), float(t[1])
+        fl = torch.tensor([1.0 if finite else 0.0], device=dev)
+        dist.all_reduce(fl, op=dist.ReduceOp.MIN)
+        finite = bool(fl.item() > 0.5)
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        mlups = world * nodes * args.steps / (ms * 1e-3) / 1e6
+        e2e_mlups = world * nodes * args.steps / e2e_s / 1e6
+        step_bytes = B_MIN_WORDS * word * nodes
+        achieved = step_bytes / (step_ms_prof * 1e-3) / 1e9
+        line = {
+            "metric": "MLUPS", "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE configs[4] throughput sweep at {n}^3: periodic two-phase box, 20 seeded drops, "
+                                   f"rho ratio 1000, fp{prec} (north_star target lattice)",
+                       "lattice": [n, n, n], "l2": f"state {sim.workspace_bytes / 1e9:.2f} GB >> 126 MB L2, no flush needed",
+                       "parallelism": "independent replica per GPU" if world > 1 else "single GPU",
+                       "finite_after_run": finite},
+            "gpu_launches": int(launches),
+            "effective_gbs": mlups * 1e6 * B_MIN_WORDS * word / 1e9 / world,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": peak_src,
+                         "kernel": dom, "algorithmic_bytes_per_step": step_bytes,
+                         "note": "achieved = 84 words/LU x nodes / (sum of the step's kernel durations, CUDA events per launch)",
+                         "kernels_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
+                         "frac_of_nominal_8TBs": achieved / 8000.0},
+            "e2e": {"value": e2e_mlups, "unit": "MLUPS", "h2d_bytes_per_step": h2d / args.steps,
+                    "d2h_bytes_per_step": d2h / args.steps,
+                    "job": f"pinned host phi0,u0 -> H2D -> clip_init -> clip_step({args.steps}) -> clip_get -> D2H, wall clock"},
+            "clocks": clocks,
+        }
+        if world == 1 and not args.no_cpu:
+            cm, cms, sample = oracle_baseline(64, 20, 2)
+            line["cpu_baseline"] = {"value": cm, "unit": "MLUPS", "cores": 1, "kind": "oracle", "sample": sample}
+        print(json.dumps(line))
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=256)
+    ap.add_argument("--precision", type=int, default=32, choices=[32, 64])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

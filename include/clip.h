@@ -84,6 +84,14 @@ const char* clip_last_error(const clip_t* h);
 /* Number of kernel launches the handle has enqueued so far (instrumentation for bench.py's gpu_launches). */
 long long clip_launch_count(const clip_t* h);
 
+/* Instrumentation for bench.py's roofline: like clip_step(h, n), but every kernel launch is bracketed by CUDA
+ * events on the handle's stream; after synchronising the stream (this call is host-synchronous) the elapsed
+ * milliseconds and launch counts are ADDED per kernel kind into ms[kind] / count[kind], kind < clip_kernel_kinds().
+ * clip_kernel_name(kind) is the kernel's name (library-owned string), NULL if kind is out of range. */
+int clip_step_profiled(clip_t* h, int n, double* ms, long long* count);
+int clip_kernel_kinds(void);
+const char* clip_kernel_name(int kind);
+
 #ifdef __cplusplus
 }
 #endif

@@ -73,6 +73,11 @@ def lib():
         L.clip_last_error.argtypes = [C.c_void_p]
         L.clip_launch_count.restype = C.c_longlong
         L.clip_launch_count.argtypes = [C.c_void_p]
+        L.clip_step_profiled.restype = C.c_int
+        L.clip_step_profiled.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+        L.clip_kernel_kinds.restype = C.c_int
+        L.clip_kernel_name.restype = C.c_char_p
+        L.clip_kernel_name.argtypes = [C.c_int]
         _lib = L
     return _lib
 
@@ -112,6 +117,15 @@ def clip_last_error(h=None) -> str:
 
 def clip_launch_count(h) -> int:
     return int(lib().clip_launch_count(h))
+
+
+def clip_step_profiled(h, n: int):
+    """Returns {kernel name: (total ms, launches)} for n steps (host-synchronous instrumentation)."""
+    k = lib().clip_kernel_kinds()
+    ms = (C.c_double * k)()
+    cnt = (C.c_longlong * k)()
+    rc = lib().clip_step_profiled(h, int(n), ms, cnt)
+    return rc, {lib().clip_kernel_name(i).decode(): (ms[i], cnt[i]) for i in range(k)}
 
 
 class ClipError(RuntimeError):
@@ -184,6 +198,12 @@ class Clip:
         with self.torch.cuda.device(self.device):
             self._check(clip_get(self._h, phi.data_ptr() if phi is not None else 0,
                                  p.data_ptr() if p is not None else 0, u.data_ptr() if u is not None else 0))
+
+    def step_profiled(self, n=1):
+        with self.torch.cuda.device(self.device):
+            rc, d = clip_step_profiled(self._h, n)
+        self._check(rc)
+        return d
 
     @property
     def launches(self) -> int:

@@ -143,11 +143,25 @@ template <typename T> int do_init(clip_handle* h, const void* phi0, const void* 
   return check_cuda(h, "k_init");
 }
 
-template <typename T> int do_step(clip_handle* h, int nsteps) {
+enum { KIND_PHI = 0, KIND_STEP = 1, KIND_COUNT = 2 };
+const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step"};
+
+struct Prof {  // optional per-launch event timing (clip_step_profiled)
+  std::vector<cudaEvent_t> ev;
+  std::vector<int> kind;
+  cudaStream_t stream;
+  void begin() { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, stream); ev.push_back(e); }
+  void end(int k) { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, stream); ev.push_back(e); kind.push_back(k); }
+};
+
+template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullptr) {
   for (int s = 0; s < nsteps; ++s) {
     clip::KP<T> P = make_kp<T>(h);
+    if (prof) prof->begin();
     clip::k_phi<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
+    if (prof) { prof->end(KIND_PHI); prof->begin(); }
     clip::k_step<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
+    if (prof) prof->end(KIND_STEP);
     h->launches += 2;
     h->cur ^= 1;
     h->t += 1;
@@ -222,6 +236,29 @@ int clip_step(clip_t* h, int n) {
   if (n < 0) { set_err(h->err, "clip_step: n must be >= 0"); return CLIP_EINVAL; }
   return h->p.precision == 32 ? do_step<float>(h, n) : do_step<double>(h, n);
 }
+
+int clip_step_profiled(clip_t* h, int n, double* ms, long long* count) {
+  if (!h) return CLIP_EINVAL;
+  if (!h->inited) { set_err(h->err, "clip_step_profiled: clip_init has not been called"); return CLIP_ESTATE; }
+  if (n < 0 || !ms || !count) { set_err(h->err, "clip_step_profiled: bad arguments"); return CLIP_EINVAL; }
+  Prof prof;
+  prof.stream = h->stream;
+  int rc = h->p.precision == 32 ? do_step<float>(h, n, &prof) : do_step<double>(h, n, &prof);
+  cudaError_t e = cudaStreamSynchronize(h->stream);
+  if (rc == CLIP_OK && e != cudaSuccess) { set_err(h->err, "clip_step_profiled: %s", cudaGetErrorString(e)); rc = CLIP_ECUDA; }
+  for (size_t k = 0; k < prof.kind.size(); ++k) {
+    float t = 0.f;
+    if (rc == CLIP_OK && cudaEventElapsedTime(&t, prof.ev[2 * k], prof.ev[2 * k + 1]) == cudaSuccess) {
+      ms[prof.kind[k]] += t;
+      count[prof.kind[k]] += 1;
+    }
+  }
+  for (cudaEvent_t ev : prof.ev) cudaEventDestroy(ev);
+  return rc;
+}
+
+int clip_kernel_kinds(void) { return KIND_COUNT; }
+const char* clip_kernel_name(int kind) { return (kind >= 0 && kind < KIND_COUNT) ? KIND_NAMES[kind] : nullptr; }
 
 int clip_get(clip_t* h, void* d_phi, void* d_p, void* d_u) {
   if (!h) return CLIP_EINVAL;
