@@ -35,6 +35,29 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+def rank_seed(rank, base=2505):
+    """Every rank runs its own seeded replica of the workload (weak scaling)."""
+    return base + int(rank)
+
+
+def whole_job_mlups(nodes_per_rank, steps, ms, world):
+    """Whole-job throughput: lattice updates of ALL ranks / max-over-ranks time."""
+    return world * nodes_per_rank * steps / (ms * 1e-3) / 1e6
+
+
+def reduce_over_ranks(ms, e2e_s, finite, world, device):
+    """MAX over ranks of the two timings, AND over ranks of the finite flag (nccl on GPU, gloo in the CPU test)."""
+    if world <= 1:
+        return float(ms), float(e2e_s), bool(finite)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms, e2e_s], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    fl = torch.tensor([1.0 if finite else 0.0], device=device)
+    dist.all_reduce(fl, op=dist.ReduceOp.MIN)
+    return float(t[0]), float(t[1]), bool(fl.item() > 0.5)
+
+
 class ClockSampler:
     """Samples nvidia-smi clocks / throttle reasons during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -144,7 +167,7 @@ def run_ours(args):
     dtype = torch.float32 if prec == 32 else torch.float64
     word = 4 if prec == 32 else 8
     # one independent lattice per rank (replicas): seed differs per rank
-    case = inputs.sweep_drops(n=n, seed=2505 + rank, precision=prec)
+    case = inputs.sweep_drops(n=n, seed=rank_seed(rank), precision=prec)
     nodes = n ** 3
     sim = clip.Clip(n, n, n, case["params"], device=dev)
     phi0_h = torch.as_tensor(case["phi0"]).to(dtype).pin_memory()
@@ -193,17 +216,11 @@ def run_ours(args):
     barrier()
     e2e_s = time.perf_counter() - t0
 
-    if world > 1:
-        t = torch.tensor([ms, e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_s = float(t[0]), float(t[1])
-        fl = torch.tensor([1.0 if finite else 0.0], device=dev)
-        dist.all_reduce(fl, op=dist.ReduceOp.MIN)
-        finite = bool(fl.item() > 0.5)
+    ms, e2e_s, finite = reduce_over_ranks(ms, e2e_s, finite, world, dev)
 
     if rank == 0:
         peak, peak_src = measured_peak()
-        mlups = world * nodes * args.steps / (ms * 1e-3) / 1e6
+        mlups = whole_job_mlups(nodes, args.steps, ms, world)
         e2e_mlups = world * nodes * args.steps / e2e_s / 1e6
         step_bytes = B_MIN_WORDS * word * nodes
         achieved = step_bytes / (step_ms_prof * 1e-3) / 1e9
