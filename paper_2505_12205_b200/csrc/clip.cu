@@ -2,10 +2,12 @@
 // workspace is carved into the arrays listed at the top of clip_kernels.cuh.
 #include "../../include/clip.h"
 #include "clip_kernels.cuh"
+#include "clip_fast.cuh"
 
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -85,6 +87,7 @@ struct clip_handle {
   cudaStream_t stream;
   int cur;      // which of the A/B population buffers holds the current post-collision state
   bool inited;
+  bool force_generic;  // CLIP_FORCE_GENERIC=1 in the environment at clip_create: generic kernels only (tests)
   long long launches;
   long long t;
   std::vector<uint8_t> mask_host;
@@ -143,8 +146,34 @@ template <typename T> int do_init(clip_handle* h, const void* phi0, const void* 
   return check_cuda(h, "k_init");
 }
 
-enum { KIND_PHI = 0, KIND_STEP = 1, KIND_COUNT = 2 };
-const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step"};
+enum { KIND_PHI = 0, KIND_STEP = 1, KIND_PHI2 = 2, KIND_STEP2 = 3, KIND_COUNT = 4 };
+const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step2"};
+
+// The pair-per-thread fast kernels (clip_fast.cuh) cover fully periodic lattices with even nx.
+bool fast_ok(const clip_handle* h) {
+  if (h->force_generic) return false;
+  for (int k = 0; k < 6; ++k) if (h->p.bc[k] != CLIP_BC_PERIODIC) return false;
+  return h->nx % 2 == 0;
+}
+void fast_shape(const clip_handle* h, dim3& grid, dim3& block) {
+  const int pairs = h->nx / 2;
+  int bx = 1;
+  while (bx < pairs && bx < 128) bx *= 2;
+  const int by = 256 / bx;
+  block = dim3(bx, by, 1);
+  grid = dim3((pairs + bx - 1) / bx, (h->ny + by - 1) / by, h->nz);
+}
+template <typename T> clip::FP<T> make_fp(const clip::KP<T>& P) {
+  clip::FP<T> F;
+  F.k = P;
+  for (int a = 0; a < clip::Q; ++a) {
+    F.fs[a] = P.f_src + (long long)a * P.n; F.gs[a] = P.g_src + (long long)a * P.n;
+    F.fd[a] = P.f_dst + (long long)a * P.n; F.gd[a] = P.g_dst + (long long)a * P.n;
+  }
+  return F;
+}
+template <typename T> struct StepMinBlocks { static constexpr int value = 2; };
+template <> struct StepMinBlocks<double> { static constexpr int value = 1; };
 
 struct Prof {  // optional per-launch event timing (clip_step_profiled)
   std::vector<cudaEvent_t> ev;
@@ -155,13 +184,20 @@ struct Prof {  // optional per-launch event timing (clip_step_profiled)
 };
 
 template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullptr) {
+  const bool fast = fast_ok(h);
+  dim3 fg, fb;
+  if (fast) fast_shape(h, fg, fb);
   for (int s = 0; s < nsteps; ++s) {
     clip::KP<T> P = make_kp<T>(h);
     if (prof) prof->begin();
-    clip::k_phi<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
-    if (prof) { prof->end(KIND_PHI); prof->begin(); }
-    clip::k_step<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
-    if (prof) prof->end(KIND_STEP);
+    clip::FP<T> F;
+    if (fast) F = make_fp<T>(P);
+    if (fast) clip::k_phi2<T><<<fg, fb, 0, h->stream>>>(F);
+    else clip::k_phi<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
+    if (prof) { prof->end(fast ? KIND_PHI2 : KIND_PHI); prof->begin(); }
+    if (fast) clip::k_step2<T, StepMinBlocks<T>::value><<<fg, fb, 0, h->stream>>>(F);
+    else clip::k_step<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
+    if (prof) prof->end(fast ? KIND_STEP2 : KIND_STEP);
     h->launches += 2;
     h->cur ^= 1;
     h->t += 1;
@@ -202,7 +238,9 @@ int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params,
   clip_handle* h = new (std::nothrow) clip_handle();
   if (!h) { set_err(g_create_error, "clip_create: out of host memory"); return CLIP_ENOMEM; }
   h->nx = nx; h->ny = ny; h->nz = nz; h->p = *params; h->L = L; h->ws = (char*)d_workspace;
-  h->stream = (cudaStream_t)cuda_stream; h->cur = 0; h->inited = false; h->launches = 0; h->t = 0; h->err[0] = 0;
+  h->stream = (cudaStream_t)cuda_stream; h->cur = 0; h->inited = false;
+  { const char* e = getenv("CLIP_FORCE_GENERIC"); h->force_generic = e && e[0] == '1'; }
+  h->launches = 0; h->t = 0; h->err[0] = 0;
   if (params->bc[4] == CLIP_BC_INLET) {  // disc mask, decided in double on the host
     h->mask_host.resize((size_t)nx * ny);
     for (int y = 0; y < ny; ++y)

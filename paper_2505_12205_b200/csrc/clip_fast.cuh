@@ -1,0 +1,274 @@
+// clip_fast.cuh -- fast kernels for fully periodic lattices with even nx: one thread owns the node pair
+// (x0, x0+1), all arithmetic two-lane packed (clip_pack.cuh).  Same equations and the same "lean" formulation as
+// clip_kernels.cuh (header comment there), reorganised by opposite-direction pairs (a, a+1):
+//   f+_a , f+_abar = w_a (A_a +- B_a),  A_a = p* - 1.5 u.u + 4.5 (e_a.u)^2 + k e_a^T D e_a,  B_a = e_a.(3u + 1.5 F/rho)
+//   g+_a , g+_abar = (1-w_phi) g + w_a (C_a +- E_a),  C_a = w_phi phi (1 - 1.5 u.u + 4.5 (e_a.u)^2),
+//                                                     E_a = e_a.(3 w_phi phi u + (1 - w_phi/2) [1-4(phi-1/2)^2]/W n)
+// (Eq. 13, 16-19, 27-28 as read in G2, 33-36).
+#pragma once
+#include "clip_kernels.cuh"
+#include "clip_pack.cuh"
+
+namespace clip {
+
+// Kernel parameters of the fast kernels: KP plus one base pointer per direction and array, so that every load / store
+// address is a single IMAD.WIDE (32-bit element index x word size + 64-bit base taken from the constant bank).
+template <typename T> struct FP {
+  KP<T> k;
+  const T* fs[Q]; const T* gs[Q];  // post-collision populations at t,   [nz][ny][nx] each
+  T* fd[Q]; T* gd[Q];              // post-collision populations at t+1
+};
+
+// Per-thread geometry of a node pair on a periodic lattice: element indices are 32-bit (n < 2^31, checked on the host).
+struct Geo {
+  int rc;                  // index of node x0 in its own row
+  int dym, dyp, dzm, dzp;  // offsets to the rows y-1, y+1, z-1, z+1 (periodic wrap, B.5-B.7)
+  int xm, xp;              // offsets from x0 to x0-1 and to x0+2 (periodic wrap)
+};
+
+template <typename T> __device__ __forceinline__ Geo make_geo(const KP<T>& P, int x0, int y, int z) {
+  Geo g;
+  const int nxy = P.nx * P.ny;
+  g.rc = (z * P.ny + y) * P.nx + x0;
+  g.dym = (y == 0) ? (P.ny - 1) * P.nx : -P.nx;
+  g.dyp = (y == P.ny - 1) ? -(P.ny - 1) * P.nx : P.nx;
+  g.dzm = (z == 0) ? (P.nz - 1) * nxy : -nxy;
+  g.dzp = (z == P.nz - 1) ? -(P.nz - 1) * nxy : nxy;
+  g.xm = (x0 == 0) ? P.nx - 1 : -1;
+  g.xp = (x0 + 2 == P.nx) ? 2 - P.nx : 2;
+  return g;
+}
+
+// row index of (y + sy, z + sz)
+template <int sy, int sz> __device__ __forceinline__ int row_of(const Geo& g) {
+  return g.rc + (sy > 0 ? g.dyp : (sy < 0 ? g.dym : 0)) + (sz > 0 ? g.dzp : (sz < 0 ? g.dzm : 0));
+}
+
+// Streaming (pull, Alg. 2 / B.3-B.6) of direction a for the node pair: value at x - e_a.
+template <typename T, int a> __device__ __forceinline__ P2<T> pull2(const T* const (&src)[Q], const Geo& g) {
+  const T* __restrict__ b = src[a];
+  const int row = row_of<-cy(a), -cz(a)>(g);
+  if (cx(a) == 0) return ld_pair<T>(b + row);
+  if (cx(a) == 1) return P2<T>(__ldg(b + (row + g.xm)), __ldg(b + row));
+  return P2<T>(__ldg(b + (row + 1)), __ldg(b + (row + g.xp)));
+}
+template <typename T, int a = 0> struct Pull2All {
+  static __device__ __forceinline__ void run(const T* const (&src)[Q], const Geo& g, P2<T> (&v)[Q]) {
+    v[a] = pull2<T, a>(src, g);
+    Pull2All<T, a + 1>::run(src, g, v);
+  }
+};
+template <typename T> struct Pull2All<T, Q> {
+  static __device__ __forceinline__ void run(const T* const (&)[Q], const Geo&, P2<T> (&)[Q]) {}
+};
+template <typename T, int a = 0> struct Store2All {
+  static __device__ __forceinline__ void run(T* const (&dst)[Q], int rc, const P2<T> (&v)[Q]) {
+    st_pair<T>(dst[a] + rc, v[a]);
+    Store2All<T, a + 1>::run(dst, rc, v);
+  }
+};
+template <typename T> struct Store2All<T, Q> {
+  static __device__ __forceinline__ void run(T* const (&)[Q], int, const P2<T> (&)[Q]) {}
+};
+
+template <typename T> __device__ __forceinline__ P2<T> sum19(const P2<T> (&g)[Q]) {
+  return ((g[0] + (g[1] + g[2])) + ((g[3] + g[4]) + (g[5] + g[6]))) +
+         (((g[7] + g[8]) + (g[9] + g[10])) + ((g[11] + g[12]) + (g[13] + g[14])) + ((g[15] + g[16]) + (g[17] + g[18])));
+}
+
+// phi at x-1, x, x+1 of one row, for both nodes of the pair
+template <typename T> struct Row3 { P2<T> L, C, R; };
+template <typename T> __device__ __forceinline__ Row3<T> ld_row3(const T* __restrict__ phi, int row, const Geo& g) {
+  Row3<T> r;
+  r.C = ld_pair<T>(phi + row);
+  const T m = __ldg(phi + (row + g.xm)), p = __ldg(phi + (row + g.xp));
+  r.L = P2<T>(m, r.C.lo());
+  r.R = P2<T>(r.C.hi(), p);
+  return r;
+}
+
+// Eq. 40a/b on differences d = phi(x+e) - phi(x) (exact zero on a uniform field).
+template <typename T>
+__device__ __forceinline__ void stencil2(const T* __restrict__ phi, const Geo& g, P2<T>& pc, P2<T> (&G)[3], P2<T>& L) {
+  typedef P2<T> V;
+  const Row3<T> c = ld_row3<T>(phi, row_of<0, 0>(g), g);
+  const Row3<T> yp = ld_row3<T>(phi, row_of<1, 0>(g), g), ym = ld_row3<T>(phi, row_of<-1, 0>(g), g);
+  const Row3<T> zp = ld_row3<T>(phi, row_of<0, 1>(g), g), zm = ld_row3<T>(phi, row_of<0, -1>(g), g);
+  const V ypzp = ld_pair<T>(phi + row_of<1, 1>(g)), ymzm = ld_pair<T>(phi + row_of<-1, -1>(g));
+  const V ypzm = ld_pair<T>(phi + row_of<1, -1>(g)), ymzp = ld_pair<T>(phi + row_of<-1, 1>(g));
+  pc = c.C;
+  const V d1 = c.R - pc, d2 = c.L - pc, d3 = yp.C - pc, d4 = ym.C - pc, d5 = zp.C - pc, d6 = zm.C - pc;
+  const V d7 = yp.R - pc, d8 = ym.L - pc, d9 = ym.R - pc, d10 = yp.L - pc;
+  const V d11 = zp.R - pc, d12 = zm.L - pc, d13 = zm.R - pc, d14 = zp.L - pc;
+  const V d15 = ypzp - pc, d16 = ymzm - pc, d17 = ypzm - pc, d18 = ymzp - pc;
+  const V s1 = ((d1 + d2) + (d3 + d4)) + (d5 + d6);
+  const V s2 = (((d7 + d8) + (d9 + d10)) + ((d11 + d12) + (d13 + d14))) + ((d15 + d16) + (d17 + d18));
+  L = fma2(V(T(1.0 / 3.0)), s1, V(T(1.0 / 6.0)) * s2);
+  const V e78 = d7 - d8, e910 = d9 - d10, e1112 = d11 - d12, e1314 = d13 - d14, e1516 = d15 - d16, e1718 = d17 - d18;
+  G[0] = fma2(V(T(1.0 / 6.0)), d1 - d2, V(T(1.0 / 12.0)) * ((e78 + e910) + (e1112 + e1314)));
+  G[1] = fma2(V(T(1.0 / 6.0)), d3 - d4, V(T(1.0 / 12.0)) * ((e78 - e910) + (e1516 + e1718)));
+  G[2] = fma2(V(T(1.0 / 6.0)), d5 - d6, V(T(1.0 / 12.0)) * ((e1112 - e1314) + (e1516 - e1718)));
+}
+
+template <typename T> struct Mat2 { P2<T> rho, inv_rho, tau, s_nu, mu; };
+template <typename T> __device__ __forceinline__ Mat2<T> materials2(const KP<T>& P, P2<T> phi, P2<T> L) {
+  typedef P2<T> V;
+  Mat2<T> m;
+  m.rho = fma2(phi, V(P.drho), V(P.rho_l));                                    // Eq. 39
+  m.inv_rho = rcp2(m.rho);
+  if (P.visc_interp == 1) m.tau = rcp2(fma2(phi, V(P.itau_h - P.itau_l), V(P.itau_l)));
+  else m.tau = fma2(phi, V(P.tau_h - P.tau_l), V(P.tau_l));                    // Eq. 24
+  m.s_nu = rcp2(m.tau + V(T(0.5)));                                            // G3
+  m.mu = fms2(V(P.beta4) * phi, (phi - V(T(1))) * (phi - V(T(0.5))), V(P.kappa) * L);  // Eq. 11 (G4)
+  return m;
+}
+
+template <typename T> struct Mom2 { P2<T> p, mx, my, mz, xx, yy, zz, xy, yz, xz; };
+template <typename T> __device__ __forceinline__ Mom2<T> moments2(const P2<T> (&f)[Q]) {
+  typedef P2<T> V;
+  Mom2<T> m;
+  const V s12 = f[1] + f[2], s34 = f[3] + f[4], s56 = f[5] + f[6];
+  const V s78 = f[7] + f[8], s910 = f[9] + f[10], s1112 = f[11] + f[12], s1314 = f[13] + f[14];
+  const V s1516 = f[15] + f[16], s1718 = f[17] + f[18];
+  const V d12 = f[1] - f[2], d34 = f[3] - f[4], d56 = f[5] - f[6];
+  const V d78 = f[7] - f[8], d910 = f[9] - f[10], d1112 = f[11] - f[12], d1314 = f[13] - f[14];
+  const V d1516 = f[15] - f[16], d1718 = f[17] - f[18];
+  const V sxy = s78 + s910, sxz = s1112 + s1314, syz = s1516 + s1718;
+  m.p = (f[0] + ((s12 + s34) + s56)) + ((sxy + sxz) + syz);
+  m.mx = d12 + ((d78 + d910) + (d1112 + d1314));
+  m.my = d34 + ((d78 - d910) + (d1516 + d1718));
+  m.mz = d56 + ((d1112 - d1314) + (d1516 - d1718));
+  m.xx = s12 + (sxy + sxz);
+  m.yy = s34 + (sxy + syz);
+  m.zz = s56 + (sxz + syz);
+  m.xy = s78 - s910;
+  m.xz = s1112 - s1314;
+  m.yz = s1516 - s1718;
+  return m;
+}
+
+// Total force (Eq. 20) and D = dev(Pi^neq); same closed forms as clip::total_force.
+template <typename T>
+__device__ __forceinline__ void total_force2(const KP<T>& P, const Mom2<T>& m, const Mat2<T>& mat, P2<T> ux, P2<T> uy,
+                                             P2<T> uz, const P2<T> (&G)[3], P2<T> (&F)[3], P2<T> (&D)[6]) {
+  typedef P2<T> V;
+  const V p3 = m.p * V(T(1.0 / 3.0));
+  const V nxx = m.xx - fma2(ux, ux, p3), nyy = m.yy - fma2(uy, uy, p3), nzz = m.zz - fma2(uz, uz, p3);
+  const V nxy = m.xy - ux * uy, nyz = m.yz - uy * uz, nxz = m.xz - ux * uz;
+  const V tr3 = ((nxx + nyy) + nzz) * V(T(1.0 / 3.0));
+  D[0] = nxx - tr3; D[1] = nyy - tr3; D[2] = nzz - tr3; D[3] = nxy; D[4] = nyz; D[5] = nxz;
+  const V s = mat.s_nu;
+  const V Sxx = fma2(s, D[0], tr3), Syy = fma2(s, D[1], tr3), Szz = fma2(s, D[2], tr3);
+  const V Sxy = s * D[3], Syz = s * D[4], Sxz = s * D[5];
+  const V cmu = -(mat.tau * V(P.drho));
+  const V cs = mat.mu - p3 * V(P.drho);
+  const V rb = mat.rho - V(P.rho_ref);
+  F[0] = fma2(cs, G[0], fma2(rb, V(P.gx), cmu * fma2(Sxx, G[0], fma2(Sxy, G[1], Sxz * G[2]))));
+  F[1] = fma2(cs, G[1], fma2(rb, V(P.gy), cmu * fma2(Sxy, G[0], fma2(Syy, G[1], Syz * G[2]))));
+  F[2] = fma2(cs, G[2], fma2(rb, V(P.gz), cmu * fma2(Sxz, G[0], fma2(Syz, G[1], Szz * G[2]))));
+}
+
+// One opposite pair (a, a+1) of both collisions.  eu = e_a.u, eDe = e_a^T D e_a, ev = e_a.(3u + h), em = e_a.mvec.
+template <typename T>
+struct Coll2 {
+  typedef P2<T> V;
+  V p, c0, k, omphi, om1;  // p*, -1.5 u.u, 4.5 (1 - s_nu), w_phi phi, 1 - w_phi
+  template <int a>
+  __device__ __forceinline__ void pair(V eu, V eDe, V ev, V em, V (&f)[Q], V (&g)[Q]) const {
+    const V w(cw<T>(a));
+    const V q = fma2(eu * V(T(4.5)), eu, c0);  // Gamma_a/w_a - 1 - 3 e.u
+    const V A = fma2(k, eDe, p + q);
+    f[a] = w * (A + ev);
+    f[a + 1] = w * (A - ev);
+    const V C = fma2(omphi, q, omphi);
+    g[a] = fma2(om1, g[a], w * (C + em));
+    g[a + 1] = fma2(om1, g[a + 1], w * (C - em));
+  }
+};
+
+// Both collisions (Alg. 1) of a node pair: g in/out in place, f+ out (a function of the moments only, because the
+// 14 non-shear moments relax at rate 1, G2).
+template <typename T>
+__device__ __forceinline__ void collide2(const KP<T>& P, const Mom2<T>& m, const Mat2<T>& mat, P2<T> phi, const P2<T> (&G)[3],
+                                         P2<T> ux, P2<T> uy, P2<T> uz, P2<T> (&f)[Q], P2<T> (&g)[Q]) {
+  typedef P2<T> V;
+  V F[3], D[6];
+  total_force2(P, m, mat, ux, uy, uz, G, F, D);
+  const V usq15 = V(T(1.5)) * fma2(ux, ux, fma2(uy, uy, uz * uz));
+  const V ir15 = V(T(1.5)) * mat.inv_rho;
+  // v = 3u + 1.5 F/rho
+  const V vx = fma2(V(T(3)), ux, F[0] * ir15), vy = fma2(V(T(3)), uy, F[1] * ir15), vz = fma2(V(T(3)), uz, F[2] * ir15);
+  // interface normal (R10) and the F^phi prefactor, Eq. 34
+  const V gn = sqrt2(fma2(G[0], G[0], fma2(G[1], G[1], G[2] * G[2]))) + V(T(1e-32));
+  const V ph = phi - V(T(0.5));
+  const V pref = fma2(V(T(-4)) * ph, ph, V(T(1))) * V(P.inv_W);
+  const V cn = (V(T(1) - T(0.5) * P.om_phi) * pref) * rcp2(gn);
+  Coll2<T> c;
+  c.p = m.p; c.c0 = -usq15; c.k = V(T(4.5)) * (V(T(1)) - mat.s_nu);
+  c.omphi = V(P.om_phi) * phi; c.om1 = V(T(1) - P.om_phi);
+  const V o3 = V(T(3)) * c.omphi;
+  const V mx = fma2(o3, ux, cn * G[0]), my = fma2(o3, uy, cn * G[1]), mz = fma2(o3, uz, cn * G[2]);
+  // rest direction
+  f[0] = V(cw<T>(0)) * (m.p - usq15);
+  g[0] = fma2(c.om1, g[0], V(cw<T>(0)) * (c.omphi - c.omphi * usq15));
+  const V Dxy2 = D[3] + D[3], Dyz2 = D[4] + D[4], Dxz2 = D[5] + D[5];
+  const V sxy = D[0] + D[1], sxz = D[0] + D[2], syz = D[1] + D[2];
+  c.template pair<1>(ux, D[0], vx, mx, f, g);
+  c.template pair<3>(uy, D[1], vy, my, f, g);
+  c.template pair<5>(uz, D[2], vz, mz, f, g);
+  c.template pair<7>(ux + uy, sxy + Dxy2, vx + vy, mx + my, f, g);
+  c.template pair<9>(ux - uy, sxy - Dxy2, vx - vy, mx - my, f, g);
+  c.template pair<11>(ux + uz, sxz + Dxz2, vx + vz, mx + mz, f, g);
+  c.template pair<13>(ux - uz, sxz - Dxz2, vx - vz, mx - mz, f, g);
+  c.template pair<15>(uy + uz, syz + Dyz2, vy + vz, my + mz, f, g);
+  c.template pair<17>(uy - uz, syz - Dyz2, vy - vz, my - mz, f, g);
+}
+
+// ------------------------------------------------------------------------------------------------ kernels
+// Launch shape: blockDim = (bx, by), grid = (ceil(nx/2/bx), ceil(ny/by), nz); thread -> pair (x0, x0+1) of row (y, z).
+template <typename T> __device__ __forceinline__ bool pair_coords(const KP<T>& P, int& x0, int& y, int& z) {
+  x0 = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
+  y = blockIdx.y * blockDim.y + threadIdx.y;
+  z = blockIdx.z;
+  return x0 < P.nx && y < P.ny;
+}
+
+// k_phi2: phi(t+1) = sum_a g_a(x,t+1) (Eq. 38) by pulling the post-collision g+(t).
+template <typename T> __global__ void __launch_bounds__(256) k_phi2(const __grid_constant__ FP<T> FPp) {
+  const KP<T>& P = FPp.k;
+  int x0, y, z;
+  if (!pair_coords(P, x0, y, z)) return;
+  const Geo geo = make_geo(P, x0, y, z);
+  P2<T> g[Q];
+  Pull2All<T>::run(FPp.gs, geo, g);
+  st_pair<T>(P.phi + geo.rc, sum19(g));
+}
+
+// k_step2: pull f+, g+ -> macros (Alg. 3) -> both collisions (Alg. 1) -> store f+, g+, u.
+template <typename T, int MINB> __global__ void __launch_bounds__(256, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
+  typedef P2<T> V;
+  const KP<T>& P = FPp.k;
+  int x0, y, z;
+  if (!pair_coords(P, x0, y, z)) return;
+  const Geo geo = make_geo(P, x0, y, z);
+  V f[Q], g[Q];
+  Pull2All<T>::run(FPp.fs, geo, f);
+  Pull2All<T>::run(FPp.gs, geo, g);
+  V ux = ld_pair<T>(P.u + geo.rc), uy = ld_pair<T>(P.u + P.n + geo.rc), uz = ld_pair<T>(P.u + 2 * P.n + geo.rc);
+  V phi, G[3], L;
+  stencil2<T>(P.phi, geo, phi, G, L);
+  const Mom2<T> m = moments2<T>(f);
+  const Mat2<T> mat = materials2<T>(P, phi, L);
+  {  // macros, Alg. 3: F from (new p*, new phi, lagged u, R13), then Eq. 31b
+    V F[3], D[6];
+    total_force2(P, m, mat, ux, uy, uz, G, F, D);
+    const V h = V(T(0.5)) * mat.inv_rho;
+    ux = fma2(h, F[0], m.mx); uy = fma2(h, F[1], m.my); uz = fma2(h, F[2], m.mz);
+  }
+  st_pair<T>(P.u + geo.rc, ux); st_pair<T>(P.u + P.n + geo.rc, uy); st_pair<T>(P.u + 2 * P.n + geo.rc, uz);
+  collide2<T>(P, m, mat, phi, G, ux, uy, uz, f, g);
+  Store2All<T>::run(FPp.fd, geo.rc, f);
+  Store2All<T>::run(FPp.gd, geo.rc, g);
+}
+
+}  // namespace clip
