@@ -3,6 +3,8 @@
 #include "../../include/clip.h"
 #include "clip_kernels.cuh"
 #include "clip_fast.cuh"
+#include "clip_march.cuh"
+#include "clip_tick.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -28,7 +30,7 @@ size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
   size_t word;  // 4 or 8
-  size_t off_f[2], off_g[2], off_phi, off_u, off_obf, off_obg, off_lam, off_mask, total;
+  size_t off_f[2], off_g[2], off_phi, off_u, off_obf, off_obg, off_lam, off_mask, off_sync, total;
 };
 
 Layout make_layout(int nx, int ny, int nz, const clip_params* p) {
@@ -46,6 +48,7 @@ Layout make_layout(int nx, int ny, int nz, const clip_params* p) {
   L.off_obg = take(outlet ? 19 * nxy * L.word : 0);
   L.off_lam = take(outlet ? nxy * L.word : 0);
   L.off_mask = take(inlet ? nxy : 0);
+  L.off_sync = take(((size_t)nz + 64) * sizeof(unsigned));  // k_tick: ticket counter + per-plane counters
   L.total = o;
   return L;
 }
@@ -87,6 +90,13 @@ struct clip_handle {
   cudaStream_t stream;
   int cur;      // which of the A/B population buffers holds the current post-collision state
   bool inited;
+  bool march_attr_set;
+  int mode;            // fast-path variant (CLIP_FAST_MODE): 0 = k_tick2, 1 = k_march, 2 = k_phi2 + k_step2 (default)
+  unsigned epoch;      // steps since clip_init (k_tick counters)
+  int tick_order;      // CLIP_TICK_ORDER (default 0): 0 = item number from blockIdx, 1 = from an atomic ticket
+  int fast_threads;    // threads per block of the pair kernels (CLIP_FAST_THREADS: 128 or 256, default 256)
+  int tick_hint;       // CLIP_TICK_HINT (default 1): streaming cache hints on single-use loads and on stores
+  int march_lz;        // planes per z segment of k_march (CLIP_MARCH_LZ, default 32)
   bool force_generic;  // CLIP_FORCE_GENERIC=1 in the environment at clip_create: generic kernels only (tests)
   long long launches;
   long long t;
@@ -138,6 +148,8 @@ int check_cuda(clip_handle* h, const char* what) {
 unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / block); }
 
 template <typename T> int do_init(clip_handle* h, const void* phi0, const void* u0) {
+  cudaMemsetAsync(h->ws + h->L.off_sync, 0, ((size_t)h->nz + 64) * sizeof(unsigned), h->stream);
+  h->epoch = 0;
   h->cur = 1;  // k_init writes into "dst"; flip afterwards so that it becomes the current state
   clip::KP<T> P = make_kp<T>(h);
   clip::k_init<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P, (const T*)phi0, (const T*)u0);
@@ -146,8 +158,9 @@ template <typename T> int do_init(clip_handle* h, const void* phi0, const void* 
   return check_cuda(h, "k_init");
 }
 
-enum { KIND_PHI = 0, KIND_STEP = 1, KIND_PHI2 = 2, KIND_STEP2 = 3, KIND_COUNT = 4 };
-const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step2"};
+enum { KIND_PHI = 0, KIND_STEP = 1, KIND_PHI2 = 2, KIND_STEP2 = 3, KIND_MARCH = 4, KIND_TICK = 5, KIND_COUNT = 6 };
+const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step2", "k_march", "k_tick"};
+constexpr int MTX = 64, MTY = 8;  // in-plane tile of the marching kernel
 
 // The pair-per-thread fast kernels (clip_fast.cuh) cover fully periodic lattices with even nx.
 bool fast_ok(const clip_handle* h) {
@@ -159,7 +172,7 @@ void fast_shape(const clip_handle* h, dim3& grid, dim3& block) {
   const int pairs = h->nx / 2;
   int bx = 1;
   while (bx < pairs && bx < 128) bx *= 2;
-  const int by = 256 / bx;
+  const int by = h->fast_threads / bx > 0 ? h->fast_threads / bx : 1;
   block = dim3(bx, by, 1);
   grid = dim3((pairs + bx - 1) / bx, (h->ny + by - 1) / by, h->nz);
 }
@@ -171,6 +184,10 @@ template <typename T> clip::FP<T> make_fp(const clip::KP<T>& P) {
     F.fd[a] = P.f_dst + (long long)a * P.n; F.gd[a] = P.g_dst + (long long)a * P.n;
   }
   return F;
+}
+// The fused marching kernel additionally needs whole tiles.
+bool march_ok(const clip_handle* h) {
+  return fast_ok(h) && h->mode == 1 && h->nx % MTX == 0 && h->ny % MTY == 0;
 }
 template <typename T> struct StepMinBlocks { static constexpr int value = 2; };
 template <> struct StepMinBlocks<double> { static constexpr int value = 1; };
@@ -186,9 +203,51 @@ struct Prof {  // optional per-launch event timing (clip_step_profiled)
 template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullptr) {
   const bool fast = fast_ok(h);
   dim3 fg, fb;
+  const bool march = march_ok(h);
+  bool tick = false;
   if (fast) fast_shape(h, fg, fb);
+  if (fast && h->mode == 0 && (h->nx / 2) % fb.x == 0 && h->ny % fb.y == 0) {
+    tick = true;
+  }
+  constexpr size_t msmem = clip::march_smem_bytes<T, MTX, MTY>();
+  auto kmarch = clip::k_march<T, MTX, MTY, StepMinBlocks<T>::value>;
+  if (march && !h->march_attr_set) {
+    if (cudaFuncSetAttribute(kmarch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msmem) != cudaSuccess)
+      return check_cuda(h, "cudaFuncSetAttribute(k_march)");
+    h->march_attr_set = true;
+  }
   for (int s = 0; s < nsteps; ++s) {
     clip::KP<T> P = make_kp<T>(h);
+    if (tick) {
+      clip::FP<T> F = make_fp<T>(P);
+      h->epoch += 1;
+      unsigned* sync = (unsigned*)(h->ws + h->L.off_sync);
+      clip::TickP tk;
+      tk.ticket = sync; tk.done_a = sync + 32;
+      tk.tp = (int)(fg.x * fg.y); tk.gx = (int)fg.x;
+      const unsigned items = ((unsigned)h->nz + 3u) * (unsigned)tk.tp;
+      tk.base = 0;
+      tk.target = (unsigned)tk.tp * h->epoch;
+      if (prof) prof->begin();
+      clip::k_tick2<T, StepMinBlocks<T>::value><<<items, fb, 0, h->stream>>>(F, tk);
+      if (prof) prof->end(KIND_TICK);
+      h->launches += 1;
+      h->cur ^= 1;
+      h->t += 1;
+      continue;
+    }
+    if (march) {
+      clip::FP<T> F = make_fp<T>(P);
+      const int LZ = h->march_lz;
+      dim3 mg(h->nx / MTX, h->ny / MTY, (h->nz + LZ - 1) / LZ);
+      if (prof) prof->begin();
+      kmarch<<<mg, clip::MarchCfg<MTX, MTY>::NT, msmem, h->stream>>>(F, LZ);
+      if (prof) prof->end(KIND_MARCH);
+      h->launches += 1;
+      h->cur ^= 1;
+      h->t += 1;
+      continue;
+    }
     if (prof) prof->begin();
     clip::FP<T> F;
     if (fast) F = make_fp<T>(P);
@@ -240,6 +299,12 @@ int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params,
   h->nx = nx; h->ny = ny; h->nz = nz; h->p = *params; h->L = L; h->ws = (char*)d_workspace;
   h->stream = (cudaStream_t)cuda_stream; h->cur = 0; h->inited = false;
   { const char* e = getenv("CLIP_FORCE_GENERIC"); h->force_generic = e && e[0] == '1'; }
+  h->march_attr_set = false;
+  { const char* e = getenv("CLIP_FAST_MODE"); h->mode = e ? atoi(e) : 2; h->epoch = 0; }
+  { const char* e = getenv("CLIP_TICK_ORDER"); h->tick_order = e ? atoi(e) : 0; }
+  { const char* e = getenv("CLIP_FAST_THREADS"); h->fast_threads = (e && atoi(e) == 128) ? 128 : 256; }
+  { const char* e = getenv("CLIP_TICK_HINT"); h->tick_hint = e ? atoi(e) : 1; }
+  { const char* e = getenv("CLIP_MARCH_LZ"); h->march_lz = e ? atoi(e) : 32; if (h->march_lz < 1) h->march_lz = 32; }
   h->launches = 0; h->t = 0; h->err[0] = 0;
   if (params->bc[4] == CLIP_BC_INLET) {  // disc mask, decided in double on the host
     h->mask_host.resize((size_t)nx * ny);

@@ -45,29 +45,29 @@ template <int sy, int sz> __device__ __forceinline__ int row_of(const Geo& g) {
 }
 
 // Streaming (pull, Alg. 2 / B.3-B.6) of direction a for the node pair: value at x - e_a.
-template <typename T, int a> __device__ __forceinline__ P2<T> pull2(const T* const (&src)[Q], const Geo& g) {
+template <typename T, int a, int H> __device__ __forceinline__ P2<T> pull2(const T* const (&src)[Q], const Geo& g) {
   const T* __restrict__ b = src[a];
   const int row = row_of<-cy(a), -cz(a)>(g);
-  if (cx(a) == 0) return ld_pair<T>(b + row);
-  if (cx(a) == 1) return P2<T>(__ldg(b + (row + g.xm)), __ldg(b + row));
-  return P2<T>(__ldg(b + (row + 1)), __ldg(b + (row + g.xp)));
+  if (cx(a) == 0) return ld_pair<T, H>(b + row);
+  if (cx(a) == 1) return P2<T>(ld_one<T, H>(b + (row + g.xm)), ld_one<T, H>(b + row));
+  return P2<T>(ld_one<T, H>(b + (row + 1)), ld_one<T, H>(b + (row + g.xp)));
 }
-template <typename T, int a = 0> struct Pull2All {
+template <typename T, int H = LD_NC, int a = 0> struct Pull2All {
   static __device__ __forceinline__ void run(const T* const (&src)[Q], const Geo& g, P2<T> (&v)[Q]) {
-    v[a] = pull2<T, a>(src, g);
-    Pull2All<T, a + 1>::run(src, g, v);
+    v[a] = pull2<T, a, H>(src, g);
+    Pull2All<T, H, a + 1>::run(src, g, v);
   }
 };
-template <typename T> struct Pull2All<T, Q> {
+template <typename T, int H> struct Pull2All<T, H, Q> {
   static __device__ __forceinline__ void run(const T* const (&)[Q], const Geo&, P2<T> (&)[Q]) {}
 };
-template <typename T, int a = 0> struct Store2All {
+template <typename T, int H = ST_WB, int a = 0> struct Store2All {
   static __device__ __forceinline__ void run(T* const (&dst)[Q], int rc, const P2<T> (&v)[Q]) {
-    st_pair<T>(dst[a] + rc, v[a]);
-    Store2All<T, a + 1>::run(dst, rc, v);
+    st_pair<T, H>(dst[a] + rc, v[a]);
+    Store2All<T, H, a + 1>::run(dst, rc, v);
   }
 };
-template <typename T> struct Store2All<T, Q> {
+template <typename T, int H> struct Store2All<T, H, Q> {
   static __device__ __forceinline__ void run(T* const (&)[Q], int, const P2<T> (&)[Q]) {}
 };
 
@@ -78,24 +78,24 @@ template <typename T> __device__ __forceinline__ P2<T> sum19(const P2<T> (&g)[Q]
 
 // phi at x-1, x, x+1 of one row, for both nodes of the pair
 template <typename T> struct Row3 { P2<T> L, C, R; };
-template <typename T> __device__ __forceinline__ Row3<T> ld_row3(const T* __restrict__ phi, int row, const Geo& g) {
+template <typename T, int H> __device__ __forceinline__ Row3<T> ld_row3(const T* __restrict__ phi, int row, const Geo& g) {
   Row3<T> r;
-  r.C = ld_pair<T>(phi + row);
-  const T m = __ldg(phi + (row + g.xm)), p = __ldg(phi + (row + g.xp));
+  r.C = ld_pair<T, H>(phi + row);
+  const T m = ld_one<T, H>(phi + (row + g.xm)), p = ld_one<T, H>(phi + (row + g.xp));
   r.L = P2<T>(m, r.C.lo());
   r.R = P2<T>(r.C.hi(), p);
   return r;
 }
 
 // Eq. 40a/b on differences d = phi(x+e) - phi(x) (exact zero on a uniform field).
-template <typename T>
+template <typename T, int H = LD_NC>
 __device__ __forceinline__ void stencil2(const T* __restrict__ phi, const Geo& g, P2<T>& pc, P2<T> (&G)[3], P2<T>& L) {
   typedef P2<T> V;
-  const Row3<T> c = ld_row3<T>(phi, row_of<0, 0>(g), g);
-  const Row3<T> yp = ld_row3<T>(phi, row_of<1, 0>(g), g), ym = ld_row3<T>(phi, row_of<-1, 0>(g), g);
-  const Row3<T> zp = ld_row3<T>(phi, row_of<0, 1>(g), g), zm = ld_row3<T>(phi, row_of<0, -1>(g), g);
-  const V ypzp = ld_pair<T>(phi + row_of<1, 1>(g)), ymzm = ld_pair<T>(phi + row_of<-1, -1>(g));
-  const V ypzm = ld_pair<T>(phi + row_of<1, -1>(g)), ymzp = ld_pair<T>(phi + row_of<-1, 1>(g));
+  const Row3<T> c = ld_row3<T, H>(phi, row_of<0, 0>(g), g);
+  const Row3<T> yp = ld_row3<T, H>(phi, row_of<1, 0>(g), g), ym = ld_row3<T, H>(phi, row_of<-1, 0>(g), g);
+  const Row3<T> zp = ld_row3<T, H>(phi, row_of<0, 1>(g), g), zm = ld_row3<T, H>(phi, row_of<0, -1>(g), g);
+  const V ypzp = ld_pair<T, H>(phi + row_of<1, 1>(g)), ymzm = ld_pair<T, H>(phi + row_of<-1, -1>(g));
+  const V ypzm = ld_pair<T, H>(phi + row_of<1, -1>(g)), ymzp = ld_pair<T, H>(phi + row_of<-1, 1>(g));
   pc = c.C;
   const V d1 = c.R - pc, d2 = c.L - pc, d3 = yp.C - pc, d4 = ym.C - pc, d5 = zp.C - pc, d6 = zm.C - pc;
   const V d7 = yp.R - pc, d8 = ym.L - pc, d9 = ym.R - pc, d10 = yp.L - pc;
@@ -233,30 +233,30 @@ template <typename T> __device__ __forceinline__ bool pair_coords(const KP<T>& P
   return x0 < P.nx && y < P.ny;
 }
 
-// k_phi2: phi(t+1) = sum_a g_a(x,t+1) (Eq. 38) by pulling the post-collision g+(t).
-template <typename T> __global__ void __launch_bounds__(256) k_phi2(const __grid_constant__ FP<T> FPp) {
-  const KP<T>& P = FPp.k;
-  int x0, y, z;
-  if (!pair_coords(P, x0, y, z)) return;
-  const Geo geo = make_geo(P, x0, y, z);
+// phi(t+1) = sum_a g_a(x,t+1) (Eq. 38) of one node pair by pulling the post-collision g+(t).
+template <typename T, int HG> __device__ __forceinline__ void phi_pair(const FP<T>& FPp, int x0, int y, int z) {
+  const Geo geo = make_geo(FPp.k, x0, y, z);
   P2<T> g[Q];
-  Pull2All<T>::run(FPp.gs, geo, g);
-  st_pair<T>(P.phi + geo.rc, sum19(g));
+  Pull2All<T, HG>::run(FPp.gs, geo, g);
+  st_pair<T>(FPp.k.phi + geo.rc, sum19(g));
 }
 
-// k_step2: pull f+, g+ -> macros (Alg. 3) -> both collisions (Alg. 1) -> store f+, g+, u.
-template <typename T, int MINB> __global__ void __launch_bounds__(256, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
+// One node pair of the step: pull f+, g+ -> macros (Alg. 3) -> both collisions (Alg. 1) -> store f+, g+, u.
+// HL: hint of the population / u loads, HP: hint of the phi loads, HS: hint of the stores.  `before_phi()` runs after
+// the population loads have been issued and before phi is touched (k_tick waits there for the phi planes).
+struct NoWait { __device__ __forceinline__ void operator()() const {} };
+template <typename T, int HL, int HP, int HS, typename W>
+__device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z, W before_phi) {
   typedef P2<T> V;
   const KP<T>& P = FPp.k;
-  int x0, y, z;
-  if (!pair_coords(P, x0, y, z)) return;
   const Geo geo = make_geo(P, x0, y, z);
   V f[Q], g[Q];
-  Pull2All<T>::run(FPp.fs, geo, f);
-  Pull2All<T>::run(FPp.gs, geo, g);
-  V ux = ld_pair<T>(P.u + geo.rc), uy = ld_pair<T>(P.u + P.n + geo.rc), uz = ld_pair<T>(P.u + 2 * P.n + geo.rc);
+  Pull2All<T, HL>::run(FPp.fs, geo, f);
+  Pull2All<T, HL>::run(FPp.gs, geo, g);
+  V ux = ld_pair<T, HL>(P.u + geo.rc), uy = ld_pair<T, HL>(P.u + P.n + geo.rc), uz = ld_pair<T, HL>(P.u + 2 * P.n + geo.rc);
+  before_phi();
   V phi, G[3], L;
-  stencil2<T>(P.phi, geo, phi, G, L);
+  stencil2<T, HP>(P.phi, geo, phi, G, L);
   const Mom2<T> m = moments2<T>(f);
   const Mat2<T> mat = materials2<T>(P, phi, L);
   {  // macros, Alg. 3: F from (new p*, new phi, lagged u, R13), then Eq. 31b
@@ -265,10 +265,21 @@ template <typename T, int MINB> __global__ void __launch_bounds__(256, MINB) k_s
     const V h = V(T(0.5)) * mat.inv_rho;
     ux = fma2(h, F[0], m.mx); uy = fma2(h, F[1], m.my); uz = fma2(h, F[2], m.mz);
   }
-  st_pair<T>(P.u + geo.rc, ux); st_pair<T>(P.u + P.n + geo.rc, uy); st_pair<T>(P.u + 2 * P.n + geo.rc, uz);
+  st_pair<T, HS>(P.u + geo.rc, ux); st_pair<T, HS>(P.u + P.n + geo.rc, uy); st_pair<T, HS>(P.u + 2 * P.n + geo.rc, uz);
   collide2<T>(P, m, mat, phi, G, ux, uy, uz, f, g);
-  Store2All<T>::run(FPp.fd, geo.rc, f);
-  Store2All<T>::run(FPp.gd, geo.rc, g);
+  Store2All<T, HS>::run(FPp.fd, geo.rc, f);
+  Store2All<T, HS>::run(FPp.gd, geo.rc, g);
+}
+
+template <typename T> __global__ void __launch_bounds__(256) k_phi2(const __grid_constant__ FP<T> FPp) {
+  int x0, y, z;
+  if (!pair_coords(FPp.k, x0, y, z)) return;
+  phi_pair<T, LD_NC>(FPp, x0, y, z);
+}
+template <typename T, int MINB> __global__ void __launch_bounds__(256, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
+  int x0, y, z;
+  if (!pair_coords(FPp.k, x0, y, z)) return;
+  step_pair<T, LD_NC, LD_NC, ST_WB>(FPp, x0, y, z, NoWait());
 }
 
 }  // namespace clip

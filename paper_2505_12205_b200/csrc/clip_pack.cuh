@@ -57,20 +57,28 @@ __device__ __forceinline__ P2<double> rcp2(P2<double> a) { return P2<double>(1.0
 __device__ __forceinline__ P2<float> sqrt2(P2<float> a) { return P2<float>(sqrtf(a.v.x), sqrtf(a.v.y)); }
 __device__ __forceinline__ P2<double> sqrt2(P2<double> a) { return P2<double>(sqrt(a.v.x), sqrt(a.v.y)); }
 
-// ---- global memory: aligned pair access (8 B for float, 16 B for double) and scalar lanes
-template <typename T> __device__ __forceinline__ P2<T> ld_pair(const T* __restrict__ p);
-template <> __device__ __forceinline__ P2<float> ld_pair<float>(const float* __restrict__ p) {
-  return P2<float>(__ldg(reinterpret_cast<const float2*>(p)));
+// ---- global memory: aligned pair access (8 B for float, 16 B for double) and scalar lanes, with a cache hint H:
+//   LD_NC  read-only path (ld.global.nc), default          ST_WB  plain store
+//   LD_CS  streaming, evict-first in L1/L2 (last use)      ST_CS  streaming store
+//   LD_CA  coherent load cached in L1 (data written earlier in the same launch by other blocks)
+enum { LD_NC = 0, LD_CS = 1, LD_CA = 2 };
+enum { ST_WB = 0, ST_CS = 1 };
+template <int H, typename U> __device__ __forceinline__ U ld_hint(const U* p) {
+  if (H == LD_CS) return __ldcs(p);
+  if (H == LD_CA) return __ldca(p);
+  return __ldg(p);
 }
-template <> __device__ __forceinline__ P2<double> ld_pair<double>(const double* __restrict__ p) {
-  return P2<double>(__ldg(reinterpret_cast<const double2*>(p)));
+template <typename T> struct PairOf;
+template <> struct PairOf<float> { typedef float2 type; };
+template <> struct PairOf<double> { typedef double2 type; };
+template <typename T, int H = LD_NC> __device__ __forceinline__ P2<T> ld_pair(const T* __restrict__ p) {
+  return P2<T>(ld_hint<H>(reinterpret_cast<const typename PairOf<T>::type*>(p)));
 }
-template <typename T> __device__ __forceinline__ void st_pair(T* __restrict__ p, P2<T> v);
-template <> __device__ __forceinline__ void st_pair<float>(float* __restrict__ p, P2<float> v) {
-  *reinterpret_cast<float2*>(p) = v.v;
-}
-template <> __device__ __forceinline__ void st_pair<double>(double* __restrict__ p, P2<double> v) {
-  *reinterpret_cast<double2*>(p) = v.v;
+template <typename T, int H = LD_NC> __device__ __forceinline__ T ld_one(const T* __restrict__ p) { return ld_hint<H>(p); }
+template <typename T, int H = ST_WB> __device__ __forceinline__ void st_pair(T* __restrict__ p, P2<T> v) {
+  typedef typename PairOf<T>::type U;
+  if (H == ST_CS) __stcs(reinterpret_cast<U*>(p), v.v);
+  else *reinterpret_cast<U*>(p) = v.v;
 }
 
 }  // namespace clip

@@ -139,3 +139,64 @@ def test_error_paths():
     assert clip.clip_step(h, 1) == clip.CLIP_ESTATE
     assert clip.clip_get(h, 0, 0, 0) == clip.CLIP_ESTATE
     assert clip.clip_destroy(h) == clip.CLIP_OK
+
+
+def _gpu_env(case, steps, precision, **env):  # fast-path variant switches are read at clip_create
+    import os
+    old = {k: os.environ.get(k) for k in env}
+    os.environ.update({k: str(v) for k, v in env.items()})
+    try:
+        return _gpu(case, steps, precision)
+    finally:
+        for k, v in old.items():
+            if v is None:
+                os.environ.pop(k, None)
+            else:
+                os.environ[k] = v
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_single_launch_paths_equal_two_kernel_path_bitwise(precision):
+    """k_tick (one ticket-ordered launch, phi through L2) and k_march (phi resolved in shared memory) run the same
+    arithmetic in the same order as k_phi2 + k_step2: their fields must agree bit for bit -- for k_march over several
+    z-segment lengths (ragged last segment included)."""
+    case = inputs.sweep_drops(shape=(128, 24, 20), ndrops=6, rmin=3, rmax=6)
+    ref = _gpu_env(case, 25, precision, CLIP_FAST_MODE=2)
+    out = _gpu_env(case, 25, precision, CLIP_FAST_MODE=0)
+    for a, b in zip(ref, out):
+        assert np.array_equal(a, b), "k_tick"
+    for lz in (32, 7, 1):
+        out = _gpu_env(case, 25, precision, CLIP_FAST_MODE=1, CLIP_MARCH_LZ=lz)
+        for a, b in zip(ref, out):
+            assert np.array_equal(a, b), lz
+
+
+def test_tick_small_nz_and_chunked_steps():
+    """k_tick's item order for nz = 1, 2, 3 (degenerate plane wrap) and its step counters across several clip_step
+    calls: equal to the two-kernel path bit for bit."""
+    for nz in (1, 2, 3):
+        case = inputs.sweep_drops(shape=(32, 16, nz), ndrops=2, rmin=3, rmax=5)
+        ref = _gpu_env(case, 12, 64, CLIP_FAST_MODE=2)
+        import os
+        old = os.environ.get("CLIP_FAST_MODE")
+        os.environ["CLIP_FAST_MODE"] = "0"
+        try:
+            out = _gpu(case, 12, 64, chunks=(5, 1, 6))
+        finally:
+            os.environ.pop("CLIP_FAST_MODE")
+            if old is not None:
+                os.environ["CLIP_FAST_MODE"] = old
+        for a, b in zip(ref, out):
+            assert np.array_equal(a, b), nz
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_fast_paths_match_generic_kernels(precision):
+    """The pair-per-thread packed kernels against the generic thread-per-node kernels (different association of the
+    same sums): round-off only."""
+    case = inputs.sweep_drops(shape=(64, 16, 12), ndrops=4, rmin=3, rmax=5)
+    a = _gpu_env(case, 50, precision, CLIP_FORCE_GENERIC=1)
+    b = _gpu_env(case, 50, precision)
+    tol = 1e-12 if precision == 64 else 2e-5
+    for x, y in zip(a, b):
+        assert np.abs(x - y).max() <= tol * max(1.0, np.abs(x).max())
