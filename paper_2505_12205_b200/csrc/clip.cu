@@ -3,7 +3,6 @@
 #include "../../include/clip.h"
 #include "clip_kernels.cuh"
 #include "clip_fast.cuh"
-#include "clip_march.cuh"
 #include "clip_tick.cuh"
 
 #include <cmath>
@@ -30,7 +29,7 @@ size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
   size_t word;  // 4 or 8
-  size_t off_f[2], off_g[2], off_phi, off_u, off_obf, off_obg, off_lam, off_mask, off_sync, total;
+  size_t off_p[2], off_phi, off_u, off_obf, off_obg, off_lam, off_mask, off_sync, total;
 };
 
 Layout make_layout(int nx, int ny, int nz, const clip_params* p) {
@@ -39,8 +38,7 @@ Layout make_layout(int nx, int ny, int nz, const clip_params* p) {
   const size_t n = (size_t)nx * ny * nz, nxy = (size_t)nx * ny;
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t r = o; o += align_up(bytes); return r; };
-  L.off_f[0] = take(19 * n * L.word); L.off_f[1] = take(19 * n * L.word);
-  L.off_g[0] = take(19 * n * L.word); L.off_g[1] = take(19 * n * L.word);
+  L.off_p[0] = take(38 * n * L.word); L.off_p[1] = take(38 * n * L.word);
   L.off_phi = take(n * L.word);
   L.off_u = take(3 * n * L.word);
   const bool outlet = p->bc[5] == CLIP_BC_OUTLET, inlet = p->bc[4] == CLIP_BC_INLET;
@@ -90,13 +88,13 @@ struct clip_handle {
   cudaStream_t stream;
   int cur;      // which of the A/B population buffers holds the current post-collision state
   bool inited;
-  bool march_attr_set;
-  int mode;            // fast-path variant (CLIP_FAST_MODE): 0 = k_tick2, 1 = k_march, 2 = k_phi2 + k_step2 (default)
+  int mode;            // fast-path variant (CLIP_FAST_MODE): 0 = k_tick2 (one launch), 2 = k_phi2 + k_step2
   unsigned epoch;      // steps since clip_init (k_tick counters)
   int tick_order;      // CLIP_TICK_ORDER (default 0): 0 = item number from blockIdx, 1 = from an atomic ticket
   int fast_threads;    // threads per block of the pair kernels (CLIP_FAST_THREADS: 128 or 256, default 256)
+  int nx_special;      // nx, or 0 when CLIP_NO_NX_SPECIAL=1 forces the runtime-nx kernels (tests)
+  int tick_lag;        // CLIP_TICK_LAG (default 4, >= 3): groups between the phi job and the collision job of a plane (k_tick2)
   int tick_hint;       // CLIP_TICK_HINT (default 1): streaming cache hints on single-use loads and on stores
-  int march_lz;        // planes per z segment of k_march (CLIP_MARCH_LZ, default 32)
   bool force_generic;  // CLIP_FORCE_GENERIC=1 in the environment at clip_create: generic kernels only (tests)
   long long launches;
   long long t;
@@ -128,8 +126,7 @@ template <typename T> clip::KP<T> make_kp(const clip_handle* h) {
   for (int k = 0; k < 3; ++k) P.uin[k] = (T)p.inlet_u[k];
   P.phi_in = (T)p.inlet_phi;
   char* ws = h->ws;
-  P.f_src = (const T*)(ws + h->L.off_f[h->cur]); P.g_src = (const T*)(ws + h->L.off_g[h->cur]);
-  P.f_dst = (T*)(ws + h->L.off_f[h->cur ^ 1]); P.g_dst = (T*)(ws + h->L.off_g[h->cur ^ 1]);
+  P.p_src = (const T*)(ws + h->L.off_p[h->cur]); P.p_dst = (T*)(ws + h->L.off_p[h->cur ^ 1]);
   P.phi = (T*)(ws + h->L.off_phi); P.u = (T*)(ws + h->L.off_u);
   P.ob_f = (T*)(ws + h->L.off_obf); P.ob_g = (T*)(ws + h->L.off_obg); P.lam = (T*)(ws + h->L.off_lam);
   P.mask = (const uint8_t*)(ws + h->L.off_mask);
@@ -159,8 +156,7 @@ template <typename T> int do_init(clip_handle* h, const void* phi0, const void* 
 }
 
 enum { KIND_PHI = 0, KIND_STEP = 1, KIND_PHI2 = 2, KIND_STEP2 = 3, KIND_MARCH = 4, KIND_TICK = 5, KIND_COUNT = 6 };
-const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step2", "k_march", "k_tick"};
-constexpr int MTX = 64, MTY = 8;  // in-plane tile of the marching kernel
+const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step2", "(unused)", "k_tick2"};
 
 // The pair-per-thread fast kernels (clip_fast.cuh) cover fully periodic lattices with even nx.
 bool fast_ok(const clip_handle* h) {
@@ -176,18 +172,37 @@ void fast_shape(const clip_handle* h, dim3& grid, dim3& block) {
   block = dim3(bx, by, 1);
   grid = dim3((pairs + bx - 1) / bx, (h->ny + by - 1) / by, h->nz);
 }
-template <typename T> clip::FP<T> make_fp(const clip::KP<T>& P) {
-  clip::FP<T> F;
-  F.k = P;
-  for (int a = 0; a < clip::Q; ++a) {
-    F.fs[a] = P.f_src + (long long)a * P.n; F.gs[a] = P.g_src + (long long)a * P.n;
-    F.fd[a] = P.f_dst + (long long)a * P.n; F.gd[a] = P.g_dst + (long long)a * P.n;
+template <typename T> clip::FP<T> make_fp(const clip::KP<T>& P) { clip::FP<T> F; F.k = P; return F; }
+
+// nx values with their own instantiation of the fast kernels (direction offsets as immediates); others take NX = 0.
+#ifndef CLIP_NX_LIST
+#define CLIP_NX_LIST(X) X(64) X(128) X(256) X(384) X(512)
+#endif
+
+template <typename T> void launch_phi2(int nx, dim3 g, dim3 b, cudaStream_t st, const clip::FP<T>& F) {
+  switch (nx) {
+#define X(N) case N: clip::k_phi2<T, N><<<g, b, 0, st>>>(F); break;
+    CLIP_NX_LIST(X)
+#undef X
+    default: clip::k_phi2<T, 0><<<g, b, 0, st>>>(F);
   }
-  return F;
 }
-// The fused marching kernel additionally needs whole tiles.
-bool march_ok(const clip_handle* h) {
-  return fast_ok(h) && h->mode == 1 && h->nx % MTX == 0 && h->ny % MTY == 0;
+template <typename T, int MB> void launch_step2(int nx, dim3 g, dim3 b, cudaStream_t st, const clip::FP<T>& F) {
+  switch (nx) {
+#define X(N) case N: clip::k_step2<T, N, MB><<<g, b, 0, st>>>(F); break;
+    CLIP_NX_LIST(X)
+#undef X
+    default: clip::k_step2<T, 0, MB><<<g, b, 0, st>>>(F);
+  }
+}
+template <typename T, int MB>
+void launch_tick2(int nx, unsigned items, dim3 b, cudaStream_t st, const clip::FP<T>& F, const clip::TickP& tk, int lag) {
+  switch (nx) {
+#define X(N) case N: clip::k_tick2<T, N, MB><<<items, b, 0, st>>>(F, tk, lag); break;
+    CLIP_NX_LIST(X)
+#undef X
+    default: clip::k_tick2<T, 0, MB><<<items, b, 0, st>>>(F, tk, lag);
+  }
 }
 template <typename T> struct StepMinBlocks { static constexpr int value = 2; };
 template <> struct StepMinBlocks<double> { static constexpr int value = 1; };
@@ -203,18 +218,10 @@ struct Prof {  // optional per-launch event timing (clip_step_profiled)
 template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullptr) {
   const bool fast = fast_ok(h);
   dim3 fg, fb;
-  const bool march = march_ok(h);
   bool tick = false;
   if (fast) fast_shape(h, fg, fb);
   if (fast && h->mode == 0 && (h->nx / 2) % fb.x == 0 && h->ny % fb.y == 0) {
     tick = true;
-  }
-  constexpr size_t msmem = clip::march_smem_bytes<T, MTX, MTY>();
-  auto kmarch = clip::k_march<T, MTX, MTY, StepMinBlocks<T>::value>;
-  if (march && !h->march_attr_set) {
-    if (cudaFuncSetAttribute(kmarch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msmem) != cudaSuccess)
-      return check_cuda(h, "cudaFuncSetAttribute(k_march)");
-    h->march_attr_set = true;
   }
   for (int s = 0; s < nsteps; ++s) {
     clip::KP<T> P = make_kp<T>(h);
@@ -225,24 +232,13 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       clip::TickP tk;
       tk.ticket = sync; tk.done_a = sync + 32;
       tk.tp = (int)(fg.x * fg.y); tk.gx = (int)fg.x;
-      const unsigned items = ((unsigned)h->nz + 3u) * (unsigned)tk.tp;
+      const unsigned lag = (unsigned)h->tick_lag;
+      const unsigned items = ((unsigned)h->nz + lag) * (unsigned)tk.tp;
       tk.base = 0;
       tk.target = (unsigned)tk.tp * h->epoch;
       if (prof) prof->begin();
-      clip::k_tick2<T, StepMinBlocks<T>::value><<<items, fb, 0, h->stream>>>(F, tk);
+      launch_tick2<T, StepMinBlocks<T>::value>(h->nx_special, items, fb, h->stream, F, tk, (int)lag);
       if (prof) prof->end(KIND_TICK);
-      h->launches += 1;
-      h->cur ^= 1;
-      h->t += 1;
-      continue;
-    }
-    if (march) {
-      clip::FP<T> F = make_fp<T>(P);
-      const int LZ = h->march_lz;
-      dim3 mg(h->nx / MTX, h->ny / MTY, (h->nz + LZ - 1) / LZ);
-      if (prof) prof->begin();
-      kmarch<<<mg, clip::MarchCfg<MTX, MTY>::NT, msmem, h->stream>>>(F, LZ);
-      if (prof) prof->end(KIND_MARCH);
       h->launches += 1;
       h->cur ^= 1;
       h->t += 1;
@@ -251,10 +247,10 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
     if (prof) prof->begin();
     clip::FP<T> F;
     if (fast) F = make_fp<T>(P);
-    if (fast) clip::k_phi2<T><<<fg, fb, 0, h->stream>>>(F);
+    if (fast) launch_phi2<T>(h->nx_special, fg, fb, h->stream, F);
     else clip::k_phi<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
     if (prof) { prof->end(fast ? KIND_PHI2 : KIND_PHI); prof->begin(); }
-    if (fast) clip::k_step2<T, StepMinBlocks<T>::value><<<fg, fb, 0, h->stream>>>(F);
+    if (fast) launch_step2<T, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
     else clip::k_step<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
     if (prof) prof->end(fast ? KIND_STEP2 : KIND_STEP);
     h->launches += 2;
@@ -299,12 +295,12 @@ int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params,
   h->nx = nx; h->ny = ny; h->nz = nz; h->p = *params; h->L = L; h->ws = (char*)d_workspace;
   h->stream = (cudaStream_t)cuda_stream; h->cur = 0; h->inited = false;
   { const char* e = getenv("CLIP_FORCE_GENERIC"); h->force_generic = e && e[0] == '1'; }
-  h->march_attr_set = false;
   { const char* e = getenv("CLIP_FAST_MODE"); h->mode = e ? atoi(e) : 2; h->epoch = 0; }
   { const char* e = getenv("CLIP_TICK_ORDER"); h->tick_order = e ? atoi(e) : 0; }
   { const char* e = getenv("CLIP_FAST_THREADS"); h->fast_threads = (e && atoi(e) == 128) ? 128 : 256; }
+  { const char* e = getenv("CLIP_NO_NX_SPECIAL"); h->nx_special = (e && e[0] == '1') ? 0 : nx; }
+  { const char* e = getenv("CLIP_TICK_LAG"); h->tick_lag = e ? atoi(e) : 4; if (h->tick_lag < 3) h->tick_lag = 3; }
   { const char* e = getenv("CLIP_TICK_HINT"); h->tick_hint = e ? atoi(e) : 1; }
-  { const char* e = getenv("CLIP_MARCH_LZ"); h->march_lz = e ? atoi(e) : 32; if (h->march_lz < 1) h->march_lz = 32; }
   h->launches = 0; h->t = 0; h->err[0] = 0;
   if (params->bc[4] == CLIP_BC_INLET) {  // disc mask, decided in double on the host
     h->mask_host.resize((size_t)nx * ny);

@@ -11,64 +11,75 @@
 
 namespace clip {
 
-// Kernel parameters of the fast kernels: KP plus one base pointer per direction and array, so that every load / store
-// address is a single IMAD.WIDE (32-bit element index x word size + 64-bit base taken from the constant bank).
-template <typename T> struct FP {
-  KP<T> k;
-  const T* fs[Q]; const T* gs[Q];  // post-collision populations at t,   [nz][ny][nx] each
-  T* fd[Q]; T* gd[Q];              // post-collision populations at t+1
-};
+// Kernel parameters of the fast kernels (kept as a separate type so that their signatures differ from the generic ones).
+template <typename T> struct FP { KP<T> k; };
 
-// Per-thread geometry of a node pair on a periodic lattice: element indices are 32-bit (n < 2^31, checked on the host).
+// Per-thread geometry of a node pair on a periodic lattice.  Plain fields (phi, u) are indexed with 32-bit element
+// indices (n < 2^31, checked on the host).  The population buffer is [nz][ny][38][nx]: the row of (y', z') starts at
+// 38 * (plain row start), so component c of node x0 in the row whose plain index is `row` sits at
+// 38 * row - 37 * x0 + c * nx  -- one 64-bit multiply-add per ROW; within a row all 38 components and the x +- 1
+// neighbours are constant offsets (load / store immediates when NX is a template parameter).
 struct Geo {
-  int rc;                  // index of node x0 in its own row
-  int dym, dyp, dzm, dzp;  // offsets to the rows y-1, y+1, z-1, z+1 (periodic wrap, B.5-B.7)
+  int rc;                  // plain index of node x0 in its own row
+  int dym, dyp, dzm, dzp;  // plain offsets to the rows y-1, y+1, z-1, z+1 (periodic wrap, B.5-B.7)
   int xm, xp;              // offsets from x0 to x0-1 and to x0+2 (periodic wrap)
+  bool wm, wp;             // x0-1 / x0+2 wrap around
+  int x0;
 };
 
 template <typename T> __device__ __forceinline__ Geo make_geo(const KP<T>& P, int x0, int y, int z) {
   Geo g;
   const int nxy = P.nx * P.ny;
+  g.x0 = x0;
   g.rc = (z * P.ny + y) * P.nx + x0;
   g.dym = (y == 0) ? (P.ny - 1) * P.nx : -P.nx;
   g.dyp = (y == P.ny - 1) ? -(P.ny - 1) * P.nx : P.nx;
   g.dzm = (z == 0) ? (P.nz - 1) * nxy : -nxy;
   g.dzp = (z == P.nz - 1) ? -(P.nz - 1) * nxy : nxy;
-  g.xm = (x0 == 0) ? P.nx - 1 : -1;
-  g.xp = (x0 + 2 == P.nx) ? 2 - P.nx : 2;
+  g.wm = (x0 == 0); g.wp = (x0 + 2 == P.nx);
+  g.xm = g.wm ? P.nx - 1 : -1;
+  g.xp = g.wp ? 2 - P.nx : 2;
   return g;
 }
 
-// row index of (y + sy, z + sz)
+// plain row index of (y + sy, z + sz)
 template <int sy, int sz> __device__ __forceinline__ int row_of(const Geo& g) {
   return g.rc + (sy > 0 ? g.dyp : (sy < 0 ? g.dym : 0)) + (sz > 0 ? g.dzp : (sz < 0 ? g.dzm : 0));
 }
-
-// Streaming (pull, Alg. 2 / B.3-B.6) of direction a for the node pair: value at x - e_a.
-template <typename T, int a, int H> __device__ __forceinline__ P2<T> pull2(const T* const (&src)[Q], const Geo& g) {
-  const T* __restrict__ b = src[a];
-  const int row = row_of<-cy(a), -cz(a)>(g);
-  if (cx(a) == 0) return ld_pair<T, H>(b + row);
-  if (cx(a) == 1) return P2<T>(ld_one<T, H>(b + (row + g.xm)), ld_one<T, H>(b + row));
-  return P2<T>(ld_one<T, H>(b + (row + 1)), ld_one<T, H>(b + (row + g.xp)));
+// pointer to component 0 of node x0 in the population row of (y + sy, z + sz)
+template <typename T, int sy, int sz> __device__ __forceinline__ const T* pop_row(const T* __restrict__ p, const Geo& g) {
+  return p + ((long long)NC * row_of<sy, sz>(g) - (NC - 1) * g.x0);
 }
-template <typename T, int H = LD_NC, int a = 0> struct Pull2All {
-  static __device__ __forceinline__ void run(const T* const (&src)[Q], const Geo& g, P2<T> (&v)[Q]) {
-    v[a] = pull2<T, a, H>(src, g);
-    Pull2All<T, H, a + 1>::run(src, g, v);
+
+// Streaming (pull, Alg. 2 / B.3-B.6) of direction a of set SET (0: f, 1: g) for the node pair: value at x - e_a.
+// NX > 0: nx known at compile time (component offsets become immediates); NX == 0: runtime nx.
+template <typename T, int a, int H, int NX, int SET>
+__device__ __forceinline__ P2<T> pull2(const T* __restrict__ src, int nx_rt, const Geo& g) {
+  const int nx = NX ? NX : nx_rt;
+  const T* __restrict__ rp = pop_row<T, -cy(a), -cz(a)>(src, g) + (SET * Q + a) * nx;
+  if (cx(a) == 0) return ld_pair<T, H>(rp);
+  if (cx(a) == 1) return P2<T>(g.wm ? ld_one<T, H>(rp + (nx - 1)) : ld_one<T, H>(rp - 1), ld_one<T, H>(rp));
+  return P2<T>(ld_one<T, H>(rp + 1), g.wp ? ld_one<T, H>(rp + (2 - nx)) : ld_one<T, H>(rp + 2));
+}
+template <typename T, int H, int NX, int SET, int a = 0> struct Pull2All {
+  static __device__ __forceinline__ void run(const T* __restrict__ src, int nx, const Geo& g, P2<T> (&v)[Q]) {
+    v[a] = pull2<T, a, H, NX, SET>(src, nx, g);
+    Pull2All<T, H, NX, SET, a + 1>::run(src, nx, g, v);
   }
 };
-template <typename T, int H> struct Pull2All<T, H, Q> {
-  static __device__ __forceinline__ void run(const T* const (&)[Q], const Geo&, P2<T> (&)[Q]) {}
+template <typename T, int H, int NX, int SET> struct Pull2All<T, H, NX, SET, Q> {
+  static __device__ __forceinline__ void run(const T* __restrict__, int, const Geo&, P2<T> (&)[Q]) {}
 };
-template <typename T, int H = ST_WB, int a = 0> struct Store2All {
-  static __device__ __forceinline__ void run(T* const (&dst)[Q], int rc, const P2<T> (&v)[Q]) {
-    st_pair<T, H>(dst[a] + rc, v[a]);
-    Store2All<T, H, a + 1>::run(dst, rc, v);
+// stores of set SET into the node pair's own population row `rd` (= pointer to component 0 of node x0)
+template <typename T, int H, int NX, int SET, int a = 0> struct Store2All {
+  static __device__ __forceinline__ void run(T* __restrict__ rd, int nx_rt, const P2<T> (&v)[Q]) {
+    const int nx = NX ? NX : nx_rt;
+    st_pair<T, H>(rd + (SET * Q + a) * nx, v[a]);
+    Store2All<T, H, NX, SET, a + 1>::run(rd, nx_rt, v);
   }
 };
-template <typename T, int H> struct Store2All<T, H, Q> {
-  static __device__ __forceinline__ void run(T* const (&)[Q], int, const P2<T> (&)[Q]) {}
+template <typename T, int H, int NX, int SET> struct Store2All<T, H, NX, SET, Q> {
+  static __device__ __forceinline__ void run(T* __restrict__, int, const P2<T> (&)[Q]) {}
 };
 
 template <typename T> __device__ __forceinline__ P2<T> sum19(const P2<T> (&g)[Q]) {
@@ -234,25 +245,26 @@ template <typename T> __device__ __forceinline__ bool pair_coords(const KP<T>& P
 }
 
 // phi(t+1) = sum_a g_a(x,t+1) (Eq. 38) of one node pair by pulling the post-collision g+(t).
-template <typename T, int HG> __device__ __forceinline__ void phi_pair(const FP<T>& FPp, int x0, int y, int z) {
-  const Geo geo = make_geo(FPp.k, x0, y, z);
+template <typename T, int HG, int NX> __device__ __forceinline__ void phi_pair(const FP<T>& FPp, int x0, int y, int z) {
+  const KP<T>& P = FPp.k;
+  const Geo geo = make_geo(P, x0, y, z);
   P2<T> g[Q];
-  Pull2All<T, HG>::run(FPp.gs, geo, g);
-  st_pair<T>(FPp.k.phi + geo.rc, sum19(g));
+  Pull2All<T, HG, NX, 1>::run(P.p_src, P.nx, geo, g);
+  st_pair<T>(P.phi + geo.rc, sum19(g));
 }
 
 // One node pair of the step: pull f+, g+ -> macros (Alg. 3) -> both collisions (Alg. 1) -> store f+, g+, u.
 // HL: hint of the population / u loads, HP: hint of the phi loads, HS: hint of the stores.  `before_phi()` runs after
-// the population loads have been issued and before phi is touched (k_tick waits there for the phi planes).
+// the population loads have been issued and before phi is touched.
 struct NoWait { __device__ __forceinline__ void operator()() const {} };
-template <typename T, int HL, int HP, int HS, typename W>
+template <typename T, int HL, int HP, int HS, int NX, typename W>
 __device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z, W before_phi) {
   typedef P2<T> V;
   const KP<T>& P = FPp.k;
   const Geo geo = make_geo(P, x0, y, z);
   V f[Q], g[Q];
-  Pull2All<T, HL>::run(FPp.fs, geo, f);
-  Pull2All<T, HL>::run(FPp.gs, geo, g);
+  Pull2All<T, HL, NX, 0>::run(P.p_src, P.nx, geo, f);
+  Pull2All<T, HL, NX, 1>::run(P.p_src, P.nx, geo, g);
   V ux = ld_pair<T, HL>(P.u + geo.rc), uy = ld_pair<T, HL>(P.u + P.n + geo.rc), uz = ld_pair<T, HL>(P.u + 2 * P.n + geo.rc);
   before_phi();
   V phi, G[3], L;
@@ -267,19 +279,20 @@ __device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z
   }
   st_pair<T, HS>(P.u + geo.rc, ux); st_pair<T, HS>(P.u + P.n + geo.rc, uy); st_pair<T, HS>(P.u + 2 * P.n + geo.rc, uz);
   collide2<T>(P, m, mat, phi, G, ux, uy, uz, f, g);
-  Store2All<T, HS>::run(FPp.fd, geo.rc, f);
-  Store2All<T, HS>::run(FPp.gd, geo.rc, g);
+  T* const rd = const_cast<T*>(pop_row<T, 0, 0>(P.p_dst, geo));
+  Store2All<T, HS, NX, 0>::run(rd, P.nx, f);
+  Store2All<T, HS, NX, 1>::run(rd, P.nx, g);
 }
 
-template <typename T> __global__ void __launch_bounds__(256) k_phi2(const __grid_constant__ FP<T> FPp) {
+template <typename T, int NX> __global__ void __launch_bounds__(256) k_phi2(const __grid_constant__ FP<T> FPp) {
   int x0, y, z;
   if (!pair_coords(FPp.k, x0, y, z)) return;
-  phi_pair<T, LD_NC>(FPp, x0, y, z);
+  phi_pair<T, LD_NC, NX>(FPp, x0, y, z);
 }
-template <typename T, int MINB> __global__ void __launch_bounds__(256, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
+template <typename T, int NX, int MINB> __global__ void __launch_bounds__(256, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
   int x0, y, z;
   if (!pair_coords(FPp.k, x0, y, z)) return;
-  step_pair<T, LD_NC, LD_NC, ST_WB>(FPp, x0, y, z, NoWait());
+  step_pair<T, LD_NC, LD_NC, ST_WB, NX>(FPp, x0, y, z, NoWait());
 }
 
 }  // namespace clip

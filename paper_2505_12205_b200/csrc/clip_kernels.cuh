@@ -1,7 +1,9 @@
 // clip_kernels.cuh -- device code of libclip (sm_100a).  See DESIGN.md for the kernel designs and the roofline.
 //
 // State kept in HBM between steps (SoA, x fastest; T = float or double):
-//   f[cur], g[cur]  POST-collision populations f+(x,t), g+(x,t)            [19][nz][ny][nx]   (A/B buffered)
+//   pop[cur]        POST-collision populations f+(x,t) (components 0..18) and g+(x,t) (19..37), row-interleaved:
+//                   [nz][ny][38][nx] -- the 38 components of one lattice row lie next to each other, so that in the
+//                   fast kernels (NX a template parameter) every direction offset is a load/store immediate (A/B buffered)
 //   phi             phi(x,t)                                                    [nz][ny][nx]
 //   u               u(x,t)                                                   [3][nz][ny][nx]   (node-local update)
 //   ob_f, ob_g      PRE-collision populations of the outlet layer z = nz-1 at t   [19][ny][nx] (outlet only)
@@ -56,8 +58,8 @@ template <typename T> struct KP {
   T gx, gy, gz, rho_ref;
   T uin[3], phi_in;
   // arrays
-  const T* f_src; const T* g_src;  // post-collision at t
-  T* f_dst; T* g_dst;              // post-collision at t+1
+  const T* p_src;  // post-collision populations at t     [nz][ny][38][nx]
+  T* p_dst;        // post-collision populations at t+1
   T* phi; T* u;
   T* ob_f; T* ob_g; T* lam;
   const uint8_t* mask;
@@ -110,13 +112,17 @@ __device__ __forceinline__ Nbr make_nbr(const KP<T>& P, int x, int y, int z) {
   return b;
 }
 
+constexpr int NC = 2 * Q;  // components per lattice row of the population buffer
+// offset, in the population buffer, from a node to the node x - e_a (rows are NC times longer there)
 template <int a> __device__ __forceinline__ long long src_off(const Nbr& b) {
-  long long o = 0;
+  long long o = 0, r = 0;
   if (cx(a) == 1) o += b.xm; else if (cx(a) == -1) o += b.xp;
-  if (cy(a) == 1) o += b.ym; else if (cy(a) == -1) o += b.yp;
-  if (cz(a) == 1) o += b.zm; else if (cz(a) == -1) o += b.zp;
-  return o;
+  if (cy(a) == 1) r += b.ym; else if (cy(a) == -1) r += b.yp;
+  if (cz(a) == 1) r += b.zm; else if (cz(a) == -1) r += b.zp;
+  return o + NC * r;
 }
+// index of component 0 of node i (x its column) in the population buffer
+__device__ __forceinline__ long long pop_base(long long i, int x) { return (long long)NC * (i - x) + x; }
 template <int a> __device__ __forceinline__ bool src_bounce(const Nbr& b) {
   return (cx(a) == 1 && b.bxm) || (cx(a) == -1 && b.bxp) || (cy(a) == 1 && b.bym) || (cy(a) == -1 && b.byp) ||
          (cz(a) == 1 && b.bzm) || (cz(a) == -1 && b.bzp);
@@ -128,23 +134,24 @@ template <int a> __device__ __forceinline__ bool src_open(const Nbr& b) {
 // Streaming (pull) of one population set at node i: Alg. 2 / B.3-B.4 with periodic wrap (B.5-B.6) and halfway
 // bounce-back (B.10-B.11; a wall crossing wins at edges and corners, R11).  Open links (inlet disc / outlet
 // face) get 0 and are filled by the caller.
+// `src` points at component 0 of the set (f: p_src, g: p_src + Q*nx); pb = pop_base of the node.
 template <typename T, int a>
-__device__ __forceinline__ T pull_one(const T* __restrict__ src, long long n, long long i, const Nbr& b, bool slow) {
-  if (!slow) return __ldg(src + (long long)a * n + i + src_off<a>(b));
-  if (src_bounce<a>(b)) return __ldg(src + (long long)copp(a) * n + i);
+__device__ __forceinline__ T pull_one(const T* __restrict__ src, int nx, long long pb, const Nbr& b, bool slow) {
+  if (!slow) return __ldg(src + pb + a * nx + src_off<a>(b));
+  if (src_bounce<a>(b)) return __ldg(src + pb + copp(a) * nx);
   if (src_open<a>(b)) return T(0);
-  return __ldg(src + (long long)a * n + i + src_off<a>(b));
+  return __ldg(src + pb + a * nx + src_off<a>(b));
 }
 
 template <typename T, int a = 0> struct PullAll {
-  static __device__ __forceinline__ void run(const T* __restrict__ src, long long n, long long i, const Nbr& b, bool slow,
+  static __device__ __forceinline__ void run(const T* __restrict__ src, int nx, long long pb, const Nbr& b, bool slow,
                                               T (&v)[Q]) {
-    v[a] = pull_one<T, a>(src, n, i, b, slow);
-    PullAll<T, a + 1>::run(src, n, i, b, slow, v);
+    v[a] = pull_one<T, a>(src, nx, pb, b, slow);
+    PullAll<T, a + 1>::run(src, nx, pb, b, slow, v);
   }
 };
 template <typename T> struct PullAll<T, Q> {
-  static __device__ __forceinline__ void run(const T* __restrict__, long long, long long, const Nbr&, bool, T (&)[Q]) {}
+  static __device__ __forceinline__ void run(const T* __restrict__, int, long long, const Nbr&, bool, T (&)[Q]) {}
 };
 
 // Gamma_a / w_a, Eq. 18
@@ -195,8 +202,9 @@ __device__ __forceinline__ void load_node(const KP<T>& P, int x, int y, int z, T
   const long long i = (long long)zs * P.nxy + (long long)y * P.nx + x;
   const Nbr b = make_nbr(P, x, y, zs);
   const bool slow = P.any_nonperiodic && b.any;
-  PullAll<T>::run(P.g_src, P.n, i, b, slow, g);
-  if (WITH_F) PullAll<T>::run(P.f_src, P.n, i, b, slow, f);
+  const long long pb = pop_base(i, x);
+  PullAll<T>::run(P.p_src + Q * P.nx, P.nx, pb, b, slow, g);
+  if (WITH_F) PullAll<T>::run(P.p_src, P.nx, pb, b, slow, f);
   if (P.has_inlet && b.ozm) {
     inlet_g(P, g);
     if (WITH_F) inlet_f(P, f);
@@ -341,13 +349,13 @@ __device__ __forceinline__ void collide(const KP<T>& P, const Mom<T>& m, const M
 }
 
 template <typename T, int a = 0> struct StoreAll {
-  static __device__ __forceinline__ void run(T* __restrict__ dst, long long n, long long i, const T (&v)[Q]) {
-    dst[(long long)a * n + i] = v[a];
-    StoreAll<T, a + 1>::run(dst, n, i, v);
+  static __device__ __forceinline__ void run(T* __restrict__ dst, int nx, long long pb, const T (&v)[Q]) {
+    dst[pb + a * nx] = v[a];
+    StoreAll<T, a + 1>::run(dst, nx, pb, v);
   }
 };
 template <typename T> struct StoreAll<T, Q> {
-  static __device__ __forceinline__ void run(T* __restrict__, long long, long long, const T (&)[Q]) {}
+  static __device__ __forceinline__ void run(T* __restrict__, int, long long, const T (&)[Q]) {}
 };
 
 // ------------------------------------------------------------------------------------------------ kernels
@@ -396,8 +404,8 @@ template <typename T> __global__ void __launch_bounds__(256) k_step(const __grid
   if (P.has_inlet && z == 0 && P.mask[(long long)y * P.nx + x]) { ux = P.uin[0]; uy = P.uin[1]; uz = P.uin[2]; }
   P.u[i] = ux; P.u[P.n + i] = uy; P.u[2 * P.n + i] = uz;
   collide(P, m, mat, phi, G, ux, uy, uz, f, g);
-  StoreAll<T>::run(P.f_dst, P.n, i, f);
-  StoreAll<T>::run(P.g_dst, P.n, i, g);
+  StoreAll<T>::run(P.p_dst, P.nx, pop_base(i, x), f);
+  StoreAll<T>::run(P.p_dst + Q * P.nx, P.nx, pop_base(i, x), g);
 }
 
 // k_init: I1-I4 of DESIGN.md (R8), then the first collision; phi0/u0 are caller buffers.
@@ -440,8 +448,8 @@ __global__ void __launch_bounds__(256) k_init(const __grid_constant__ KP<T> P, c
   P.u[i] = ux; P.u[P.n + i] = uy; P.u[2 * P.n + i] = uz;
   const Mom<T> m = moments(f);
   collide(P, m, mat, phi, G, ux, uy, uz, f, g);
-  StoreAll<T>::run(P.f_dst, P.n, i, f);
-  StoreAll<T>::run(P.g_dst, P.n, i, g);
+  StoreAll<T>::run(P.p_dst, P.nx, pop_base(i, x), f);
+  StoreAll<T>::run(P.p_dst + Q * P.nx, P.nx, pop_base(i, x), g);
 }
 
 // k_get: phi, p = p* rho c_s^2 with p* = sum_a f+_a (the collision conserves sum f), u.
@@ -456,7 +464,8 @@ __global__ void __launch_bounds__(256) k_get(const __grid_constant__ KP<T> P, T*
   if (p_out) {
     T f[Q];
 #pragma unroll
-    for (int a = 0; a < Q; ++a) f[a] = P.f_src[(long long)a * P.n + i];
+    const int x = (int)(i % P.nx);
+    for (int a = 0; a < Q; ++a) f[a] = P.p_src[pop_base(i, x) + a * P.nx];
     const Mom<T> m = moments(f);
     p_out[i] = m.p * (P.rho_l + phi * P.drho) * T(1.0 / 3.0);
   }

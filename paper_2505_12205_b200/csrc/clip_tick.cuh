@@ -27,20 +27,20 @@ __device__ __forceinline__ unsigned ld_volatile_u32(const unsigned* p) {
 }
 
 // k_tick2: every block does BOTH jobs for one tile: phi(t+1) of plane p = (i + nz - 1) mod nz (if i < nz) and the
-// macros + collisions of plane z = i - 3 (if i >= 3), where i = blockIdx.x / tp is the "group" (nz + 3 groups).
+// macros + collisions of plane z = i - lag (if i >= lag >= 3), where i = blockIdx.x / tp is the "group" (nz + lag groups).
 // B(z) needs the phi planes z-1, z, z+1, which groups <= i - 1 produced: a block only ever waits for blocks with a
 // smaller index (handed out earlier, hence resident or finished); a wait longer than ~0.1 s traps instead of hanging.
 // All loads of the block (g pull of plane p, f / u of plane z) are in flight before the first use; the second pull
 // of g (plane z, read two groups earlier by A) hits L2.  One barrier per block.
-template <typename T, int MINB>
-__global__ void __launch_bounds__(256, MINB) k_tick2(const __grid_constant__ FP<T> FPp, const TickP tk) {
+template <typename T, int NX, int MINB>
+__global__ void __launch_bounds__(256, MINB) k_tick2(const __grid_constant__ FP<T> FPp, const TickP tk, const int lag) {
   typedef P2<T> V;
   const KP<T>& P = FPp.k;
   const int tid = threadIdx.y * blockDim.x + threadIdx.x;
   const int nz = P.nz;
   const int grp = blockIdx.x / tk.tp, r = blockIdx.x - grp * tk.tp;
-  const bool has_a = grp < nz, has_b = grp >= 3;
-  const int pa = (grp + nz - 1) % nz, z = grp - 3;
+  const bool has_a = grp < nz, has_b = grp >= lag;
+  const int pa = (grp + nz - 1) % nz, z = grp - lag;
   const int bxi = r % tk.gx, byi = r / tk.gx;
   const int x0 = 2 * (bxi * blockDim.x + threadIdx.x), y = byi * blockDim.y + threadIdx.y;
   unsigned c0 = 0, c1 = 0, c2 = 0;
@@ -52,16 +52,16 @@ __global__ void __launch_bounds__(256, MINB) k_tick2(const __grid_constant__ FP<
   Geo geo_a, geo;
   if (has_a) {
     geo_a = make_geo(P, x0, y, pa);
-    Pull2All<T, LD_NC>::run(FPp.gs, geo_a, ga);
+    Pull2All<T, LD_NC, NX, 1>::run(P.p_src, P.nx, geo_a, ga);
   }
   if (has_b) {
     geo = make_geo(P, x0, y, z);
-    Pull2All<T, LD_NC>::run(FPp.fs, geo, f);
+    Pull2All<T, LD_NC, NX, 0>::run(P.p_src, P.nx, geo, f);
     ux = ld_pair<T>(P.u + geo.rc); uy = ld_pair<T>(P.u + P.n + geo.rc); uz = ld_pair<T>(P.u + 2 * P.n + geo.rc);
   }
   if (has_a) st_pair<T>(P.phi + geo_a.rc, sum19(ga));
   if (has_b) {
-    Pull2All<T, LD_NC>::run(FPp.gs, geo, g);
+    Pull2All<T, LD_NC, NX, 1>::run(P.p_src, P.nx, geo, g);
     if (tid == 0) {
       unsigned spins = 0;
       while ((int)(c0 - tk.target) < 0) { __nanosleep(32); c0 = ld_volatile_u32(tk.done_a + zp); if (++spins > (1u << 21)) __trap(); }
@@ -85,8 +85,9 @@ __global__ void __launch_bounds__(256, MINB) k_tick2(const __grid_constant__ FP<
   }
   st_pair<T>(P.u + geo.rc, ux); st_pair<T>(P.u + P.n + geo.rc, uy); st_pair<T>(P.u + 2 * P.n + geo.rc, uz);
   collide2<T>(P, m, mat, phi, G, ux, uy, uz, f, g);
-  Store2All<T>::run(FPp.fd, geo.rc, f);
-  Store2All<T>::run(FPp.gd, geo.rc, g);
+  T* const rd = const_cast<T*>(pop_row<T, 0, 0>(P.p_dst, geo));
+  Store2All<T, ST_WB, NX, 0>::run(rd, P.nx, f);
+  Store2All<T, ST_WB, NX, 1>::run(rd, P.nx, g);
 }
 
 }  // namespace clip

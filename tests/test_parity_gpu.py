@@ -157,18 +157,20 @@ def _gpu_env(case, steps, precision, **env):  # fast-path variant switches are r
 
 @pytest.mark.parametrize("precision", [64, 32])
 def test_single_launch_paths_equal_two_kernel_path_bitwise(precision):
-    """k_tick (one ticket-ordered launch, phi through L2) and k_march (phi resolved in shared memory) run the same
-    arithmetic in the same order as k_phi2 + k_step2: their fields must agree bit for bit -- for k_march over several
-    z-segment lengths (ragged last segment included)."""
+    """k_tick2 (one launch, blocks ordered plane by plane, second g read from L2) runs the same arithmetic in the same
+    order as k_phi2 + k_step2: the fields must agree bit for bit; so must the nx-specialised and runtime-nx kernels."""
     case = inputs.sweep_drops(shape=(128, 24, 20), ndrops=6, rmin=3, rmax=6)
     ref = _gpu_env(case, 25, precision, CLIP_FAST_MODE=2)
     out = _gpu_env(case, 25, precision, CLIP_FAST_MODE=0)
     for a, b in zip(ref, out):
         assert np.array_equal(a, b), "k_tick"
-    for lz in (32, 7, 1):
-        out = _gpu_env(case, 25, precision, CLIP_FAST_MODE=1, CLIP_MARCH_LZ=lz)
-        for a, b in zip(ref, out):
-            assert np.array_equal(a, b), lz
+    # a lattice whose nx has its own instantiation (direction offsets as immediates) against the runtime-nx form
+    case = inputs.sweep_drops(shape=(64, 24, 10), ndrops=4, rmin=3, rmax=5)
+    a = _gpu_env(case, 25, precision, CLIP_FAST_MODE=2)
+    b = _gpu_env(case, 25, precision, CLIP_FAST_MODE=0)
+    c = _gpu_env(case, 25, precision, CLIP_FAST_MODE=2, CLIP_NO_NX_SPECIAL=1)
+    for x, y, z in zip(a, b, c):
+        assert np.array_equal(x, y) and np.array_equal(x, z)
 
 
 def test_tick_small_nz_and_chunked_steps():
