@@ -158,10 +158,10 @@ template <typename T> int do_init(clip_handle* h, const void* phi0, const void* 
 enum { KIND_PHI = 0, KIND_STEP = 1, KIND_PHI2 = 2, KIND_STEP2 = 3, KIND_MARCH = 4, KIND_TICK = 5, KIND_COUNT = 6 };
 const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step2", "(unused)", "k_tick2"};
 
-// The pair-per-thread fast kernels (clip_fast.cuh) cover fully periodic lattices with even nx.
+// The pair-per-thread fast kernels (clip_fast.cuh) cover lattices whose faces are PERIODIC or WALL, with even nx.
 bool fast_ok(const clip_handle* h) {
   if (h->force_generic) return false;
-  for (int k = 0; k < 6; ++k) if (h->p.bc[k] != CLIP_BC_PERIODIC) return false;
+  for (int k = 0; k < 6; ++k) if (h->p.bc[k] != CLIP_BC_PERIODIC && h->p.bc[k] != CLIP_BC_WALL) return false;
   return h->nx % 2 == 0;
 }
 void fast_shape(const clip_handle* h, dim3& grid, dim3& block) {
@@ -179,29 +179,29 @@ template <typename T> clip::FP<T> make_fp(const clip::KP<T>& P) { clip::FP<T> F;
 #define CLIP_NX_LIST(X) X(64) X(128) X(256) X(384) X(512)
 #endif
 
-template <typename T> void launch_phi2(int nx, dim3 g, dim3 b, cudaStream_t st, const clip::FP<T>& F) {
+template <typename T, bool W> void launch_phi2(int nx, dim3 g, dim3 b, cudaStream_t st, const clip::FP<T>& F) {
   switch (nx) {
-#define X(N) case N: clip::k_phi2<T, N><<<g, b, 0, st>>>(F); break;
+#define X(N) case N: clip::k_phi2<T, N, W><<<g, b, 0, st>>>(F); break;
     CLIP_NX_LIST(X)
 #undef X
-    default: clip::k_phi2<T, 0><<<g, b, 0, st>>>(F);
+    default: clip::k_phi2<T, 0, W><<<g, b, 0, st>>>(F);
   }
 }
-template <typename T, int MB> void launch_step2(int nx, dim3 g, dim3 b, cudaStream_t st, const clip::FP<T>& F) {
+template <typename T, bool W, int MB> void launch_step2(int nx, dim3 g, dim3 b, cudaStream_t st, const clip::FP<T>& F) {
   switch (nx) {
-#define X(N) case N: clip::k_step2<T, N, MB><<<g, b, 0, st>>>(F); break;
+#define X(N) case N: clip::k_step2<T, N, W, MB><<<g, b, 0, st>>>(F); break;
     CLIP_NX_LIST(X)
 #undef X
-    default: clip::k_step2<T, 0, MB><<<g, b, 0, st>>>(F);
+    default: clip::k_step2<T, 0, W, MB><<<g, b, 0, st>>>(F);
   }
 }
-template <typename T, int MB>
+template <typename T, bool W, int MB>
 void launch_tick2(int nx, unsigned items, dim3 b, cudaStream_t st, const clip::FP<T>& F, const clip::TickP& tk, int lag) {
   switch (nx) {
-#define X(N) case N: clip::k_tick2<T, N, MB><<<items, b, 0, st>>>(F, tk, lag); break;
+#define X(N) case N: clip::k_tick2<T, N, W, MB><<<items, b, 0, st>>>(F, tk, lag); break;
     CLIP_NX_LIST(X)
 #undef X
-    default: clip::k_tick2<T, 0, MB><<<items, b, 0, st>>>(F, tk, lag);
+    default: clip::k_tick2<T, 0, W, MB><<<items, b, 0, st>>>(F, tk, lag);
   }
 }
 template <typename T> struct StepMinBlocks { static constexpr int value = 2; };
@@ -217,6 +217,8 @@ struct Prof {  // optional per-launch event timing (clip_step_profiled)
 
 template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullptr) {
   const bool fast = fast_ok(h);
+  bool walls = false;
+  for (int k = 0; k < 6; ++k) walls = walls || h->p.bc[k] == CLIP_BC_WALL;
   dim3 fg, fb;
   bool tick = false;
   if (fast) fast_shape(h, fg, fb);
@@ -237,7 +239,8 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       tk.base = 0;
       tk.target = (unsigned)tk.tp * h->epoch;
       if (prof) prof->begin();
-      launch_tick2<T, StepMinBlocks<T>::value>(h->nx_special, items, fb, h->stream, F, tk, (int)lag);
+      if (walls) launch_tick2<T, true, StepMinBlocks<T>::value>(h->nx_special, items, fb, h->stream, F, tk, (int)lag);
+      else launch_tick2<T, false, StepMinBlocks<T>::value>(h->nx_special, items, fb, h->stream, F, tk, (int)lag);
       if (prof) prof->end(KIND_TICK);
       h->launches += 1;
       h->cur ^= 1;
@@ -247,10 +250,12 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
     if (prof) prof->begin();
     clip::FP<T> F;
     if (fast) F = make_fp<T>(P);
-    if (fast) launch_phi2<T>(h->nx_special, fg, fb, h->stream, F);
+    if (fast && walls) launch_phi2<T, true>(h->nx_special, fg, fb, h->stream, F);
+    else if (fast) launch_phi2<T, false>(h->nx_special, fg, fb, h->stream, F);
     else clip::k_phi<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
     if (prof) { prof->end(fast ? KIND_PHI2 : KIND_PHI); prof->begin(); }
-    if (fast) launch_step2<T, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
+    if (fast && walls) launch_step2<T, true, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
+    else if (fast) launch_step2<T, false, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
     else clip::k_step<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
     if (prof) prof->end(fast ? KIND_STEP2 : KIND_STEP);
     h->launches += 2;

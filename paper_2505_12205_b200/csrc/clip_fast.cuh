@@ -1,4 +1,4 @@
-// clip_fast.cuh -- fast kernels for fully periodic lattices with even nx: one thread owns the node pair
+// clip_fast.cuh -- fast kernels for lattices with periodic and / or wall faces and even nx: one thread owns the node pair
 // (x0, x0+1), all arithmetic two-lane packed (clip_pack.cuh).  Same equations and the same "lean" formulation as
 // clip_kernels.cuh (header comment there), reorganised by opposite-direction pairs (a, a+1):
 //   f+_a , f+_abar = w_a (A_a +- B_a),  A_a = p* - 1.5 u.u + 4.5 (e_a.u)^2 + k e_a^T D e_a,  B_a = e_a.(3u + 1.5 F/rho)
@@ -25,9 +25,14 @@ struct Geo {
   int xm, xp;              // offsets from x0 to x0-1 and to x0+2 (periodic wrap)
   bool wm, wp;             // x0-1 / x0+2 wrap around
   int x0;
+  // walls (WALLS instantiations only): links of this pair that cross a halfway bounce-back face (B.10-B.11) ...
+  bool bym, byp, bzm, bzp;  // ... towards y-1, y+1, z-1, z+1 (both nodes of the pair)
+  bool bxm, bxp;            // ... towards x0-1 (node x0 only) and towards x0+2 (node x0+1 only)
+  // ... and the phi ghost rule there (clamp = mirror across the wall, R9): plain offsets for the stencil rows / columns
+  int cym, cyp, czm, czp, cxm, cxp;
 };
 
-template <typename T> __device__ __forceinline__ Geo make_geo(const KP<T>& P, int x0, int y, int z) {
+template <typename T, bool WALLS = false> __device__ __forceinline__ Geo make_geo(const KP<T>& P, int x0, int y, int z) {
   Geo g;
   const int nxy = P.nx * P.ny;
   g.x0 = x0;
@@ -39,7 +44,24 @@ template <typename T> __device__ __forceinline__ Geo make_geo(const KP<T>& P, in
   g.wm = (x0 == 0); g.wp = (x0 + 2 == P.nx);
   g.xm = g.wm ? P.nx - 1 : -1;
   g.xp = g.wp ? 2 - P.nx : 2;
+  g.cym = g.dym; g.cyp = g.dyp; g.czm = g.dzm; g.czp = g.dzp; g.cxm = g.xm; g.cxp = g.xp;
+  g.bym = g.byp = g.bzm = g.bzp = g.bxm = g.bxp = false;
+  if (WALLS) {
+    g.bxm = g.wm && P.bc[0] != BC_PERIODIC; g.bxp = g.wp && P.bc[1] != BC_PERIODIC;
+    g.bym = (y == 0) && P.bc[2] != BC_PERIODIC; g.byp = (y == P.ny - 1) && P.bc[3] != BC_PERIODIC;
+    g.bzm = (z == 0) && P.bc[4] != BC_PERIODIC; g.bzp = (z == P.nz - 1) && P.bc[5] != BC_PERIODIC;
+    if (g.bxm) g.cxm = 0;
+    if (g.bxp) g.cxp = 1;
+    if (g.bym) g.cym = 0;
+    if (g.byp) g.cyp = 0;
+    if (g.bzm) g.czm = 0;
+    if (g.bzp) g.czp = 0;
+  }
   return g;
+}
+// plain row index of (y + sy, z + sz) under the phi ghost rule
+template <int sy, int sz> __device__ __forceinline__ int phi_row_of(const Geo& g) {
+  return g.rc + (sy > 0 ? g.cyp : (sy < 0 ? g.cym : 0)) + (sz > 0 ? g.czp : (sz < 0 ? g.czm : 0));
 }
 
 // plain row index of (y + sy, z + sz)
@@ -53,21 +75,30 @@ template <typename T, int sy, int sz> __device__ __forceinline__ const T* pop_ro
 
 // Streaming (pull, Alg. 2 / B.3-B.6) of direction a of set SET (0: f, 1: g) for the node pair: value at x - e_a.
 // NX > 0: nx known at compile time (component offsets become immediates); NX == 0: runtime nx.
-template <typename T, int a, int H, int NX, int SET>
+// WALLS: a link that crosses a wall face takes the opposite population of the node itself (B.10-B.11; any wall crossing
+// wins at edges and corners, R11).
+template <typename T, int a, int H, int NX, int SET, bool WALLS>
 __device__ __forceinline__ P2<T> pull2(const T* __restrict__ src, int nx_rt, const Geo& g) {
   const int nx = NX ? NX : nx_rt;
   const T* __restrict__ rp = pop_row<T, -cy(a), -cz(a)>(src, g) + (SET * Q + a) * nx;
+  if (WALLS && a > 0) {
+    const T* __restrict__ own = pop_row<T, 0, 0>(src, g) + (SET * Q + copp(a)) * nx;
+    const bool rb = (cy(a) == 1 && g.bym) || (cy(a) == -1 && g.byp) || (cz(a) == 1 && g.bzm) || (cz(a) == -1 && g.bzp);
+    if (rb) return ld_pair<T, H>(own);
+    if (cx(a) == 1 && g.bxm) return P2<T>(ld_one<T, H>(own), ld_one<T, H>(rp));
+    if (cx(a) == -1 && g.bxp) return P2<T>(ld_one<T, H>(rp + 1), ld_one<T, H>(own + 1));
+  }
   if (cx(a) == 0) return ld_pair<T, H>(rp);
   if (cx(a) == 1) return P2<T>(g.wm ? ld_one<T, H>(rp + (nx - 1)) : ld_one<T, H>(rp - 1), ld_one<T, H>(rp));
   return P2<T>(ld_one<T, H>(rp + 1), g.wp ? ld_one<T, H>(rp + (2 - nx)) : ld_one<T, H>(rp + 2));
 }
-template <typename T, int H, int NX, int SET, int a = 0> struct Pull2All {
+template <typename T, int H, int NX, int SET, bool WALLS, int a = 0> struct Pull2All {
   static __device__ __forceinline__ void run(const T* __restrict__ src, int nx, const Geo& g, P2<T> (&v)[Q]) {
-    v[a] = pull2<T, a, H, NX, SET>(src, nx, g);
-    Pull2All<T, H, NX, SET, a + 1>::run(src, nx, g, v);
+    v[a] = pull2<T, a, H, NX, SET, WALLS>(src, nx, g);
+    Pull2All<T, H, NX, SET, WALLS, a + 1>::run(src, nx, g, v);
   }
 };
-template <typename T, int H, int NX, int SET> struct Pull2All<T, H, NX, SET, Q> {
+template <typename T, int H, int NX, int SET, bool WALLS> struct Pull2All<T, H, NX, SET, WALLS, Q> {
   static __device__ __forceinline__ void run(const T* __restrict__, int, const Geo&, P2<T> (&)[Q]) {}
 };
 // stores of set SET into the node pair's own population row `rd` (= pointer to component 0 of node x0)
@@ -92,7 +123,7 @@ template <typename T> struct Row3 { P2<T> L, C, R; };
 template <typename T, int H> __device__ __forceinline__ Row3<T> ld_row3(const T* __restrict__ phi, int row, const Geo& g) {
   Row3<T> r;
   r.C = ld_pair<T, H>(phi + row);
-  const T m = ld_one<T, H>(phi + (row + g.xm)), p = ld_one<T, H>(phi + (row + g.xp));
+  const T m = ld_one<T, H>(phi + (row + g.cxm)), p = ld_one<T, H>(phi + (row + g.cxp));
   r.L = P2<T>(m, r.C.lo());
   r.R = P2<T>(r.C.hi(), p);
   return r;
@@ -102,11 +133,11 @@ template <typename T, int H> __device__ __forceinline__ Row3<T> ld_row3(const T*
 template <typename T, int H = LD_NC>
 __device__ __forceinline__ void stencil2(const T* __restrict__ phi, const Geo& g, P2<T>& pc, P2<T> (&G)[3], P2<T>& L) {
   typedef P2<T> V;
-  const Row3<T> c = ld_row3<T, H>(phi, row_of<0, 0>(g), g);
-  const Row3<T> yp = ld_row3<T, H>(phi, row_of<1, 0>(g), g), ym = ld_row3<T, H>(phi, row_of<-1, 0>(g), g);
-  const Row3<T> zp = ld_row3<T, H>(phi, row_of<0, 1>(g), g), zm = ld_row3<T, H>(phi, row_of<0, -1>(g), g);
-  const V ypzp = ld_pair<T, H>(phi + row_of<1, 1>(g)), ymzm = ld_pair<T, H>(phi + row_of<-1, -1>(g));
-  const V ypzm = ld_pair<T, H>(phi + row_of<1, -1>(g)), ymzp = ld_pair<T, H>(phi + row_of<-1, 1>(g));
+  const Row3<T> c = ld_row3<T, H>(phi, phi_row_of<0, 0>(g), g);
+  const Row3<T> yp = ld_row3<T, H>(phi, phi_row_of<1, 0>(g), g), ym = ld_row3<T, H>(phi, phi_row_of<-1, 0>(g), g);
+  const Row3<T> zp = ld_row3<T, H>(phi, phi_row_of<0, 1>(g), g), zm = ld_row3<T, H>(phi, phi_row_of<0, -1>(g), g);
+  const V ypzp = ld_pair<T, H>(phi + phi_row_of<1, 1>(g)), ymzm = ld_pair<T, H>(phi + phi_row_of<-1, -1>(g));
+  const V ypzm = ld_pair<T, H>(phi + phi_row_of<1, -1>(g)), ymzp = ld_pair<T, H>(phi + phi_row_of<-1, 1>(g));
   pc = c.C;
   const V d1 = c.R - pc, d2 = c.L - pc, d3 = yp.C - pc, d4 = ym.C - pc, d5 = zp.C - pc, d6 = zm.C - pc;
   const V d7 = yp.R - pc, d8 = ym.L - pc, d9 = ym.R - pc, d10 = yp.L - pc;
@@ -245,11 +276,11 @@ template <typename T> __device__ __forceinline__ bool pair_coords(const KP<T>& P
 }
 
 // phi(t+1) = sum_a g_a(x,t+1) (Eq. 38) of one node pair by pulling the post-collision g+(t).
-template <typename T, int HG, int NX> __device__ __forceinline__ void phi_pair(const FP<T>& FPp, int x0, int y, int z) {
+template <typename T, int HG, int NX, bool WALLS> __device__ __forceinline__ void phi_pair(const FP<T>& FPp, int x0, int y, int z) {
   const KP<T>& P = FPp.k;
-  const Geo geo = make_geo(P, x0, y, z);
+  const Geo geo = make_geo<T, WALLS>(P, x0, y, z);
   P2<T> g[Q];
-  Pull2All<T, HG, NX, 1>::run(P.p_src, P.nx, geo, g);
+  Pull2All<T, HG, NX, 1, WALLS>::run(P.p_src, P.nx, geo, g);
   st_pair<T>(P.phi + geo.rc, sum19(g));
 }
 
@@ -257,14 +288,14 @@ template <typename T, int HG, int NX> __device__ __forceinline__ void phi_pair(c
 // HL: hint of the population / u loads, HP: hint of the phi loads, HS: hint of the stores.  `before_phi()` runs after
 // the population loads have been issued and before phi is touched.
 struct NoWait { __device__ __forceinline__ void operator()() const {} };
-template <typename T, int HL, int HP, int HS, int NX, typename W>
+template <typename T, int HL, int HP, int HS, int NX, bool WALLS, typename W>
 __device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z, W before_phi) {
   typedef P2<T> V;
   const KP<T>& P = FPp.k;
-  const Geo geo = make_geo(P, x0, y, z);
+  const Geo geo = make_geo<T, WALLS>(P, x0, y, z);
   V f[Q], g[Q];
-  Pull2All<T, HL, NX, 0>::run(P.p_src, P.nx, geo, f);
-  Pull2All<T, HL, NX, 1>::run(P.p_src, P.nx, geo, g);
+  Pull2All<T, HL, NX, 0, WALLS>::run(P.p_src, P.nx, geo, f);
+  Pull2All<T, HL, NX, 1, WALLS>::run(P.p_src, P.nx, geo, g);
   V ux = ld_pair<T, HL>(P.u + geo.rc), uy = ld_pair<T, HL>(P.u + P.n + geo.rc), uz = ld_pair<T, HL>(P.u + 2 * P.n + geo.rc);
   before_phi();
   V phi, G[3], L;
@@ -284,15 +315,16 @@ __device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z
   Store2All<T, HS, NX, 1>::run(rd, P.nx, g);
 }
 
-template <typename T, int NX> __global__ void __launch_bounds__(256) k_phi2(const __grid_constant__ FP<T> FPp) {
+template <typename T, int NX, bool WALLS> __global__ void __launch_bounds__(256) k_phi2(const __grid_constant__ FP<T> FPp) {
   int x0, y, z;
   if (!pair_coords(FPp.k, x0, y, z)) return;
-  phi_pair<T, LD_NC, NX>(FPp, x0, y, z);
+  phi_pair<T, LD_NC, NX, WALLS>(FPp, x0, y, z);
 }
-template <typename T, int NX, int MINB> __global__ void __launch_bounds__(256, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
+template <typename T, int NX, bool WALLS, int MINB>
+__global__ void __launch_bounds__(256, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
   int x0, y, z;
   if (!pair_coords(FPp.k, x0, y, z)) return;
-  step_pair<T, LD_NC, LD_NC, ST_WB, NX>(FPp, x0, y, z, NoWait());
+  step_pair<T, LD_NC, LD_NC, ST_WB, NX, WALLS>(FPp, x0, y, z, NoWait());
 }
 
 }  // namespace clip

@@ -32,7 +32,7 @@ __device__ __forceinline__ unsigned ld_volatile_u32(const unsigned* p) {
 // smaller index (handed out earlier, hence resident or finished); a wait longer than ~0.1 s traps instead of hanging.
 // All loads of the block (g pull of plane p, f / u of plane z) are in flight before the first use; the second pull
 // of g (plane z, read two groups earlier by A) hits L2.  One barrier per block.
-template <typename T, int NX, int MINB>
+template <typename T, int NX, bool WALLS, int MINB>
 __global__ void __launch_bounds__(256, MINB) k_tick2(const __grid_constant__ FP<T> FPp, const TickP tk, const int lag) {
   typedef P2<T> V;
   const KP<T>& P = FPp.k;
@@ -51,17 +51,17 @@ __global__ void __launch_bounds__(256, MINB) k_tick2(const __grid_constant__ FP<
   V ga[Q], f[Q], g[Q], ux, uy, uz;
   Geo geo_a, geo;
   if (has_a) {
-    geo_a = make_geo(P, x0, y, pa);
-    Pull2All<T, LD_NC, NX, 1>::run(P.p_src, P.nx, geo_a, ga);
+    geo_a = make_geo<T, WALLS>(P, x0, y, pa);
+    Pull2All<T, LD_NC, NX, 1, WALLS>::run(P.p_src, P.nx, geo_a, ga);
   }
   if (has_b) {
-    geo = make_geo(P, x0, y, z);
-    Pull2All<T, LD_NC, NX, 0>::run(P.p_src, P.nx, geo, f);
+    geo = make_geo<T, WALLS>(P, x0, y, z);
+    Pull2All<T, LD_NC, NX, 0, WALLS>::run(P.p_src, P.nx, geo, f);
     ux = ld_pair<T>(P.u + geo.rc); uy = ld_pair<T>(P.u + P.n + geo.rc); uz = ld_pair<T>(P.u + 2 * P.n + geo.rc);
   }
   if (has_a) st_pair<T>(P.phi + geo_a.rc, sum19(ga));
   if (has_b) {
-    Pull2All<T, LD_NC, NX, 1>::run(P.p_src, P.nx, geo, g);
+    Pull2All<T, LD_NC, NX, 1, WALLS>::run(P.p_src, P.nx, geo, g);
     if (tid == 0) {
       unsigned spins = 0;
       while ((int)(c0 - tk.target) < 0) { __nanosleep(32); c0 = ld_volatile_u32(tk.done_a + zp); if (++spins > (1u << 21)) __trap(); }

@@ -202,3 +202,43 @@ def test_fast_paths_match_generic_kernels(precision):
     tol = 1e-12 if precision == 64 else 2e-5
     for x, y in zip(a, b):
         assert np.abs(x - y).max() <= tol * max(1.0, np.abs(x).max())
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_full_size_256_equals_tiled_64(precision):
+    """BASELINE configs[4] at the full bench size (256^3, the launch configuration bench.py times: nx-specialised
+    pair kernels, same block shape): a periodic 64^3 field tiled 4 x 4 x 4 must evolve into the tiled 64^3 solution,
+    bit for bit (every node runs the same arithmetic; only indexing, wrap-around and tiling differ) -- and the 64^3
+    solution itself is checked against the oracle element by element in test_parity[sweep64]."""
+    import torch
+    from paper_2505_12205_b200 import clip
+    small = inputs.sweep_drops(n=64)
+    steps = 20
+    ref = _gpu(small, steps, precision)
+    big = dict(small)
+    big["nx"] = big["ny"] = big["nz"] = 256
+    big["phi0"] = np.tile(small["phi0"], (4, 4, 4))
+    big["u0"] = np.tile(small["u0"], (1, 4, 4, 4))
+    sim = clip.Clip.from_case(big, precision=precision)
+    sim.step(steps)
+    phi, p, u = sim.get()
+    torch.cuda.synchronize()
+    for got, want in ((phi, ref[0]), (p, ref[1]), (u, ref[2])):
+        want_t = torch.as_tensor(np.tile(want, (1,) * (want.ndim - 3) + (4, 4, 4))).to(got.device)
+        assert torch.equal(got.double(), want_t)
+    sim.close()
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_walled_fast_paths(precision):
+    """Walls in the pair-per-thread kernels (bounce-back of either node of a pair in x, of both in y / z, edges and
+    corners, clamped phi ghosts): close to the generic thread-per-node kernels, and k_tick2 bit-identical to
+    k_phi2 + k_step2 with wall faces in every direction."""
+    for case in (inputs.walled_box(), inputs.rayleigh_taylor(L=16, W=3.0), inputs.poiseuille(nx=4, ny=32, nz=4)):
+        a = _gpu_env(case, 40, precision, CLIP_FORCE_GENERIC=1)
+        b = _gpu_env(case, 40, precision, CLIP_FAST_MODE=2)
+        c = _gpu_env(case, 40, precision, CLIP_FAST_MODE=0)
+        tol = 1e-12 if precision == 64 else 5e-5
+        for x, y, z in zip(a, b, c):
+            assert np.abs(x - y).max() <= tol * max(1.0, np.abs(x).max()), case["name"]
+            assert np.array_equal(y, z), case["name"]
