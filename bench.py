@@ -167,9 +167,13 @@ def run_ours(args):
     dtype = torch.float32 if prec == 32 else torch.float64
     word = 4 if prec == 32 else 8
     # one independent lattice per rank (replicas): seed differs per rank
-    case = inputs.sweep_drops(n=n, seed=rank_seed(rank), precision=prec)
-    nodes = n ** 3
-    sim = clip.Clip(n, n, n, case["params"], device=dev)
+    if args.workload == "rt":  # BASELINE configs[2]: Rayleigh-Taylor 128 x 512 x 128, walls in y (not the headline workload)
+        case = inputs.rayleigh_taylor(L=n // 2, precision=prec)
+    else:
+        case = inputs.sweep_drops(n=n, seed=rank_seed(rank), precision=prec)
+    nxl, nyl, nzl = case["nx"], case["ny"], case["nz"]
+    nodes = nxl * nyl * nzl
+    sim = clip.Clip(nxl, nyl, nzl, case["params"], device=dev)
     phi0_h = torch.as_tensor(case["phi0"]).to(dtype).pin_memory()
     u0_h = torch.as_tensor(case["u0"]).to(dtype).pin_memory()
     sim.init(phi0_h, u0_h)
@@ -204,9 +208,9 @@ def run_ours(args):
     dom = max(prof, key=lambda k: prof[k][0])
 
     # ---- end to end through the host-buffer call: H2D(phi0,u0) -> init -> K steps -> get -> D2H(phi,p,u)
-    out_phi = torch.empty((n, n, n), dtype=dtype).pin_memory()
-    out_p = torch.empty((n, n, n), dtype=dtype).pin_memory()
-    out_u = torch.empty((3, n, n, n), dtype=dtype).pin_memory()
+    out_phi = torch.empty((nzl, nyl, nxl), dtype=dtype).pin_memory()
+    out_p = torch.empty((nzl, nyl, nxl), dtype=dtype).pin_memory()
+    out_u = torch.empty((3, nzl, nyl, nxl), dtype=dtype).pin_memory()
     bufs = (torch.empty_like(phi0_h, device=dev), torch.empty_like(u0_h, device=dev), torch.empty_like(out_phi, device=dev),
             torch.empty_like(out_p, device=dev), torch.empty_like(out_u, device=dev))
     clip.run_host(sim, phi0_h, u0_h, 2, out_phi, out_p, out_u, bufs)  # warm-up job
@@ -228,9 +232,10 @@ def run_ours(args):
             "metric": "MLUPS", "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
-            "config": {"workload": f"BASELINE configs[4] throughput sweep at {n}^3: periodic two-phase box, 20 seeded drops, "
-                                   f"rho ratio 1000, fp{prec} (north_star target lattice)",
-                       "lattice": [n, n, n], "l2": f"state {sim.workspace_bytes / 1e9:.2f} GB >> 126 MB L2, no flush needed",
+            "config": {"workload": (f"BASELINE configs[2] Rayleigh-Taylor {nxl}x{nyl}x{nzl}, walls in y, fp{prec}" if args.workload == "rt" else
+                                    f"BASELINE configs[4] throughput sweep at {n}^3: periodic two-phase box, 20 seeded drops, "
+                                    f"rho ratio 1000, fp{prec} (north_star target lattice)"),
+                       "lattice": [nxl, nyl, nzl], "l2": f"state {sim.workspace_bytes / 1e9:.2f} GB >> 126 MB L2, no flush needed",
                        "parallelism": "independent replica per GPU" if world > 1 else "single GPU",
                        "finite_after_run": finite},
             "gpu_launches": int(launches),
@@ -264,6 +269,8 @@ def main():
     ap.add_argument("--n", type=int, default=256)
     ap.add_argument("--precision", type=int, default=32, choices=[32, 64])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--workload", default="sweep", choices=["sweep", "rt"],
+                    help="sweep = BASELINE configs[4] (headline); rt = configs[2] lattice (n/2 x 2n x n/2), walls in y")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

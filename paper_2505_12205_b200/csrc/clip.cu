@@ -168,6 +168,7 @@ void fast_shape(const clip_handle* h, dim3& grid, dim3& block) {
   const int pairs = h->nx / 2;
   int bx = 1;
   while (bx < pairs && bx < 128) bx *= 2;
+  while (bx > 32 && pairs % bx != 0) bx /= 2;  // e.g. nx = 384: 192 pairs -> 64-wide blocks, no idle threads
   const int by = h->fast_threads / bx > 0 ? h->fast_threads / bx : 1;
   block = dim3(bx, by, 1);
   grid = dim3((pairs + bx - 1) / bx, (h->ny + by - 1) / by, h->nz);
