@@ -274,6 +274,13 @@ template <typename T> __device__ __forceinline__ bool pair_coords(const KP<T>& P
   z = blockIdx.z;
   return x0 < P.nx && y < P.ny;
 }
+// Block-uniform: does any node of the block (rows y0 .. y0+rows-1 of plane z, all x) sit next to a wall face?  Blocks
+// that do not run the plain periodic code even in a lattice with walls.
+template <typename T> __device__ __forceinline__ bool block_touches_wall(const KP<T>& P, int y0, int rows, int z) {
+  return (P.bc[0] != BC_PERIODIC) || (P.bc[1] != BC_PERIODIC) ||
+         (y0 == 0 && P.bc[2] != BC_PERIODIC) || (y0 + rows >= P.ny && P.bc[3] != BC_PERIODIC) ||
+         (z == 0 && P.bc[4] != BC_PERIODIC) || (z == P.nz - 1 && P.bc[5] != BC_PERIODIC);
+}
 
 // phi(t+1) = sum_a g_a(x,t+1) (Eq. 38) of one node pair by pulling the post-collision g+(t).
 template <typename T, int HG, int NX, bool WALLS> __device__ __forceinline__ void phi_pair(const FP<T>& FPp, int x0, int y, int z) {
@@ -318,13 +325,15 @@ __device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z
 template <typename T, int NX, bool WALLS> __global__ void __launch_bounds__(256) k_phi2(const __grid_constant__ FP<T> FPp) {
   int x0, y, z;
   if (!pair_coords(FPp.k, x0, y, z)) return;
-  phi_pair<T, LD_NC, NX, WALLS>(FPp, x0, y, z);
+  if (WALLS && !block_touches_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) phi_pair<T, LD_NC, NX, false>(FPp, x0, y, z);
+  else phi_pair<T, LD_NC, NX, WALLS>(FPp, x0, y, z);
 }
 template <typename T, int NX, bool WALLS, int MINB>
 __global__ void __launch_bounds__(256, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
   int x0, y, z;
   if (!pair_coords(FPp.k, x0, y, z)) return;
-  step_pair<T, LD_NC, LD_NC, ST_WB, NX, WALLS>(FPp, x0, y, z, NoWait());
+  if (WALLS && !block_touches_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) step_pair<T, LD_NC, LD_NC, ST_WB, NX, false>(FPp, x0, y, z, NoWait());
+  else step_pair<T, LD_NC, LD_NC, ST_WB, NX, WALLS>(FPp, x0, y, z, NoWait());
 }
 
 }  // namespace clip
