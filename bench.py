@@ -169,6 +169,8 @@ def run_ours(args):
     # one independent lattice per rank (replicas): seed differs per rank
     if args.workload == "rt":  # BASELINE configs[2]: Rayleigh-Taylor 128 x 512 x 128, walls in y (not the headline workload)
         case = inputs.rayleigh_taylor(L=n // 2, precision=prec)
+    elif args.workload == "jet":  # BASELINE configs[3]: liquid jet 192 x 192 x 1536, inlet disc, convective outlet, side walls
+        case = inputs.jet(nxy=3 * n // 4, nz=6 * n, r_nozzle=12.0 * n / 256, precision=prec)
     else:
         case = inputs.sweep_drops(n=n, seed=rank_seed(rank), precision=prec)
     nxl, nyl, nzl = case["nx"], case["ny"], case["nz"]
@@ -233,6 +235,7 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
             "config": {"workload": (f"BASELINE configs[2] Rayleigh-Taylor {nxl}x{nyl}x{nzl}, walls in y, fp{prec}" if args.workload == "rt" else
+                                    f"BASELINE configs[3] liquid jet {nxl}x{nyl}x{nzl}, inlet disc + convective outlet + side walls, fp{prec}" if args.workload == "jet" else
                                     f"BASELINE configs[4] throughput sweep at {n}^3: periodic two-phase box, 20 seeded drops, "
                                     f"rho ratio 1000, fp{prec} (north_star target lattice)"),
                        "lattice": [nxl, nyl, nzl], "l2": f"state {sim.workspace_bytes / 1e9:.2f} GB >> 126 MB L2, no flush needed",
@@ -269,8 +272,8 @@ def main():
     ap.add_argument("--n", type=int, default=256)
     ap.add_argument("--precision", type=int, default=32, choices=[32, 64])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
-    ap.add_argument("--workload", default="sweep", choices=["sweep", "rt"],
-                    help="sweep = BASELINE configs[4] (headline); rt = configs[2] lattice (n/2 x 2n x n/2), walls in y")
+    ap.add_argument("--workload", default="sweep", choices=["sweep", "rt", "jet"],
+                    help="sweep = BASELINE configs[4] (headline); rt = configs[2] lattice (n/2 x 2n x n/2), walls in y; jet = configs[3] lattice (3n/4 x 3n/4 x 6n)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

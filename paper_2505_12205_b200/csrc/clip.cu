@@ -112,6 +112,7 @@ template <typename T> clip::KP<T> make_kp(const clip_handle* h) {
   P.nxy = (long long)h->nx * h->ny;
   P.any_nonperiodic = 0;
   for (int k = 0; k < 6; ++k) { P.bc[k] = p.bc[k]; if (p.bc[k] != CLIP_BC_PERIODIC) P.any_nonperiodic = 1; }
+  P.z_lo = 0; P.z_cnt = h->nz;
   P.has_inlet = p.bc[4] == CLIP_BC_INLET;
   P.has_outlet = p.bc[5] == CLIP_BC_OUTLET;
   P.visc_interp = p.visc_interp;
@@ -158,11 +159,12 @@ template <typename T> int do_init(clip_handle* h, const void* phi0, const void* 
 enum { KIND_PHI = 0, KIND_STEP = 1, KIND_PHI2 = 2, KIND_STEP2 = 3, KIND_MARCH = 4, KIND_TICK = 5, KIND_COUNT = 6 };
 const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step2", "(unused)", "k_tick2"};
 
-// The pair-per-thread fast kernels (clip_fast.cuh) cover lattices whose faces are PERIODIC or WALL, with even nx.
+// The pair-per-thread fast kernels (clip_fast.cuh) cover planes whose neighbourhood has only PERIODIC or WALL faces, even nx.
 bool fast_ok(const clip_handle* h) {
   if (h->force_generic) return false;
-  for (int k = 0; k < 6; ++k) if (h->p.bc[k] != CLIP_BC_PERIODIC && h->p.bc[k] != CLIP_BC_WALL) return false;
-  return h->nx % 2 == 0;
+  for (int k = 0; k < 4; ++k) if (h->p.bc[k] != CLIP_BC_PERIODIC && h->p.bc[k] != CLIP_BC_WALL) return false;
+  // an INLET (-z) / OUTLET (+z) face is served by the generic kernels on its own plane (hybrid launches, do_step)
+  return h->nx % 2 == 0 && h->nz >= 4;
 }
 void fast_shape(const clip_handle* h, dim3& grid, dim3& block) {
   const int pairs = h->nx / 2;
@@ -223,7 +225,8 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
   dim3 fg, fb;
   bool tick = false;
   if (fast) fast_shape(h, fg, fb);
-  if (fast && h->mode == 0 && (h->nx / 2) % fb.x == 0 && h->ny % fb.y == 0) {
+  if (fast && h->mode == 0 && h->p.bc[4] != CLIP_BC_INLET && h->p.bc[5] != CLIP_BC_OUTLET && (h->nx / 2) % fb.x == 0 &&
+      h->ny % fb.y == 0) {
     tick = true;
   }
   for (int s = 0; s < nsteps; ++s) {
@@ -248,18 +251,41 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       h->t += 1;
       continue;
     }
-    if (prof) prof->begin();
+    // planes next to an INLET / OUTLET face: generic kernels; all other planes: pair kernels (when the lattice allows)
+    const int glo = (fast && h->p.bc[4] == CLIP_BC_INLET) ? 1 : 0, ghi = (fast && h->p.bc[5] == CLIP_BC_OUTLET) ? 1 : 0;
+    clip::KP<T> Plo = P, Phi = P;
+    Plo.z_lo = 0; Plo.z_cnt = glo; Phi.z_lo = h->nz - ghi; Phi.z_cnt = ghi;
     clip::FP<T> F;
-    if (fast) F = make_fp<T>(P);
-    if (fast && walls) launch_phi2<T, true>(h->nx_special, fg, fb, h->stream, F);
-    else if (fast) launch_phi2<T, false>(h->nx_special, fg, fb, h->stream, F);
-    else clip::k_phi<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
-    if (prof) { prof->end(fast ? KIND_PHI2 : KIND_PHI); prof->begin(); }
-    if (fast && walls) launch_step2<T, true, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
-    else if (fast) launch_step2<T, false, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
-    else clip::k_step<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
-    if (prof) prof->end(fast ? KIND_STEP2 : KIND_STEP);
-    h->launches += 2;
+    if (fast) { F = make_fp<T>(P); F.k.z_lo = glo; F.k.z_cnt = h->nz - glo - ghi; fg.z = (unsigned)F.k.z_cnt; }
+    for (int pass = 0; pass < 2; ++pass) {  // pass 0: phi(t+1); pass 1: macros + collisions
+      if (prof) prof->begin();
+      if (!fast) {
+        if (pass == 0) clip::k_phi<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
+        else clip::k_step<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
+        h->launches += 1;
+        if (prof) prof->end(pass == 0 ? KIND_PHI : KIND_STEP);
+        continue;
+      }
+      if (glo) {
+        if (pass == 0) clip::k_phi<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Plo);
+        else clip::k_step<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Plo);
+        h->launches += 1;
+      }
+      if (ghi) {
+        if (pass == 0) clip::k_phi<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Phi);
+        else clip::k_step<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Phi);
+        h->launches += 1;
+      }
+      if (pass == 0) {
+        if (walls) launch_phi2<T, true>(h->nx_special, fg, fb, h->stream, F);
+        else launch_phi2<T, false>(h->nx_special, fg, fb, h->stream, F);
+      } else {
+        if (walls) launch_step2<T, true, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
+        else launch_step2<T, false, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
+      }
+      h->launches += 1;
+      if (prof) prof->end(pass == 0 ? KIND_PHI2 : KIND_STEP2);
+    }
     h->cur ^= 1;
     h->t += 1;
   }

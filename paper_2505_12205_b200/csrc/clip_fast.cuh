@@ -271,7 +271,7 @@ __device__ __forceinline__ void collide2(const KP<T>& P, const Mom2<T>& m, const
 template <typename T> __device__ __forceinline__ bool pair_coords(const KP<T>& P, int& x0, int& y, int& z) {
   x0 = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
   y = blockIdx.y * blockDim.y + threadIdx.y;
-  z = blockIdx.z;
+  z = P.z_lo + blockIdx.z;
   return x0 < P.nx && y < P.ny;
 }
 // Block-uniform: does any node of the block (rows y0 .. y0+rows-1 of plane z, all x) sit next to a wall face?  Blocks

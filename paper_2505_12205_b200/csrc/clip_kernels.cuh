@@ -52,6 +52,7 @@ template <typename T> struct KP {
   long long nxy;  // nodes per z layer
   int bc[6];
   int has_inlet, has_outlet, any_nonperiodic, visc_interp;
+  int z_lo, z_cnt;  // planes [z_lo, z_lo + z_cnt) a k_phi* / k_step* launch covers (whole lattice: 0, nz)
   T rho_h, rho_l, drho;
   T tau_h, tau_l, itau_h, itau_l;
   T beta4, kappa, inv_W, om_phi;
@@ -361,8 +362,9 @@ template <typename T> struct StoreAll<T, Q> {
 // ------------------------------------------------------------------------------------------------ kernels
 // k_phi: phi(t+1) = sum_a g_a(x,t+1)  (Eq. 38) from the post-collision g+(t); inlet nodes get phi_in.
 template <typename T> __global__ void __launch_bounds__(256) k_phi(const __grid_constant__ KP<T> P) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= P.n) return;
+  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= P.z_cnt * P.nxy) return;
+  const long long i = j + P.z_lo * P.nxy;
   const int x = (int)(i % P.nx);
   const long long r = i / P.nx;
   const int y = (int)(r % P.ny), z = (int)(r / P.ny);
@@ -376,8 +378,9 @@ template <typename T> __global__ void __launch_bounds__(256) k_phi(const __grid_
 
 // k_step: the fused stream -> BC -> macro -> collide kernel.
 template <typename T> __global__ void __launch_bounds__(256) k_step(const __grid_constant__ KP<T> P) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= P.n) return;
+  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= P.z_cnt * P.nxy) return;
+  const long long i = j + P.z_lo * P.nxy;
   const int x = (int)(i % P.nx);
   const long long r = i / P.nx;
   const int y = (int)(r % P.ny), z = (int)(r / P.ny);

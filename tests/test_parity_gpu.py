@@ -234,7 +234,8 @@ def test_walled_fast_paths(precision):
     """Walls in the pair-per-thread kernels (bounce-back of either node of a pair in x, of both in y / z, edges and
     corners, clamped phi ghosts): close to the generic thread-per-node kernels, and k_tick2 bit-identical to
     k_phi2 + k_step2 with wall faces in every direction."""
-    for case in (inputs.walled_box(), inputs.rayleigh_taylor(L=16, W=3.0), inputs.poiseuille(nx=4, ny=32, nz=4)):
+    for case in (inputs.walled_box(), inputs.rayleigh_taylor(L=16, W=3.0), inputs.poiseuille(nx=4, ny=32, nz=4),
+                 inputs.jet(nxy=24, nz=32, r_nozzle=4.0)):  # jet: inlet / outlet planes by the generic kernels (hybrid)
         a = _gpu_env(case, 40, precision, CLIP_FORCE_GENERIC=1)
         b = _gpu_env(case, 40, precision, CLIP_FAST_MODE=2)
         c = _gpu_env(case, 40, precision, CLIP_FAST_MODE=0)
