@@ -179,7 +179,7 @@ template <typename T> clip::FP<T> make_fp(const clip::KP<T>& P) { clip::FP<T> F;
 
 // nx values with their own instantiation of the fast kernels (direction offsets as immediates); others take NX = 0.
 #ifndef CLIP_NX_LIST
-#define CLIP_NX_LIST(X) X(64) X(128) X(256) X(384) X(512)
+#define CLIP_NX_LIST(X) X(64) X(128) X(192) X(256) X(384) X(512)
 #endif
 
 template <typename T, bool W> void launch_phi2(int nx, dim3 g, dim3 b, cudaStream_t st, const clip::FP<T>& F) {

@@ -277,7 +277,8 @@ template <typename T> __device__ __forceinline__ bool pair_coords(const KP<T>& P
 // Block-uniform: does any node of the block (rows y0 .. y0+rows-1 of plane z, all x) sit next to a wall face?  Blocks
 // that do not run the plain periodic code even in a lattice with walls.
 template <typename T> __device__ __forceinline__ bool block_touches_wall(const KP<T>& P, int y0, int rows, int z) {
-  return (P.bc[0] != BC_PERIODIC) || (P.bc[1] != BC_PERIODIC) ||
+  const int xb = 2 * blockIdx.x * blockDim.x;  // first node column of the block
+  return (xb == 0 && P.bc[0] != BC_PERIODIC) || (xb + 2 * (int)blockDim.x >= P.nx && P.bc[1] != BC_PERIODIC) ||
          (y0 == 0 && P.bc[2] != BC_PERIODIC) || (y0 + rows >= P.ny && P.bc[3] != BC_PERIODIC) ||
          (z == 0 && P.bc[4] != BC_PERIODIC) || (z == P.nz - 1 && P.bc[5] != BC_PERIODIC);
 }
