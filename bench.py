@@ -24,6 +24,10 @@ if ROOT not in sys.path:
 
 B_MIN_WORDS = 84  # f 19R+19W, g 19R+19W, phi 1R+1W, u 3R+3W
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
+# captures (profiles/r01_fast_256_fp32.md); reported as roofline.traffic when the run matches that configuration.
+NCU_TRAFFIC = {("k_step2", 256, 32, "sweep"): 2.821e9 + 2.698e9}
+
 
 def measured_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -244,7 +248,7 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "effective_gbs": mlups * 1e6 * B_MIN_WORDS * word / 1e9 / world,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "peak_source": peak_src,
+                         "traffic": NCU_TRAFFIC.get((dom, n, prec, args.workload)), "peak_source": peak_src,
                          "kernel": dom, "algorithmic_bytes_per_step": step_bytes,
                          "note": "achieved = 84 words/LU x nodes / (sum of the step's kernel durations, CUDA events per launch)",
                          "kernels_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},

@@ -63,6 +63,8 @@ CASES = {
     "jet_replica": (lambda: inputs.jet(nxy=24, nz=96, r_nozzle=4.0), 200),              # configs[3] replica
     "odd_box": (lambda: inputs.sweep_drops(shape=(20, 12, 36), ndrops=4, rmin=3, rmax=5), 100),
     "walled_box": (lambda: inputs.walled_box(), 100),
+    "odd_nx": (lambda: inputs.sweep_drops(shape=(21, 12, 10), ndrops=3, rmin=3, rmax=4), 60),   # generic kernels only
+    "thin_z": (lambda: inputs.sweep_drops(shape=(32, 16, 2), ndrops=2, rmin=3, rmax=4), 60),   # nz < 4: generic kernels
 }
 
 _ref_cache = {}
