@@ -35,6 +35,9 @@ enum { CLIP_OK = 0, CLIP_EINVAL = -1, CLIP_ENOMEM = -2, CLIP_ESTATE = -3, CLIP_E
  * App. B.5 (:1094-1129), only on the +z face. */
 enum { CLIP_BC_PERIODIC = 0, CLIP_BC_WALL = 1, CLIP_BC_INLET = 2, CLIP_BC_OUTLET = 3 };
 
+/* Hydrodynamic collision operator: weighted MRT (the paper's choice for 3-D, :849) or BGK. */
+enum { CLIP_COLL_WMRT = 0, CLIP_COLL_BGK = 1 };
+
 typedef struct clip_params {
   int precision;           /* 32 or 64: element type of every device array incl. user I/O */
   double rho_h, rho_l;     /* densities of the phi=1 (heavy) and phi=0 (light) fluid, Eq. 39 (:301) */
@@ -48,6 +51,7 @@ typedef struct clip_params {
   double inlet_r;          /* nozzle radius; nodes of the -z face outside the disc are WALL */
   int outlet_u_mode;       /* 0 = U_local of B.22 (:1104); 1 (U_ave) and 2 (U_max) are not implemented */
   int visc_interp;         /* 0 = linear tau, Eq. 24 (paper); 1 = harmonic (1/tau linear in phi; non-paper) */
+  int collision;           /* CLIP_COLL_WMRT (0, default): Eq. 27-28 + F_mu of Eq. 30; CLIP_COLL_BGK (1): Eq. 26 + F_mu of Eq. 29 */
 } clip_params;
 
 typedef struct clip_handle clip_t;

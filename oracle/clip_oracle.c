@@ -39,6 +39,7 @@ typedef struct clipo_params {
   double inlet_u[3], inlet_phi, inlet_c[2], inlet_r;
   int outlet_u_mode;       /* 0 = U_local only */
   int visc_interp;         /* 0: Eq. 24 linear tau; 1: harmonic (1/tau linear; non-paper) */
+  int collision;           /* 0: WMRT, Eq. 27-28, 30; 1: BGK, Eq. 26, 29 */
 } clipo_params;
 
 typedef struct clipo {
@@ -90,6 +91,14 @@ static void build_basis(clipo *h) {
 /* S-hat of Eq. 28 read as: rate s_nu on the 5 traceless second-order moments (rows 4..8), rate 1
  * on the other 14 [G2]. */
 static double S_of(int k, double s_nu) { return (k >= 4 && k <= 8) ? s_nu : 1.0; }
+
+/* Collision operator applied to r = f - feq_bar (or f - feq in the viscous force):
+ * WMRT: M^-1 S M r (Eq. 27);  BGK: r / (tau + 1/2) (Eq. 26; the same factor multiplies the stress in Eq. 29). */
+static void apply_MSM(const clipo *h, double s_nu, const double *r, double *out);
+static void apply_collision(const clipo *h, double s_nu, const double *r, double *out) {
+  if (h->p.collision == 1) { for (int a = 0; a < Q; ++a) out[a] = s_nu * r[a]; }
+  else apply_MSM(h, s_nu, r, out);
+}
 
 /* out = M^-1 S M r  (Eq. 27) */
 static void apply_MSM(const clipo *h, double s_nu, const double *r, double *out) {
@@ -173,7 +182,7 @@ static void total_force(const clipo *h, const double *f, double pstar, double ux
   double drho = h->p.rho_h - h->p.rho_l;
   double r[Q], t[Q];
   for (int a = 0; a < Q; ++a) r[a] = f[a] - (pstar * h->w[a] + (Gamma(h, a, ux, uy, uz) - h->w[a])); /* f - feq, Eq. 17 */
-  apply_MSM(h, s_nu, r, t);
+  apply_collision(h, s_nu, r, t);
   double Pi[3][3] = {{0}};
   for (int b = 0; b < Q; ++b) {
     double e[3] = {(double)EX[b], (double)EY[b], (double)EZ[b]};
@@ -209,7 +218,7 @@ static void collide_node(const clipo *h, const double *phi_field, int x, int y, 
     double feqbar = feq - 0.5 * Fa[a];
     r[a] = fin[a] - feqbar;
   }
-  apply_MSM(h, s_nu, r, t);
+  apply_collision(h, s_nu, r, t);
   for (int a = 0; a < Q; ++a) fout[a] = fin[a] - t[a] + Fa[a];
   /* phase-field collision: Eq. 33-36, tau_phi = M / c_s^2 (Eq. 37) */
   double tau_phi = 3.0 * h->p.M, om = 1.0 / (tau_phi + 0.5);

@@ -27,7 +27,7 @@ class clip_params(C.Structure):
         ("bc", C.c_int * 6),
         ("inlet_u", C.c_double * 3), ("inlet_phi", C.c_double),
         ("inlet_c", C.c_double * 2), ("inlet_r", C.c_double),
-        ("outlet_u_mode", C.c_int), ("visc_interp", C.c_int),
+        ("outlet_u_mode", C.c_int), ("visc_interp", C.c_int), ("collision", C.c_int),
     ]
 
 
@@ -42,6 +42,7 @@ def make_params(p: dict) -> clip_params:
     s.inlet_c = (C.c_double * 2)(*[float(v) for v in p["inlet_c"]])
     s.outlet_u_mode = int(p["outlet_u_mode"])
     s.visc_interp = int(p["visc_interp"])
+    s.collision = int(p.get("collision", 0))
     return s
 
 

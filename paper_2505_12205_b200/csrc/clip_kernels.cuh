@@ -51,7 +51,7 @@ template <typename T> struct KP {
   long long n;    // nodes
   long long nxy;  // nodes per z layer
   int bc[6];
-  int has_inlet, has_outlet, any_nonperiodic, visc_interp;
+  int has_inlet, has_outlet, any_nonperiodic, visc_interp, collision;
   int z_lo, z_cnt;  // planes [z_lo, z_lo + z_cnt) a k_phi* / k_step* launch covers (whole lattice: 0, nz)
   T rho_h, rho_l, drho;
   T tau_h, tau_l, itau_h, itau_l;
@@ -311,7 +311,8 @@ __device__ __forceinline__ void total_force(const KP<T>& P, const Mom<T>& m, con
   const T tr3 = (nxx + nyy + nzz) * T(1.0 / 3.0);
   D[0] = nxx - tr3; D[1] = nyy - tr3; D[2] = nzz - tr3; D[3] = nxy; D[4] = nyz; D[5] = nxz;
   const T s = mat.s_nu;
-  const T Sxx = s * D[0] + tr3, Syy = s * D[1] + tr3, Szz = s * D[2] + tr3;
+  const T trs = P.collision == 1 ? s * tr3 : tr3;  // BGK relaxes the trace at s_nu too (Eq. 29); WMRT at rate 1 (Eq. 30)
+  const T Sxx = s * D[0] + trs, Syy = s * D[1] + trs, Szz = s * D[2] + trs;
   const T Sxy = s * D[3], Syz = s * D[4], Sxz = s * D[5];
   const T cmu = -mat.tau * P.drho;
   const T cs = mat.mu - p3 * P.drho;  // F_s + F_p = (mu_phi - p* c_s^2 (rho_h - rho_l)) grad phi
@@ -344,7 +345,10 @@ __device__ __forceinline__ void collide(const KP<T>& P, const Mom<T>& m, const M
     const T eu = ex * ux + ey * uy + ez * uz;
     const T gam = T(3) * eu + T(4.5) * eu * eu - usq15;  // Gamma_a / w_a - 1
     const T eDe = ex * ex * D[0] + ey * ey * D[1] + ez * ez * D[2] + T(2) * (ex * ey * D[3] + ey * ez * D[4] + ex * ez * D[5]);
-    f[a] = cw<T>(a) * ((m.p + gam) + (ex * hx + ey * hy + ez * hz) + k * eDe);
+    if (P.collision == 1)  // BGK, Eq. 26: f+ = (1 - s) f + s feq_bar + F_a
+      f[a] = (T(1) - mat.s_nu) * f[a] + cw<T>(a) * (mat.s_nu * (m.p + gam) + (T(2) - mat.s_nu) * (ex * hx + ey * hy + ez * hz));
+    else
+      f[a] = cw<T>(a) * ((m.p + gam) + (ex * hx + ey * hy + ez * hz) + k * eDe);
     g[a] = om1 * g[a] + cw<T>(a) * (omphi * (T(1) + gam) + (ex * nx_ + ey * ny_ + ez * nz_));
   }
 }

@@ -32,10 +32,11 @@ def laplace_drop(n=32, R=8.0, W=4.0, sigma=0.01, steps=1000):
 
 
 def poiseuille_steady(ny=128, tau_a=5.0, tau_b=0.5, rho_a=1.0, rho_b=1.0, gx=1e-6, visc_interp=0, tol=1e-10,
-                      max_steps=400000, check_every=500):
+                      max_steps=400000, check_every=500, collision=0):
     """Layered Poiseuille (BASELINE configs[1] family) run until max|u(t) - u(t-1)| < tol."""
     case = inputs.poiseuille(nx=4, ny=ny, nz=4, tau_a=tau_a, tau_b=tau_b, rho_a=rho_a, rho_b=rho_b, gx=gx,
                              visc_interp=visc_interp)
+    case["params"]["collision"] = collision
     o = Oracle.from_case(case)
     du = np.inf
     while o.time < max_steps:
@@ -51,7 +52,7 @@ def poiseuille_steady(ny=128, tau_a=5.0, tau_b=0.5, rho_a=1.0, rho_b=1.0, gx=1e-
                 params=dict(ny=ny, tau_a=tau_a, tau_b=tau_b, rho_a=rho_a, rho_b=rho_b, gx=gx, visc_interp=visc_interp))
 
 
-def shear_wave(orient="xy", tau=0.8, n=64, steps=1000, A=1e-4, rho=1.0):
+def shear_wave(orient="xy", tau=0.8, n=64, steps=1000, A=1e-4, rho=1.0, collision=0):
     """P8: single-phase (phi = 1) decaying shear wave; returns the projected amplitude history.
 
     orient: "xy" u_x(y), "yz" u_y(z), "zx" u_z(x) on a 4-thick slab; "diag" u along (1,-1,0)/sqrt2 varying along
@@ -74,7 +75,7 @@ def shear_wave(orient="xy", tau=0.8, n=64, steps=1000, A=1e-4, rho=1.0):
         mode = np.sin(k0 * (x + y)); comp = np.array([1.0, -1.0, 0]) / np.sqrt(2); k2 = 2 * k0 ** 2
     for c in range(3):
         u0[c] = A * comp[c] * mode
-    p = inputs.default_params(rho_h=rho, rho_l=rho, tau_h=tau, tau_l=tau, sigma=0.0)
+    p = inputs.default_params(rho_h=rho, rho_l=rho, tau_h=tau, tau_l=tau, sigma=0.0, collision=collision)
     o = Oracle(nx, ny, nz, p)
     o.init(np.ones((nz, ny, nx)), u0)
     amp = []
@@ -127,6 +128,8 @@ JOBS = {
     "tanh_wide": (tanh_relax, dict(W0_factor=2.0)),
     "tanh_narrow": (tanh_relax, dict(W0_factor=0.5)),
     "galilean": (galilean_drift, {}),
+    "wave_diag_bgk": (shear_wave, dict(orient="diag", n=64, steps=600, tau=0.6, collision=1)),
+    "pois_rho10_bgk": (poiseuille_steady, dict(ny=64, tau_a=5.0, tau_b=0.5, rho_a=10.0, rho_b=1.0, gx=1e-7, tol=1e-12, collision=1)),
 }
 
 

@@ -41,7 +41,7 @@ def runs():
 
 
 # ------------------------------------------------------------------------------------------------ P8: viscosity
-@pytest.mark.parametrize("name", ["wave_xy", "wave_yz", "wave_zx", "wave_diag"])
+@pytest.mark.parametrize("name", ["wave_xy", "wave_yz", "wave_zx", "wave_diag", "wave_diag_bgk"])
 def test_shear_wave_decay_P8(runs, name):
     """P8: a small shear wave in a single-phase fluid decays as exp(-nu k^2 t) with nu = tau c_s^2 (Eq. 23,
     PAPER.md:209) and relaxation rate s_nu = 1/(tau + 1/2) (G3) on the 5 traceless second-order moments (G2); the
@@ -139,6 +139,18 @@ def test_poiseuille_sharp_closed_form_P6ii(runs):
         err = cf.l2_rel(r["ux"], sharp)
         print("sharp-form L2:", "harmonic" if pr["visc_interp"] else "linear", err)
         assert err < bound, (pr["visc_interp"], err)
+
+
+def test_poiseuille_density_ratio_bgk(runs):
+    """SURVEY 8(f) NEXT-1, BGK mode (Eq. 26 with the viscous force of Eq. 29): the same
+    rho* = 10, mu* = 100 Poiseuille case against the quadrature of Eq. 45 -- Eq. 29's prefactor nu / ((tau + 1/2) c_s^2)
+    is what makes the stress in F_mu the physical one when every moment relaxes at 1 / (tau + 1/2)."""
+    r = runs.get("pois_rho10_bgk")
+    assert r["du"] < 1e-12
+    rho_of, mu_of = _mu_rho(r["params"])
+    ref = cf.poiseuille_quadrature(r["phi"], rho_of, mu_of, r["params"]["gx"])
+    err = cf.l2_rel(r["ux"], ref)
+    assert err < 0.02, err
 
 
 def test_poiseuille_density_ratio_P7(runs):

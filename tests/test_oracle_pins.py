@@ -83,12 +83,13 @@ def test_moment_identities_P12():
         assert np.abs(geqb @ e - (phi * u - 0.5 * pref * nv / 3)).max() < 1e-16
 
 
-def test_viscous_force_closed_form():
+@pytest.mark.parametrize("coll", [0, 1])  # 1 = BGK: Eq. 29, every moment (the trace of Pi too) carries 1/(tau + 1/2)
+def test_viscous_force_closed_form(coll):
     """Eq. 30 with Eq. 32 evaluated through the dense M^-1 S M must equal the closed form
     F_mu = -tau (rho_h-rho_l) [s_nu dev(Pi) + tr(Pi)/3 I] grad phi, Pi = sum e e (f - feq); F_p = -p* c_s^2 grad rho
     (Eq. 21); F_s = mu_phi grad phi (Eq. 10); F_b = (rho - rho_ref) g."""
     p = inputs.default_params(rho_h=3.0, rho_l=1.0, tau_h=0.3, tau_l=0.9, sigma=0.02, W=4.0, g=(1e-4, -2e-4, 3e-4),
-                              rho_ref=0.7)
+                              rho_ref=0.7, collision=coll)
     o = Oracle(4, 4, 4, p)
     e, w = o.lattice()
     rng = np.random.default_rng(3)
@@ -101,7 +102,7 @@ def test_viscous_force_closed_form():
         f += (ps - f.sum()) * w  # keep sum f = p*
         tau = 0.9 + phi * (0.3 - 0.9); s = 1 / (tau + 0.5); rho = 1 + 2 * phi
         Pi = np.einsum("a,ai,aj->ij", f - feq, e, e)
-        S = s * (Pi - np.trace(Pi) / 3 * np.eye(3)) + np.trace(Pi) / 3 * np.eye(3)
+        S = s * Pi if coll == 1 else s * (Pi - np.trace(Pi) / 3 * np.eye(3)) + np.trace(Pi) / 3 * np.eye(3)
         beta, kappa = 12 * 0.02 / 4, 1.5 * 0.02 * 4
         mu = 4 * beta * phi * (phi - 1) * (phi - 0.5) - kappa * L
         F_expect = mu * G + (rho - 0.7) * np.array(p["g"]) - ps / 3 * 2.0 * G - tau * 2.0 * (S @ G)

@@ -55,6 +55,11 @@ def _compare(case, steps, precision, ref=None):
         assert ephi <= FP32_PHI and eu <= FP32_U
 
 
+def _with(case, **kw):
+    case["params"].update(kw)
+    return case
+
+
 CASES = {
     "drop32": (lambda: inputs.drop(), 100),                                              # BASELINE configs[0]
     "sweep64": (lambda: inputs.sweep_drops(n=64), 100),                                 # configs[4] at 64^3
@@ -63,6 +68,8 @@ CASES = {
     "jet_replica": (lambda: inputs.jet(nxy=24, nz=96, r_nozzle=4.0), 200),              # configs[3] replica
     "odd_box": (lambda: inputs.sweep_drops(shape=(20, 12, 36), ndrops=4, rmin=3, rmax=5), 100),
     "walled_box": (lambda: inputs.walled_box(), 100),
+    "drop32_bgk": (lambda: _with(inputs.drop(), collision=1), 100),                       # BGK mode
+    "jet_replica_bgk": (lambda: _with(inputs.jet(nxy=24, nz=48, r_nozzle=4.0), collision=1), 100),
     "odd_nx": (lambda: inputs.sweep_drops(shape=(21, 12, 10), ndrops=3, rmin=3, rmax=4), 60),   # generic kernels only
     "thin_z": (lambda: inputs.sweep_drops(shape=(32, 16, 2), ndrops=2, rmin=3, rmax=4), 60),   # nz < 4: generic kernels
 }
