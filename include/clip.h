@@ -52,6 +52,9 @@ typedef struct clip_params {
   int outlet_u_mode;       /* 0 = U_local of B.22 (:1104); 1 (U_ave) and 2 (U_max) are not implemented */
   int visc_interp;         /* 0 = linear tau, Eq. 24 (paper); 1 = harmonic (1/tau linear in phi; non-paper) */
   int collision;           /* CLIP_COLL_WMRT (0, default): Eq. 27-28 + F_mu of Eq. 30; CLIP_COLL_BGK (1): Eq. 26 + F_mu of Eq. 29 */
+  int phase_only;          /* 0 (default): full two-phase flow.  1: only the phase-field equation (Eq. 33) is advanced and
+                              u is prescribed by the caller (clip_set_u) -- the set-up of the interface-in-shear-flow test,
+                              PAPER.md:675-713 (Sec. 5.4); f stays 0, p is returned as 0 */
 } clip_params;
 
 typedef struct clip_handle clip_t;
@@ -73,6 +76,12 @@ int clip_init(clip_t* h, const void* d_phi0, const void* d_u0);
 
 /* Advance n >= 0 time steps (Eq. 13, 33 with all of App. B); asynchronous on the stream. */
 int clip_step(clip_t* h, int n);
+
+/* phase_only mode: prescribe the velocity field u [3][nz][ny][nx] (device) that the following collisions use; the
+ * buffer is copied asynchronously on the stream and not retained.  Because the populations are stored post-collision,
+ * the field passed before clip_step(h, 1) at time t must be u(t+1) (clip_init takes u(0)).  CLIP_ESTATE outside
+ * phase_only mode or before clip_init. */
+int clip_set_u(clip_t* h, const void* d_u);
 
 /* Write phi, the physical pressure p = p* rho c_s^2 (:189) and u at the current time into caller buffers
  * (device; any may be NULL); asynchronous on the stream. */

@@ -40,6 +40,8 @@ typedef struct clipo_params {
   int outlet_u_mode;       /* 0 = U_local only */
   int visc_interp;         /* 0: Eq. 24 linear tau; 1: harmonic (1/tau linear; non-paper) */
   int collision;           /* 0: WMRT, Eq. 27-28, 30; 1: BGK, Eq. 26, 29 */
+  int phase_only;          /* 1: only the phase-field LBE (Eq. 33) is advanced; u is prescribed (clipo_set_u), f stays 0:
+                              the set-up of the interface-in-shear-flow test, PAPER.md:675-713 (Sec. 5.4) */
 } clipo_params;
 
 typedef struct clipo {
@@ -208,18 +210,22 @@ static void collide_node(const clipo *h, const double *phi_field, int x, int y, 
   stencils(h, phi_field, x, y, z, G, &L);
   double pstar = 0.0;
   for (int a = 0; a < Q; ++a) pstar += fin[a]; /* Eq. 31a */
-  total_force(h, fin, pstar, ux, uy, uz, phi, G, L, F);
-  double rho = rho_of(h, phi), tau = tau_of(h, phi), s_nu = 1.0 / (tau + 0.5);
-  /* hydrodynamic collision: Eq. 13, 16, 17, 19, 27 */
-  double r[Q], t[Q], Fa[Q];
-  for (int a = 0; a < Q; ++a) {
-    double feq = pstar * h->w[a] + (Gamma(h, a, ux, uy, uz) - h->w[a]);
-    Fa[a] = h->w[a] * (EX[a] * F[0] + EY[a] * F[1] + EZ[a] * F[2]) / (rho * (1.0 / 3.0));
-    double feqbar = feq - 0.5 * Fa[a];
-    r[a] = fin[a] - feqbar;
+  if (h->p.phase_only) { /* prescribed u: the hydrodynamic populations are not advanced */
+    for (int a = 0; a < Q; ++a) fout[a] = fin[a];
+  } else {
+    total_force(h, fin, pstar, ux, uy, uz, phi, G, L, F);
+    double rho = rho_of(h, phi), tau = tau_of(h, phi), s_nu = 1.0 / (tau + 0.5);
+    /* hydrodynamic collision: Eq. 13, 16, 17, 19, 27 */
+    double r[Q], t[Q], Fa[Q];
+    for (int a = 0; a < Q; ++a) {
+      double feq = pstar * h->w[a] + (Gamma(h, a, ux, uy, uz) - h->w[a]);
+      Fa[a] = h->w[a] * (EX[a] * F[0] + EY[a] * F[1] + EZ[a] * F[2]) / (rho * (1.0 / 3.0));
+      double feqbar = feq - 0.5 * Fa[a];
+      r[a] = fin[a] - feqbar;
+    }
+    apply_collision(h, s_nu, r, t);
+    for (int a = 0; a < Q; ++a) fout[a] = fin[a] - t[a] + Fa[a];
   }
-  apply_collision(h, s_nu, r, t);
-  for (int a = 0; a < Q; ++a) fout[a] = fin[a] - t[a] + Fa[a];
   /* phase-field collision: Eq. 33-36, tau_phi = M / c_s^2 (Eq. 37) */
   double tau_phi = 3.0 * h->p.M, om = 1.0 / (tau_phi + 0.5);
   double nrm = sqrt(G[0] * G[0] + G[1] * G[1] + G[2] * G[2]) + 1e-32; /* [R10] */
@@ -261,6 +267,7 @@ static void macros(clipo *h) {
     for (int a = 0; a < Q; ++a) s += h->g[i * Q + a]; /* Eq. 38 */
     h->phi[i] = is_inlet_node(h, x, y, z) ? h->p.inlet_phi : s;
   }
+  if (h->p.phase_only) return; /* u stays as prescribed, p* = 0 */
   for (int z = 0; z < h->nz; ++z) for (int y = 0; y < h->ny; ++y) for (int x = 0; x < h->nx; ++x) {
     size_t i = IDX(h, x, y, z);
     const double *f = h->f + i * Q;
@@ -321,7 +328,7 @@ int clipo_init(clipo *h, const double *phi0, const double *u0) {
       double Fphi = pref * h->w[a] * (EX[a] * G[0] / nrm + EY[a] * G[1] / nrm + EZ[a] * G[2] / nrm);
       double Fa = h->w[a] * (EX[a] * F[0] + EY[a] * F[1] + EZ[a] * F[2]) / (rho * (1.0 / 3.0));
       h->g[i * Q + a] = phi * Gam - 0.5 * Fphi;
-      h->f[i * Q + a] = (Gam - h->w[a]) - 0.5 * Fa;
+      h->f[i * Q + a] = h->p.phase_only ? 0.0 : (Gam - h->w[a]) - 0.5 * Fa;
     }
     h->pstar[i] = 0.0;
   }
@@ -392,6 +399,13 @@ static void step_once(clipo *h) {
 int clipo_step(clipo *h, int n) {
   if (h->p.bc[5] == BC_OUTLET && h->nz < 2) return -1;
   for (int k = 0; k < n; ++k) step_once(h);
+  return 0;
+}
+
+/* Prescribe the velocity field used by the following collisions (phase_only mode; u = [3][n]). */
+int clipo_set_u(clipo *h, const double *u) {
+  size_t n = h->n;
+  memcpy(h->ux, u, n * 8); memcpy(h->uy, u + n, n * 8); memcpy(h->uz, u + 2 * n, n * 8);
   return 0;
 }
 

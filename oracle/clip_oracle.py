@@ -34,7 +34,7 @@ class _Params(C.Structure):
         ("bc", C.c_int * 6),
         ("inlet_u", C.c_double * 3), ("inlet_phi", C.c_double), ("inlet_c", C.c_double * 2),
         ("inlet_r", C.c_double),
-        ("outlet_u_mode", C.c_int), ("visc_interp", C.c_int), ("collision", C.c_int),
+        ("outlet_u_mode", C.c_int), ("visc_interp", C.c_int), ("collision", C.c_int), ("phase_only", C.c_int),
     ]
 
 
@@ -49,6 +49,7 @@ def _marshal(p: dict) -> _Params:
     s.outlet_u_mode = int(p["outlet_u_mode"])
     s.visc_interp = int(p["visc_interp"])
     s.collision = int(p.get("collision", 0))
+    s.phase_only = int(p.get("phase_only", 0))
     return s
 
 
@@ -65,6 +66,7 @@ def lib():
         _lib.clipo_destroy.argtypes = [C.c_void_p]
         _lib.clipo_init.argtypes = [C.c_void_p, d, d]
         _lib.clipo_step.argtypes = [C.c_void_p, C.c_int]
+        _lib.clipo_set_u.argtypes = [C.c_void_p, d]
         _lib.clipo_get.argtypes = [C.c_void_p, d, d, d]
         _lib.clipo_get_populations.argtypes = [C.c_void_p, d, d]
         _lib.clipo_set_populations.argtypes = [C.c_void_p, d, d]
@@ -117,6 +119,10 @@ class Oracle:
         phi0 = np.ascontiguousarray(phi0, dtype=np.float64).reshape(self.nz, self.ny, self.nx)
         u0 = np.ascontiguousarray(u0, dtype=np.float64).reshape(3, self.nz, self.ny, self.nx)
         lib().clipo_init(self._h, _dp(phi0), _dp(u0))
+
+    def set_u(self, u):
+        u = np.ascontiguousarray(u, dtype=np.float64).reshape(3, self.nz, self.ny, self.nx)
+        lib().clipo_set_u(self._h, _dp(u))
 
     def step(self, n: int = 1):
         if lib().clipo_step(self._h, int(n)) != 0:

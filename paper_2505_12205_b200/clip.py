@@ -27,7 +27,7 @@ class clip_params(C.Structure):
         ("bc", C.c_int * 6),
         ("inlet_u", C.c_double * 3), ("inlet_phi", C.c_double),
         ("inlet_c", C.c_double * 2), ("inlet_r", C.c_double),
-        ("outlet_u_mode", C.c_int), ("visc_interp", C.c_int), ("collision", C.c_int),
+        ("outlet_u_mode", C.c_int), ("visc_interp", C.c_int), ("collision", C.c_int), ("phase_only", C.c_int),
     ]
 
 
@@ -43,6 +43,7 @@ def make_params(p: dict) -> clip_params:
     s.outlet_u_mode = int(p["outlet_u_mode"])
     s.visc_interp = int(p["visc_interp"])
     s.collision = int(p.get("collision", 0))
+    s.phase_only = int(p.get("phase_only", 0))
     return s
 
 
@@ -66,6 +67,8 @@ def lib():
         L.clip_init.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.clip_step.restype = C.c_int
         L.clip_step.argtypes = [C.c_void_p, C.c_int]
+        L.clip_set_u.restype = C.c_int
+        L.clip_set_u.argtypes = [C.c_void_p, C.c_void_p]
         L.clip_get.restype = C.c_int
         L.clip_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.clip_destroy.restype = C.c_int
@@ -101,6 +104,10 @@ def clip_init(h, d_phi0: int, d_u0: int) -> int:
 
 def clip_step(h, n: int) -> int:
     return lib().clip_step(h, int(n))
+
+
+def clip_set_u(h, d_u: int) -> int:
+    return lib().clip_set_u(h, C.c_void_p(d_u))
 
 
 def clip_get(h, d_phi: int, d_p: int, d_u: int) -> int:
@@ -180,6 +187,13 @@ class Clip:
         with t.cuda.device(self.device), t.cuda.stream(self.stream):
             self._check(clip_init(self._h, phi0.data_ptr(), u0.data_ptr()))
             phi0.record_stream(self.stream); u0.record_stream(self.stream)
+
+    def set_u(self, u):
+        t = self.torch
+        u = u.to(device=self.device, dtype=self.dtype).contiguous().reshape(3, self.nz, self.ny, self.nx)
+        with t.cuda.device(self.device), t.cuda.stream(self.stream):
+            self._check(clip_set_u(self._h, u.data_ptr()))
+            u.record_stream(self.stream)
 
     def step(self, n=1):
         with self.torch.cuda.device(self.device):

@@ -62,6 +62,7 @@ const char* validate(int nx, int ny, int nz, const clip_params* p) {
   if (p->visc_interp == 1 && (!(p->tau_h > 0.0) || !(p->tau_l > 0.0))) return "harmonic interpolation needs tau > 0";
   if (p->visc_interp != 0 && p->visc_interp != 1) return "visc_interp must be 0 or 1";
   if (p->collision != CLIP_COLL_WMRT && p->collision != CLIP_COLL_BGK) return "collision must be CLIP_COLL_WMRT (0) or CLIP_COLL_BGK (1)";
+  if (p->phase_only != 0 && p->phase_only != 1) return "phase_only must be 0 or 1";
   if (!(3.0 * p->M + 0.5 > 0.0)) return "tau_phi + 1/2 must be positive";
   if (!(p->W > 0.0)) return "W must be positive";
   if (!std::isfinite(p->sigma)) return "sigma must be finite";
@@ -118,6 +119,7 @@ template <typename T> clip::KP<T> make_kp(const clip_handle* h) {
   P.has_outlet = p.bc[5] == CLIP_BC_OUTLET;
   P.visc_interp = p.visc_interp;
   P.collision = p.collision;
+  P.phase_only = p.phase_only;
   P.rho_h = (T)p.rho_h; P.rho_l = (T)p.rho_l; P.drho = (T)(p.rho_h - p.rho_l);
   P.tau_h = (T)p.tau_h; P.tau_l = (T)p.tau_l;
   P.itau_h = (T)(p.tau_h != 0.0 ? 1.0 / p.tau_h : 0.0); P.itau_l = (T)(p.tau_l != 0.0 ? 1.0 / p.tau_l : 0.0);
@@ -164,7 +166,7 @@ const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step
 // The pair-per-thread fast kernels (clip_fast.cuh) cover planes whose neighbourhood has only PERIODIC or WALL faces, even nx.
 bool fast_ok(const clip_handle* h) {
   if (h->force_generic) return false;
-  if (h->p.collision != CLIP_COLL_WMRT) return false;  // BGK keeps all 19 f in the collision: generic kernels only (round 1)
+  if (h->p.collision != CLIP_COLL_WMRT || h->p.phase_only) return false;  // BGK keeps all 19 f in the collision: generic kernels only (round 1)
   for (int k = 0; k < 4; ++k) if (h->p.bc[k] != CLIP_BC_PERIODIC && h->p.bc[k] != CLIP_BC_WALL) return false;
   // an INLET (-z) / OUTLET (+z) face is served by the generic kernels on its own plane (hybrid launches, do_step)
   return h->nx % 2 == 0 && h->nz >= 4;
@@ -365,6 +367,17 @@ int clip_init(clip_t* h, const void* d_phi0, const void* d_u0) {
   int rc = h->p.precision == 32 ? do_init<float>(h, d_phi0, d_u0) : do_init<double>(h, d_phi0, d_u0);
   if (rc == CLIP_OK) { h->inited = true; h->t = 0; }
   return rc;
+}
+
+int clip_set_u(clip_t* h, const void* d_u) {
+  if (!h) return CLIP_EINVAL;
+  if (!h->p.phase_only) { set_err(h->err, "clip_set_u: the handle is not in phase_only mode"); return CLIP_ESTATE; }
+  if (!h->inited) { set_err(h->err, "clip_set_u: clip_init has not been called"); return CLIP_ESTATE; }
+  if (!d_u || ((uintptr_t)d_u) % 16) { set_err(h->err, "clip_set_u: u must be a 16-byte aligned device pointer"); return CLIP_EINVAL; }
+  const size_t bytes = 3 * (size_t)h->nx * h->ny * h->nz * h->L.word;
+  cudaError_t e = cudaMemcpyAsync(h->ws + h->L.off_u, d_u, bytes, cudaMemcpyDeviceToDevice, h->stream);
+  if (e != cudaSuccess) { set_err(h->err, "clip_set_u: %s", cudaGetErrorString(e)); return CLIP_ECUDA; }
+  return CLIP_OK;
 }
 
 int clip_step(clip_t* h, int n) {

@@ -51,7 +51,7 @@ template <typename T> struct KP {
   long long n;    // nodes
   long long nxy;  // nodes per z layer
   int bc[6];
-  int has_inlet, has_outlet, any_nonperiodic, visc_interp, collision;
+  int has_inlet, has_outlet, any_nonperiodic, visc_interp, collision, phase_only;
   int z_lo, z_cnt;  // planes [z_lo, z_lo + z_cnt) a k_phi* / k_step* launch covers (whole lattice: 0, nz)
   T rho_h, rho_l, drho;
   T tau_h, tau_l, itau_h, itau_l;
@@ -326,8 +326,8 @@ __device__ __forceinline__ void total_force(const KP<T>& P, const Mom<T>& m, con
 template <typename T>
 __device__ __forceinline__ void collide(const KP<T>& P, const Mom<T>& m, const Mat<T>& mat, T phi, const T (&G)[3], T ux,
                                         T uy, T uz, T (&f)[Q], T (&g)[Q]) {
-  T F[3], D[6];
-  total_force(P, m, mat, ux, uy, uz, G, F, D);
+  T F[3] = {T(0), T(0), T(0)}, D[6] = {T(0), T(0), T(0), T(0), T(0), T(0)};
+  if (!P.phase_only) total_force(P, m, mat, ux, uy, uz, G, F, D);
   const T usq15 = T(1.5) * (ux * ux + uy * uy + uz * uz);
   const T hx = T(1.5) * F[0] * mat.inv_rho, hy = T(1.5) * F[1] * mat.inv_rho, hz = T(1.5) * F[2] * mat.inv_rho;
   const T k = T(4.5) * (T(1) - mat.s_nu);
@@ -345,7 +345,9 @@ __device__ __forceinline__ void collide(const KP<T>& P, const Mom<T>& m, const M
     const T eu = ex * ux + ey * uy + ez * uz;
     const T gam = T(3) * eu + T(4.5) * eu * eu - usq15;  // Gamma_a / w_a - 1
     const T eDe = ex * ex * D[0] + ey * ey * D[1] + ez * ez * D[2] + T(2) * (ex * ey * D[3] + ey * ez * D[4] + ex * ez * D[5]);
-    if (P.collision == 1)  // BGK, Eq. 26: f+ = (1 - s) f + s feq_bar + F_a
+    if (P.phase_only)  // prescribed u (Sec. 5.4): the hydrodynamic populations are not advanced
+      f[a] = T(0);
+    else if (P.collision == 1)  // BGK, Eq. 26: f+ = (1 - s) f + s feq_bar + F_a
       f[a] = (T(1) - mat.s_nu) * f[a] + cw<T>(a) * (mat.s_nu * (m.p + gam) + (T(2) - mat.s_nu) * (ex * hx + ey * hy + ez * hz));
     else
       f[a] = cw<T>(a) * ((m.p + gam) + (ex * hx + ey * hy + ez * hz) + k * eDe);
@@ -402,7 +404,7 @@ template <typename T> __global__ void __launch_bounds__(256) k_step(const __grid
   const Mom<T> m = moments(f);
   // macros, Alg. 3: F from (new p*, new phi, lagged u), then Eq. 31b
   T ux = P.u[i], uy = P.u[P.n + i], uz = P.u[2 * P.n + i];
-  {
+  if (!P.phase_only) {
     T F[3], D[6];
     total_force(P, m, mat, ux, uy, uz, G, F, D);
     const T h = T(0.5) * mat.inv_rho;

@@ -10,7 +10,7 @@ Layout everywhere: phi0[z, y, x] (x fastest), u0[c, z, y, x].  Node j sits at co
 
 Parameter dictionary keys (both the oracle binding and the CUDA binding marshal these into their own structs):
   precision (32|64), rho_h, rho_l, tau_h, tau_l, sigma, W, M, g (3), rho_ref, bc (6: -x,+x,-y,+y,-z,+z),
-  inlet_u (3), inlet_phi, inlet_c (2), inlet_r, outlet_u_mode, visc_interp, collision (0 WMRT, 1 BGK)
+  inlet_u (3), inlet_phi, inlet_c (2), inlet_r, outlet_u_mode, visc_interp, collision (0 WMRT, 1 BGK), phase_only (1: prescribed u)
 """
 from __future__ import annotations
 
@@ -29,7 +29,7 @@ def default_params(**kw) -> dict:
         bc=(PERIODIC,) * 6,
         inlet_u=(0.0, 0.0, 0.0), inlet_phi=1.0,
         inlet_c=(0.0, 0.0), inlet_r=0.0,
-        outlet_u_mode=0, visc_interp=0, collision=0,
+        outlet_u_mode=0, visc_interp=0, collision=0, phase_only=0,
     )
     p.update(kw)
     return p

@@ -116,6 +116,40 @@ def galilean_drift(n=24, steps=400, u0=(0.01, 0.02, 0.005)):
                 pmax=float(np.abs(p).max()), steps=steps, u0=u0)
 
 
+def shear_interface(L0=200, U0=0.04, W=3.0, Pe=600.0, center=(0.5, 0.3), period_factor=2.0):
+    """Sec. 5.4: circular interface of radius L0/5 in the reversing shear flow of Eq. 48 on a periodic
+    L0 x L0 (x 1) lattice, phase-field equation only (u prescribed), M = U0 W / Pe (Eq. 49).  The velocity carries
+    cos(pi t / T) with T = period_factor * T_f, T_f = L0 / U0 (Eq. 51): it reverses at t = T_f and the run ends at 2 T_f
+    (PAPER.md:705), which fixes period_factor = 2 (the text's bare "T" is ambiguous).
+    Returns the error of Eq. 50 and the mass drift."""
+    M = U0 * W / Pe
+    p = inputs.default_params(W=W, M=M, sigma=0.0, rho_h=1.0, rho_l=1.0, phase_only=1)
+    y, x = np.meshgrid(np.arange(L0, dtype=float), np.arange(L0, dtype=float), indexing="ij")
+    r = np.sqrt((x - center[0] * L0) ** 2 + (y - center[1] * L0) ** 2)
+    phi0 = 0.5 + 0.5 * np.tanh(2.0 * (L0 / 5.0 - r) / W)
+    Tf = L0 / U0
+    T = period_factor * Tf
+    sx, sy = np.sin(np.pi * x / L0) ** 2 * np.sin(2 * np.pi * y / L0), -np.sin(np.pi * y / L0) ** 2 * np.sin(2 * np.pi * x / L0)
+
+    def vel(t):
+        c = U0 * np.cos(np.pi * t / T)
+        return np.stack([c * sx, c * sy, np.zeros_like(sx)])[:, None]
+
+    o = Oracle(L0, L0, 1, p)
+    o.init(phi0[None], vel(0))
+    n = int(round(2 * Tf))
+    phi_half = None
+    for k in range(n):
+        o.set_u(vel(k))
+        o.step(1)
+        if k + 1 == n // 2:
+            phi_half = o.get()[0][0].copy()
+    phi = o.get()[0][0]
+    err = float(np.sqrt(((phi - phi0) ** 2).sum() / (phi0 ** 2).sum()))
+    return dict(err=err, mass=float(phi.sum() / phi0.sum() - 1.0), steps=n, L0=L0,
+                stretch=float(np.sqrt(((phi_half - phi0) ** 2).sum() / (phi0 ** 2).sum())))
+
+
 JOBS = {
     "laplace": (laplace_drop, {}),
     "pois_linear": (poiseuille_steady, dict(visc_interp=0)),

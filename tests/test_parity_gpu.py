@@ -252,3 +252,39 @@ def test_walled_fast_paths(precision):
         for x, y, z in zip(a, b, c):
             assert np.abs(x - y).max() <= tol * max(1.0, np.abs(x).max()), case["name"]
             assert np.array_equal(y, z), case["name"]
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_phase_only_prescribed_velocity(precision):
+    """phase-field equation alone with a prescribed, time-dependent velocity (the set-up of
+    PAPER.md:675-713, Sec. 5.4, at reduced size and on a 3-D slab): GPU (clip_set_u + clip_step) vs the oracle.  The
+    GPU stores post-collision populations, so it takes u(k+1) before step k+1 where the oracle takes u(k)."""
+    import torch
+    from oracle.clip_oracle import Oracle
+    from paper_2505_12205_b200 import clip
+    nx, ny, nz, U0, W = 40, 36, 3, 0.04, 3.0
+    p = inputs.default_params(W=W, M=U0 * W / 600.0, sigma=0.0, rho_h=1.0, rho_l=1.0, phase_only=1, precision=precision)
+    z, y, x = np.meshgrid(np.arange(nz, dtype=float), np.arange(ny, dtype=float), np.arange(nx, dtype=float), indexing="ij")
+    phi0 = 0.5 + 0.5 * np.tanh(2.0 * (8.0 - np.sqrt((x - 20) ** 2 + (y - 12) ** 2)) / W)
+    steps, T = 120, 200.0
+
+    def vel(t):
+        c = U0 * np.cos(np.pi * t / T)
+        return np.stack([c * np.sin(np.pi * x / nx) ** 2 * np.sin(2 * np.pi * y / ny),
+                         -c * np.sin(np.pi * y / ny) ** 2 * np.sin(2 * np.pi * x / nx), 0.01 * c * np.ones_like(x)])
+
+    o = Oracle(nx, ny, nz, p)
+    o.init(phi0, vel(0))
+    for k in range(steps):
+        o.set_u(vel(k)); o.step(1)
+    rphi = o.get()[0]
+    sim = clip.Clip(nx, ny, nz, p)
+    sim.init(torch.as_tensor(phi0), torch.as_tensor(vel(0)))
+    for k in range(steps):
+        sim.set_u(torch.as_tensor(vel(k + 1))); sim.step(1)
+    phi, pr, u = (t.double().cpu().numpy() for t in sim.get())
+    assert np.abs(pr).max() == 0.0 and np.abs(u - vel(steps)).max() < (1e-15 if precision == 64 else 1e-8)
+    err = np.abs(phi - rphi).max()
+    print(f"phase_only fp{precision}: max-abs phi {err:.2e}, moved {np.abs(rphi - phi0).max():.2f}")
+    assert err <= (FP64_ABS if precision == 64 else FP32_PHI) and np.abs(rphi - phi0).max() > 0.2
+    sim.close()
