@@ -146,7 +146,8 @@ def shear_interface(L0=200, U0=0.04, W=3.0, Pe=600.0, center=(0.5, 0.3), period_
             phi_half = o.get()[0][0].copy()
     phi = o.get()[0][0]
     err = float(np.sqrt(((phi - phi0) ** 2).sum() / (phi0 ** 2).sum()))
-    return dict(err=err, mass=float(phi.sum() / phi0.sum() - 1.0), steps=n, L0=L0,
+    return dict(err=err, mass=float(phi.sum() / phi0.sum() - 1.0), steps=n, L0=L0, s_in=float((phi0 ** 2).sum()),
+                s_out=float(((1 - phi0) ** 2).sum()),
                 stretch=float(np.sqrt(((phi_half - phi0) ** 2).sum() / (phi0 ** 2).sum())))
 
 

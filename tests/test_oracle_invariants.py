@@ -176,3 +176,14 @@ def test_outlet_recurrence_R12():
         for a0, a1 in ((f0, f1), (g0, g1)):
             assert np.abs(a1[-1] * (1 + lam) - a0[-1] - lam * a1[-2]).max() < 1e-15
     assert np.isfinite(f1).all() and np.isfinite(g1).all()
+
+
+def test_phase_only_mode():
+    """Prescribed-velocity mode (PAPER.md:675-713 set-up, small): f stays 0, p = 0, u is returned as prescribed, total
+    phi is conserved to round-off, and the reversed flow brings the interface back (Eq. 50 error small)."""
+    import sys, os
+    sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+    import oracle_jobs
+    r = oracle_jobs.shear_interface(L0=40)
+    assert abs(r["mass"]) < 1e-12
+    assert r["err"] < 0.1 and r["stretch"] > 0.5     # strongly deformed at t = T_f, restored at 2 T_f
