@@ -4,6 +4,7 @@
 #include "clip_kernels.cuh"
 #include "clip_fast.cuh"
 #include "clip_tick.cuh"
+#include "clip_fused.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -29,8 +30,63 @@ size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
   size_t word;  // 4 or 8
-  size_t off_p[2], off_phi, off_u, off_obf, off_obg, off_lam, off_mask, off_sync, total;
+  size_t off_p[2], off_phi, off_u, off_obf, off_obg, off_lam, off_mask, off_sync, off_phi2, off_part, total;
 };
+
+// Tiling of the single-pass kernel k_fused (clip_fused.cuh): tiles of `ty` rows x one z chunk; the number of tiles is
+// chosen close to (and not above) a whole number of waves of resident blocks on the 148 SMs of a B200.
+struct FusedPlan {
+  bool ok, fills_gpu;
+  int ty, ytiles, nchunks, tzmax, threads, blocks_per_sm;
+  size_t part_words, smem_bytes;
+};
+constexpr int B200_SMS = 148;
+
+
+// Resident threads per SM the k_fused instantiations are compiled for (__launch_bounds__): fp32 384 (<= 168 registers;
+// 12 warps with every load of a row in flight beat 16 warps at 128 registers, measured 17.3 vs 16.8 GLUPS at 256^3),
+// except 256-thread blocks (nx = 512 and the runtime-nx form), which keep 2 blocks; fp64 256 (255 registers).
+constexpr int fused_threads_per_sm(int precision, int block_threads) {
+  return precision == 32 ? (block_threads >= 256 ? 512 : 384) : 256;
+}
+
+FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
+  FusedPlan f{};
+  if (p->collision != CLIP_COLL_WMRT || p->phase_only) return f;
+  for (int k = 0; k < 6; ++k) if (p->bc[k] != CLIP_BC_PERIODIC && p->bc[k] != CLIP_BC_WALL) return f;
+  if (nx % 64 != 0 || nx > 512 || ny % 4 != 0 || nz < 4) return f;
+  f.ty = 4;  // small tiles leave more of the SM's L1 to the phi stencil and the shifted population loads (measured)
+  { const char* e = getenv("CLIP_FUSED_TY"); if (e && (atoi(e) == 4 || atoi(e) == 8 || atoi(e) == 16) && ny % atoi(e) == 0) f.ty = atoi(e); }
+  f.ytiles = ny / f.ty;
+  f.threads = nx / 2;
+  const int word = p->precision == 32 ? 4 : 8;
+  const int nwarps = f.threads / 32;
+  f.smem_bytes = (size_t)clip::FUSED_SLOTS * (f.ty + 2) * (nx + 2 * nwarps) * word;
+  int bps = fused_threads_per_sm(p->precision, f.threads) / f.threads;
+  if (bps > 32) bps = 32;
+  if (bps < 1) bps = 1;
+  while (bps > 1 && (f.smem_bytes + 1024) * bps > 227 * 1024) --bps;
+  if (f.smem_bytes + 1024 > 227 * 1024) return f;
+  f.blocks_per_sm = bps;
+  const long long cap = (long long)B200_SMS * bps;
+  int nchunks = 0;
+  const int max_chunks = nz / 4 > 0 ? nz / 4 : 1;
+  f.fills_gpu = (long long)f.ytiles * max_chunks >= cap;
+  for (int m = 1; m <= 64; ++m) {
+    long long c = m * cap / f.ytiles;
+    if (c < 1) continue;
+    if (c > max_chunks) { if (nchunks == 0) nchunks = max_chunks; break; }
+    nchunks = (int)c;
+    if ((nz + nchunks - 1) / nchunks <= 16) break;
+  }
+  if (nchunks < 1) nchunks = 1;
+  { const char* e = getenv("CLIP_FUSED_CHUNKS"); if (e && atoi(e) >= 1 && atoi(e) <= nz) nchunks = atoi(e); }
+  f.nchunks = nchunks;
+  f.tzmax = (nz + nchunks - 1) / nchunks;
+  f.part_words = (size_t)f.ytiles * nchunks * (2 * f.tzmax + 2 * (f.ty + 2)) * nx;
+  f.ok = true;
+  return f;
+}
 
 Layout make_layout(int nx, int ny, int nz, const clip_params* p) {
   Layout L{};
@@ -47,6 +103,9 @@ Layout make_layout(int nx, int ny, int nz, const clip_params* p) {
   L.off_lam = take(outlet ? nxy * L.word : 0);
   L.off_mask = take(inlet ? nxy : 0);
   L.off_sync = take(((size_t)nz + 64) * sizeof(unsigned));  // k_tick: ticket counter + per-plane counters
+  const FusedPlan fp = fused_plan(nx, ny, nz, p);                // k_fused: second phi buffer + tile-halo partial sums
+  L.off_phi2 = take(fp.ok ? n * L.word : 0);
+  L.off_part = take(fp.ok ? fp.part_words * L.word : 0);
   L.total = o;
   return L;
 }
@@ -89,11 +148,15 @@ struct clip_handle {
   char* ws;
   cudaStream_t stream;
   int cur;      // which of the A/B population buffers holds the current post-collision state
+  int phi_cur;  // which phi buffer holds phi(t) (flips only on the k_fused path)
+  bool phi_ahead;  // k_fused path: the other phi buffer already holds phi(t+1)
+  FusedPlan fplan;
   bool inited;
-  int mode;            // fast-path variant (CLIP_FAST_MODE): 0 = k_tick2 (one launch), 2 = k_phi2 + k_step2
+  int mode;            // fast-path variant (CLIP_FAST_MODE): unset = automatic (k_fused + k_fix on wide lattices, else k_phi2 + k_step2);
+                       // 3 = k_fused wherever the lattice allows; 2 = k_phi2 + k_step2; 0 = k_tick2 (one launch)
   unsigned epoch;      // steps since clip_init (k_tick counters)
   int tick_order;      // CLIP_TICK_ORDER (default 0): 0 = item number from blockIdx, 1 = from an atomic ticket
-  int fast_threads;    // threads per block of the pair kernels (CLIP_FAST_THREADS: 128 or 256; default 256 for fp32, 128 for fp64)
+  int fast_threads;    // threads per block of the pair kernels (128)
   int nx_special;      // nx, or 0 when CLIP_NO_NX_SPECIAL=1 forces the runtime-nx kernels (tests)
   int tick_lag;        // CLIP_TICK_LAG (default 4, >= 3): groups between the phi job and the collision job of a plane (k_tick2)
   int tick_hint;       // CLIP_TICK_HINT (default 1): streaming cache hints on single-use loads and on stores
@@ -132,7 +195,7 @@ template <typename T> clip::KP<T> make_kp(const clip_handle* h) {
   P.phi_in = (T)p.inlet_phi;
   char* ws = h->ws;
   P.p_src = (const T*)(ws + h->L.off_p[h->cur]); P.p_dst = (T*)(ws + h->L.off_p[h->cur ^ 1]);
-  P.phi = (T*)(ws + h->L.off_phi); P.u = (T*)(ws + h->L.off_u);
+  P.phi = (T*)(ws + (h->phi_cur ? h->L.off_phi2 : h->L.off_phi)); P.u = (T*)(ws + h->L.off_u);
   P.ob_f = (T*)(ws + h->L.off_obf); P.ob_g = (T*)(ws + h->L.off_obg); P.lam = (T*)(ws + h->L.off_lam);
   P.mask = (const uint8_t*)(ws + h->L.off_mask);
   return P;
@@ -152,6 +215,7 @@ unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / 
 template <typename T> int do_init(clip_handle* h, const void* phi0, const void* u0) {
   cudaMemsetAsync(h->ws + h->L.off_sync, 0, ((size_t)h->nz + 64) * sizeof(unsigned), h->stream);
   h->epoch = 0;
+  h->phi_cur = 0; h->phi_ahead = false;
   h->cur = 1;  // k_init writes into "dst"; flip afterwards so that it becomes the current state
   clip::KP<T> P = make_kp<T>(h);
   clip::k_init<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P, (const T*)phi0, (const T*)u0);
@@ -160,8 +224,8 @@ template <typename T> int do_init(clip_handle* h, const void* phi0, const void* 
   return check_cuda(h, "k_init");
 }
 
-enum { KIND_PHI = 0, KIND_STEP = 1, KIND_PHI2 = 2, KIND_STEP2 = 3, KIND_MARCH = 4, KIND_TICK = 5, KIND_COUNT = 6 };
-const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step2", "(unused)", "k_tick2"};
+enum { KIND_PHI = 0, KIND_STEP = 1, KIND_PHI2 = 2, KIND_STEP2 = 3, KIND_FIX = 4, KIND_TICK = 5, KIND_FUSED = 6, KIND_COUNT = 7 };
+const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step2", "k_fix", "k_tick2", "k_fused"};
 
 // The pair-per-thread fast kernels (clip_fast.cuh) cover planes whose neighbourhood has only PERIODIC or WALL faces, even nx.
 bool fast_ok(const clip_handle* h) {
@@ -212,8 +276,28 @@ void launch_tick2(int nx, unsigned items, dim3 b, cudaStream_t st, const clip::F
     default: clip::k_tick2<T, 0, W, MB><<<items, b, 0, st>>>(F, tk, lag);
   }
 }
-template <typename T> struct StepMinBlocks { static constexpr int value = 2; };
+template <typename T> struct StepMinBlocks { static constexpr int value = 3; };  // k_step2 (128-thread blocks)
 template <> struct StepMinBlocks<double> { static constexpr int value = 1; };
+template <typename T> struct TickMinBlocks { static constexpr int value = 2; };  // k_tick2 (__launch_bounds__(256, .))
+template <> struct TickMinBlocks<double> { static constexpr int value = 1; };
+
+template <typename T, int NX, bool W> void launch_fused_nx(dim3 g, dim3 b, size_t smem, cudaStream_t st, const clip::FP<T>& F, const clip::FusedP<T>& U) {
+  constexpr int MAXT = NX ? NX / 2 : 256;
+  constexpr int TPSM = fused_threads_per_sm(sizeof(T) == 4 ? 32 : 64, MAXT);
+  constexpr int MINB = TPSM / MAXT > 0 ? TPSM / MAXT : 1;
+  auto kern = clip::k_fused<T, NX, W, MAXT, MINB>;
+  static bool attr_done = false;  // per instantiation
+  if (!attr_done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024); attr_done = true; }
+  kern<<<g, b, smem, st>>>(F, U);
+}
+template <typename T, bool W> void launch_fused(int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const clip::FP<T>& F, const clip::FusedP<T>& U) {
+  switch (nx) {
+#define X(N) case N: launch_fused_nx<T, N, W>(g, b, smem, st, F, U); break;
+    CLIP_NX_LIST(X)
+#undef X
+    default: launch_fused_nx<T, 0, W>(g, b, smem, st, F, U);
+  }
+}
 
 struct Prof {  // optional per-launch event timing (clip_step_profiled)
   std::vector<cudaEvent_t> ev;
@@ -234,8 +318,43 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       h->ny % fb.y == 0) {
     tick = true;
   }
+  // k_fused pays on wide lattices with enough tiles to fill the GPU (measured: +4 .. +11 % at nx >= 256, slower at nx <= 128)
+  const bool fused = fast && h->fplan.ok && (h->mode == 3 || (h->mode < 0 && h->nx >= 256 && h->fplan.fills_gpu));
   for (int s = 0; s < nsteps; ++s) {
     clip::KP<T> P = make_kp<T>(h);
+    if (fused) {  // one pass over f and g (clip_fused.cuh) + the tile-surface fix-up of phi(t+2)
+      // State between fused steps: populations f+(t), g+(t); phi buffer `phi_cur` = phi(t) (what clip_get returns), the
+      // other buffer = phi(t+1) = sum_a g+_a(x - e_a, t), which the collision at t+1 needs (first step: one k_phi2).
+      const FusedPlan& fp = h->fplan;
+      clip::FP<T> F = make_fp<T>(P);
+      T* const phi_now = (T*)(h->ws + (h->phi_cur ? h->L.off_phi2 : h->L.off_phi));
+      T* const phi_next = (T*)(h->ws + (h->phi_cur ? h->L.off_phi : h->L.off_phi2));
+      F.k.phi = phi_next;
+      if (!h->phi_ahead) {
+        if (prof) prof->begin();
+        if (walls) launch_phi2<T, true>(h->nx_special, fg, fb, h->stream, F);
+        else launch_phi2<T, false>(h->nx_special, fg, fb, h->stream, F);
+        if (prof) prof->end(KIND_PHI2);
+        h->launches += 1;
+        h->phi_ahead = true;
+      }
+      clip::FusedP<T> U;
+      U.phi_dst = phi_now;  // becomes phi(t+2); phi(t) is no longer needed once the time is t+1
+      U.part = (T*)(h->ws + h->L.off_part);
+      U.ty = fp.ty; U.ytiles = fp.ytiles; U.nchunks = fp.nchunks; U.tzmax = fp.tzmax;
+      U.tile_stride = (long long)(2 * fp.tzmax + 2 * (fp.ty + 2)) * h->nx;
+      if (prof) prof->begin();
+      if (walls) launch_fused<T, true>(h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+      else launch_fused<T, false>(h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+      if (prof) { prof->end(KIND_FUSED); prof->begin(); }
+      clip::k_fix<T><<<dim3(fp.ytiles, fp.nchunks, (2 * fp.tzmax + 2 * (fp.ty - 2) + clip::FIX_ROWS - 1) / clip::FIX_ROWS), 128, 0, h->stream>>>(F, U);
+      if (prof) prof->end(KIND_FIX);
+      h->launches += 2;
+      h->cur ^= 1;
+      h->phi_cur ^= 1;
+      h->t += 1;
+      continue;
+    }
     if (tick) {
       clip::FP<T> F = make_fp<T>(P);
       h->epoch += 1;
@@ -248,8 +367,8 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       tk.base = 0;
       tk.target = (unsigned)tk.tp * h->epoch;
       if (prof) prof->begin();
-      if (walls) launch_tick2<T, true, StepMinBlocks<T>::value>(h->nx_special, items, fb, h->stream, F, tk, (int)lag);
-      else launch_tick2<T, false, StepMinBlocks<T>::value>(h->nx_special, items, fb, h->stream, F, tk, (int)lag);
+      if (walls) launch_tick2<T, true, TickMinBlocks<T>::value>(h->nx_special, items, fb, h->stream, F, tk, (int)lag);
+      else launch_tick2<T, false, TickMinBlocks<T>::value>(h->nx_special, items, fb, h->stream, F, tk, (int)lag);
       if (prof) prof->end(KIND_TICK);
       h->launches += 1;
       h->cur ^= 1;
@@ -330,14 +449,12 @@ int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params,
   clip_handle* h = new (std::nothrow) clip_handle();
   if (!h) { set_err(g_create_error, "clip_create: out of host memory"); return CLIP_ENOMEM; }
   h->nx = nx; h->ny = ny; h->nz = nz; h->p = *params; h->L = L; h->ws = (char*)d_workspace;
-  h->stream = (cudaStream_t)cuda_stream; h->cur = 0; h->inited = false;
+  h->stream = (cudaStream_t)cuda_stream; h->cur = 0; h->phi_cur = 0; h->phi_ahead = false; h->inited = false;
+  h->fplan = fused_plan(nx, ny, nz, params);
   { const char* e = getenv("CLIP_FORCE_GENERIC"); h->force_generic = e && e[0] == '1'; }
-  { const char* e = getenv("CLIP_FAST_MODE"); h->mode = e ? atoi(e) : 2; h->epoch = 0; }
+  { const char* e = getenv("CLIP_FAST_MODE"); h->mode = e ? atoi(e) : -1; h->epoch = 0; }
   { const char* e = getenv("CLIP_TICK_ORDER"); h->tick_order = e ? atoi(e) : 0; }
-  {  // fp64 holds a node pair in ~250 registers: 128-thread blocks schedule better there (measured 8.2 vs 7.6 GLUPS)
-    const char* e = getenv("CLIP_FAST_THREADS");
-    h->fast_threads = e ? (atoi(e) == 128 ? 128 : 256) : (params->precision == 64 ? 128 : 256);
-  }
+  h->fast_threads = 128;  // measured: fp64 8.2 vs 7.6 GLUPS, fp32 (with 3 blocks per SM) +2 % against 256-thread blocks
   { const char* e = getenv("CLIP_NO_NX_SPECIAL"); h->nx_special = (e && e[0] == '1') ? 0 : nx; }
   { const char* e = getenv("CLIP_TICK_LAG"); h->tick_lag = e ? atoi(e) : 4; if (h->tick_lag < 3) h->tick_lag = 3; }
   { const char* e = getenv("CLIP_TICK_HINT"); h->tick_hint = e ? atoi(e) : 1; }

@@ -9,6 +9,12 @@
 #include "clip_kernels.cuh"
 #include "clip_pack.cuh"
 
+// Compiler-level fence between the two load rounds of step_pair (keeps nvcc from hoisting part of round 2 into round 1
+// and splitting round 1 instead; no instruction is emitted).
+#ifndef CLIP_LOAD_FENCE
+#define CLIP_LOAD_FENCE() asm volatile("" ::: "memory")
+#endif
+
 namespace clip {
 
 // Kernel parameters of the fast kernels (kept as a separate type so that their signatures differ from the generic ones).
@@ -210,29 +216,34 @@ __device__ __forceinline__ void total_force2(const KP<T>& P, const Mom2<T>& m, c
   F[2] = fma2(cs, G[2], fma2(rb, V(P.gz), cmu * fma2(Sxz, G[0], fma2(Syz, G[1], Szz * G[2]))));
 }
 
-// One opposite pair (a, a+1) of both collisions.  eu = e_a.u, eDe = e_a^T D e_a, ev = e_a.(3u + h), em = e_a.mvec.
+// One opposite pair (a, a+1) of the two collisions.  eu = e_a.u, eDe = e_a^T D e_a, ev = e_a.(3u + h), em = e_a.mvec.
+// The f half and the g half are separate so that g can still be in flight while f+ is computed and stored (step_pair).
 template <typename T>
 struct Coll2 {
   typedef P2<T> V;
   V p, c0, k, omphi, om1;  // p*, -1.5 u.u, 4.5 (1 - s_nu), w_phi phi, 1 - w_phi
-  template <int a>
-  __device__ __forceinline__ void pair(V eu, V eDe, V ev, V em, V (&f)[Q], V (&g)[Q]) const {
+  __device__ __forceinline__ V q(V eu) const { return fma2(eu * V(T(4.5)), eu, c0); }  // Gamma_a/w_a - 1 - 3 e.u
+  template <int a> __device__ __forceinline__ void pair_f(V eu, V eDe, V ev, V (&f)[Q]) const {
     const V w(cw<T>(a));
-    const V q = fma2(eu * V(T(4.5)), eu, c0);  // Gamma_a/w_a - 1 - 3 e.u
-    const V A = fma2(k, eDe, p + q);
+    const V A = fma2(k, eDe, p + q(eu));
     f[a] = w * (A + ev);
     f[a + 1] = w * (A - ev);
-    const V C = fma2(omphi, q, omphi);
+  }
+  template <int a> __device__ __forceinline__ void pair_g(V eu, V em, V (&g)[Q]) const {
+    const V w(cw<T>(a));
+    const V C = fma2(omphi, q(eu), omphi);
     g[a] = fma2(om1, g[a], w * (C + em));
     g[a + 1] = fma2(om1, g[a + 1], w * (C - em));
   }
 };
+// what the g collision needs from the f collision of the same node pair
+template <typename T> struct GCtx { Coll2<T> c; P2<T> ux, uy, uz, mx, my, mz, usq15; };
 
-// Both collisions (Alg. 1) of a node pair: g in/out in place, f+ out (a function of the moments only, because the
-// 14 non-shear moments relax at rate 1, G2).
+// f collision (Alg. 1) of a node pair: f+ out (a function of the moments only, because the 14 non-shear moments relax at
+// rate 1, G2); fills the context of the g collision.
 template <typename T>
-__device__ __forceinline__ void collide2(const KP<T>& P, const Mom2<T>& m, const Mat2<T>& mat, P2<T> phi, const P2<T> (&G)[3],
-                                         P2<T> ux, P2<T> uy, P2<T> uz, P2<T> (&f)[Q], P2<T> (&g)[Q]) {
+__device__ __forceinline__ void collide2_f(const KP<T>& P, const Mom2<T>& m, const Mat2<T>& mat, P2<T> phi, const P2<T> (&G)[3],
+                                           P2<T> ux, P2<T> uy, P2<T> uz, P2<T> (&f)[Q], GCtx<T>& x) {
   typedef P2<T> V;
   V F[3], D[6];
   total_force2(P, m, mat, ux, uy, uz, G, F, D);
@@ -245,25 +256,47 @@ __device__ __forceinline__ void collide2(const KP<T>& P, const Mom2<T>& m, const
   const V ph = phi - V(T(0.5));
   const V pref = fma2(V(T(-4)) * ph, ph, V(T(1))) * V(P.inv_W);
   const V cn = (V(T(1) - T(0.5) * P.om_phi) * pref) * rcp2(gn);
-  Coll2<T> c;
+  Coll2<T>& c = x.c;
   c.p = m.p; c.c0 = -usq15; c.k = V(T(4.5)) * (V(T(1)) - mat.s_nu);
   c.omphi = V(P.om_phi) * phi; c.om1 = V(T(1) - P.om_phi);
   const V o3 = V(T(3)) * c.omphi;
-  const V mx = fma2(o3, ux, cn * G[0]), my = fma2(o3, uy, cn * G[1]), mz = fma2(o3, uz, cn * G[2]);
-  // rest direction
+  x.mx = fma2(o3, ux, cn * G[0]); x.my = fma2(o3, uy, cn * G[1]); x.mz = fma2(o3, uz, cn * G[2]);
+  x.ux = ux; x.uy = uy; x.uz = uz; x.usq15 = usq15;
   f[0] = V(cw<T>(0)) * (m.p - usq15);
-  g[0] = fma2(c.om1, g[0], V(cw<T>(0)) * (c.omphi - c.omphi * usq15));
   const V Dxy2 = D[3] + D[3], Dyz2 = D[4] + D[4], Dxz2 = D[5] + D[5];
   const V sxy = D[0] + D[1], sxz = D[0] + D[2], syz = D[1] + D[2];
-  c.template pair<1>(ux, D[0], vx, mx, f, g);
-  c.template pair<3>(uy, D[1], vy, my, f, g);
-  c.template pair<5>(uz, D[2], vz, mz, f, g);
-  c.template pair<7>(ux + uy, sxy + Dxy2, vx + vy, mx + my, f, g);
-  c.template pair<9>(ux - uy, sxy - Dxy2, vx - vy, mx - my, f, g);
-  c.template pair<11>(ux + uz, sxz + Dxz2, vx + vz, mx + mz, f, g);
-  c.template pair<13>(ux - uz, sxz - Dxz2, vx - vz, mx - mz, f, g);
-  c.template pair<15>(uy + uz, syz + Dyz2, vy + vz, my + mz, f, g);
-  c.template pair<17>(uy - uz, syz - Dyz2, vy - vz, my - mz, f, g);
+  c.template pair_f<1>(ux, D[0], vx, f);
+  c.template pair_f<3>(uy, D[1], vy, f);
+  c.template pair_f<5>(uz, D[2], vz, f);
+  c.template pair_f<7>(ux + uy, sxy + Dxy2, vx + vy, f);
+  c.template pair_f<9>(ux - uy, sxy - Dxy2, vx - vy, f);
+  c.template pair_f<11>(ux + uz, sxz + Dxz2, vx + vz, f);
+  c.template pair_f<13>(ux - uz, sxz - Dxz2, vx - vz, f);
+  c.template pair_f<15>(uy + uz, syz + Dyz2, vy + vz, f);
+  c.template pair_f<17>(uy - uz, syz - Dyz2, vy - vz, f);
+}
+// g collision (Eq. 33-36): g in/out in place
+template <typename T> __device__ __forceinline__ void collide2_g(const GCtx<T>& x, P2<T> (&g)[Q]) {
+  typedef P2<T> V;
+  const Coll2<T>& c = x.c;
+  g[0] = fma2(c.om1, g[0], V(cw<T>(0)) * (c.omphi - c.omphi * x.usq15));
+  c.template pair_g<1>(x.ux, x.mx, g);
+  c.template pair_g<3>(x.uy, x.my, g);
+  c.template pair_g<5>(x.uz, x.mz, g);
+  c.template pair_g<7>(x.ux + x.uy, x.mx + x.my, g);
+  c.template pair_g<9>(x.ux - x.uy, x.mx - x.my, g);
+  c.template pair_g<11>(x.ux + x.uz, x.mx + x.mz, g);
+  c.template pair_g<13>(x.ux - x.uz, x.mx - x.mz, g);
+  c.template pair_g<15>(x.uy + x.uz, x.my + x.mz, g);
+  c.template pair_g<17>(x.uy - x.uz, x.my - x.mz, g);
+}
+
+template <typename T>
+__device__ __forceinline__ void collide2(const KP<T>& P, const Mom2<T>& m, const Mat2<T>& mat, P2<T> phi, const P2<T> (&G)[3],
+                                         P2<T> ux, P2<T> uy, P2<T> uz, P2<T> (&f)[Q], P2<T> (&g)[Q]) {
+  GCtx<T> gx;
+  collide2_f<T>(P, m, mat, phi, G, ux, uy, uz, f, gx);
+  collide2_g<T>(gx, g);
 }
 
 // ------------------------------------------------------------------------------------------------ kernels
@@ -294,21 +327,27 @@ template <typename T, int HG, int NX, bool WALLS> __device__ __forceinline__ voi
 
 // One node pair of the step: pull f+, g+ -> macros (Alg. 3) -> both collisions (Alg. 1) -> store f+, g+, u.
 // HL: hint of the population / u loads, HP: hint of the phi loads, HS: hint of the stores.  `before_phi()` runs after
-// the population loads have been issued and before phi is touched.
+// the f loads have been issued and before phi is touched.
+// `after(geo, g)` runs last with the post-collision g+ of the pair (the fused kernel accumulates phi(t+1) from it).
+// Load schedule (128 registers hold about 75 loaded values, not all 110): round 1 = f, u, phi stencil; the g loads are
+// issued as soon as f has been reduced to its 10 moments and phi to (grad, laplacian), and stay in flight while the
+// macros and f+ are computed and stored.
 struct NoWait { __device__ __forceinline__ void operator()() const {} };
-template <typename T, int HL, int HP, int HS, int NX, bool WALLS, typename W>
-__device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z, W before_phi) {
+struct NoAfter { template <typename T> __device__ __forceinline__ void operator()(const Geo&, const P2<T> (&)[Q]) const {} };
+template <typename T, int HL, int HP, int HS, int NX, bool WALLS, typename W, typename A = NoAfter>
+__device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z, W before_phi, A after = A()) {
   typedef P2<T> V;
   const KP<T>& P = FPp.k;
   const Geo geo = make_geo<T, WALLS>(P, x0, y, z);
   V f[Q], g[Q];
   Pull2All<T, HL, NX, 0, WALLS>::run(P.p_src, P.nx, geo, f);
-  Pull2All<T, HL, NX, 1, WALLS>::run(P.p_src, P.nx, geo, g);
   V ux = ld_pair<T, HL>(P.u + geo.rc), uy = ld_pair<T, HL>(P.u + P.n + geo.rc), uz = ld_pair<T, HL>(P.u + 2 * P.n + geo.rc);
   before_phi();
   V phi, G[3], L;
   stencil2<T, HP>(P.phi, geo, phi, G, L);
   const Mom2<T> m = moments2<T>(f);
+  CLIP_LOAD_FENCE();
+  Pull2All<T, HL, NX, 1, WALLS>::run(P.p_src, P.nx, geo, g);
   const Mat2<T> mat = materials2<T>(P, phi, L);
   {  // macros, Alg. 3: F from (new p*, new phi, lagged u, R13), then Eq. 31b
     V F[3], D[6];
@@ -317,10 +356,13 @@ __device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z
     ux = fma2(h, F[0], m.mx); uy = fma2(h, F[1], m.my); uz = fma2(h, F[2], m.mz);
   }
   st_pair<T, HS>(P.u + geo.rc, ux); st_pair<T, HS>(P.u + P.n + geo.rc, uy); st_pair<T, HS>(P.u + 2 * P.n + geo.rc, uz);
-  collide2<T>(P, m, mat, phi, G, ux, uy, uz, f, g);
+  GCtx<T> gx;
+  collide2_f<T>(P, m, mat, phi, G, ux, uy, uz, f, gx);
   T* const rd = const_cast<T*>(pop_row<T, 0, 0>(P.p_dst, geo));
   Store2All<T, HS, NX, 0>::run(rd, P.nx, f);
+  collide2_g<T>(gx, g);
   Store2All<T, HS, NX, 1>::run(rd, P.nx, g);
+  after(geo, g);
 }
 
 template <typename T, int NX, bool WALLS> __global__ void __launch_bounds__(256) k_phi2(const __grid_constant__ FP<T> FPp) {
@@ -329,8 +371,10 @@ template <typename T, int NX, bool WALLS> __global__ void __launch_bounds__(256)
   if (WALLS && !block_touches_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) phi_pair<T, LD_NC, NX, false>(FPp, x0, y, z);
   else phi_pair<T, LD_NC, NX, WALLS>(FPp, x0, y, z);
 }
+// 128-thread blocks; fp32: 3 blocks per SM (<= 168 registers: all ~100 loads of a node pair in flight at once, measured
+// faster than 4 blocks at 128 registers), fp64: what 255 registers allow.
 template <typename T, int NX, bool WALLS, int MINB>
-__global__ void __launch_bounds__(256, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
+__global__ void __launch_bounds__(128, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
   int x0, y, z;
   if (!pair_coords(FPp.k, x0, y, z)) return;
   if (WALLS && !block_touches_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) step_pair<T, LD_NC, LD_NC, ST_WB, NX, false>(FPp, x0, y, z, NoWait());

@@ -1,0 +1,253 @@
+// clip_fused.cuh -- the whole step as ONE pass over f and g ("D4" of DESIGN.md): k_fused = step_pair of clip_fast.cuh
+// plus phi(t+1) = sum_a g+_a(x - e_a, t) (Eq. 38 after streaming, B.4 :990) accumulated ON CHIP from
+// the post-collision g+ the block has just computed, so g is never read a second time.
+//
+// A block owns a TILE: all x of `ty` consecutive lattice rows, planes z0 .. z1-1 (chunk c of the z axis), and walks
+// it row by row (one thread = one node pair of the row, as in k_step2).  Source node x' sends g+_a(x') to node
+// x' + e_a: 9 target rows (dy, dz); within a target row the three directions (0, +x, -x) are combined by warp
+// shuffles, so every thread only ever adds into ITS OWN column pair of a shared-memory ring of 4 planes x (ty+2)
+// rows -- no atomics, no per-row barrier (warp edges: lanes 0 / 31 keep private edge accumulators that the
+// neighbouring warp's edge lane adds when the plane is flushed).  A ring plane is complete (as far as this tile is
+// concerned) once the next plane has been processed; it is then flushed:
+//   rows inside the tile            -> phi_dst (own sum; complete for rows not on the tile surface)
+//   rows y0-1, y0+ty and the planes z0-1, z1 (the tile's halo) -> `part`, a per-tile partial-sum buffer
+// k_fix then adds, in a fixed order, the <= 5 neighbour partials to every row on a tile surface.  Deterministic
+// (no floating-point atomics); summation ORDER differs from k_phi2's sum19, so the fields agree with the two-kernel
+// path to round-off, not bit for bit (G21).
+//
+// Walls (halfway bounce-back, B.10-B.11 :1034-1037): a link that would leave through a wall face returns to the
+// sending node as the opposite population, i.e. its g+ lands on the sender's own row and column.
+#pragma once
+#include "clip_fast.cuh"
+
+namespace clip {
+
+constexpr int FUSED_SLOTS = 4;  // ring planes of k_fused: z-1, z, z+1 and the one being flushed
+
+template <typename T> struct FusedP {
+  T* phi_dst;             // phi(t+1)                         [nz][ny][nx]
+  T* part;                // partial sums of the tile halos   [tiles][2 tzmax + 2 (ty + 2)][nx]
+  int ty, ytiles, nchunks, tzmax;
+  long long tile_stride;  // elements of `part` per tile
+};
+__host__ __device__ __forceinline__ int chunk_z0(int c, int nz, int nchunks) { return (int)((long long)c * nz / nchunks); }
+// rows of a tile's slab in `part`
+__host__ __device__ __forceinline__ int slot_ym(int k) { return k; }
+__host__ __device__ __forceinline__ int slot_yp(int k, int tzmax) { return tzmax + k; }
+__host__ __device__ __forceinline__ int slot_zm(int j, int tzmax) { return 2 * tzmax + j; }
+__host__ __device__ __forceinline__ int slot_zp(int j, int tzmax, int ty) { return 2 * tzmax + ty + 2 + j; }
+
+template <typename T> __device__ __forceinline__ T shfl_up1(T v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+template <typename T> __device__ __forceinline__ T shfl_dn1(T v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+
+// Accumulation of one source row into the ring.  Column-private shared memory: acc[(slot * rows + j) * nx + x0 .. +1].
+// The nine contributions are formed in registers first; the shared-memory read-modify-writes are then issued as one
+// batch of loads followed by one batch of stores (the rows are distinct, which the compiler cannot know).
+template <typename T, bool WALLS> struct Scatter {
+  typedef P2<T> V;
+  T* ring;     // ring base
+  T* edge_p;   // [slots * rows][nwarps]: lane 31's +x sends (land in the next warp's first column)
+  T* edge_m;   // [slots * rows][nwarps]: lane 0's  -x sends (land in the previous warp's last column)
+  int nx, rows, nwarps, warp, lane;
+  int sm, sc, sp;  // ring slots of the planes z-1, z, z+1
+  int j;           // ring row of the source row (ly + 1)
+
+  template <int dz> __device__ __forceinline__ int slot() const { return dz < 0 ? sm : (dz > 0 ? sp : sc); }
+  template <int dy, int dz> __device__ __forceinline__ bool behind_wall(const Geo& geo) const {
+    // the row (dy, dz) lies behind a wall: everything returns to the sender (B.10-B.11)
+    return WALLS && ((dy > 0 && geo.byp) || (dy < 0 && geo.bym) || (dz > 0 && geo.bzp) || (dz < 0 && geo.bzm));
+  }
+  // target row (dy, dz) with the three directions a0 (e_x = 0), ap (e_x = +1), am (e_x = -1): c = what lands in this
+  // thread's columns, ep / em = what lane 31 / lane 0 sends across the warp edge; bounced links go to `own`
+  template <int dy, int dz, int a0, int ap, int am>
+  __device__ __forceinline__ void xrow(const Geo& geo, const V (&g)[Q], V& own, V& c, T& ep, T& em) const {
+    V v0 = g[a0], vp = g[ap], vm = g[am];
+    if (WALLS) {
+      if (behind_wall<dy, dz>(geo)) { own = own + ((v0 + vp) + vm); v0 = V(T(0)); vp = V(T(0)); vm = V(T(0)); }
+      else {  // x walls: node x0+1 sending +x through the +x face / node x0 sending -x through the -x face
+        if (geo.bxp) { own = own + V(T(0), vp.hi()); vp = V(vp.lo(), T(0)); }
+        if (geo.bxm) { own = own + V(vm.lo(), T(0)); vm = V(T(0), vm.hi()); }
+      }
+    }
+    T up = shfl_up1(vp.hi()), dn = shfl_dn1(vm.lo());  // executed by every lane (wall rows are uniform over the block)
+    if (lane == 0) up = T(0);
+    if (lane == 31) dn = T(0);
+    c = (v0 + V(up, vp.lo())) + V(vm.hi(), dn);
+    ep = vp.hi(); em = vm.lo();
+  }
+  template <int dy, int dz, int a0> __device__ __forceinline__ void diag(const Geo& geo, const V (&g)[Q], V& own, V& c) const {
+    c = g[a0];
+    if (WALLS && behind_wall<dy, dz>(geo)) { own = own + c; c = V(T(0)); }
+  }
+  __device__ __forceinline__ void operator()(const Geo& geo, const V (&g)[Q]) const {
+    typedef typename PairOf<T>::type U;
+    V own(T(0)), c[9];
+    T ep[5], em[5];
+    xrow<1, 0, 3, 7, 10>(geo, g, own, c[0], ep[0], em[0]);
+    xrow<-1, 0, 4, 9, 8>(geo, g, own, c[1], ep[1], em[1]);
+    xrow<0, 1, 5, 11, 14>(geo, g, own, c[2], ep[2], em[2]);
+    xrow<0, -1, 6, 13, 12>(geo, g, own, c[3], ep[3], em[3]);
+    diag<1, 1, 15>(geo, g, own, c[5]);
+    diag<-1, -1, 16>(geo, g, own, c[6]);
+    diag<1, -1, 17>(geo, g, own, c[7]);
+    diag<-1, 1, 18>(geo, g, own, c[8]);
+    xrow<0, 0, 0, 1, 2>(geo, g, own, c[4], ep[4], em[4]);  // own row last: with walls it also collects what bounced back
+    c[4] = c[4] + own;
+    const int r[9] = {sc * rows + j + 1, sc * rows + j - 1, sp * rows + j, sm * rows + j, sc * rows + j,
+                      sp * rows + j + 1, sm * rows + j - 1, sm * rows + j + 1, sp * rows + j - 1};
+    U* p[9];
+    U o[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) { p[k] = reinterpret_cast<U*>(ring + (size_t)r[k] * nx + geo.x0); o[k] = *p[k]; }
+#pragma unroll
+    for (int k = 0; k < 9; ++k) *p[k] = (V(o[k]) + c[k]).v;
+    if (lane == 0 || lane == 31) {
+      T* const e = (lane ? edge_p : edge_m) + warp;
+      T t[5];
+#pragma unroll
+      for (int k = 0; k < 5; ++k) t[k] = e[r[k] * nwarps];
+#pragma unroll
+      for (int k = 0; k < 5; ++k) e[r[k] * nwarps] = t[k] + (lane ? ep[k] : em[k]);
+    }
+  }
+};
+
+// Flush ring slot `s` (ty + 2 rows): column sums + the neighbouring warps' edge sends; the slot is left zeroed.
+// dst_row(j) gives the destination of ring row j (pointer to column 0) or nullptr to drop the row.
+template <typename T, typename D>
+__device__ __forceinline__ void flush_slot(T* ring, T* edge_p, T* edge_m, int nx, int rows, int nwarps, int warp, int lane,
+                                           int x0, int s, D dst_row) {
+  typedef P2<T> V;
+  typedef typename PairOf<T>::type U;
+  const int wl = warp == 0 ? nwarps - 1 : warp - 1, wr = warp == nwarps - 1 ? 0 : warp + 1;
+  for (int j = 0; j < rows; ++j) {
+    const int row = s * rows + j;
+    U* p = reinterpret_cast<U*>(ring + (size_t)row * nx + x0);
+    V v = V(*p);
+    *p = V(T(0)).v;
+    if (lane == 0) { T& e = edge_p[row * nwarps + wl]; v = v + V(e, T(0)); e = T(0); }
+    if (lane == 31) { T& e = edge_m[row * nwarps + wr]; v = v + V(T(0), e); e = T(0); }
+    T* d = dst_row(j);
+    if (d) st_pair<T>(d + x0, v);
+  }
+}
+
+// grid = (ytiles, nchunks); block = nx/2 threads (nx % 64 == 0); dynamic shared memory = ring + edges.
+template <typename T, int NX, bool WALLS, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP<T> FPp, const FusedP<T> U) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const KP<T>& P = FPp.k;
+  const int nx = NX ? NX : P.nx;
+  const int rows = U.ty + 2;
+  const int nwarps = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  T* ring = reinterpret_cast<T*>(smem_raw);
+  constexpr int nslots = FUSED_SLOTS;
+  T* edge_p = ring + (size_t)nslots * rows * nx;
+  T* edge_m = edge_p + nslots * rows * nwarps;
+  const int x0 = 2 * threadIdx.x;
+  const int iy = blockIdx.x, c = blockIdx.y;
+  const int y0 = iy * U.ty, z0 = chunk_z0(c, P.nz, U.nchunks), z1 = chunk_z0(c + 1, P.nz, U.nchunks);
+  const int tz = z1 - z0;
+  for (int i = threadIdx.x; i < nslots * rows * (nx + 2 * nwarps); i += blockDim.x) ring[i] = T(0);
+  __syncthreads();
+  T* const slab = U.part + (long long)(c * U.ytiles + iy) * U.tile_stride;
+  Scatter<T, WALLS> sc;
+  sc.ring = ring; sc.edge_p = edge_p; sc.edge_m = edge_m; sc.nx = nx; sc.rows = rows; sc.nwarps = nwarps; sc.warp = warp; sc.lane = lane;
+  // flush of plane k (-1 .. tz) of the tile, held in ring slot (k + 1) % slots
+  auto flush = [&](int k) {
+    const int s = (k + 1) % nslots;
+    if (k < 0 || k >= tz) {
+      flush_slot<T>(ring, edge_p, edge_m, nx, rows, nwarps, warp, lane, x0, s, [&](int j) -> T* {
+        return slab + (long long)(k < 0 ? slot_zm(j, U.tzmax) : slot_zp(j, U.tzmax, U.ty)) * nx;
+      });
+    } else {
+      T* const plane = U.phi_dst + ((long long)(z0 + k) * P.ny + y0) * nx;
+      flush_slot<T>(ring, edge_p, edge_m, nx, rows, nwarps, warp, lane, x0, s, [&](int j) -> T* {
+        if (j == 0) return slab + (long long)slot_ym(k) * nx;
+        if (j == rows - 1) return slab + (long long)slot_yp(k, U.tzmax) * nx;
+        return plane + (long long)(j - 1) * nx;
+      });
+    }
+  };
+  // FOUR ring slots for three live planes: the slot flushed after plane lz (plane lz-1) is not touched while plane lz+1
+  // is processed, so one barrier per plane suffices (a warp's flush overlaps the other warps' next plane).
+#pragma unroll 1
+  for (int lz = 0; lz < tz; ++lz) {
+    const int z = z0 + lz;
+    sc.sm = lz % nslots; sc.sc = (lz + 1) % nslots; sc.sp = (lz + 2) % nslots;
+#pragma unroll 1
+    for (int ly = 0; ly < U.ty; ++ly) {
+      const int y = y0 + ly;
+      sc.j = ly + 1;
+      bool wall_row = false;
+      if (WALLS) {
+        wall_row = P.bc[0] != BC_PERIODIC || P.bc[1] != BC_PERIODIC || (y == 0 && P.bc[2] != BC_PERIODIC) ||
+                   (y == P.ny - 1 && P.bc[3] != BC_PERIODIC) || (z == 0 && P.bc[4] != BC_PERIODIC) ||
+                   (z == P.nz - 1 && P.bc[5] != BC_PERIODIC);
+      }
+      if (WALLS && wall_row) {
+        step_pair<T, LD_NC, LD_NC, ST_WB, NX, true>(FPp, x0, y, z, NoWait(), sc);
+      } else {
+        Scatter<T, false> sp;
+        sp.ring = ring; sp.edge_p = edge_p; sp.edge_m = edge_m; sp.nx = nx; sp.rows = rows; sp.nwarps = nwarps; sp.warp = warp; sp.lane = lane;
+        sp.sm = sc.sm; sp.sc = sc.sc; sp.sp = sc.sp; sp.j = sc.j;
+        step_pair<T, LD_NC, LD_NC, ST_WB, NX, false>(FPp, x0, y, z, NoWait(), sp);
+      }
+    }
+    __syncthreads();
+    flush(lz - 1);
+  }
+  flush(tz - 1);
+  flush(tz);
+}
+
+// phi(t+1) of the rows on a tile surface: own sum + the neighbour tiles' partials, fixed order.
+// Surface rows of a tile are numbered s = 0 .. 2 tzmax + 2 (ty - 2) - 1: [0, tzmax) the row ly = 0 of plane lz = s;
+// [tzmax, 2 tzmax) the row ly = ty-1; then the rows 1 .. ty-2 of the first plane and (if the tile has more than one
+// plane) of the last plane.  grid = (ytiles, nchunks, ceil(rows / FIX_ROWS)); block = 128 threads over the x pairs.
+constexpr int FIX_ROWS = 4;
+template <typename T> __global__ void __launch_bounds__(128) k_fix(const __grid_constant__ FP<T> FPp, const FusedP<T> U) {
+  typedef P2<T> V;
+  const KP<T>& P = FPp.k;
+  const int nx = P.nx;
+  const int iy = blockIdx.x, c = blockIdx.y;
+  const int z0 = chunk_z0(c, P.nz, U.nchunks), tz = chunk_z0(c + 1, P.nz, U.nchunks) - z0;
+  const int iym = iy == 0 ? U.ytiles - 1 : iy - 1, iyp = iy == U.ytiles - 1 ? 0 : iy + 1;
+  const int cm = c == 0 ? U.nchunks - 1 : c - 1, cp = c == U.nchunks - 1 ? 0 : c + 1;
+  auto slab = [&](int cc, int ii, int slot) -> const T* {
+    return U.part + (long long)(cc * U.ytiles + ii) * U.tile_stride + (long long)slot * nx;
+  };
+  const int nrows = 2 * U.tzmax + 2 * (U.ty - 2);
+#pragma unroll 1
+  for (int i = 0; i < FIX_ROWS; ++i) {
+    int s = blockIdx.z * FIX_ROWS + i, ly, lz;
+    if (s >= nrows) return;
+    if (s < 2 * U.tzmax) { ly = s < U.tzmax ? 0 : U.ty - 1; lz = s < U.tzmax ? s : s - U.tzmax; if (lz >= tz) continue; }
+    else {
+      s -= 2 * U.tzmax;
+      ly = 1 + (s < U.ty - 2 ? s : s - (U.ty - 2));
+      lz = s < U.ty - 2 ? 0 : tz - 1;
+      if (s >= U.ty - 2 && tz == 1) continue;
+    }
+    const int y = iy * U.ty + ly;
+    const bool ylo = ly == 0, yhi = ly == U.ty - 1, zlo = lz == 0, zhi = lz == tz - 1;
+    const T* src[8];
+    int ns = 0;
+    if (ylo) src[ns++] = slab(c, iym, slot_yp(lz, U.tzmax));
+    if (yhi) src[ns++] = slab(c, iyp, slot_ym(lz));
+    if (zlo) src[ns++] = slab(cm, iy, slot_zp(ly + 1, U.tzmax, U.ty));
+    if (zhi) src[ns++] = slab(cp, iy, slot_zm(ly + 1, U.tzmax));
+    if (ylo && zlo) src[ns++] = slab(cm, iym, slot_zp(U.ty + 1, U.tzmax, U.ty));
+    if (ylo && zhi) src[ns++] = slab(cp, iym, slot_zm(U.ty + 1, U.tzmax));
+    if (yhi && zlo) src[ns++] = slab(cm, iyp, slot_zp(0, U.tzmax, U.ty));
+    if (yhi && zhi) src[ns++] = slab(cp, iyp, slot_zm(0, U.tzmax));
+    T* const row = U.phi_dst + ((long long)(z0 + lz) * P.ny + y) * nx;
+    for (int x0 = 2 * threadIdx.x; x0 < nx; x0 += 2 * blockDim.x) {
+      V v = ld_pair<T, LD_CA>(row + x0);
+      for (int k = 0; k < ns; ++k) v = v + ld_pair<T, LD_CA>(src[k] + x0);
+      st_pair<T>(row + x0, v);
+    }
+  }
+}
+
+}  // namespace clip

@@ -213,29 +213,104 @@ def test_fast_paths_match_generic_kernels(precision):
         assert np.abs(x - y).max() <= tol * max(1.0, np.abs(x).max())
 
 
+@pytest.mark.parametrize("mode", [3, 2])
 @pytest.mark.parametrize("precision", [32, 64])
-def test_full_size_256_equals_tiled_64(precision):
-    """BASELINE configs[4] at the full bench size (256^3, the launch configuration bench.py times: nx-specialised
-    pair kernels, same block shape): a periodic 64^3 field tiled 4 x 4 x 4 must evolve into the tiled 64^3 solution,
-    bit for bit (every node runs the same arithmetic; only indexing, wrap-around and tiling differ) -- and the 64^3
-    solution itself is checked against the oracle element by element in test_parity[sweep64]."""
+def test_full_size_256_equals_tiled_64(precision, mode):
+    """BASELINE configs[4] at the full bench size (256^3, the launch configurations bench.py times: nx-specialised
+    kernels, same block shapes): a periodic 64^3 field tiled 4 x 4 x 4 must evolve into the tiled 64^3 solution --
+    and the 64^3 solution itself is checked against the oracle element by element in test_parity[sweep64].
+    mode 2 (k_phi2 + k_step2): bit for bit (every node runs the same arithmetic; only indexing, wrap-around and tiling
+    differ).  mode 3 (k_fused + k_fix, the default): phi(t+1) is summed tile by tile, so the association of the 19-term
+    sum depends on where a node sits in its tile: round-off only."""
+    import os
     import torch
     from paper_2505_12205_b200 import clip
     small = inputs.sweep_drops(n=64)
     steps = 20
-    ref = _gpu(small, steps, precision)
+    ref = _gpu_env(small, steps, precision, CLIP_FAST_MODE=mode)
     big = dict(small)
     big["nx"] = big["ny"] = big["nz"] = 256
     big["phi0"] = np.tile(small["phi0"], (4, 4, 4))
     big["u0"] = np.tile(small["u0"], (1, 4, 4, 4))
-    sim = clip.Clip.from_case(big, precision=precision)
+    old = os.environ.get("CLIP_FAST_MODE")
+    os.environ["CLIP_FAST_MODE"] = str(mode)
+    try:
+        sim = clip.Clip.from_case(big, precision=precision)
+    finally:
+        os.environ.pop("CLIP_FAST_MODE")
+        if old is not None:
+            os.environ["CLIP_FAST_MODE"] = old
     sim.step(steps)
     phi, p, u = sim.get()
     torch.cuda.synchronize()
+    tol = 0.0 if mode == 2 else (1e-13 if precision == 64 else 2e-5)
     for got, want in ((phi, ref[0]), (p, ref[1]), (u, ref[2])):
         want_t = torch.as_tensor(np.tile(want, (1,) * (want.ndim - 3) + (4, 4, 4))).to(got.device)
-        assert torch.equal(got.double(), want_t)
+        if mode == 2:
+            assert torch.equal(got.double(), want_t)
+        else:
+            assert float((got.double() - want_t).abs().max()) <= tol * max(1.0, float(want_t.abs().max()))
     sim.close()
+
+
+FUSED_LATTICES = {
+    "periodic_128x24x20": lambda: inputs.sweep_drops(shape=(128, 24, 20), ndrops=6, rmin=3, rmax=6),
+    "periodic_64x4x5": lambda: inputs.sweep_drops(shape=(64, 4, 5), ndrops=2, rmin=2, rmax=3),      # one y tile: the halo wraps onto the tile itself
+    "walled_64x12x9": lambda: inputs.walled_box(nx=64, ny=12, nz=9),
+    "walled_128x8x17": lambda: inputs.walled_box(nx=128, ny=8, nz=17),
+    "rt_64": lambda: inputs.rayleigh_taylor(L=64, W=3.0),                                       # y walls, x / z periodic
+}
+
+
+@pytest.mark.parametrize("name", list(FUSED_LATTICES))
+@pytest.mark.parametrize("precision", [64, 32])
+def test_fused_single_pass_path(name, precision):
+    """k_fused + k_fix (one pass over f and g; phi(t+1) scattered on chip, tile halos through partial sums) against
+    k_phi2 + k_step2: same arithmetic except the association of phi's 19-term sum -> round-off only, for several
+    tilings (default; one z chunk; one plane per chunk; 8-row tiles), with and without walls."""
+    case = FUSED_LATTICES[name]()
+    steps = 30
+    ref = _gpu_env(case, steps, precision, CLIP_FAST_MODE=2)
+    tol = 1e-12 if precision == 64 else 3e-5
+    tilings = [{}, {"CLIP_FUSED_CHUNKS": 1}, {"CLIP_FUSED_CHUNKS": case["nz"]}, {"CLIP_FUSED_CHUNKS": 3}]
+    if case["ny"] % 8 == 0:
+        tilings.append({"CLIP_FUSED_TY": 8, "CLIP_FUSED_CHUNKS": 2})
+    for env in tilings:
+        out = _gpu_env(case, steps, precision, CLIP_FAST_MODE=3, **env)
+        for a, b in zip(ref, out):
+            assert np.isfinite(b).all()
+            assert np.abs(a - b).max() <= tol * max(1.0, np.abs(a).max()), (name, env)
+
+
+def test_fused_path_time_semantics():
+    """The fused path keeps phi one step ahead of the populations internally: clip_get must still return phi(t), a
+    clip_get between steps must not disturb the run, and clip_step(a); clip_step(b) == clip_step(a + b) bit for bit."""
+    import torch
+    from paper_2505_12205_b200 import clip
+    case = inputs.sweep_drops(shape=(64, 16, 12), ndrops=4, rmin=3, rmax=5)
+    whole = _gpu_env(case, 25, 64, CLIP_FAST_MODE=3)
+    import os
+    os.environ["CLIP_FAST_MODE"] = "3"
+    try:
+        sim = clip.Clip.from_case(case, precision=64)
+    finally:
+        os.environ.pop("CLIP_FAST_MODE")
+    phi0 = sim.get()[0].cpu().numpy()
+    assert np.array_equal(phi0, case["phi0"])
+    sim.step(7)
+    mid = [t.double().cpu().numpy() for t in sim.get()]
+    sim.step(0)
+    sim.step(18)
+    out = [t.double().cpu().numpy() for t in sim.get()]
+    torch.cuda.synchronize()
+    names = clip.clip_step_profiled(sim._h, 0)[1]
+    assert "k_fused" in names
+    sim.close()
+    for a, b in zip(whole, out):
+        assert np.array_equal(a, b)
+    ref7 = _gpu_env(case, 7, 64, CLIP_FAST_MODE=2)
+    for a, b in zip(ref7, mid):
+        assert np.abs(a - b).max() <= 1e-12
 
 
 @pytest.mark.parametrize("precision", [64, 32])
