@@ -32,8 +32,10 @@ enum { CLIP_OK = 0, CLIP_EINVAL = -1, CLIP_ENOMEM = -2, CLIP_ESTATE = -3, CLIP_E
 
 /* Boundary type of one lattice face.  PERIODIC: App. B.1 (:971-1003).  WALL: halfway bounce-back, App. B.3
  * (:1028-1038).  INLET: velocity inlet, App. B.4 (:1042-1088), only on the -z face.  OUTLET: convective outlet,
- * App. B.5 (:1094-1129), only on the +z face. */
-enum { CLIP_BC_PERIODIC = 0, CLIP_BC_WALL = 1, CLIP_BC_INLET = 2, CLIP_BC_OUTLET = 3 };
+ * App. B.5 (:1094-1129), only on the +z face.  FREESLIP: specular reflection half a cell outside the last node, App. B.2
+ * (B.8-B.9, :1017-1026): zero normal velocity, free tangential velocity; where a link also crosses a WALL face the
+ * bounce-back wins.  The phi stencils (Eq. 40) take the mirror value behind WALL, FREESLIP, INLET and OUTLET faces. */
+enum { CLIP_BC_PERIODIC = 0, CLIP_BC_WALL = 1, CLIP_BC_INLET = 2, CLIP_BC_OUTLET = 3, CLIP_BC_FREESLIP = 4 };
 
 /* Hydrodynamic collision operator: weighted MRT (the paper's choice for 3-D, :849) or BGK. */
 enum { CLIP_COLL_WMRT = 0, CLIP_COLL_BGK = 1 };
@@ -50,7 +52,8 @@ typedef struct clip_params {
   double inlet_c[2];       /* nozzle disc centre (x, y) in node coordinates */
   double inlet_r;          /* nozzle radius; nodes of the -z face outside the disc are WALL */
   int outlet_u_mode;       /* 0 = U_local of B.22 (:1104); 1 (U_ave) and 2 (U_max) are not implemented */
-  int visc_interp;         /* 0 = linear tau, Eq. 24 (paper); 1 = harmonic (1/tau linear in phi; non-paper) */
+  int visc_interp;         /* 0 = linear tau, Eq. 24 (paper, Alg. 1); 1 = harmonic (1/tau linear in phi; non-paper);
+                              2 = linear dynamic viscosity, Eq. 25 (:219): mu = rho tau / 3, tau = 3 mu(phi) / rho(phi) */
   int collision;           /* CLIP_COLL_WMRT (0, default): Eq. 27-28 + F_mu of Eq. 30; CLIP_COLL_BGK (1): Eq. 26 + F_mu of Eq. 29 */
   int phase_only;          /* 0 (default): full two-phase flow.  1: only the phase-field equation (Eq. 33) is advanced and
                               u is prescribed by the caller (clip_set_u) -- the set-up of the interface-in-shear-flow test,

@@ -13,7 +13,8 @@
  * race, reading G15), dense 19x19 M^-1 S M (Eq. 27).  No fusion, blocking or reordering.
  *
  * Readings of garbled / silent passages are marked [Gn]/[Rn] below.
- * Parity pins: see tests/test_oracle_pins.py.  "parity unpinned" items: R9 (phi ghost at walls / open faces),
+ * Parity pins: see tests/test_oracle_pins.py, test_oracle_invariants.py (free-slip = mirror plane), test_oracle_physics.py.
+ * "parity unpinned" items: R9 (phi ghost at walls / open faces),
  * R12 (outlet U_local from stored u(t)), R13 (lagged u inside the macro update's F_mu).
  */
 #include <math.h>
@@ -21,7 +22,7 @@
 #include <string.h>
 
 #define Q 19
-enum { BC_PERIODIC = 0, BC_WALL = 1, BC_INLET = 2, BC_OUTLET = 3 };
+enum { BC_PERIODIC = 0, BC_WALL = 1, BC_INLET = 2, BC_OUTLET = 3, BC_FREESLIP = 4 };
 
 /* D3Q19 velocities, Eq. 14, in the ordering consistent with the inlet set {1,7,9,11,13} being
  * the +x-pointing directions [G1]; opposite pairs adjacent. */
@@ -38,7 +39,8 @@ typedef struct clipo_params {
   int bc[6];               /* -x,+x,-y,+y,-z,+z */
   double inlet_u[3], inlet_phi, inlet_c[2], inlet_r;
   int outlet_u_mode;       /* 0 = U_local only */
-  int visc_interp;         /* 0: Eq. 24 linear tau; 1: harmonic (1/tau linear; non-paper) */
+  int visc_interp;         /* 0: Eq. 24 linear tau; 1: harmonic (1/tau linear; non-paper);
+                              2: Eq. 25 linear dynamic viscosity mu = rho tau c_s^2, tau = 3 mu(phi) / rho(phi) */
   int collision;           /* 0: WMRT, Eq. 27-28, 30; 1: BGK, Eq. 26, 29 */
   int phase_only;          /* 1: only the phase-field LBE (Eq. 33) is advanced; u is prescribed (clipo_set_u), f stays 0:
                               the set-up of the interface-in-shear-flow test, PAPER.md:675-713 (Sec. 5.4) */
@@ -159,6 +161,11 @@ static void stencils(const clipo *h, const double *phi, int x, int y, int z, dou
 
 static double tau_of(const clipo *h, double phi) {
   if (h->p.visc_interp == 1) return 1.0 / (1.0 / h->p.tau_l + phi * (1.0 / h->p.tau_h - 1.0 / h->p.tau_l));
+  if (h->p.visc_interp == 2) { /* Eq. 25 with mu_X = rho_X tau_X c_s^2 (Eq. 23), phi_L = 0; then tau = mu / (rho c_s^2) */
+    const double mu_l = h->p.rho_l * h->p.tau_l / 3.0, mu_h = h->p.rho_h * h->p.tau_h / 3.0;
+    const double mu = mu_l + phi * (mu_h - mu_l);
+    return 3.0 * mu / (h->p.rho_l + phi * (h->p.rho_h - h->p.rho_l));
+  }
   return h->p.tau_l + phi * (h->p.tau_h - h->p.tau_l); /* Eq. 24, phi_L = 0 */
 }
 static double rho_of(const clipo *h, double phi) { return h->p.rho_l + phi * (h->p.rho_h - h->p.rho_l); } /* Eq. 39 */
@@ -344,13 +351,17 @@ static void step_once(clipo *h) {
     size_t i = IDX(h, x, y, z);
     collide_node(h, h->phi, x, y, z, h->f + i * Q, h->g + i * Q, h->ux[i], h->uy[i], h->uz[i], h->fp + i * Q, h->gp + i * Q);
   }
-  /* step 7: streaming (B.3-B.6) with halfway bounce-back (B.10-B.11) into the second buffer */
+  /* step 7: streaming (B.3-B.6) with halfway bounce-back (B.10-B.11) and free-slip (B.8-B.9) into the second buffer.
+   * Free-slip: a population that leaves node x_b through a free-slip face comes back with its wall-normal
+   * velocity component reversed and the tangential ones kept, and lands on x_b + e_tangential.  Pull form: the population
+   * a arriving at x whose upstream node x - e_a lies behind a free-slip face in dimension d was sent, as direction a' = a
+   * with component d reversed, by the node that has x's coordinate in d and the upstream coordinates in the other dimensions. */
   for (int z = 0; z < nz; ++z) for (int y = 0; y < ny; ++y) for (int x = 0; x < nx; ++x) {
     size_t i = IDX(h, x, y, z);
     for (int a = 0; a < Q; ++a) {
       int sx = x - EX[a], sy = y - EY[a], sz = z - EZ[a];
       int bounce = 0, open = 0;
-      int s[3] = {sx, sy, sz}, nn[3] = {nx, ny, nz};
+      int s[3] = {sx, sy, sz}, nn[3] = {nx, ny, nz}, here[3] = {x, y, z}, e[3] = {EX[a], EY[a], EZ[a]};
       for (int d = 0; d < 3; ++d) {
         int face = -1;
         if (s[d] < 0) face = 2 * d; else if (s[d] >= nn[d]) face = 2 * d + 1;
@@ -358,18 +369,24 @@ static void step_once(clipo *h) {
         int type = bc[face];
         if (type == BC_PERIODIC) s[d] += (s[d] < 0) ? nn[d] : -nn[d];
         else if (type == BC_WALL) bounce = 1;
+        else if (type == BC_FREESLIP) { s[d] = here[d]; e[d] = -e[d]; }
         else if (type == BC_INLET) { if (in_disc(h, x, y)) open = 1; else bounce = 1; }
         else open = 1; /* OUTLET: the destination layer is overwritten in step 9 */
       }
-      if (bounce) { /* a wall crossing wins at edges / corners [R11] */
+      if (bounce) { /* a no-slip wall crossing wins at edges / corners [R11] */
         h->f2[i * Q + a] = h->fp[i * Q + opp(a)];
         h->g2[i * Q + a] = h->gp[i * Q + opp(a)];
       } else if (open) { /* unknown: filled by step 8 or 9; keep a defined value */
         h->f2[i * Q + a] = 0.0; h->g2[i * Q + a] = 0.0;
       } else {
+        int as = a;
+        if (e[0] != EX[a] || e[1] != EY[a] || e[2] != EZ[a]) {
+          as = -1;
+          for (int b = 0; b < Q; ++b) if (EX[b] == e[0] && EY[b] == e[1] && EZ[b] == e[2]) as = b;
+        }
         size_t j = IDX(h, s[0], s[1], s[2]);
-        h->f2[i * Q + a] = h->fp[j * Q + a];
-        h->g2[i * Q + a] = h->gp[j * Q + a];
+        h->f2[i * Q + a] = h->fp[j * Q + as];
+        h->g2[i * Q + a] = h->gp[j * Q + as];
       }
     }
   }

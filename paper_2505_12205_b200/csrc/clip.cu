@@ -119,7 +119,7 @@ const char* validate(int nx, int ny, int nz, const clip_params* p) {
   if (!(p->rho_h > 0.0) || !(p->rho_l > 0.0)) return "densities must be positive";
   if (!(p->tau_h + 0.5 > 0.0) || !(p->tau_l + 0.5 > 0.0)) return "tau + 1/2 must be positive";
   if (p->visc_interp == 1 && (!(p->tau_h > 0.0) || !(p->tau_l > 0.0))) return "harmonic interpolation needs tau > 0";
-  if (p->visc_interp != 0 && p->visc_interp != 1) return "visc_interp must be 0 or 1";
+  if (p->visc_interp < 0 || p->visc_interp > 2) return "visc_interp must be 0, 1 or 2";
   if (p->collision != CLIP_COLL_WMRT && p->collision != CLIP_COLL_BGK) return "collision must be CLIP_COLL_WMRT (0) or CLIP_COLL_BGK (1)";
   if (p->phase_only != 0 && p->phase_only != 1) return "phase_only must be 0 or 1";
   if (!(3.0 * p->M + 0.5 > 0.0)) return "tau_phi + 1/2 must be positive";
@@ -127,9 +127,10 @@ const char* validate(int nx, int ny, int nz, const clip_params* p) {
   if (!std::isfinite(p->sigma)) return "sigma must be finite";
   for (int d = 0; d < 3; ++d) {
     const int lo = p->bc[2 * d], hi = p->bc[2 * d + 1];
-    if (lo < 0 || lo > 3 || hi < 0 || hi > 3) return "unknown boundary type";
+    if (lo < 0 || lo > 4 || hi < 0 || hi > 4) return "unknown boundary type";
     if ((lo == CLIP_BC_PERIODIC) != (hi == CLIP_BC_PERIODIC)) return "PERIODIC faces must come in pairs";
-    if (d < 2 && (lo >= CLIP_BC_INLET || hi >= CLIP_BC_INLET)) return "INLET / OUTLET are only supported on the z faces";
+    const bool open_lo = lo == CLIP_BC_INLET || lo == CLIP_BC_OUTLET, open_hi = hi == CLIP_BC_INLET || hi == CLIP_BC_OUTLET;
+    if (d < 2 && (open_lo || open_hi)) return "INLET / OUTLET are only supported on the z faces";
   }
   if (p->bc[4] == CLIP_BC_OUTLET) return "OUTLET is only supported on the +z face";
   if (p->bc[5] == CLIP_BC_INLET) return "INLET is only supported on the -z face";
@@ -185,6 +186,7 @@ template <typename T> clip::KP<T> make_kp(const clip_handle* h) {
   P.phase_only = p.phase_only;
   P.rho_h = (T)p.rho_h; P.rho_l = (T)p.rho_l; P.drho = (T)(p.rho_h - p.rho_l);
   P.tau_h = (T)p.tau_h; P.tau_l = (T)p.tau_l;
+  P.rt_h = (T)(p.rho_h * p.tau_h); P.rt_l = (T)(p.rho_l * p.tau_l);
   P.itau_h = (T)(p.tau_h != 0.0 ? 1.0 / p.tau_h : 0.0); P.itau_l = (T)(p.tau_l != 0.0 ? 1.0 / p.tau_l : 0.0);
   P.beta4 = (T)(4.0 * 12.0 * p.sigma / p.W);  // 4 beta, Eq. 12
   P.kappa = (T)(1.5 * p.sigma * p.W);
@@ -232,6 +234,7 @@ bool fast_ok(const clip_handle* h) {
   if (h->force_generic) return false;
   if (h->p.collision != CLIP_COLL_WMRT || h->p.phase_only) return false;  // BGK keeps all 19 f in the collision: generic kernels only (round 1)
   for (int k = 0; k < 4; ++k) if (h->p.bc[k] != CLIP_BC_PERIODIC && h->p.bc[k] != CLIP_BC_WALL) return false;
+  if (h->p.bc[4] == CLIP_BC_FREESLIP || h->p.bc[5] == CLIP_BC_FREESLIP) return false;  // free-slip: generic kernels only
   // an INLET (-z) / OUTLET (+z) face is served by the generic kernels on its own plane (hybrid launches, do_step)
   return h->nx % 2 == 0 && h->nz >= 4;
 }

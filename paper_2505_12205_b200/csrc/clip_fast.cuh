@@ -165,6 +165,7 @@ template <typename T> __device__ __forceinline__ Mat2<T> materials2(const KP<T>&
   m.rho = fma2(phi, V(P.drho), V(P.rho_l));                                    // Eq. 39
   m.inv_rho = rcp2(m.rho);
   if (P.visc_interp == 1) m.tau = rcp2(fma2(phi, V(P.itau_h - P.itau_l), V(P.itau_l)));
+  else if (P.visc_interp == 2) m.tau = fma2(phi, V(P.rt_h - P.rt_l), V(P.rt_l)) * m.inv_rho;  // Eq. 25: mu linear, tau = 3 mu / rho
   else m.tau = fma2(phi, V(P.tau_h - P.tau_l), V(P.tau_l));                    // Eq. 24
   m.s_nu = rcp2(m.tau + V(T(0.5)));                                            // G3
   m.mu = fms2(V(P.beta4) * phi, (phi - V(T(1))) * (phi - V(T(0.5))), V(P.kappa) * L);  // Eq. 11 (G4)

@@ -26,7 +26,7 @@
 
 namespace clip {
 
-enum { BC_PERIODIC = 0, BC_WALL = 1, BC_INLET = 2, BC_OUTLET = 3 };
+enum { BC_PERIODIC = 0, BC_WALL = 1, BC_INLET = 2, BC_OUTLET = 3, BC_FREESLIP = 4 };
 constexpr int Q = 19;
 
 // D3Q19 velocity set, Eq. 14; ordering chosen so that the +x set is {1,7,9,11,13}
@@ -54,7 +54,7 @@ template <typename T> struct KP {
   int has_inlet, has_outlet, any_nonperiodic, visc_interp, collision, phase_only;
   int z_lo, z_cnt;  // planes [z_lo, z_lo + z_cnt) a k_phi* / k_step* launch covers (whole lattice: 0, nz)
   T rho_h, rho_l, drho;
-  T tau_h, tau_l, itau_h, itau_l;
+  T tau_h, tau_l, itau_h, itau_l, rt_h, rt_l;  // rt = rho tau = 3 mu (Eq. 23, 25)
   T beta4, kappa, inv_W, om_phi;
   T gx, gy, gz, rho_ref;
   T uin[3], phi_in;
@@ -81,6 +81,8 @@ struct Nbr {
   bool bxm, bxp, bym, byp, bzm, bzp;
   // the link crosses the inlet disc (unknown, B.4) / the outlet face (layer overwritten, B.5)
   bool ozm, ozp;
+  // the link towards that side crosses a free-slip face and is reflected specularly (B.8-B.9)
+  bool sxm, sxp, sym, syp, szm, szp;
   bool any;
 };
 
@@ -94,22 +96,25 @@ __device__ __forceinline__ Nbr make_nbr(const KP<T>& P, int x, int y, int z) {
   b.zm = ((z == 0) ? (long long)(P.nz - 1) : -1LL) * P.nxy;
   b.zp = ((z == P.nz - 1) ? -(long long)(P.nz - 1) : 1LL) * P.nxy;
   b.bxm = b.bxp = b.bym = b.byp = b.bzm = b.bzp = b.ozm = b.ozp = false;
+  b.sxm = b.sxp = b.sym = b.syp = b.szm = b.szp = false;
   if (P.any_nonperiodic) {
-    b.bxm = (x == 0) && P.bc[0] != BC_PERIODIC;
-    b.bxp = (x == P.nx - 1) && P.bc[1] != BC_PERIODIC;
-    b.bym = (y == 0) && P.bc[2] != BC_PERIODIC;
-    b.byp = (y == P.ny - 1) && P.bc[3] != BC_PERIODIC;
+    b.bxm = (x == 0) && P.bc[0] == BC_WALL;            b.sxm = (x == 0) && P.bc[0] == BC_FREESLIP;
+    b.bxp = (x == P.nx - 1) && P.bc[1] == BC_WALL;     b.sxp = (x == P.nx - 1) && P.bc[1] == BC_FREESLIP;
+    b.bym = (y == 0) && P.bc[2] == BC_WALL;            b.sym = (y == 0) && P.bc[2] == BC_FREESLIP;
+    b.byp = (y == P.ny - 1) && P.bc[3] == BC_WALL;     b.syp = (y == P.ny - 1) && P.bc[3] == BC_FREESLIP;
     if (z == 0 && P.bc[4] != BC_PERIODIC) {
       const bool disc = (P.bc[4] == BC_INLET) && P.mask[(long long)y * P.nx + x];
-      b.bzm = !disc;
+      b.szm = P.bc[4] == BC_FREESLIP;
+      b.bzm = !disc && !b.szm;
       b.ozm = disc;
     }
     if (z == P.nz - 1 && P.bc[5] != BC_PERIODIC) {
       b.bzp = (P.bc[5] == BC_WALL);
       b.ozp = (P.bc[5] == BC_OUTLET);
+      b.szp = (P.bc[5] == BC_FREESLIP);
     }
   }
-  b.any = b.bxm | b.bxp | b.bym | b.byp | b.bzm | b.bzp | b.ozm | b.ozp;
+  b.any = b.bxm | b.bxp | b.bym | b.byp | b.bzm | b.bzp | b.ozm | b.ozp | b.sxm | b.sxp | b.sym | b.syp | b.szm | b.szp;
   return b;
 }
 
@@ -136,11 +141,39 @@ template <int a> __device__ __forceinline__ bool src_open(const Nbr& b) {
 // bounce-back (B.10-B.11; a wall crossing wins at edges and corners, R11).  Open links (inlet disc / outlet
 // face) get 0 and are filled by the caller.
 // `src` points at component 0 of the set (f: p_src, g: p_src + Q*nx); pb = pop_base of the node.
+// index of the direction with velocity (ex, ey, ez) (must be one of the 19)
+__host__ __device__ constexpr int dir_of(int ex, int ey, int ez) {
+  for (int a = 0; a < Q; ++a) if (cx(a) == ex && cy(a) == ey && cz(a) == ez) return a;
+  return 0;
+}
+// Free-slip (B.8-B.9), pull form: the population a arriving at a node whose upstream node lies
+// behind a free-slip face in dimension d was sent as direction a' = a with component d reversed by the node that has
+// the same coordinate in d and the upstream coordinates in the other dimensions (specular reflection half a cell out).
+template <typename T, int a, int FX, int FY, int FZ>
+__device__ __forceinline__ T pull_reflected(const T* __restrict__ src, int nx, long long pb, const Nbr& b) {
+  constexpr int ar = dir_of(FX ? -cx(a) : cx(a), FY ? -cy(a) : cy(a), FZ ? -cz(a) : cz(a));
+  long long o = 0, r = 0;
+  if (!FX) { if (cx(a) == 1) o += b.xm; else if (cx(a) == -1) o += b.xp; }
+  if (!FY) { if (cy(a) == 1) r += b.ym; else if (cy(a) == -1) r += b.yp; }
+  if (!FZ) { if (cz(a) == 1) r += b.zm; else if (cz(a) == -1) r += b.zp; }
+  return __ldg(src + pb + ar * nx + o + NC * r);
+}
 template <typename T, int a>
 __device__ __forceinline__ T pull_one(const T* __restrict__ src, int nx, long long pb, const Nbr& b, bool slow) {
   if (!slow) return __ldg(src + pb + a * nx + src_off<a>(b));
-  if (src_bounce<a>(b)) return __ldg(src + pb + copp(a) * nx);
+  if (src_bounce<a>(b)) return __ldg(src + pb + copp(a) * nx);  // a no-slip crossing wins at edges and corners (R11)
   if (src_open<a>(b)) return T(0);
+  const bool fx = (cx(a) == 1 && b.sxm) || (cx(a) == -1 && b.sxp);
+  const bool fy = (cy(a) == 1 && b.sym) || (cy(a) == -1 && b.syp);
+  const bool fz = (cz(a) == 1 && b.szm) || (cz(a) == -1 && b.szp);
+  if (fx | fy | fz) {  // D3Q19: at most two components are non-zero
+    if (fx && fy) return pull_reflected<T, a, 1, 1, 0>(src, nx, pb, b);
+    if (fx && fz) return pull_reflected<T, a, 1, 0, 1>(src, nx, pb, b);
+    if (fy && fz) return pull_reflected<T, a, 0, 1, 1>(src, nx, pb, b);
+    if (fx) return pull_reflected<T, a, 1, 0, 0>(src, nx, pb, b);
+    if (fy) return pull_reflected<T, a, 0, 1, 0>(src, nx, pb, b);
+    return pull_reflected<T, a, 0, 0, 1>(src, nx, pb, b);
+  }
   return __ldg(src + pb + a * nx + src_off<a>(b));
 }
 
@@ -268,6 +301,7 @@ template <typename T> __device__ __forceinline__ Mat<T> materials(const KP<T>& P
   m.rho = P.rho_l + phi * P.drho;                                              // Eq. 39
   m.inv_rho = T(1) / m.rho;
   if (P.visc_interp == 1) m.tau = T(1) / (P.itau_l + phi * (P.itau_h - P.itau_l));
+  else if (P.visc_interp == 2) m.tau = (P.rt_l + phi * (P.rt_h - P.rt_l)) * m.inv_rho;  // Eq. 25: mu linear, tau = 3 mu / rho
   else m.tau = P.tau_l + phi * (P.tau_h - P.tau_l);                            // Eq. 24
   m.s_nu = T(1) / (m.tau + T(0.5));                                            // G3
   m.mu = P.beta4 * phi * (phi - T(1)) * (phi - T(0.5)) - P.kappa * L;          // Eq. 11 (sign corrected, G4)

@@ -16,7 +16,7 @@ from __future__ import annotations
 
 import numpy as np
 
-PERIODIC, WALL, INLET, OUTLET = 0, 1, 2, 3
+PERIODIC, WALL, INLET, OUTLET, FREESLIP = 0, 1, 2, 3, 4
 
 
 def default_params(**kw) -> dict:

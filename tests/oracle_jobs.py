@@ -164,6 +164,7 @@ JOBS = {
     "tanh_narrow": (tanh_relax, dict(W0_factor=0.5)),
     "galilean": (galilean_drift, {}),
     "wave_diag_bgk": (shear_wave, dict(orient="diag", n=64, steps=600, tau=0.6, collision=1)),
+    "pois_rho10_mu": (poiseuille_steady, dict(ny=64, tau_a=5.0, tau_b=0.5, rho_a=10.0, rho_b=1.0, gx=1e-7, tol=1e-12, visc_interp=2)),
     "pois_rho10_bgk": (poiseuille_steady, dict(ny=64, tau_a=5.0, tau_b=0.5, rho_a=10.0, rho_b=1.0, gx=1e-7, tol=1e-12, collision=1)),
 }
 

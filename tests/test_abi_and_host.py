@@ -56,6 +56,8 @@ def test_validation_without_gpu():
         (dict(precision=16), "precision"),
         (dict(bc=(0, 1, 0, 0, 0, 0)), "PERIODIC"),
         (dict(bc=(2, 3, 0, 0, 0, 0)), "z faces"),
+        (dict(bc=(5, 5, 0, 0, 0, 0)), "unknown boundary"),
+        (dict(bc=(4, 0, 0, 0, 0, 0)), "PERIODIC"),
         (dict(rho_l=0.0), "densit"),
         (dict(W=0.0), "W"),
         (dict(tau_l=-0.5), "tau"),
@@ -66,6 +68,9 @@ def test_validation_without_gpu():
         q = dict(p); q.update(bad)
         assert clip.clip_workspace_bytes(8, 8, 8, clip.make_params(q)) == 0
         assert word in clip.clip_last_error(None), (bad, clip.clip_last_error(None))
+    for good in (dict(bc=(4, 4, 1, 4, 4, 1)), dict(bc=(4, 4, 4, 4, 2, 3)), dict(visc_interp=2)):   # FREESLIP faces, Eq. 25
+        q = dict(p); q.update(good)
+        assert clip.clip_workspace_bytes(8, 8, 8, clip.make_params(q)) > 0, good
     assert clip.clip_workspace_bytes(0, 8, 8, ok) == 0
     rc, h = clip.clip_create(8, 8, 8, ok, 0, 1 << 30, 0)          # NULL workspace
     assert rc == clip.CLIP_EINVAL and not h

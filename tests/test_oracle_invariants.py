@@ -118,6 +118,64 @@ def test_lattice_symmetry_P9():
     assert np.abs(u3 - np.stack([-fl(u[0]), fl(u[1]), fl(u[2])])).max() < 1e-13
 
 
+def _mirror_extend(v, axes, sign_axis=None):
+    """Even (or, for the vector component normal to the mirror, odd) extension of v[z, y, x] across the halfway planes
+    of the given axes: index n + k <- n - 1 - k."""
+    for ax in axes:
+        m = np.flip(v, axis=ax)
+        if sign_axis is not None and ax == sign_axis:
+            m = -m
+        v = np.concatenate([v, m], axis=ax)
+    return v
+
+
+@pytest.mark.parametrize("faces", ["y", "xyz"])
+def test_free_slip_is_a_mirror_plane(faces):
+    """SURVEY 8(f) NEXT-3, free-slip faces (B.8-B.9): specular reflection half a cell outside the
+    last node makes the face a symmetry plane, so a box with free-slip faces must evolve exactly like one octant of
+    the mirror-extended PERIODIC box (phi, p, tangential u even; normal u odd) -- a run that never enters the
+    free-slip branch.  'y': free-slip on the two y faces, x / z periodic; 'xyz': all six faces (edges and corners
+    reflect two / three components).  Round-off only (the order of the sums over a changes)."""
+    nx, ny, nz = 10, 8, 6
+    case = inputs.sweep_drops(shape=(nx, ny, nz), ndrops=2, rmin=2.5, rmax=3.5, W=3.0, precision=64, u_amp=0.01)
+    FS, PE = inputs.FREESLIP, inputs.PERIODIC
+    axes = {"y": (1,), "xyz": (0, 1, 2)}[faces]              # numpy axes of [z, y, x] arrays
+    case["params"]["bc"] = tuple(FS if (2 - d) in axes else PE for d in (0, 0, 1, 1, 2, 2))
+    case["params"]["g"] = (2e-5, 0.0, 0.0) if faces == "y" else (0.0, 0.0, 0.0)   # gravity only along a tangential, unmirrored axis
+    phi, p, u = _run(case, 40)
+    big = dict(case)
+    big["params"] = dict(case["params"]); big["params"]["bc"] = (PE,) * 6
+    big["phi0"] = _mirror_extend(case["phi0"], axes)
+    big["u0"] = np.stack([_mirror_extend(case["u0"][c], axes, sign_axis=2 - c) for c in range(3)])
+    big["nz"], big["ny"], big["nx"] = big["phi0"].shape
+    phi2, p2, u2 = _run(big, 40)
+    sub = (slice(0, nz), slice(0, ny), slice(0, nx))
+    assert np.abs(phi2[sub] - phi).max() < 1e-13 and np.abs(p2[sub] - p).max() < 1e-13
+    assert np.abs(u2[(slice(None),) + sub] - u).max() < 1e-13
+    assert np.abs(phi - case["phi0"]).max() > 1e-3          # the run did something
+    # the normal velocity at the node next to the face stays small but the tangential one is free
+    assert np.abs(u).max() > 1e-3
+
+
+def test_free_slip_keeps_tangential_momentum():
+    """Free-slip y faces exert no tangential stress: with x / z periodic and no body force the total x- and z-momentum
+    sum rho u stays constant, whereas the same box with halfway bounce-back (B.10) loses it."""
+    FS, PE, WA = inputs.FREESLIP, inputs.PERIODIC, inputs.WALL
+    out = {}
+    for name, wall in (("slip", FS), ("noslip", WA)):
+        case = inputs.sweep_drops(shape=(8, 10, 6), ndrops=1, rmin=2.5, rmax=3.0, W=3.0, precision=64, u_amp=0.0)
+        case["params"].update(bc=(PE, PE, wall, wall, PE, PE), rho_h=1.0, rho_l=1.0, sigma=0.0)
+        case["u0"][0] += 0.02
+        case["u0"][2] -= 0.01
+        phi, p, u = _run(case, 60)
+        out[name] = (u[0].sum(), u[2].sum())
+        m0 = (0.02 * 480, -0.01 * 480)
+        if name == "slip":
+            assert abs(out[name][0] - m0[0]) < 1e-12 and abs(out[name][1] - m0[1]) < 1e-12
+        else:
+            assert out[name][0] < 0.95 * m0[0]
+
+
 def test_inlet_invariants_P13_G6():
     """P13: after the velocity-inlet rule (B.12-B.20 as read in G6) a node satisfies the two conditions the paper
     says it must: sum_a f_a e_a = u_in (B.12; F = 0 at the inlet, :1088) and sum_a g_a = phi_in

@@ -107,6 +107,8 @@ def test_tanh_equilibrium_profile_P3(runs, name):
 def _mu_rho(params):
     ta, tb, ra, rb = params["tau_a"], params["tau_b"], params["rho_a"], params["rho_b"]
     rho_of = lambda phi: rb + phi * (ra - rb)
+    if params["visc_interp"] == 2:  # Eq. 25 / 46b: the dynamic viscosity itself is linear in phi
+        return rho_of, (lambda phi: rb * tb / 3.0 + phi * (ra * ta / 3.0 - rb * tb / 3.0))
     if params["visc_interp"] == 1:
         tau_of = lambda phi: 1.0 / (1.0 / tb + phi * (1.0 / ta - 1.0 / tb))
     else:
@@ -151,6 +153,25 @@ def test_poiseuille_density_ratio_bgk(runs):
     ref = cf.poiseuille_quadrature(r["phi"], rho_of, mu_of, r["params"]["gx"])
     err = cf.l2_rel(r["ux"], ref)
     assert err < 0.02, err
+
+
+def test_poiseuille_linear_mu_eq25(runs):
+    """SURVEY 8(f) NEXT-6, visc_interp = 2 (Eq. 25): mu, not tau, is linear in phi -- exactly the
+    viscosity field of the paper's Poiseuille comparison, Eq. 46b.  The rho* = 10, mu* = 100 case
+    against the quadrature of Eq. 45 with mu(y) = mu_L + phi (mu_H - mu_L); the same run must NOT fit the
+    quadrature with the linear-tau viscosity of Eq. 24 (the two differ by ~10 % at this density ratio), so a mode
+    that silently fell back to Eq. 24 fails."""
+    r = runs.get("pois_rho10_mu")
+    assert r["du"] < 1e-12
+    rho_of, mu_of = _mu_rho(r["params"])
+    ref = cf.poiseuille_quadrature(r["phi"], rho_of, mu_of, r["params"]["gx"])
+    err = cf.l2_rel(r["ux"], ref)
+    print("Eq. 25 Poiseuille L2:", err)
+    assert err < 0.01, err
+    other = dict(r["params"]); other["visc_interp"] = 0
+    rho0, mu0 = _mu_rho(other)
+    err0 = cf.l2_rel(r["ux"], cf.poiseuille_quadrature(r["phi"], rho0, mu0, r["params"]["gx"]))
+    assert err0 > 5 * err and err0 > 0.02, (err, err0)
 
 
 def test_poiseuille_density_ratio_P7(runs):

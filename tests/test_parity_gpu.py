@@ -70,6 +70,14 @@ CASES = {
     "walled_box": (lambda: inputs.walled_box(), 100),
     "drop32_bgk": (lambda: _with(inputs.drop(), collision=1), 100),                       # BGK mode
     "jet_replica_bgk": (lambda: _with(inputs.jet(nxy=24, nz=48, r_nozzle=4.0), collision=1), 100),
+    # free-slip faces (B.8-B.9) -- all six (edges, corners), mixed with no-slip walls (wall wins), and the
+    # paper's jet set-up with free-slip side walls (PAPER.md:Sec. 6); NEXT-6: Eq. 25 viscosity interpolation
+    "freeslip_box": (lambda: _with(inputs.walled_box(), bc=(inputs.FREESLIP,) * 6), 100),
+    "freeslip_mixed": (lambda: _with(inputs.walled_box(nx=14, ny=12, nz=10), bc=(inputs.FREESLIP, inputs.WALL, inputs.WALL, inputs.FREESLIP, inputs.FREESLIP, inputs.FREESLIP)), 100),
+    "freeslip_channel": (lambda: _with(inputs.rayleigh_taylor(L=16, W=3.0), bc=(inputs.PERIODIC, inputs.PERIODIC, inputs.FREESLIP, inputs.FREESLIP, inputs.PERIODIC, inputs.PERIODIC)), 100),
+    "jet_freeslip_sides": (lambda: _with(inputs.jet(nxy=24, nz=48, r_nozzle=4.0), bc=(inputs.FREESLIP,) * 4 + (inputs.INLET, inputs.OUTLET)), 100),
+    "sweep64_linear_mu": (lambda: _with(inputs.sweep_drops(n=64), visc_interp=2, tau_l=0.3), 100),   # fused-free fast path
+    "rt_replica_linear_mu": (lambda: _with(inputs.rayleigh_taylor(L=16, W=3.0), visc_interp=2), 100),
     "odd_nx": (lambda: inputs.sweep_drops(shape=(21, 12, 10), ndrops=3, rmin=3, rmax=4), 60),   # generic kernels only
     "thin_z": (lambda: inputs.sweep_drops(shape=(32, 16, 2), ndrops=2, rmin=3, rmax=4), 60),   # nz < 4: generic kernels
 }
