@@ -350,7 +350,8 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       if (walls) launch_fused<T, true>(h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
       else launch_fused<T, false>(h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
       if (prof) { prof->end(KIND_FUSED); prof->begin(); }
-      clip::k_fix<T><<<dim3(fp.ytiles, fp.nchunks, (2 * fp.tzmax + 2 * (fp.ty - 2) + clip::FIX_ROWS - 1) / clip::FIX_ROWS), 128, 0, h->stream>>>(F, U);
+      const int fix_rpb = clip::FIX_ROWS * (clip::FIX_THREADS / clip::fix_threads_per_row(h->nx, clip::Vec16<T>::EV));  // rows per block
+      clip::k_fix<T><<<dim3(fp.ytiles, fp.nchunks, (2 * fp.tzmax + 2 * (fp.ty - 2) + fix_rpb - 1) / fix_rpb), clip::FIX_THREADS, 0, h->stream>>>(F, U);
       if (prof) prof->end(KIND_FIX);
       h->launches += 2;
       h->cur ^= 1;

@@ -204,10 +204,21 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP
 // phi(t+1) of the rows on a tile surface: own sum + the neighbour tiles' partials, fixed order.
 // Surface rows of a tile are numbered s = 0 .. 2 tzmax + 2 (ty - 2) - 1: [0, tzmax) the row ly = 0 of plane lz = s;
 // [tzmax, 2 tzmax) the row ly = ty-1; then the rows 1 .. ty-2 of the first plane and (if the tile has more than one
-// plane) of the last plane.  grid = (ytiles, nchunks, ceil(rows / FIX_ROWS)); block = 128 threads over the x pairs.
-constexpr int FIX_ROWS = 4;
-template <typename T> __global__ void __launch_bounds__(128) k_fix(const __grid_constant__ FP<T> FPp, const FusedP<T> U) {
-  typedef P2<T> V;
+// plane) of the last plane.  grid = (ytiles, nchunks, ceil(rows / (FIX_ROWS * rows_per_pass))); block = FIX_THREADS.
+constexpr int FIX_ROWS = 4;     // passes per block
+constexpr int FIX_THREADS = 128;
+// 16-byte accesses: 4 floats / 2 doubles per thread; a block covers rows_per_pass = FIX_THREADS / min(nx / EV, FIX_THREADS)
+// surface rows per pass.
+template <typename T> struct Vec16;
+template <> struct Vec16<float> { typedef float4 type; static constexpr int EV = 4; };
+template <> struct Vec16<double> { typedef double2 type; static constexpr int EV = 2; };
+__device__ __forceinline__ float4 vadd(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
+__device__ __forceinline__ double2 vadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__host__ __device__ __forceinline__ int fix_threads_per_row(int nx, int ev) { return nx / ev < FIX_THREADS ? nx / ev : FIX_THREADS; }
+
+template <typename T> __global__ void __launch_bounds__(FIX_THREADS) k_fix(const __grid_constant__ FP<T> FPp, const FusedP<T> U) {
+  typedef typename Vec16<T>::type W;
+  constexpr int EV = Vec16<T>::EV;
   const KP<T>& P = FPp.k;
   const int nx = P.nx;
   const int iy = blockIdx.x, c = blockIdx.y;
@@ -218,9 +229,12 @@ template <typename T> __global__ void __launch_bounds__(128) k_fix(const __grid_
     return U.part + (long long)(cc * U.ytiles + ii) * U.tile_stride + (long long)slot * nx;
   };
   const int nrows = 2 * U.tzmax + 2 * (U.ty - 2);
+  const int vpr = nx / EV, tv = fix_threads_per_row(nx, EV), rpp = FIX_THREADS / tv;
+  const int myrow = threadIdx.x / tv, v0 = threadIdx.x - myrow * tv;
+  if (myrow >= rpp) return;
 #pragma unroll 1
   for (int i = 0; i < FIX_ROWS; ++i) {
-    int s = blockIdx.z * FIX_ROWS + i, ly, lz;
+    int s = (blockIdx.z * FIX_ROWS + i) * rpp + myrow, ly, lz;
     if (s >= nrows) return;
     if (s < 2 * U.tzmax) { ly = s < U.tzmax ? 0 : U.ty - 1; lz = s < U.tzmax ? s : s - U.tzmax; if (lz >= tz) continue; }
     else {
@@ -242,10 +256,10 @@ template <typename T> __global__ void __launch_bounds__(128) k_fix(const __grid_
     if (yhi && zlo) src[ns++] = slab(cm, iyp, slot_zp(0, U.tzmax, U.ty));
     if (yhi && zhi) src[ns++] = slab(cp, iyp, slot_zm(0, U.tzmax));
     T* const row = U.phi_dst + ((long long)(z0 + lz) * P.ny + y) * nx;
-    for (int x0 = 2 * threadIdx.x; x0 < nx; x0 += 2 * blockDim.x) {
-      V v = ld_pair<T, LD_CA>(row + x0);
-      for (int k = 0; k < ns; ++k) v = v + ld_pair<T, LD_CA>(src[k] + x0);
-      st_pair<T>(row + x0, v);
+    for (int v = v0; v < vpr; v += tv) {
+      W a = __ldca(reinterpret_cast<const W*>(row) + v);
+      for (int k = 0; k < ns; ++k) a = vadd(a, __ldca(reinterpret_cast<const W*>(src[k]) + v));
+      reinterpret_cast<W*>(row)[v] = a;
     }
   }
 }

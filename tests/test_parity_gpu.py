@@ -261,6 +261,51 @@ def test_full_size_256_equals_tiled_64(precision, mode):
     sim.close()
 
 
+_full_size_ref = {}
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_full_size_lattices_against_the_oracle(precision):
+    """Direct oracle parity AT THE FULL BENCH SIZES, in the launch configurations bench.py times: the oracle runs one
+    periodic cell of the field, the GPU the full lattice made of 4 x 4 (x 4) copies of it, and every GPU node is compared
+    with the oracle value of its image (north_star tolerances, 20 steps).
+      * BASELINE configs[4] at 256^3 (k_fused + k_fix): cell = the 64^3 sweep field;
+      * BASELINE configs[2] lattice 128 x 512 x 128 with the RT parameters of the full case (walls in y; k_phi2 + k_step2,
+        walls instantiation): cell = 32 x 512 x 32 with the interface perturbed at wavelength 32 instead of 128."""
+    import torch
+    from paper_2505_12205_b200 import clip
+    steps = 20
+    small = inputs.sweep_drops(n=64)
+    rt = inputs.rayleigh_taylor(L=128)
+    z, y, x = np.meshgrid(np.arange(32.0), np.arange(512.0), np.arange(32.0), indexing="ij")
+    y0 = 256.0 + 0.05 * 128 * (np.cos(2 * np.pi * x / 32) + np.cos(2 * np.pi * z / 32))
+    cell = dict(rt, nx=32, ny=512, nz=32, phi0=0.5 + 0.5 * np.tanh(2.0 * (y - y0) / 5.0), u0=np.zeros((3, 32, 512, 32)),
+                name="rt_cell")
+    for case, reps, kernel in ((small, (4, 4, 4), "k_fused"), (cell, (4, 1, 4), "k_step2")):
+        if case["name"] not in _full_size_ref:
+            _full_size_ref[case["name"]] = _oracle(case, steps)
+        rphi, rp, ru = _full_size_ref[case["name"]]
+        big = dict(case)
+        big["nz"], big["ny"], big["nx"] = (case["nz"] * reps[0], case["ny"] * reps[1], case["nx"] * reps[2])
+        big["phi0"] = np.tile(case["phi0"], reps)
+        big["u0"] = np.tile(case["u0"], (1,) + reps)
+        sim = clip.Clip.from_case(big, precision=precision)
+        sim.step(steps)
+        phi, p, u = sim.get()
+        ran = {k for k, v in sim.step_profiled(1).items() if v[1]}
+        torch.cuda.synchronize()
+        assert kernel in ran, (case["name"], ran)        # the path bench.py times on this lattice
+        for name, got, want in (("phi", phi, rphi), ("p", p, rp), ("u", u, ru)):
+            want_t = torch.as_tensor(np.tile(want, (1,) * (want.ndim - 3) + reps)).to(got.device)
+            err = float((got.double() - want_t).abs().max())
+            scale = float(want_t.abs().max())
+            if precision == 64:
+                assert err <= FP64_ABS, (case["name"], name, err)
+            elif name != "p":
+                assert err <= (FP32_PHI if name == "phi" else FP32_U) * scale, (case["name"], name, err, scale)
+        sim.close()
+
+
 FUSED_LATTICES = {
     "periodic_128x24x20": lambda: inputs.sweep_drops(shape=(128, 24, 20), ndrops=6, rmin=3, rmax=6),
     "periodic_64x4x5": lambda: inputs.sweep_drops(shape=(64, 4, 5), ndrops=2, rmin=2, rmax=3),      # one y tile: the halo wraps onto the tile itself
