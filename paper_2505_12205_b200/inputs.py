@@ -122,6 +122,21 @@ def jet(nxy=192, nz=1536, r_nozzle=12.0, We=2.2, W=4.0, U=0.05, precision=32):
     return _case(nx, ny, nz, p, phi0, u0, f"jet{nxy}x{nz}")
 
 
+def capillary_wave(L0=256, nu=0.005, sigma=1.0e-4, W=4.0, M=0.02, rho_h=1.0, rho_l=0.1, eta0_rel=0.02, precision=64):
+    """PAPER.md Sec. 5.1 (:559-595, Fig. 7): L0 x 2 L0 (x 1) box, free-slip faces in x, no-slip walls in y; heavy fluid
+    below the interface y = L0 + eta0 cos(2 pi x / L0), eta0 = 0.02 L0; equal kinematic viscosity nu in both fluids;
+    sigma = 1e-4, xi = 4, M = 0.02 as printed.  The paper does not print the densities: rho_h / rho_l = 10 here.
+    Quasi-2D: nz = 1, periodic in z (D3Q19 with no z dependence)."""
+    nx, ny, nz = L0, 2 * L0, 1
+    x, y, z = _grid(nx, ny, nz)
+    yi = L0 + eta0_rel * L0 * np.cos(2 * np.pi * (x + 0.5) / L0)      # nodes at j + 1/2, faces at 0 and n
+    phi0 = 0.5 - 0.5 * np.tanh(2.0 * (y + 0.5 - yi) / W)
+    u0 = np.zeros((3, nz, ny, nx))
+    p = default_params(precision=precision, rho_h=rho_h, rho_l=rho_l, tau_h=3.0 * nu, tau_l=3.0 * nu, sigma=sigma, W=W, M=M,
+                       bc=(FREESLIP, FREESLIP, WALL, WALL, PERIODIC, PERIODIC))
+    return _case(nx, ny, nz, p, phi0, u0, f"capwave{L0}")
+
+
 def sweep_drops(n=64, seed=2505, ndrops=20, rmin=6.0, rmax=20.0, W=4.0, u_amp=0.01, precision=32,
                 shape=None):
     """BASELINE.json configs[4]: periodic box with `ndrops` seeded spherical drops and i.i.d. uniform u0.

@@ -68,3 +68,26 @@ def tanh_width_fit(phi_line, lo=0.05, hi=0.95):
         fit = 0.5 + 0.5 * np.tanh(s * r + c)
         out.append((W, float(np.abs(fit - phi_line[r]).max())))
     return out
+
+
+def prosperetti_capillary_wave(t, nu, k, sigma, rho_h, rho_l):
+    """Eq. 41-42 (Prosperetti 1981): eta(t)/eta0 of a small-amplitude capillary wave between two
+    fluids of equal kinematic viscosity nu, no gravity.  omega0^2 = sigma k^3 / (rho_h + rho_l), gamma = rho_h rho_l /
+    (rho_h + rho_l)^2, z_i the four roots of Eq. 42, Z_i = prod_{j != i} (z_j - z_i).  As printed, Eq. 41's first term reads
+    ".../(8(1-4 gamma) nu^2 k^4 + omega0)" and Eq. 42's constant term "(1-4 gamma) nu k^2 + omega0^2": dimensionally both
+    need omega0^2 and (nu k^2)^2 (Prosperetti's Eq. 21-22), which is what is evaluated here; eta(0) = 1 and the inviscid
+    limit cos(omega0 t) pin that reading (tests/test_oracle_pins.py).  erfc of a complex argument through the Faddeeva
+    function: erfc(x) = exp(-x^2) w(i x)."""
+    from scipy.special import wofz
+    t = np.maximum(np.asarray(t, dtype=np.float64), 1e-12)
+    w0sq = sigma * k ** 3 / (rho_h + rho_l)
+    gam = rho_h * rho_l / (rho_h + rho_l) ** 2
+    nk2 = nu * k * k
+    erfc = lambda x: np.exp(-x * x) * wofz(1j * x)
+    z = np.roots([1.0, -4 * gam * np.sqrt(nk2), 2 * (1 - 6 * gam) * nk2, 4 * (1 - 3 * gam) * nk2 ** 1.5,
+                  (1 - 4 * gam) * nk2 ** 2 + w0sq])
+    out = 4 * (1 - 4 * gam) * nk2 ** 2 / (8 * (1 - 4 * gam) * nk2 ** 2 + w0sq) * erfc(np.sqrt(nk2 * t) + 0j)
+    for i in range(4):
+        Z = np.prod([z[j] - z[i] for j in range(4) if j != i])
+        out = out + z[i] / Z * w0sq / (z[i] ** 2 - nk2) * np.exp((z[i] ** 2 - nk2) * t) * erfc(z[i] * np.sqrt(t))
+    return out.real

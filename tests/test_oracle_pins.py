@@ -184,3 +184,20 @@ def test_chemical_potential_on_tanh_P4_G4():
     G2, _, mu2 = o2.stencil_field(np.broadcast_to(prof2[:, None, None], (128, 4, 4)).copy())
     assert abs(1.5 * sigma * W2 * (G2[2][:, 0, 0] ** 2).sum() / sigma - 1) < 0.015
     assert np.abs(mu2).max() < 0.01 * (12 * sigma / W2)
+
+
+def test_prosperetti_closed_form_limits():
+    """The capillary-wave reference of Eq. 41-42 as restated in closed_forms.py: eta(0) = eta0; for
+    nu -> 0 it tends to the inviscid standing wave cos(omega0 t); for weak damping the envelope decays at about
+    2 nu k^2 (Lamb) -- fixes the two places where the printed formulas are dimensionally garbled."""
+    import closed_forms as cf
+    k, sigma, rh, rl = 2 * np.pi / 256, 1e-4, 1.0, 0.1
+    w0 = np.sqrt(sigma * k ** 3 / (rh + rl))
+    t = np.linspace(0.0, 3 * 2 * np.pi / w0, 400)
+    assert abs(cf.prosperetti_capillary_wave(np.array([0.0]), 0.005, k, sigma, rh, rl)[0] - 1.0) < 1e-6
+    inviscid = cf.prosperetti_capillary_wave(t, 1e-9, k, sigma, rh, rl)
+    assert np.abs(inviscid - np.cos(w0 * t)).max() < 2e-3
+    weak = cf.prosperetti_capillary_wave(t, 2e-4, k, sigma, rh, rl)
+    peaks = [i for i in range(1, len(t) - 1) if weak[i] > weak[i - 1] and weak[i] > weak[i + 1]]
+    rate = -np.log(weak[peaks[-1]] / weak[peaks[0]]) / (t[peaks[-1]] - t[peaks[0]])
+    assert 0.8 * 2 * 2e-4 * k * k < rate < 2.5 * 2 * 2e-4 * k * k, (rate, 2 * 2e-4 * k * k)
