@@ -281,6 +281,8 @@ void launch_tick2(int nx, unsigned items, dim3 b, cudaStream_t st, const clip::F
 }
 template <typename T> struct StepMinBlocks { static constexpr int value = 3; };  // k_step2 (128-thread blocks)
 template <> struct StepMinBlocks<double> { static constexpr int value = 1; };
+template <typename T> struct StepMinBlocksXWalls { static constexpr int value = 4; };  // 128 registers, 16 warps
+template <> struct StepMinBlocksXWalls<double> { static constexpr int value = 1; };
 template <typename T> struct TickMinBlocks { static constexpr int value = 2; };  // k_tick2 (__launch_bounds__(256, .))
 template <> struct TickMinBlocks<double> { static constexpr int value = 1; };
 
@@ -314,6 +316,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
   const bool fast = fast_ok(h);
   bool walls = false;
   for (int k = 0; k < 6; ++k) walls = walls || h->p.bc[k] == CLIP_BC_WALL;
+  const bool xwalls = h->p.bc[0] == CLIP_BC_WALL || h->p.bc[1] == CLIP_BC_WALL;
   dim3 fg, fb;
   bool tick = false;
   if (fast) fast_shape(h, fg, fb);
@@ -408,7 +411,9 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
         if (walls) launch_phi2<T, true>(h->nx_special, fg, fb, h->stream, F);
         else launch_phi2<T, false>(h->nx_special, fg, fb, h->stream, F);
       } else {
-        if (walls) launch_step2<T, true, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
+        // walls in x: most blocks run the branchy wall code, which wants warps more than registers (jet lattice: +6 %)
+        if (walls && xwalls) launch_step2<T, true, StepMinBlocksXWalls<T>::value>(h->nx_special, fg, fb, h->stream, F);
+        else if (walls) launch_step2<T, true, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
         else launch_step2<T, false, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
       }
       h->launches += 1;
