@@ -51,7 +51,8 @@ typedef struct clip_params {
   double inlet_phi;        /* phi_in, B.16 (:1069) */
   double inlet_c[2];       /* nozzle disc centre (x, y) in node coordinates */
   double inlet_r;          /* nozzle radius; nodes of the -z face outside the disc are WALL */
-  int outlet_u_mode;       /* 0 = U_local of B.22 (:1104); 1 (U_ave) and 2 (U_max) are not implemented */
+  int outlet_u_mode;       /* characteristic outlet velocity of B.22 (:1104), from u_z of layer N-1 at the previous time, clamped
+                              at 0: 0 = U_local (per column), 1 = U_ave (mean over the layer), 2 = U_max */
   int visc_interp;         /* 0 = linear tau, Eq. 24 (paper, Alg. 1); 1 = harmonic (1/tau linear in phi; non-paper);
                               2 = linear dynamic viscosity, Eq. 25 (:219): mu = rho tau / 3, tau = 3 mu(phi) / rho(phi) */
   int collision;           /* CLIP_COLL_WMRT (0, default): Eq. 27-28 + F_mu of Eq. 30; CLIP_COLL_BGK (1): Eq. 26 + F_mu of Eq. 29 */

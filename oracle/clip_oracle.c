@@ -38,7 +38,7 @@ typedef struct clipo_params {
   double g[3], rho_ref;    /* F_b = (rho - rho_ref) g [G16] */
   int bc[6];               /* -x,+x,-y,+y,-z,+z */
   double inlet_u[3], inlet_phi, inlet_c[2], inlet_r;
-  int outlet_u_mode;       /* 0 = U_local only */
+  int outlet_u_mode;       /* B.22: 0 = U_local, 1 = U_ave, 2 = U_max of u_z over layer N-1 */
   int visc_interp;         /* 0: Eq. 24 linear tau; 1: harmonic (1/tau linear; non-paper);
                               2: Eq. 25 linear dynamic viscosity mu = rho tau c_s^2, tau = 3 mu(phi) / rho(phi) */
   int collision;           /* 0: WMRT, Eq. 27-28, 30; 1: BGK, Eq. 26, 29 */
@@ -397,15 +397,25 @@ static void step_once(clipo *h) {
       inlet_node(h, h->f2 + i * Q, h->g2 + i * Q);
     }
   /* step 9: convective outlet on layer N = nz-1 (B.26-B.27), U_local = max(0, u_z(x,y,N-1,t)) [R12] */
-  if (bc[5] == BC_OUTLET)
+  if (bc[5] == BC_OUTLET) {
+    /* B.22: the plane-wide schemes take the mean / the maximum of the normal velocity over layer N-1 at the previous time */
+    double usum = 0.0, umax = h->uz[IDX(h, 0, 0, nz - 2)];
+    for (int y = 0; y < ny; ++y) for (int x = 0; x < nx; ++x) {
+      double v = h->uz[IDX(h, x, y, nz - 2)];
+      usum += v;
+      if (v > umax) umax = v;
+    }
+    double uplane = h->p.outlet_u_mode == 1 ? usum / ((double)nx * ny) : umax;
     for (int y = 0; y < ny; ++y) for (int x = 0; x < nx; ++x) {
       size_t iN = IDX(h, x, y, nz - 1), iM = IDX(h, x, y, nz - 2);
-      double lam = h->uz[iM] > 0.0 ? h->uz[iM] : 0.0;
+      double U = h->p.outlet_u_mode == 0 ? h->uz[iM] : uplane;
+      double lam = U > 0.0 ? U : 0.0; /* [R12] */
       for (int a = 0; a < Q; ++a) {
         h->f2[iN * Q + a] = (h->f[iN * Q + a] + lam * h->f2[iM * Q + a]) / (1.0 + lam);
         h->g2[iN * Q + a] = (h->g[iN * Q + a] + lam * h->g2[iM * Q + a]) / (1.0 + lam);
       }
     }
+  }
   double *tf = h->f; h->f = h->f2; h->f2 = tf;
   double *tg = h->g; h->g = h->g2; h->g2 = tg;
   /* step 10 */

@@ -136,7 +136,7 @@ const char* validate(int nx, int ny, int nz, const clip_params* p) {
   if (p->bc[5] == CLIP_BC_INLET) return "INLET is only supported on the -z face";
   if (p->bc[5] == CLIP_BC_OUTLET && nz < 2) return "OUTLET needs nz >= 2";
   if (p->bc[4] == CLIP_BC_INLET && !(p->inlet_r >= 0.0)) return "inlet_r must be >= 0";
-  if (p->outlet_u_mode != 0) return "outlet_u_mode 1 (U_ave) and 2 (U_max) are not implemented";
+  if (p->outlet_u_mode < 0 || p->outlet_u_mode > 2) return "outlet_u_mode must be 0 (U_local), 1 (U_ave) or 2 (U_max)";
   return nullptr;
 }
 
@@ -182,6 +182,7 @@ template <typename T> clip::KP<T> make_kp(const clip_handle* h) {
   P.has_inlet = p.bc[4] == CLIP_BC_INLET;
   P.has_outlet = p.bc[5] == CLIP_BC_OUTLET;
   P.visc_interp = p.visc_interp;
+  P.outlet_u_mode = p.outlet_u_mode;
   P.collision = p.collision;
   P.phase_only = p.phase_only;
   P.rho_h = (T)p.rho_h; P.rho_l = (T)p.rho_l; P.drho = (T)(p.rho_h - p.rho_l);
@@ -388,6 +389,10 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
     Plo.z_lo = 0; Plo.z_cnt = glo; Phi.z_lo = h->nz - ghi; Phi.z_cnt = ghi;
     clip::FP<T> F;
     if (fast) { F = make_fp<T>(P); F.k.z_lo = glo; F.k.z_cnt = h->nz - glo - ghi; fg.z = (unsigned)F.k.z_cnt; }
+    if (P.has_outlet && P.outlet_u_mode != 0) {  // B.22 U_ave / U_max from u(t), before anything of this step reads lam
+      clip::k_outlet_u<T><<<1, 1024, 0, h->stream>>>(P);
+      h->launches += 1;
+    }
     for (int pass = 0; pass < 2; ++pass) {  // pass 0: phi(t+1); pass 1: macros + collisions
       if (prof) prof->begin();
       if (!fast) {

@@ -51,7 +51,7 @@ template <typename T> struct KP {
   long long n;    // nodes
   long long nxy;  // nodes per z layer
   int bc[6];
-  int has_inlet, has_outlet, any_nonperiodic, visc_interp, collision, phase_only;
+  int has_inlet, has_outlet, any_nonperiodic, visc_interp, collision, phase_only, outlet_u_mode;
   int z_lo, z_cnt;  // planes [z_lo, z_lo + z_cnt) a k_phi* / k_step* launch covers (whole lattice: 0, nz)
   T rho_h, rho_l, drho;
   T tau_h, tau_l, itau_h, itau_l, rt_h, rt_l;  // rt = rho tau = 3 mu (Eq. 23, 25)
@@ -246,12 +246,12 @@ __device__ __forceinline__ void load_node(const KP<T>& P, int x, int y, int z, T
   if (outlet_layer) {
     const long long c = (long long)y * P.nx + x;
     T lam;
-    if (LAM_FROM_U) {  // U_local of B.22 from the stored u(t) of layer N-1, clamped at 0 (R12)
+    if (LAM_FROM_U && P.outlet_u_mode == 0) {  // U_local of B.22 from the stored u(t) of layer N-1, clamped at 0 (R12)
       lam = P.u[2 * P.n + i];
       lam = lam > T(0) ? lam : T(0);
       P.lam[c] = lam;
     } else {
-      lam = P.lam[c];
+      lam = P.lam[c];  // second pass of the step, or a plane-wide scheme (k_outlet_u)
     }
     const T inv = T(1) / (T(1) + lam);
 #pragma unroll
@@ -401,6 +401,31 @@ template <typename T> struct StoreAll<T, Q> {
 
 // ------------------------------------------------------------------------------------------------ kernels
 // k_phi: phi(t+1) = sum_a g_a(x,t+1)  (Eq. 38) from the post-collision g+(t); inlet nodes get phi_in.
+// Plane-wide outlet velocity of B.22: U_ave (mode 1) or U_max (mode 2) of u_z(., ., N-1, t), clamped at 0
+// (R12), written to every entry of `lam`.  One block, fixed reduction order (deterministic).
+template <typename T> __global__ void __launch_bounds__(1024) k_outlet_u(const __grid_constant__ KP<T> P) {
+  __shared__ T sh[1024];
+  const T* __restrict__ uz = P.u + 2 * P.n + (long long)(P.nz - 2) * P.nxy;
+  const bool ave = P.outlet_u_mode == 1;
+  T acc = ave ? T(0) : uz[0];
+  for (long long c = threadIdx.x; c < P.nxy; c += blockDim.x) {
+    const T v = uz[c];
+    acc = ave ? acc + v : (v > acc ? v : acc);
+  }
+  sh[threadIdx.x] = acc;
+  __syncthreads();
+  for (int s = blockDim.x / 2; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s) {
+      const T a = sh[threadIdx.x], b = sh[threadIdx.x + s];
+      sh[threadIdx.x] = ave ? a + b : (b > a ? b : a);
+    }
+    __syncthreads();
+  }
+  T U = ave ? sh[0] / T(P.nxy) : sh[0];
+  U = U > T(0) ? U : T(0);
+  for (long long c = threadIdx.x; c < P.nxy; c += blockDim.x) P.lam[c] = U;
+}
+
 template <typename T> __global__ void __launch_bounds__(256) k_phi(const __grid_constant__ KP<T> P) {
   const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= P.z_cnt * P.nxy) return;

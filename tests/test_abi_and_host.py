@@ -62,7 +62,7 @@ def test_validation_without_gpu():
         (dict(W=0.0), "W"),
         (dict(tau_l=-0.5), "tau"),
         (dict(M=-0.2), "tau_phi"),
-        (dict(outlet_u_mode=1), "outlet_u_mode"),
+        (dict(outlet_u_mode=3), "outlet_u_mode"),
         (dict(visc_interp=7), "visc_interp"),
     ):
         q = dict(p); q.update(bad)

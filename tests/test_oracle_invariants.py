@@ -219,21 +219,28 @@ def test_inlet_nodes_in_a_run():
     assert np.abs(g[0].sum(-1)[disc] - pp["inlet_phi"]).max() < 1e-15
 
 
-def test_outlet_recurrence_R12():
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_outlet_recurrence_R12(mode):
     """B.26-B.27: chi(N,t+1) (1 + lam) - chi(N,t) = lam chi(N-1,t+1) for all 38 populations,
-    with lam = max(0, u_z(N-1, t)) (U_local of B.22, reading R12)."""
+    with lam = max(0, U) and U one of the three schemes of B.22 evaluated on u_z(N-1, t) (reading R12):
+    0 = U_local (per column), 1 = U_ave (mean over the layer), 2 = U_max."""
     case = _jet_case()
+    case["params"]["outlet_u_mode"] = mode
+    rng = np.random.default_rng(5)
+    case["u0"][2] += 0.02 + 0.015 * rng.uniform(-1.0, 1.0, size=case["u0"][2].shape)   # outflow that varies over the layer
     o = Oracle.from_case(case)
-    o.step(12)
+    o.step(2)
     for _ in range(3):
         f0, g0 = o.populations()
         uz = o.get()[2][2]
         o.step(1)
         f1, g1 = o.populations()
-        lam = np.maximum(uz[-2], 0.0)[..., None]
+        U = uz[-2] if mode == 0 else (np.full_like(uz[-2], uz[-2].mean()) if mode == 1 else np.full_like(uz[-2], uz[-2].max()))
+        lam = np.maximum(U, 0.0)[..., None]
         for a0, a1 in ((f0, f1), (g0, g1)):
             assert np.abs(a1[-1] * (1 + lam) - a0[-1] - lam * a1[-2]).max() < 1e-15
     assert np.isfinite(f1).all() and np.isfinite(g1).all()
+    assert uz[-2].max() > 1.2 * uz[-2].mean() > 0 and np.ptp(uz[-2]) > 0.3 * uz[-2].mean()   # the three schemes really differ here
 
 
 def test_phase_only_mode():

@@ -78,6 +78,8 @@ CASES = {
     "jet_freeslip_sides": (lambda: _with(inputs.jet(nxy=24, nz=48, r_nozzle=4.0), bc=(inputs.FREESLIP,) * 4 + (inputs.INLET, inputs.OUTLET)), 100),
     "sweep64_linear_mu": (lambda: _with(inputs.sweep_drops(n=64), visc_interp=2, tau_l=0.3), 100),   # fused-free fast path
     "rt_replica_linear_mu": (lambda: _with(inputs.rayleigh_taylor(L=16, W=3.0), visc_interp=2), 100),
+    "jet_replica_uave": (lambda: _with(inputs.jet(nxy=24, nz=48, r_nozzle=4.0), outlet_u_mode=1), 150),   # B.22 U_ave
+    "jet_replica_umax": (lambda: _with(inputs.jet(nxy=24, nz=48, r_nozzle=4.0), outlet_u_mode=2), 150),   # B.22 U_max
     "capwave_replica": (lambda: inputs.capillary_wave(L0=32, sigma=5e-3), 200),     # Sec. 5.1 set-up at reduced size (nz = 1)
     "odd_nx": (lambda: inputs.sweep_drops(shape=(21, 12, 10), ndrops=3, rmin=3, rmax=4), 60),   # generic kernels only
     "thin_z": (lambda: inputs.sweep_drops(shape=(32, 16, 2), ndrops=2, rmin=3, rmax=4), 60),   # nz < 4: generic kernels
