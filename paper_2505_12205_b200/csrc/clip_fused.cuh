@@ -194,7 +194,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP
         step_pair<T, LD_NC, LD_NC, ST_WB, NX, false>(FPp, x0, y, z, NoWait(), sp);
       }
     }
-    __syncthreads();
+    __syncthreads();  // also keeps the block's warps on the same plane: without it the kernel is 4 % slower (L1 reuse)
     flush(lz - 1);
   }
   flush(tz - 1);
