@@ -78,7 +78,14 @@ int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params,
  * only says "Initialization", :341 -- DESIGN.md reading R8). */
 int clip_init(clip_t* h, const void* d_phi0, const void* d_u0);
 
-/* Advance n >= 0 time steps (Eq. 13, 33 with all of App. B); asynchronous on the stream. */
+/* Advance n >= 0 time steps (Eq. 13, 33 with all of App. B); asynchronous on the stream.
+ * Which kernels run is decided per lattice at clip_create: k_fused + k_fix on wide periodic / walled lattices,
+ * k_phi2 + k_step2 on the other lattices with even nx, the generic k_phi + k_step otherwise (and on the planes next to an
+ * INLET / OUTLET face, for FREESLIP faces, BGK and phase_only).  All paths compute the same step; they agree to round-off, and
+ * each is deterministic: clip_step(a); clip_step(b) equals clip_step(a + b) bit for bit.  Test / tuning switches read from the
+ * environment at clip_create (and, for the k_fused tiling, at clip_workspace_bytes): CLIP_FAST_MODE (3 = k_fused wherever the
+ * lattice admits it, 2 = k_phi2 + k_step2, 0 = k_tick2), CLIP_FORCE_GENERIC=1, CLIP_NO_NX_SPECIAL=1, CLIP_FUSED_TY,
+ * CLIP_FUSED_CHUNKS, CLIP_TICK_LAG. */
 int clip_step(clip_t* h, int n);
 
 /* phase_only mode: prescribe the velocity field u [3][nz][ny][nx] (device) that the following collisions use; the

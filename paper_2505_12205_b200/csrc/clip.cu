@@ -5,6 +5,7 @@
 #include "clip_fast.cuh"
 #include "clip_tick.cuh"
 #include "clip_fused.cuh"
+#include "clip_launch.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -43,13 +44,6 @@ struct FusedPlan {
 constexpr int B200_SMS = 148;
 
 
-// Resident threads per SM the k_fused instantiations are compiled for (__launch_bounds__): fp32 384 (<= 168 registers;
-// 12 warps with every load of a row in flight beat 16 warps at 128 registers, measured 17.3 vs 16.8 GLUPS at 256^3),
-// except 256-thread blocks (nx = 512 and the runtime-nx form), which keep 2 blocks; fp64 256 (255 registers).
-constexpr int fused_threads_per_sm(int precision, int block_threads) {
-  return precision == 32 ? (block_threads >= 256 ? 512 : 384) : 256;
-}
-
 FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   FusedPlan f{};
   if (p->collision != CLIP_COLL_WMRT || p->phase_only) return f;
@@ -62,7 +56,7 @@ FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   const int word = p->precision == 32 ? 4 : 8;
   const int nwarps = f.threads / 32;
   f.smem_bytes = (size_t)clip::FUSED_SLOTS * (f.ty + 2) * (nx + 2 * nwarps) * word;
-  int bps = fused_threads_per_sm(p->precision, f.threads) / f.threads;
+  int bps = clip::fused_threads_per_sm(p->precision, f.threads) / f.threads;
   if (bps > 32) bps = 32;
   if (bps < 1) bps = 1;
   while (bps > 1 && (f.smem_bytes + 1024) * bps > 227 * 1024) --bps;
@@ -156,11 +150,9 @@ struct clip_handle {
   int mode;            // fast-path variant (CLIP_FAST_MODE): unset = automatic (k_fused + k_fix on wide lattices, else k_phi2 + k_step2);
                        // 3 = k_fused wherever the lattice allows; 2 = k_phi2 + k_step2; 0 = k_tick2 (one launch)
   unsigned epoch;      // steps since clip_init (k_tick counters)
-  int tick_order;      // CLIP_TICK_ORDER (default 0): 0 = item number from blockIdx, 1 = from an atomic ticket
   int fast_threads;    // threads per block of the pair kernels (128)
   int nx_special;      // nx, or 0 when CLIP_NO_NX_SPECIAL=1 forces the runtime-nx kernels (tests)
   int tick_lag;        // CLIP_TICK_LAG (default 4, >= 3): groups between the phi job and the collision job of a plane (k_tick2)
-  int tick_hint;       // CLIP_TICK_HINT (default 1): streaming cache hints on single-use loads and on stores
   bool force_generic;  // CLIP_FORCE_GENERIC=1 in the environment at clip_create: generic kernels only (tests)
   long long launches;
   long long t;
@@ -250,60 +242,6 @@ void fast_shape(const clip_handle* h, dim3& grid, dim3& block) {
 }
 template <typename T> clip::FP<T> make_fp(const clip::KP<T>& P) { clip::FP<T> F; F.k = P; return F; }
 
-// nx values with their own instantiation of the fast kernels (direction offsets as immediates); others take NX = 0.
-#ifndef CLIP_NX_LIST
-#define CLIP_NX_LIST(X) X(64) X(128) X(192) X(256) X(384) X(512)
-#endif
-
-template <typename T, bool W> void launch_phi2(int nx, dim3 g, dim3 b, cudaStream_t st, const clip::FP<T>& F) {
-  switch (nx) {
-#define X(N) case N: clip::k_phi2<T, N, W><<<g, b, 0, st>>>(F); break;
-    CLIP_NX_LIST(X)
-#undef X
-    default: clip::k_phi2<T, 0, W><<<g, b, 0, st>>>(F);
-  }
-}
-template <typename T, bool W, int MB> void launch_step2(int nx, dim3 g, dim3 b, cudaStream_t st, const clip::FP<T>& F) {
-  switch (nx) {
-#define X(N) case N: clip::k_step2<T, N, W, MB><<<g, b, 0, st>>>(F); break;
-    CLIP_NX_LIST(X)
-#undef X
-    default: clip::k_step2<T, 0, W, MB><<<g, b, 0, st>>>(F);
-  }
-}
-template <typename T, bool W, int MB>
-void launch_tick2(int nx, unsigned items, dim3 b, cudaStream_t st, const clip::FP<T>& F, const clip::TickP& tk, int lag) {
-  switch (nx) {
-#define X(N) case N: clip::k_tick2<T, N, W, MB><<<items, b, 0, st>>>(F, tk, lag); break;
-    CLIP_NX_LIST(X)
-#undef X
-    default: clip::k_tick2<T, 0, W, MB><<<items, b, 0, st>>>(F, tk, lag);
-  }
-}
-template <typename T> struct StepMinBlocks { static constexpr int value = 3; };  // k_step2 (128-thread blocks)
-template <> struct StepMinBlocks<double> { static constexpr int value = 1; };
-template <typename T> struct StepMinBlocksXWalls { static constexpr int value = 4; };  // 128 registers, 16 warps
-template <> struct StepMinBlocksXWalls<double> { static constexpr int value = 1; };
-template <typename T> struct TickMinBlocks { static constexpr int value = 2; };  // k_tick2 (__launch_bounds__(256, .))
-template <> struct TickMinBlocks<double> { static constexpr int value = 1; };
-
-template <typename T, int NX, bool W> void launch_fused_nx(dim3 g, dim3 b, size_t smem, cudaStream_t st, const clip::FP<T>& F, const clip::FusedP<T>& U) {
-  constexpr int MAXT = NX ? NX / 2 : 256;
-  constexpr int TPSM = fused_threads_per_sm(sizeof(T) == 4 ? 32 : 64, MAXT);
-  constexpr int MINB = TPSM / MAXT > 0 ? TPSM / MAXT : 1;
-  auto kern = clip::k_fused<T, NX, W, MAXT, MINB>;
-  static bool attr_done = false;  // per instantiation
-  if (!attr_done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024); attr_done = true; }
-  kern<<<g, b, smem, st>>>(F, U);
-}
-template <typename T, bool W> void launch_fused(int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const clip::FP<T>& F, const clip::FusedP<T>& U) {
-  switch (nx) {
-#define X(N) case N: launch_fused_nx<T, N, W>(g, b, smem, st, F, U); break;
-    CLIP_NX_LIST(X)
-#undef X
-    default: launch_fused_nx<T, 0, W>(g, b, smem, st, F, U);
-  }
-}
 
 struct Prof {  // optional per-launch event timing (clip_step_profiled)
   std::vector<cudaEvent_t> ev;
@@ -339,8 +277,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       F.k.phi = phi_next;
       if (!h->phi_ahead) {
         if (prof) prof->begin();
-        if (walls) launch_phi2<T, true>(h->nx_special, fg, fb, h->stream, F);
-        else launch_phi2<T, false>(h->nx_special, fg, fb, h->stream, F);
+        clip::launch_phi2<T>(walls, h->nx_special, fg, fb, h->stream, F);
         if (prof) prof->end(KIND_PHI2);
         h->launches += 1;
         h->phi_ahead = true;
@@ -351,11 +288,10 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       U.ty = fp.ty; U.ytiles = fp.ytiles; U.nchunks = fp.nchunks; U.tzmax = fp.tzmax;
       U.tile_stride = (long long)(2 * fp.tzmax + 2 * (fp.ty + 2)) * h->nx;
       if (prof) prof->begin();
-      if (walls) launch_fused<T, true>(h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
-      else launch_fused<T, false>(h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+      clip::launch_fused<T>(walls, h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
       if (prof) { prof->end(KIND_FUSED); prof->begin(); }
       const int fix_rpb = clip::FIX_ROWS * (clip::FIX_THREADS / clip::fix_threads_per_row(h->nx, clip::Vec16<T>::EV));  // rows per block
-      clip::k_fix<T><<<dim3(fp.ytiles, fp.nchunks, (2 * fp.tzmax + 2 * (fp.ty - 2) + fix_rpb - 1) / fix_rpb), clip::FIX_THREADS, 0, h->stream>>>(F, U);
+      clip::launch_fix<T>(dim3(fp.ytiles, fp.nchunks, (2 * fp.tzmax + 2 * (fp.ty - 2) + fix_rpb - 1) / fix_rpb), h->stream, F, U);
       if (prof) prof->end(KIND_FIX);
       h->launches += 2;
       h->cur ^= 1;
@@ -375,8 +311,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       tk.base = 0;
       tk.target = (unsigned)tk.tp * h->epoch;
       if (prof) prof->begin();
-      if (walls) launch_tick2<T, true, TickMinBlocks<T>::value>(h->nx_special, items, fb, h->stream, F, tk, (int)lag);
-      else launch_tick2<T, false, TickMinBlocks<T>::value>(h->nx_special, items, fb, h->stream, F, tk, (int)lag);
+      clip::launch_tick2<T>(walls, h->nx_special, items, fb, h->stream, F, tk, (int)lag);
       if (prof) prof->end(KIND_TICK);
       h->launches += 1;
       h->cur ^= 1;
@@ -413,13 +348,9 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
         h->launches += 1;
       }
       if (pass == 0) {
-        if (walls) launch_phi2<T, true>(h->nx_special, fg, fb, h->stream, F);
-        else launch_phi2<T, false>(h->nx_special, fg, fb, h->stream, F);
+        clip::launch_phi2<T>(walls, h->nx_special, fg, fb, h->stream, F);
       } else {
-        // walls in x: most blocks run the branchy wall code, which wants warps more than registers (jet lattice: +6 %)
-        if (walls && xwalls) launch_step2<T, true, StepMinBlocksXWalls<T>::value>(h->nx_special, fg, fb, h->stream, F);
-        else if (walls) launch_step2<T, true, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
-        else launch_step2<T, false, StepMinBlocks<T>::value>(h->nx_special, fg, fb, h->stream, F);
+        clip::launch_step2<T>(walls, xwalls, h->nx_special, fg, fb, h->stream, F);
       }
       h->launches += 1;
       if (prof) prof->end(pass == 0 ? KIND_PHI2 : KIND_STEP2);
@@ -467,11 +398,9 @@ int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params,
   h->fplan = fused_plan(nx, ny, nz, params);
   { const char* e = getenv("CLIP_FORCE_GENERIC"); h->force_generic = e && e[0] == '1'; }
   { const char* e = getenv("CLIP_FAST_MODE"); h->mode = e ? atoi(e) : -1; h->epoch = 0; }
-  { const char* e = getenv("CLIP_TICK_ORDER"); h->tick_order = e ? atoi(e) : 0; }
   h->fast_threads = 128;  // measured: fp64 8.2 vs 7.6 GLUPS, fp32 (with 3 blocks per SM) +2 % against 256-thread blocks
   { const char* e = getenv("CLIP_NO_NX_SPECIAL"); h->nx_special = (e && e[0] == '1') ? 0 : nx; }
   { const char* e = getenv("CLIP_TICK_LAG"); h->tick_lag = e ? atoi(e) : 4; if (h->tick_lag < 3) h->tick_lag = 3; }
-  { const char* e = getenv("CLIP_TICK_HINT"); h->tick_hint = e ? atoi(e) : 1; }
   h->launches = 0; h->t = 0; h->err[0] = 0;
   if (params->bc[4] == CLIP_BC_INLET) {  // disc mask, decided in double on the host
     h->mask_host.resize((size_t)nx * ny);

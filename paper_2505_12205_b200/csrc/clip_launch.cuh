@@ -1,0 +1,26 @@
+// clip_launch.cuh -- host-side launch functions of the nx-specialised fast kernels.  They are declared here and DEFINED in
+// clip_launch_impl.cuh, which only the small clip_inst_*.cu translation units include (one per kernel family and precision,
+// explicit instantiations), so that the ~170 kernel instantiations compile in parallel instead of in one 3-minute unit.
+#pragma once
+#include "clip_fast.cuh"
+#include "clip_tick.cuh"
+#include "clip_fused.cuh"
+
+namespace clip {
+
+// Resident threads per SM the k_fused instantiations are compiled for (__launch_bounds__): fp32 384 (<= 168 registers;
+// 12 warps with every load of a row in flight beat 16 warps at 128 registers, measured 17.3 vs 16.8 GLUPS at 256^3),
+// except 256-thread blocks (nx = 512 and the runtime-nx form), which keep 2 blocks; fp64 256 (255 registers).
+constexpr int fused_threads_per_sm(int precision, int block_threads) {
+  return precision == 32 ? (block_threads >= 256 ? 512 : 384) : 256;
+}
+
+
+// walls: the lattice has WALL faces (WALLS instantiation); xwalls: it has them in x (k_step2 then keeps 16 warps per SM)
+template <typename T> void launch_phi2(bool walls, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F);
+template <typename T> void launch_step2(bool walls, bool xwalls, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F);
+template <typename T> void launch_tick2(bool walls, int nx, unsigned items, dim3 b, cudaStream_t st, const FP<T>& F, const TickP& tk, int lag);
+template <typename T> void launch_fused(bool walls, int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
+template <typename T> void launch_fix(dim3 g, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
+
+}  // namespace clip
