@@ -338,6 +338,29 @@ def test_fused_single_pass_path(name, precision):
             assert np.abs(a - b).max() <= tol * max(1.0, np.abs(a).max()), (name, env)
 
 
+def test_fused_path_is_deterministic_at_full_size():
+    """k_fused keeps phi's partial sums in a shared-memory ring that warps of a block fill and flush at different times
+    (one barrier per plane, warp-edge sends through side arrays) and hands tile halos over through `part`: any race would
+    show up as run-to-run differences.  Two runs of the bench lattice (256^3 fp32, 12 steps, default path) must agree bit
+    for bit, and sum(phi) must be conserved to fp32 round-off (a lost or doubled halo contribution would break it)."""
+    import torch
+    from paper_2505_12205_b200 import clip
+    case = inputs.sweep_drops(n=256)
+    outs = []
+    for _ in range(2):
+        sim = clip.Clip.from_case(case, precision=32)
+        sim.step(12)
+        outs.append([t.clone() for t in sim.get()])
+        ran = {k for k, v in sim.step_profiled(1).items() if v[1]}
+        sim.close()
+        assert "k_fused" in ran
+    torch.cuda.synchronize()
+    for a, b in zip(*outs):
+        assert torch.equal(a, b)
+    s0 = float(torch.as_tensor(case["phi0"]).double().sum())
+    assert abs(float(outs[0][0].double().sum()) - s0) / s0 < 1e-6
+
+
 def test_fused_path_time_semantics():
     """The fused path keeps phi one step ahead of the populations internally: clip_get must still return phi(t), a
     clip_get between steps must not disturb the run, and clip_step(a); clip_step(b) == clip_step(a + b) bit for bit."""
