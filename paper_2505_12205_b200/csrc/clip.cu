@@ -39,6 +39,7 @@ struct Layout {
 struct FusedPlan {
   bool ok, fills_gpu;
   int ty, ytiles, nchunks, tzmax, threads, blocks_per_sm;
+  int zc[clip::FUSED_MAX_CHUNKS + 1];  // chunk boundaries along z
   size_t part_words, smem_bytes;
 };
 constexpr int B200_SMS = 148;
@@ -63,20 +64,39 @@ FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   if (f.smem_bytes + 1024 > 227 * 1024) return f;
   f.blocks_per_sm = bps;
   const long long cap = (long long)B200_SMS * bps;
-  int nchunks = 0;
   const int max_chunks = nz / 4 > 0 ? nz / 4 : 1;
   f.fills_gpu = (long long)f.ytiles * max_chunks >= cap;
-  for (int m = 1; m <= 64; ++m) {
-    long long c = m * cap / f.ytiles;
-    if (c < 1) continue;
-    if (c > max_chunks) { if (nchunks == 0) nchunks = max_chunks; break; }
-    nchunks = (int)c;
-    if ((nz + nchunks - 1) / nchunks <= 16) break;
+  // Chunks along z, dispatched in order (blockIdx.y): long ones (<= 16 planes: little halo traffic) first, then about one
+  // wave of 8-plane and one wave of 4-plane chunks, so that the last blocks to finish are short ones (uniform chunks leave
+  // ~4 % of the SM time idle in the last wave).  Small lattices and CLIP_FUSED_CHUNKS=n (tests) take n equal chunks.
+  int nchunks = 0, uniform = 0;
+  { const char* e = getenv("CLIP_FUSED_CHUNKS"); if (e && atoi(e) >= 1 && atoi(e) <= nz) uniform = atoi(e); }
+  const int per_wave = (int)((cap + f.ytiles - 1) / f.ytiles);  // chunks that are resident at the same time
+  if (!uniform && 12 * per_wave <= nz / 2) {
+    const int rest = nz - 12 * per_wave, nl = (rest + 15) / 16;
+    int z = 0;
+    for (int k = 0; k < nl; ++k) { f.zc[nchunks++] = z; z += rest / nl + (k < rest % nl ? 1 : 0); }
+    for (int k = 0; k < per_wave; ++k) { f.zc[nchunks++] = z; z += 8; }
+    for (int k = 0; k < per_wave; ++k) { f.zc[nchunks++] = z; z += 4; }
+    f.zc[nchunks] = nz;
+  } else {
+    if (!uniform) {  // as many equal chunks as fill a whole number of waves, at most 16 planes each
+      for (int m = 1; m <= 64; ++m) {
+        long long c = m * cap / f.ytiles;
+        if (c < 1) continue;
+        if (c > max_chunks) { if (uniform == 0) uniform = max_chunks; break; }
+        uniform = (int)c;
+        if ((nz + uniform - 1) / uniform <= 16) break;
+      }
+      if (uniform < 1) uniform = 1;
+    }
+    nchunks = uniform;
+    for (int c = 0; c <= nchunks; ++c) f.zc[c] = (int)((long long)c * nz / nchunks);
   }
-  if (nchunks < 1) nchunks = 1;
-  { const char* e = getenv("CLIP_FUSED_CHUNKS"); if (e && atoi(e) >= 1 && atoi(e) <= nz) nchunks = atoi(e); }
+  if (nchunks > clip::FUSED_MAX_CHUNKS) return f;
   f.nchunks = nchunks;
-  f.tzmax = (nz + nchunks - 1) / nchunks;
+  f.tzmax = 1;
+  for (int c = 0; c < nchunks; ++c) f.tzmax = f.zc[c + 1] - f.zc[c] > f.tzmax ? f.zc[c + 1] - f.zc[c] : f.tzmax;
   f.part_words = (size_t)f.ytiles * nchunks * (2 * f.tzmax + 2 * (f.ty + 2)) * nx;
   f.ok = true;
   return f;
@@ -286,6 +306,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       U.phi_dst = phi_now;  // becomes phi(t+2); phi(t) is no longer needed once the time is t+1
       U.part = (T*)(h->ws + h->L.off_part);
       U.ty = fp.ty; U.ytiles = fp.ytiles; U.nchunks = fp.nchunks; U.tzmax = fp.tzmax;
+      for (int c = 0; c <= fp.nchunks; ++c) U.zc[c] = fp.zc[c];
       U.tile_stride = (long long)(2 * fp.tzmax + 2 * (fp.ty + 2)) * h->nx;
       if (prof) prof->begin();
       clip::launch_fused<T>(walls, h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);

@@ -24,13 +24,15 @@ namespace clip {
 
 constexpr int FUSED_SLOTS = 4;  // ring planes of k_fused: z-1, z, z+1 and the one being flushed
 
+constexpr int FUSED_MAX_CHUNKS = 256;
+
 template <typename T> struct FusedP {
   T* phi_dst;             // phi(t+1)                         [nz][ny][nx]
   T* part;                // partial sums of the tile halos   [tiles][2 tzmax + 2 (ty + 2)][nx]
   int ty, ytiles, nchunks, tzmax;
+  int zc[FUSED_MAX_CHUNKS + 1];  // chunk c covers the planes zc[c] .. zc[c+1]-1 (sizes <= tzmax; clip.cu: fused_plan)
   long long tile_stride;  // elements of `part` per tile
 };
-__host__ __device__ __forceinline__ int chunk_z0(int c, int nz, int nchunks) { return (int)((long long)c * nz / nchunks); }
 // rows of a tile's slab in `part`
 __host__ __device__ __forceinline__ int slot_ym(int k) { return k; }
 __host__ __device__ __forceinline__ int slot_yp(int k, int tzmax) { return tzmax + k; }
@@ -146,7 +148,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP
   T* edge_m = edge_p + nslots * rows * nwarps;
   const int x0 = 2 * threadIdx.x;
   const int iy = blockIdx.x, c = blockIdx.y;
-  const int y0 = iy * U.ty, z0 = chunk_z0(c, P.nz, U.nchunks), z1 = chunk_z0(c + 1, P.nz, U.nchunks);
+  const int y0 = iy * U.ty, z0 = U.zc[c], z1 = U.zc[c + 1];
   const int tz = z1 - z0;
   for (int i = threadIdx.x; i < nslots * rows * (nx + 2 * nwarps); i += blockDim.x) ring[i] = T(0);
   __syncthreads();
@@ -222,7 +224,7 @@ template <typename T> __global__ void __launch_bounds__(FIX_THREADS) k_fix(const
   const KP<T>& P = FPp.k;
   const int nx = P.nx;
   const int iy = blockIdx.x, c = blockIdx.y;
-  const int z0 = chunk_z0(c, P.nz, U.nchunks), tz = chunk_z0(c + 1, P.nz, U.nchunks) - z0;
+  const int z0 = U.zc[c], tz = U.zc[c + 1] - z0;
   const int iym = iy == 0 ? U.ytiles - 1 : iy - 1, iyp = iy == U.ytiles - 1 ? 0 : iy + 1;
   const int cm = c == 0 ? U.nchunks - 1 : c - 1, cp = c == U.nchunks - 1 ? 0 : c + 1;
   auto slab = [&](int cc, int ii, int slot) -> const T* {
