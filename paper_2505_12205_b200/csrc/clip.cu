@@ -37,7 +37,7 @@ struct Layout {
 // Tiling of the single-pass kernel k_fused (clip_fused.cuh): tiles of `ty` rows x one z chunk; the number of tiles is
 // chosen close to (and not above) a whole number of waves of resident blocks on the 148 SMs of a B200.
 struct FusedPlan {
-  bool ok, fills_gpu;
+  bool ok, fills_gpu, pays;
   int ty, ytiles, nchunks, tzmax, threads, blocks_per_sm;
   int zc[clip::FUSED_MAX_CHUNKS + 1];  // chunk boundaries along z
   size_t part_words, smem_bytes;
@@ -66,6 +66,8 @@ FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   const long long cap = (long long)B200_SMS * bps;
   const int max_chunks = nz / 4 > 0 ? nz / 4 : 1;
   f.fills_gpu = (long long)f.ytiles * max_chunks >= cap;
+  // measured: +4 .. +11 % at nx >= 256; at nx = 128 only with many waves of tiles (RT 128x512x128: +1 % fp32, +6 % fp64; 128^3: slower)
+  f.pays = (nx >= 256 && f.fills_gpu) || (nx >= 128 && (long long)f.ytiles * max_chunks >= 4 * cap);
   // Chunks along z, dispatched in order (blockIdx.y): long ones (<= 16 planes: little halo traffic) first, then about one
   // wave of 8-plane and one wave of 4-plane chunks, so that the last blocks to finish are short ones (uniform chunks leave
   // ~4 % of the SM time idle in the last wave).  Small lattices and CLIP_FUSED_CHUNKS=n (tests) take n equal chunks.
@@ -283,8 +285,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       h->ny % fb.y == 0) {
     tick = true;
   }
-  // k_fused pays on wide lattices with enough tiles to fill the GPU (measured: +4 .. +11 % at nx >= 256, slower at nx <= 128)
-  const bool fused = fast && h->fplan.ok && (h->mode == 3 || (h->mode < 0 && h->nx >= 256 && h->fplan.fills_gpu));
+  const bool fused = fast && h->fplan.ok && (h->mode == 3 || (h->mode < 0 && h->fplan.pays));
   for (int s = 0; s < nsteps; ++s) {
     clip::KP<T> P = make_kp<T>(h);
     if (fused) {  // one pass over f and g (clip_fused.cuh) + the tile-surface fix-up of phi(t+2)

@@ -273,7 +273,7 @@ def test_full_size_lattices_against_the_oracle(precision):
     periodic cell of the field, the GPU the full lattice made of 4 x 4 (x 4) copies of it, and every GPU node is compared
     with the oracle value of its image (north_star tolerances, 20 steps).
       * BASELINE configs[4] at 256^3 (k_fused + k_fix): cell = the 64^3 sweep field;
-      * BASELINE configs[2] lattice 128 x 512 x 128 with the RT parameters of the full case (walls in y; k_phi2 + k_step2,
+      * BASELINE configs[2] lattice 128 x 512 x 128 with the RT parameters of the full case (walls in y; k_fused + k_fix,
         walls instantiation): cell = 32 x 512 x 32 with the interface perturbed at wavelength 32 instead of 128."""
     import torch
     from paper_2505_12205_b200 import clip
@@ -284,7 +284,7 @@ def test_full_size_lattices_against_the_oracle(precision):
     y0 = 256.0 + 0.05 * 128 * (np.cos(2 * np.pi * x / 32) + np.cos(2 * np.pi * z / 32))
     cell = dict(rt, nx=32, ny=512, nz=32, phi0=0.5 + 0.5 * np.tanh(2.0 * (y - y0) / 5.0), u0=np.zeros((3, 32, 512, 32)),
                 name="rt_cell")
-    for case, reps, kernel in ((small, (4, 4, 4), "k_fused"), (cell, (4, 1, 4), "k_step2")):
+    for case, reps, kernel in ((small, (4, 4, 4), "k_fused"), (cell, (4, 1, 4), "k_fused")):
         if case["name"] not in _full_size_ref:
             _full_size_ref[case["name"]] = _oracle(case, steps)
         rphi, rp, ru = _full_size_ref[case["name"]]
