@@ -98,6 +98,23 @@ int clip_set_u(clip_t* h, const void* d_u);
  * (device; any may be NULL); asynchronous on the stream. */
 int clip_get(clip_t* h, void* d_phi, void* d_p, void* d_u);
 
+/* z-slab decomposition over several GPUs.  Streaming pulls every population from a neighbour at most one
+ * plane away (Eq. 13, 33; Alg. 2 :432-459) and the stencils of Eq. 40 (:309-331) read phi(t+1) = sum_a g+_a(x - e_a, t)
+ * one further plane away, so a slab that carries TWO ghost planes beyond each interior cut, refreshed after every step with the
+ * neighbour's outermost owned planes, computes its owned planes exactly as the undivided lattice does (the ghost planes
+ * themselves come out wrong and are overwritten).  clip_halo_pack copies the complete state of the planes [z0, z0 + nplanes)
+ * -- post-collision populations, phi(t), on the k_fused path also phi(t+1), u(t) -- into `d_buf` (device, 16-byte aligned,
+ * clip_halo_bytes(h, nplanes) bytes); clip_halo_unpack writes such a record, packed by a handle of the same nx, ny, precision,
+ * parameters and kernel path at the same time step, over the planes [z0, z0 + nplanes).  Both are asynchronous on the
+ * handle's stream and are device-to-device copies of contiguous plane ranges (no kernel, except that the first call after
+ * clip_init on a k_fused handle runs that path's one-time phi(t+1) pre-pass, so that the record is complete: the ghost planes
+ * must be refreshed once before the first step, because k_init's gradient is wrong on the outermost one); the transfer between GPUs is the
+ * caller's (paper_2505_12205_b200/slab.py: NCCL send / recv between z neighbours).  CLIP_ESTATE before clip_init,
+ * CLIP_EINVAL for planes outside the lattice or a bad buffer; clip_halo_bytes returns 0 for bad arguments. */
+size_t clip_halo_bytes(const clip_t* h, int nplanes);
+int clip_halo_pack(clip_t* h, int z0, int nplanes, void* d_buf);
+int clip_halo_unpack(clip_t* h, int z0, int nplanes, const void* d_buf);
+
 /* Free the handle (not the workspace). */
 int clip_destroy(clip_t* h);
 

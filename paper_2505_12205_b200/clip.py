@@ -80,6 +80,12 @@ def lib():
         L.clip_step_profiled.restype = C.c_int
         L.clip_step_profiled.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.clip_kernel_kinds.restype = C.c_int
+        L.clip_halo_bytes.restype = C.c_size_t
+        L.clip_halo_bytes.argtypes = [C.c_void_p, C.c_int]
+        L.clip_halo_pack.restype = C.c_int
+        L.clip_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        L.clip_halo_unpack.restype = C.c_int
+        L.clip_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.clip_kernel_name.restype = C.c_char_p
         L.clip_kernel_name.argtypes = [C.c_int]
         _lib = L
@@ -125,6 +131,18 @@ def clip_last_error(h=None) -> str:
 
 def clip_launch_count(h) -> int:
     return int(lib().clip_launch_count(h))
+
+
+def clip_halo_bytes(h, nplanes: int) -> int:
+    return int(lib().clip_halo_bytes(h, int(nplanes)))
+
+
+def clip_halo_pack(h, z0: int, nplanes: int, d_buf: int) -> int:
+    return lib().clip_halo_pack(h, int(z0), int(nplanes), C.c_void_p(d_buf))
+
+
+def clip_halo_unpack(h, z0: int, nplanes: int, d_buf: int) -> int:
+    return lib().clip_halo_unpack(h, int(z0), int(nplanes), C.c_void_p(d_buf))
 
 
 def clip_step_profiled(h, n: int):
@@ -213,6 +231,18 @@ class Clip:
         with self.torch.cuda.device(self.device):
             self._check(clip_get(self._h, phi.data_ptr() if phi is not None else 0,
                                  p.data_ptr() if p is not None else 0, u.data_ptr() if u is not None else 0))
+
+    def halo_buffer(self, nplanes):
+        """Device buffer (uint8) for the state record of `nplanes` planes (clip_halo_pack / clip_halo_unpack)."""
+        return self.torch.empty(clip_halo_bytes(self._h, nplanes), dtype=self.torch.uint8, device=self.device)
+
+    def halo_pack(self, z0, nplanes, buf):
+        with self.torch.cuda.device(self.device):
+            self._check(clip_halo_pack(self._h, z0, nplanes, buf.data_ptr()))
+
+    def halo_unpack(self, z0, nplanes, buf):
+        with self.torch.cuda.device(self.device):
+            self._check(clip_halo_unpack(self._h, z0, nplanes, buf.data_ptr()))
 
     def step_profiled(self, n=1):
         with self.torch.cuda.device(self.device):

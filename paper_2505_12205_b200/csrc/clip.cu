@@ -273,6 +273,24 @@ struct Prof {  // optional per-launch event timing (clip_step_profiled)
   void end(int k) { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, stream); ev.push_back(e); kind.push_back(k); }
 };
 
+bool use_fused(const clip_handle* h) { return fast_ok(h) && h->fplan.ok && (h->mode == 3 || (h->mode < 0 && h->fplan.pays)); }
+
+// k_fused path, once after clip_init: phi(t+1) = sum_a g+_a(x - e_a, t) into the second phi buffer (one k_phi2 launch).
+template <typename T> void fused_prepass(clip_handle* h, Prof* prof) {
+  if (h->phi_ahead) return;
+  bool walls = false;
+  for (int k = 0; k < 6; ++k) walls = walls || h->p.bc[k] == CLIP_BC_WALL;
+  dim3 fg, fb;
+  fast_shape(h, fg, fb);
+  clip::FP<T> F = make_fp<T>(make_kp<T>(h));
+  F.k.phi = (T*)(h->ws + (h->phi_cur ? h->L.off_phi : h->L.off_phi2));
+  if (prof) prof->begin();
+  clip::launch_phi2<T>(walls, h->nx_special, fg, fb, h->stream, F);
+  if (prof) prof->end(KIND_PHI2);
+  h->launches += 1;
+  h->phi_ahead = true;
+}
+
 template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullptr) {
   const bool fast = fast_ok(h);
   bool walls = false;
@@ -285,7 +303,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       h->ny % fb.y == 0) {
     tick = true;
   }
-  const bool fused = fast && h->fplan.ok && (h->mode == 3 || (h->mode < 0 && h->fplan.pays));
+  const bool fused = use_fused(h);
   for (int s = 0; s < nsteps; ++s) {
     clip::KP<T> P = make_kp<T>(h);
     if (fused) {  // one pass over f and g (clip_fused.cuh) + the tile-surface fix-up of phi(t+2)
@@ -296,13 +314,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       T* const phi_now = (T*)(h->ws + (h->phi_cur ? h->L.off_phi2 : h->L.off_phi));
       T* const phi_next = (T*)(h->ws + (h->phi_cur ? h->L.off_phi : h->L.off_phi2));
       F.k.phi = phi_next;
-      if (!h->phi_ahead) {
-        if (prof) prof->begin();
-        clip::launch_phi2<T>(walls, h->nx_special, fg, fb, h->stream, F);
-        if (prof) prof->end(KIND_PHI2);
-        h->launches += 1;
-        h->phi_ahead = true;
-      }
+      fused_prepass<T>(h, prof);
       clip::FusedP<T> U;
       U.phi_dst = phi_now;  // becomes phi(t+2); phi(t) is no longer needed once the time is t+1
       U.part = (T*)(h->ws + h->L.off_part);
@@ -390,9 +402,58 @@ template <typename T> int do_get(clip_handle* h, void* phi, void* p, void* u) {
   return check_cuda(h, "k_get");
 }
 
+// z-slab decomposition (clip.h): the state of `np` consecutive planes is six contiguous segments of the workspace
+// (z is the slowest index of every array): populations, phi(t), phi(t+1) (k_fused only), u_x, u_y, u_z.
+struct HaloSeg { size_t off, bytes; };
+int halo_segments(const clip_handle* h, int z0, int np, HaloSeg* seg) {
+  const size_t w = h->L.word, nxy = (size_t)h->nx * h->ny, n = nxy * h->nz;
+  int k = 0;
+  seg[k++] = {h->L.off_p[h->cur] + 38 * nxy * z0 * w, 38 * nxy * np * w};
+  seg[k++] = {(h->phi_cur ? h->L.off_phi2 : h->L.off_phi) + nxy * z0 * w, nxy * np * w};
+  if (h->fplan.ok) seg[k++] = {(h->phi_cur ? h->L.off_phi : h->L.off_phi2) + nxy * z0 * w, h->phi_ahead ? nxy * np * w : 0};
+  for (int c = 0; c < 3; ++c) seg[k++] = {h->L.off_u + (c * n + nxy * z0) * w, nxy * np * w};
+  return k;
+}
+int halo_copy(clip_handle* h, int z0, int np, char* buf, bool pack, const char* who) {
+  if (!h->inited) { set_err(h->err, "%s: clip_init has not been called", who); return CLIP_ESTATE; }
+  if (z0 < 0 || np < 0 || z0 + np > h->nz) { set_err(h->err, "%s: planes [%d, %d) are outside the lattice", who, z0, z0 + np); return CLIP_EINVAL; }
+  if (!buf || ((uintptr_t)buf) % 16) { set_err(h->err, "%s: buffer must be a 16-byte aligned device pointer", who); return CLIP_EINVAL; }
+  if (use_fused(h) && !h->phi_ahead) {  // the record of a k_fused handle carries phi(t+1): bring it into being first
+    if (h->p.precision == 32) fused_prepass<float>(h, nullptr); else fused_prepass<double>(h, nullptr);
+    const int rc = check_cuda(h, who);
+    if (rc != CLIP_OK) return rc;
+  }
+  HaloSeg seg[6];
+  const int ns = halo_segments(h, z0, np, seg);
+  const size_t slot = (size_t)h->nx * h->ny * np * h->L.word;  // the phi(t+1) slot is kept even while it is not yet valid
+  size_t o = 0;
+  for (int k = 0; k < ns; ++k) {
+    if (seg[k].bytes) {
+      cudaError_t e = pack ? cudaMemcpyAsync(buf + o, h->ws + seg[k].off, seg[k].bytes, cudaMemcpyDeviceToDevice, h->stream)
+                           : cudaMemcpyAsync(h->ws + seg[k].off, buf + o, seg[k].bytes, cudaMemcpyDeviceToDevice, h->stream);
+      if (e != cudaSuccess) { set_err(h->err, "%s: %s", who, cudaGetErrorString(e)); return CLIP_ECUDA; }
+    }
+    o += k == 0 ? seg[k].bytes : slot;
+  }
+  return CLIP_OK;
+}
+
 }  // namespace
 
 extern "C" {
+
+size_t clip_halo_bytes(const clip_t* h, int nplanes) {
+  if (!h || nplanes < 0) return 0;
+  return (size_t)h->nx * h->ny * nplanes * h->L.word * (38 + 1 + (h->fplan.ok ? 1 : 0) + 3);
+}
+int clip_halo_pack(clip_t* h, int z0, int nplanes, void* d_buf) {
+  if (!h) return CLIP_EINVAL;
+  return halo_copy(h, z0, nplanes, (char*)d_buf, true, "clip_halo_pack");
+}
+int clip_halo_unpack(clip_t* h, int z0, int nplanes, const void* d_buf) {
+  if (!h) return CLIP_EINVAL;
+  return halo_copy(h, z0, nplanes, (char*)d_buf, false, "clip_halo_unpack");
+}
 
 size_t clip_workspace_bytes(int nx, int ny, int nz, const clip_params* params) {
   const char* why = validate(nx, ny, nz, params);

@@ -1,0 +1,130 @@
+"""z-slab decomposition (include/clip.h clip_halo_pack / clip_halo_unpack; paper_2505_12205_b200/slab.py) on ONE GPU:
+the slabs of a lattice live in one process and are stepped one after the other (no kernel waits on another), the halo records
+change hands by device copies.  The owned planes must equal the undivided lattice -- bit for bit on the generic and the
+two-kernel paths (same arithmetic per node), to round-off on k_fused (phi is summed in tile order) -- and the oracle within
+the north_star tolerances."""
+import numpy as np
+import pytest
+
+from paper_2505_12205_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+def _whole(case, steps, precision):
+    import torch
+    from paper_2505_12205_b200 import clip
+    sim = clip.Clip.from_case(case, precision=precision)
+    sim.step(steps)
+    out = sim.get()
+    torch.cuda.synchronize()
+    sim.close()
+    return out
+
+
+def _slabs(case, steps, precision, world, chunks=None):
+    import torch
+    from paper_2505_12205_b200 import slab
+    params = dict(case["params"]); params["precision"] = precision
+    phi0, u0 = torch.as_tensor(case["phi0"]), torch.as_tensor(case["u0"])
+    group = [slab.SlabClip(case["nx"], case["ny"], case["nz"], params, r, world) for r in range(world)]
+    for s in group:
+        s.init(phi0, u0)
+    for c in (chunks or (steps,)):
+        slab.step_group(group, c)
+    parts = [s.get() for s in group]
+    torch.cuda.synchronize()
+    out = (torch.cat([p[0] for p in parts], 0), torch.cat([p[1] for p in parts], 0), torch.cat([p[2] for p in parts], 1))
+    assert all(s.exchanges == steps + 1 for s in group)
+    launches = sum(s.sim.launches for s in group)
+    for s in group:
+        s.close()
+    return out, launches
+
+
+CASES = {
+    "sweep64": (lambda: inputs.sweep_drops(n=64), 30, (1, 2, 4)),                       # periodic z, pair kernels
+    "rt_replica": (lambda: inputs.rayleigh_taylor(L=16, W=3.0), 30, (2, 4)),            # y walls, periodic z
+    "walled_box": (lambda: inputs.walled_box(nx=12, ny=10, nz=16), 30, (2, 4)),         # z walls: end slabs have one ghost side
+    "odd_box": (lambda: inputs.sweep_drops(shape=(21, 12, 36), ndrops=4, rmin=3, rmax=5), 30, (3,)),   # odd nx: generic kernels
+}
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("name", sorted(CASES))
+def test_slabs_equal_the_undivided_lattice(name, precision, monkeypatch):
+    import torch
+    monkeypatch.setenv("CLIP_FAST_MODE", "2")   # same per-node arithmetic whatever the tiling: bit for bit
+    make, steps, worlds = CASES[name]
+    case = make()
+    ref = _whole(case, steps, precision)
+    for world in worlds:
+        out, launches = _slabs(case, steps, precision, world, chunks=(steps - 7, 7))
+        assert launches > 0
+        for a, b, what in zip(out, ref, ("phi", "p", "u")):
+            assert torch.isfinite(a).all()
+            assert torch.equal(a, b), f"{name} fp{precision} {world} slabs: {what} differs, max {float((a - b).abs().max()):.3e}"
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_slabs_on_the_fused_path(precision, monkeypatch):
+    """k_fused keeps phi(t+1) as state: the record carries it (clip.h).  Equal to the undivided two-kernel run to round-off."""
+    import torch
+    case = inputs.sweep_drops(n=64)
+    steps = 30
+    monkeypatch.setenv("CLIP_FAST_MODE", "2")
+    ref = _whole(case, steps, precision)
+    monkeypatch.setenv("CLIP_FAST_MODE", "3")
+    for world in (2, 4):
+        out, _ = _slabs(case, steps, precision, world, chunks=(1, steps - 1))
+        tol = 1e-12 if precision == 64 else 3e-5
+        for a, b, what in zip(out, ref, ("phi", "p", "u")):
+            scale = float(b.abs().max())
+            err = float((a - b).abs().max()) / max(scale, 1e-300)
+            print(f"fused slabs fp{precision} world {world} {what}: {err:.2e} of field scale")
+            assert err <= tol or (precision == 32 and what == "p"), (what, world, err)   # fp32 p is not gated (north_star)
+
+
+def test_slabs_against_the_oracle():
+    """BASELINE configs[0] (drop, 32^3, 100 steps) on two and four slabs vs the CPU oracle: fp64 <= 1e-10, fp32 1e-4 / 1e-3."""
+    from oracle.clip_oracle import Oracle
+    case = inputs.drop()
+    o = Oracle.from_case(case)
+    o.step(100)
+    rphi, rp, ru = o.get()
+    for precision, world in ((64, 2), (64, 4), (32, 2)):
+        (phi, p, u), _ = _slabs(case, 100, precision, world)
+        phi, p, u = (t.double().cpu().numpy() for t in (phi, p, u))
+        if precision == 64:
+            assert np.abs(phi - rphi).max() <= 1e-10 and np.abs(p - rp).max() <= 1e-10 and np.abs(u - ru).max() <= 1e-10
+        else:
+            assert np.abs(phi - rphi).max() / np.abs(rphi).max() <= 1e-4
+            assert np.abs(u - ru).max() / max(np.abs(ru).max(), 1e-30) <= 1e-3
+
+
+def test_halo_abi_errors_and_roundtrip():
+    import torch
+    from paper_2505_12205_b200 import clip
+    case = inputs.sweep_drops(n=16, ndrops=3, rmin=3.0, rmax=5.0, W=3.0, precision=64)
+    sim = clip.Clip(16, 16, 16, case["params"])
+    buf = sim.halo_buffer(2)
+    assert buf.numel() == 16 * 16 * 2 * 8 * (38 + 1 + 3)     # no k_fused on this lattice: no phi(t+1) slot
+    assert clip.clip_halo_pack(sim._h, 0, 2, buf.data_ptr()) == clip.CLIP_ESTATE          # before clip_init
+    sim.init(torch.as_tensor(case["phi0"]), torch.as_tensor(case["u0"]))
+    assert clip.clip_halo_pack(sim._h, 15, 2, buf.data_ptr()) == clip.CLIP_EINVAL         # planes outside the lattice
+    assert clip.clip_halo_pack(sim._h, -1, 2, buf.data_ptr()) == clip.CLIP_EINVAL
+    assert clip.clip_halo_pack(sim._h, 0, 2, 0) == clip.CLIP_EINVAL
+    assert clip.clip_halo_bytes(sim._h, -1) == 0
+    sim.step(3)
+    before = sim.get()
+    n0 = sim.launches
+    sim.halo_pack(5, 2, buf)
+    sim.halo_unpack(5, 2, buf)                        # writing a record back where it came from changes nothing
+    assert sim.launches == n0                         # copies only, no kernel
+    after = sim.get()
+    assert all(torch.equal(a, b) for a, b in zip(before, after))
+    sim.halo_unpack(9, 2, buf)                        # planes 5, 6 now also sit at 9, 10
+    phi, p, u = sim.get()
+    assert torch.equal(phi[9:11], before[0][5:7]) and torch.equal(u[:, 9:11], before[2][:, 5:7]) and torch.equal(p[9:11], before[1][5:7])
+    assert torch.equal(phi[:9], before[0][:9]) and torch.equal(phi[11:], before[0][11:])
+    sim.close()
