@@ -269,6 +269,99 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_slab(args):
+    """`--decomp slab`: ONE periodic lattice n x n x (n * N) cut into N z slabs, one per GPU (weak scaling: n^3 owned nodes per
+    GPU), halo exchange of two planes per cut after every step (paper_2505_12205_b200/slab.py).  With N = 1
+    the slab is its own neighbour: the line then shows what packing, copying and unpacking the halos costs on one GPU."""
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as g
+    g.build()
+    from paper_2505_12205_b200 import inputs, slab
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    n, prec = args.n, args.precision
+    dtype = torch.float32 if prec == 32 else torch.float64
+    word = 4 if prec == 32 else 8
+    case = inputs.sweep_drops(shape=(n, n, n * world), seed=2505, ndrops=20 * world, precision=prec)   # same recipe, same drop density
+    sl = slab.SlabClip(n, n, n * world, case["params"], rank, world, device=dev)
+    idx = torch.as_tensor(sl.planes)
+    phi0_h = torch.as_tensor(case["phi0"]).index_select(0, idx).to(dtype).pin_memory()
+    u0_h = torch.as_tensor(case["u0"]).index_select(1, idx).to(dtype).pin_memory()
+    del case
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sl.sim.init(phi0_h, u0_h)
+    sl.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = sl.sim.launches
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(sl.sim.stream)
+    sl.step(args.steps)
+    e1.record(sl.sim.stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = sl.sim.launches - l0
+    clocks = sampler.stop() if rank == 0 else None
+    phi, p, u = sl.get()
+    finite = bool(torch.isfinite(phi).all() and torch.isfinite(u).all() and torch.isfinite(p).all())
+    # end to end: pinned host slab -> H2D -> init -> K steps with exchanges -> get -> D2H of the owned planes
+    own = sl.z1 - sl.z0
+    out = [torch.empty((own, n, n), dtype=dtype).pin_memory(), torch.empty((own, n, n), dtype=dtype).pin_memory(),
+           torch.empty((3, own, n, n), dtype=dtype).pin_memory()]
+    barrier()
+    t0 = time.perf_counter()
+    sl.exchanges = 0
+    sl.sim.init(phi0_h, u0_h)
+    sl.step(args.steps)
+    for o, d in zip(out, sl.get()):
+        o.copy_(d, non_blocking=True)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    ms, e2e_s, finite = reduce_over_ranks(ms, e2e_s, finite, world, dev)
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        nodes = n * n * n
+        mlups = whole_job_mlups(nodes, args.steps, ms, world)
+        achieved = B_MIN_WORDS * word * nodes / (ms / args.steps * 1e-3) / 1e9
+        h2d = (phi0_h.numel() + u0_h.numel()) * word
+        d2h = sum(o.numel() for o in out) * word
+        print(json.dumps({
+            "metric": "MLUPS", "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE configs[4] recipe on ONE periodic lattice {n}x{n}x{n * world} cut into {world} z slab(s), fp{prec}",
+                       "lattice": [n, n, n * world], "parallelism": f"z slabs, {slab.HALO} ghost planes per cut, neighbour send/recv after every step",
+                       "halo_bytes_sent_per_rank_per_step": sl.halo_bytes_per_step, "local_planes": sl.nz_local,
+                       "l2": f"state {sl.sim.workspace_bytes / 1e9:.2f} GB >> 126 MB L2, no flush needed", "finite_after_run": finite},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                         "peak_source": peak_src, "kernel": "whole step incl. ghost planes and halo copies",
+                         "note": "achieved = 84 words/LU x OWNED nodes / step time (CUDA events around the timed steps)"},
+            "e2e": {"value": world * nodes * args.steps / e2e_s / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": h2d / args.steps,
+                    "d2h_bytes_per_step": d2h / args.steps,
+                    "job": "pinned host slab -> H2D -> clip_init -> K x (clip_step(1) + halo exchange) -> clip_get -> D2H, wall clock"},
+            "clocks": clocks}))
+    sl.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -280,9 +373,13 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--workload", default="sweep", choices=["sweep", "rt", "jet"],
                     help="sweep = BASELINE configs[4] (headline); rt = configs[2] lattice (n/2 x 2n x n/2), walls in y; jet = configs[3] lattice (3n/4 x 3n/4 x 6n)")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replica per GPU (default) or one lattice n x n x (n N) cut into z slabs with halo exchange")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.decomp == "slab":
+        run_slab(args)
     else:
         run_ours(args)
 
