@@ -106,9 +106,10 @@ int clip_get(clip_t* h, void* d_phi, void* d_p, void* d_u);
  * -- post-collision populations, phi(t), on the k_fused path also phi(t+1), u(t) -- into `d_buf` (device, 16-byte aligned,
  * clip_halo_bytes(h, nplanes) bytes); clip_halo_unpack writes such a record, packed by a handle of the same nx, ny, precision,
  * parameters and kernel path at the same time step, over the planes [z0, z0 + nplanes).  Both are asynchronous on the
- * handle's stream and are device-to-device copies of contiguous plane ranges (no kernel, except that the first call after
- * clip_init on a k_fused handle runs that path's one-time phi(t+1) pre-pass, so that the record is complete: the ghost planes
- * must be refreshed once before the first step, because k_init's gradient is wrong on the outermost one); the transfer between GPUs is the
+ * handle's stream: ONE launch of a copy kernel over the record's contiguous plane ranges (16-byte accesses) per call (the
+ * first call after clip_init on a k_fused handle also runs that path's one-time phi(t+1) pre-pass, so that the record is
+ * complete: the ghost planes must be refreshed once before the first step, because k_init's gradient is wrong on the
+ * outermost one); the transfer between GPUs is the
  * caller's (paper_2505_12205_b200/slab.py: NCCL send / recv between z neighbours).  CLIP_ESTATE before clip_init,
  * CLIP_EINVAL for planes outside the lattice or a bad buffer; clip_halo_bytes returns 0 for bad arguments. */
 size_t clip_halo_bytes(const clip_t* h, int nplanes);

@@ -405,6 +405,22 @@ template <typename T> int do_get(clip_handle* h, void* phi, void* p, void* u) {
 // z-slab decomposition (clip.h): the state of `np` consecutive planes is six contiguous segments of the workspace
 // (z is the slowest index of every array): populations, phi(t), phi(t+1) (k_fused only), u_x, u_y, u_z.
 struct HaloSeg { size_t off, bytes; };
+struct HaloJob {  // up to six (source, destination) ranges, copied by ONE launch in units of U bytes
+  const char* src[6];
+  char* dst[6];
+  unsigned long long end[6];  // running sum of the ranges' unit counts
+  int ns;
+};
+template <typename U> __global__ void __launch_bounds__(256) k_halo(const HaloJob J) {
+  const unsigned long long total = J.end[J.ns - 1], stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride) {
+    int k = 0;
+#pragma unroll
+    for (int q = 0; q < 5; ++q) k += (q < J.ns - 1 && i >= J.end[q]) ? 1 : 0;
+    const unsigned long long j = i - (k ? J.end[k - 1] : 0ull);
+    reinterpret_cast<U*>(J.dst[k])[j] = reinterpret_cast<const U*>(J.src[k])[j];
+  }
+}
 int halo_segments(const clip_handle* h, int z0, int np, HaloSeg* seg) {
   const size_t w = h->L.word, nxy = (size_t)h->nx * h->ny, n = nxy * h->nz;
   int k = 0;
@@ -418,6 +434,7 @@ int halo_copy(clip_handle* h, int z0, int np, char* buf, bool pack, const char* 
   if (!h->inited) { set_err(h->err, "%s: clip_init has not been called", who); return CLIP_ESTATE; }
   if (z0 < 0 || np < 0 || z0 + np > h->nz) { set_err(h->err, "%s: planes [%d, %d) are outside the lattice", who, z0, z0 + np); return CLIP_EINVAL; }
   if (!buf || ((uintptr_t)buf) % 16) { set_err(h->err, "%s: buffer must be a 16-byte aligned device pointer", who); return CLIP_EINVAL; }
+  if (np == 0) return CLIP_OK;
   if (use_fused(h) && !h->phi_ahead) {  // the record of a k_fused handle carries phi(t+1): bring it into being first
     if (h->p.precision == 32) fused_prepass<float>(h, nullptr); else fused_prepass<double>(h, nullptr);
     const int rc = check_cuda(h, who);
@@ -426,16 +443,29 @@ int halo_copy(clip_handle* h, int z0, int np, char* buf, bool pack, const char* 
   HaloSeg seg[6];
   const int ns = halo_segments(h, z0, np, seg);
   const size_t slot = (size_t)h->nx * h->ny * np * h->L.word;  // the phi(t+1) slot is kept even while it is not yet valid
+  bool wide = true;  // 16-byte units when every range allows it (always on the lattices of the fast kernels), else 4-byte units
   size_t o = 0;
+  HaloJob J{};
   for (int k = 0; k < ns; ++k) {
     if (seg[k].bytes) {
-      cudaError_t e = pack ? cudaMemcpyAsync(buf + o, h->ws + seg[k].off, seg[k].bytes, cudaMemcpyDeviceToDevice, h->stream)
-                           : cudaMemcpyAsync(h->ws + seg[k].off, buf + o, seg[k].bytes, cudaMemcpyDeviceToDevice, h->stream);
-      if (e != cudaSuccess) { set_err(h->err, "%s: %s", who, cudaGetErrorString(e)); return CLIP_ECUDA; }
+      char* in_ws = h->ws + seg[k].off;
+      J.src[J.ns] = pack ? in_ws : buf + o;
+      J.dst[J.ns] = pack ? buf + o : in_ws;
+      J.end[J.ns] = seg[k].bytes;  // bytes for now
+      wide = wide && seg[k].bytes % 16 == 0 && ((uintptr_t)in_ws) % 16 == 0 && o % 16 == 0;
+      J.ns += 1;
     }
     o += k == 0 ? seg[k].bytes : slot;
   }
-  return CLIP_OK;
+  const unsigned unit = wide ? 16u : 4u;
+  unsigned long long run = 0;
+  for (int k = 0; k < J.ns; ++k) { run += J.end[k] / unit; J.end[k] = run; }
+  unsigned long long blocks = (run + 255) / 256;
+  if (blocks > (unsigned long long)B200_SMS * 8) blocks = (unsigned long long)B200_SMS * 8;
+  if (wide) k_halo<uint4><<<(unsigned)blocks, 256, 0, h->stream>>>(J);
+  else k_halo<unsigned><<<(unsigned)blocks, 256, 0, h->stream>>>(J);
+  h->launches += 1;
+  return check_cuda(h, who);
 }
 
 }  // namespace
