@@ -59,6 +59,11 @@ typedef struct clip_params {
   int phase_only;          /* 0 (default): full two-phase flow.  1: only the phase-field equation (Eq. 33) is advanced and
                               u is prescribed by the caller (clip_set_u) -- the set-up of the interface-in-shear-flow test,
                               PAPER.md:675-713 (Sec. 5.4); f stays 0, p is returned as 0 */
+  int path;                /* kernel path of clip_step (not part of the method; all paths compute the same step): 0 = automatic
+                              (see clip_step), 1 = generic kernels only, 2 = never k_fused (pair kernels where the lattice admits
+                              them), 3 = k_fused wherever the lattice admits it.  The slabs of one lattice must agree on whether
+                              phi(t+1) is part of the state (clip_halo_pack), so slabs with different faces are created with 2.
+                              The environment switches listed at clip_step override this field (tests) */
 } clip_params;
 
 typedef struct clip_handle clip_t;
@@ -110,8 +115,11 @@ int clip_get(clip_t* h, void* d_phi, void* d_p, void* d_u);
  * first call after clip_init on a k_fused handle also runs that path's one-time phi(t+1) pre-pass, so that the record is
  * complete: the ghost planes must be refreshed once before the first step, because k_init's gradient is wrong on the
  * outermost one); the transfer between GPUs is the
- * caller's (paper_2505_12205_b200/slab.py: NCCL send / recv between z neighbours).  CLIP_ESTATE before clip_init,
- * CLIP_EINVAL for planes outside the lattice or a bad buffer; clip_halo_bytes returns 0 for bad arguments. */
+ * caller's (paper_2505_12205_b200/slab.py: NCCL send / recv between z neighbours).  A physical z face of the whole lattice
+ * (WALL, FREESLIP, INLET, OUTLET) belongs to the first / last slab only; the cut faces of a slab may carry any non-periodic type
+ * (slab.py uses WALL), their planes are ghosts.  The outlet's U_ave / U_max (B.22) are taken over one x-y plane, which lies in the
+ * last slab: no reduction between slabs.  CLIP_ESTATE before clip_init, CLIP_EINVAL for planes outside the lattice or a bad buffer;
+ * clip_halo_bytes returns 0 for bad arguments. */
 size_t clip_halo_bytes(const clip_t* h, int nplanes);
 int clip_halo_pack(clip_t* h, int z0, int nplanes, void* d_buf);
 int clip_halo_unpack(clip_t* h, int z0, int nplanes, const void* d_buf);

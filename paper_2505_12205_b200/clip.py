@@ -28,6 +28,7 @@ class clip_params(C.Structure):
         ("inlet_u", C.c_double * 3), ("inlet_phi", C.c_double),
         ("inlet_c", C.c_double * 2), ("inlet_r", C.c_double),
         ("outlet_u_mode", C.c_int), ("visc_interp", C.c_int), ("collision", C.c_int), ("phase_only", C.c_int),
+        ("path", C.c_int),
     ]
 
 
@@ -44,6 +45,7 @@ def make_params(p: dict) -> clip_params:
     s.visc_interp = int(p["visc_interp"])
     s.collision = int(p.get("collision", 0))
     s.phase_only = int(p.get("phase_only", 0))
+    s.path = int(p.get("path", 0))
     return s
 
 

@@ -153,6 +153,7 @@ const char* validate(int nx, int ny, int nz, const clip_params* p) {
   if (p->bc[5] == CLIP_BC_OUTLET && nz < 2) return "OUTLET needs nz >= 2";
   if (p->bc[4] == CLIP_BC_INLET && !(p->inlet_r >= 0.0)) return "inlet_r must be >= 0";
   if (p->outlet_u_mode < 0 || p->outlet_u_mode > 2) return "outlet_u_mode must be 0 (U_local), 1 (U_ave) or 2 (U_max)";
+  if (p->path < 0 || p->path > 3) return "path must be 0 (automatic), 1 (generic), 2 (no k_fused) or 3 (k_fused where admitted)";
   return nullptr;
 }
 
@@ -426,7 +427,7 @@ int halo_segments(const clip_handle* h, int z0, int np, HaloSeg* seg) {
   int k = 0;
   seg[k++] = {h->L.off_p[h->cur] + 38 * nxy * z0 * w, 38 * nxy * np * w};
   seg[k++] = {(h->phi_cur ? h->L.off_phi2 : h->L.off_phi) + nxy * z0 * w, nxy * np * w};
-  if (h->fplan.ok) seg[k++] = {(h->phi_cur ? h->L.off_phi : h->L.off_phi2) + nxy * z0 * w, h->phi_ahead ? nxy * np * w : 0};
+  if (use_fused(h)) seg[k++] = {(h->phi_cur ? h->L.off_phi : h->L.off_phi2) + nxy * z0 * w, h->phi_ahead ? nxy * np * w : 0};
   for (int c = 0; c < 3; ++c) seg[k++] = {h->L.off_u + (c * n + nxy * z0) * w, nxy * np * w};
   return k;
 }
@@ -474,7 +475,7 @@ extern "C" {
 
 size_t clip_halo_bytes(const clip_t* h, int nplanes) {
   if (!h || nplanes < 0) return 0;
-  return (size_t)h->nx * h->ny * nplanes * h->L.word * (38 + 1 + (h->fplan.ok ? 1 : 0) + 3);
+  return (size_t)h->nx * h->ny * nplanes * h->L.word * (38 + 1 + (use_fused(h) ? 1 : 0) + 3);
 }
 int clip_halo_pack(clip_t* h, int z0, int nplanes, void* d_buf) {
   if (!h) return CLIP_EINVAL;
@@ -509,8 +510,8 @@ int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params,
   h->nx = nx; h->ny = ny; h->nz = nz; h->p = *params; h->L = L; h->ws = (char*)d_workspace;
   h->stream = (cudaStream_t)cuda_stream; h->cur = 0; h->phi_cur = 0; h->phi_ahead = false; h->inited = false;
   h->fplan = fused_plan(nx, ny, nz, params);
-  { const char* e = getenv("CLIP_FORCE_GENERIC"); h->force_generic = e && e[0] == '1'; }
-  { const char* e = getenv("CLIP_FAST_MODE"); h->mode = e ? atoi(e) : -1; h->epoch = 0; }
+  { const char* e = getenv("CLIP_FORCE_GENERIC"); h->force_generic = e ? e[0] == '1' : params->path == 1; }
+  { const char* e = getenv("CLIP_FAST_MODE"); h->mode = e ? atoi(e) : (params->path == 2 ? 2 : params->path == 3 ? 3 : -1); h->epoch = 0; }
   h->fast_threads = 128;  // measured: fp64 8.2 vs 7.6 GLUPS, fp32 (with 3 blocks per SM) +2 % against 256-thread blocks
   { const char* e = getenv("CLIP_NO_NX_SPECIAL"); h->nx_special = (e && e[0] == '1') ? 0 : nx; }
   { const char* e = getenv("CLIP_TICK_LAG"); h->tick_lag = e ? atoi(e) : 4; if (h->tick_lag < 3) h->tick_lag = 3; }

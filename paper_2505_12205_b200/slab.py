@@ -14,7 +14,7 @@ from __future__ import annotations
 
 HALO = 2  # ghost planes per interior cut (see the module docstring)
 
-_OPEN_BC = (2, 3)  # CLIP_BC_INLET, CLIP_BC_OUTLET
+_WALL = 1  # CLIP_BC_WALL
 
 
 def slab_range(nz: int, rank: int, world: int):
@@ -86,14 +86,11 @@ def exchange(send_lo, send_hi, recv_lo, recv_hi, rank: int, world: int, z_period
 
 
 class SlabClip:
-    """One rank's slab of a global nx x ny x nz lattice.  `params["bc"]` are the GLOBAL faces (z: PERIODIC, WALL or FREESLIP)."""
+    """One rank's slab of a global nx x ny x nz lattice.  `params["bc"]` are the GLOBAL faces (any type the library takes)."""
 
     def __init__(self, nx, ny, nz, params: dict, rank: int, world: int, device="cuda:0", stream=None):
         from . import clip
         bc = [int(v) for v in params["bc"]]
-        if bc[4] in _OPEN_BC or bc[5] in _OPEN_BC:
-            raise ValueError("slab decomposition: INLET / OUTLET z faces are not supported (the outlet's U_ave / U_max would "
-                             "need a reduction, SURVEY.md 8(e))")
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
         self.rank, self.world = int(rank), int(world)
         self.z_periodic = bc[4] == 0
@@ -101,8 +98,17 @@ class SlabClip:
         self.lo, self.hi = slab_ghosts(self.rank, self.world, self.z_periodic)
         self.planes = slab_plane_index(self.nz, self.rank, self.world, self.z_periodic)
         self.nz_local = len(self.planes)
-        # the local lattice keeps the global z boundary type on both faces: a ghost face may apply any rule, its planes are overwritten
-        self.sim = clip.Clip(self.nx, self.ny, self.nz_local, params, device=device, stream=stream)
+        # Local faces: a physical z face belongs to the first / last slab; a cut face may apply any rule (its planes are ghosts and are
+        # overwritten): PERIODIC on a periodic lattice (all slabs alike), else WALL.  Slabs with different faces or plane counts could
+        # choose different kernel paths; the record must agree on whether phi(t+1) is state, so they are created with path = 2.
+        local = dict(params)
+        if not self.z_periodic:
+            bc[4] = bc[4] if self.rank == 0 else _WALL
+            bc[5] = bc[5] if self.rank == self.world - 1 else _WALL
+            local["bc"] = tuple(bc)
+            if self.world > 1 and int(params.get("path", 0)) in (0, 3):
+                local["path"] = 2
+        self.sim = clip.Clip(self.nx, self.ny, self.nz_local, local, device=device, stream=stream)
         self.torch = self.sim.torch
         self.device = self.sim.device
         self.hp = halo_planes(self.nz_local, self.lo, self.hi)

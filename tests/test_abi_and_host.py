@@ -64,6 +64,7 @@ def test_validation_without_gpu():
         (dict(M=-0.2), "tau_phi"),
         (dict(outlet_u_mode=3), "outlet_u_mode"),
         (dict(visc_interp=7), "visc_interp"),
+        (dict(path=4), "path"),
     ):
         q = dict(p); q.update(bad)
         assert clip.clip_workspace_bytes(8, 8, 8, clip.make_params(q)) == 0

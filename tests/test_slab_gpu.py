@@ -42,11 +42,22 @@ def _slabs(case, steps, precision, world, chunks=None):
     return out, launches
 
 
-CASES = {
-    "sweep64": (lambda: inputs.sweep_drops(n=64), 30, (1, 2, 4)),                       # periodic z, pair kernels
-    "rt_replica": (lambda: inputs.rayleigh_taylor(L=16, W=3.0), 30, (2, 4)),            # y walls, periodic z
-    "walled_box": (lambda: inputs.walled_box(nx=12, ny=10, nz=16), 30, (2, 4)),         # z walls: end slabs have one ghost side
-    "odd_box": (lambda: inputs.sweep_drops(shape=(21, 12, 36), ndrops=4, rmin=3, rmax=5), 30, (3,)),   # odd nx: generic kernels
+def _with(case, **kw):
+    case["params"].update(kw)
+    return case
+
+
+CASES = {   # name: (case, steps, slab counts, environment)
+    "sweep64": (lambda: inputs.sweep_drops(n=64), 30, (1, 2, 4), {}),                       # periodic z, pair kernels
+    "rt_replica": (lambda: inputs.rayleigh_taylor(L=16, W=3.0), 30, (2, 4), {}),            # y walls, periodic z
+    "walled_box": (lambda: inputs.walled_box(nx=12, ny=10, nz=16), 30, (2, 4), {}),         # z walls: end slabs have one ghost side
+    "odd_box": (lambda: inputs.sweep_drops(shape=(21, 12, 36), ndrops=4, rmin=3, rmax=5), 30, (3,), {}),   # odd nx: generic kernels
+    # open z faces (BASELINE configs[3] replica): the inlet belongs to the first slab, the convective outlet to the last; planes
+    # z = 0 and nz-1 by the generic kernels in the slabs as in the undivided lattice.  U_max: the plane maximum lives in the last slab
+    "jet_replica": (lambda: inputs.jet(nxy=24, nz=96, r_nozzle=4.0), 40, (2, 3, 4), {}),
+    "jet_replica_umax": (lambda: _with(inputs.jet(nxy=24, nz=48, r_nozzle=4.0), outlet_u_mode=2), 40, (2,), {}),
+    # free-slip on all six faces: generic kernels everywhere (the cut faces of the inner slabs would otherwise take the pair kernels)
+    "freeslip_box": (lambda: _with(inputs.walled_box(nx=12, ny=10, nz=16), bc=(inputs.FREESLIP,) * 6), 30, (2, 4), {"CLIP_FORCE_GENERIC": "1"}),
 }
 
 
@@ -55,7 +66,9 @@ CASES = {
 def test_slabs_equal_the_undivided_lattice(name, precision, monkeypatch):
     import torch
     monkeypatch.setenv("CLIP_FAST_MODE", "2")   # same per-node arithmetic whatever the tiling: bit for bit
-    make, steps, worlds = CASES[name]
+    make, steps, worlds, env = CASES[name]
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
     case = make()
     ref = _whole(case, steps, precision)
     for world in worlds:
@@ -83,6 +96,22 @@ def test_slabs_on_the_fused_path(precision, monkeypatch):
             err = float((a - b).abs().max()) / max(scale, 1e-300)
             print(f"fused slabs fp{precision} world {world} {what}: {err:.2e} of field scale")
             assert err <= tol or (precision == 32 and what == "p"), (what, world, err)   # fp32 p is not gated (north_star)
+
+
+def test_walled_slabs_never_take_the_fused_path():
+    """Slabs with different faces / plane counts are created with path = 2 (clip.h): no phi(t+1) slot in the record, and the
+    result equals the undivided lattice created with the same path -- without any environment switch."""
+    import torch
+    case = inputs.sweep_drops(shape=(64, 16, 32), ndrops=4, rmin=3, rmax=6)
+    case["params"].update(bc=(inputs.PERIODIC,) * 4 + (inputs.WALL, inputs.WALL), path=2)
+    ref = _whole(case, 20, 32)
+    case["params"]["path"] = 0
+    from paper_2505_12205_b200 import slab
+    probe = slab.SlabClip(64, 16, 32, dict(case["params"], precision=32), 0, 2)
+    assert probe.send_lo is None and probe.send_hi.numel() == 64 * 16 * 2 * 4 * 42
+    probe.close()
+    out, _ = _slabs(case, 20, 32, 2)
+    assert all(torch.equal(a, b) for a, b in zip(out, ref))
 
 
 def test_slabs_against_the_oracle():
