@@ -30,6 +30,7 @@ def default_params(**kw) -> dict:
         inlet_u=(0.0, 0.0, 0.0), inlet_phi=1.0,
         inlet_c=(0.0, 0.0), inlet_r=0.0,
         outlet_u_mode=0, visc_interp=0, collision=0, phase_only=0,
+        path=0,  # libclip only: kernel path (include/clip.h); the oracle ignores it
     )
     p.update(kw)
     return p

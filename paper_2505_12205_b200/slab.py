@@ -71,6 +71,16 @@ def exchange(send_lo, send_hi, recv_lo, recv_hi, rank: int, world: int, z_period
             recv_hi.copy_(send_lo)
             recv_lo.copy_(send_hi)
         return
+    ref = send_lo if send_lo is not None else send_hi
+    if ref is not None and ref.is_cuda and dist.get_backend(group) == "gloo":
+        # no NCCL (tests: two processes sharing one GPU; boxes without peer access): stage the records through host memory
+        host = [None if t is None else t.cpu() for t in (send_lo, send_hi, recv_lo, recv_hi)]
+        exchange(*host, rank, world, z_periodic, group)
+        if recv_lo is not None:
+            recv_lo.copy_(host[2])
+        if recv_hi is not None:
+            recv_hi.copy_(host[3])
+        return
     ops = []
     if above is not None:
         ops.append(dist.P2POp(dist.isend, send_hi, above, group))

@@ -3,6 +3,11 @@ the slabs of a lattice live in one process and are stepped one after the other (
 change hands by device copies.  The owned planes must equal the undivided lattice -- bit for bit on the generic and the
 two-kernel paths (same arithmetic per node), to round-off on k_fused (phi is summed in tile order) -- and the oracle within
 the north_star tolerances."""
+import json
+import os
+import subprocess
+import sys
+
 import numpy as np
 import pytest
 
@@ -157,3 +162,58 @@ def test_halo_abi_errors_and_roundtrip():
     assert torch.equal(phi[9:11], before[0][5:7]) and torch.equal(u[:, 9:11], before[2][:, 5:7]) and torch.equal(p[9:11], before[1][5:7])
     assert torch.equal(phi[:9], before[0][:9]) and torch.equal(phi[11:], before[0][11:])
     sim.close()
+
+
+_DIST_WORKER = r"""
+import json, os, sys
+sys.path.insert(0, {root!r})
+os.environ["CLIP_FAST_MODE"] = "2"     # per-node arithmetic independent of the tiling: bit for bit
+import torch
+import torch.distributed as dist
+from paper_2505_12205_b200 import clip, inputs, slab
+
+dist.init_process_group("gloo")        # NCCL refuses two ranks on one GPU; the records are staged through the host
+rank, world = dist.get_rank(), dist.get_world_size()
+ok = True
+for make, steps in ((lambda: inputs.sweep_drops(shape=(32, 32, 36), ndrops=5, rmin=3, rmax=6), 25), (lambda: inputs.jet(nxy=24, nz=48, r_nozzle=4.0), 25)):
+    case = make()
+    params = dict(case["params"]); params["precision"] = 64
+    sl = slab.SlabClip(case["nx"], case["ny"], case["nz"], params, rank, world, device="cuda:0")
+    sl.init(torch.as_tensor(case["phi0"]), torch.as_tensor(case["u0"]))
+    sl.step(steps - 5)
+    sl.step(5)
+    mine = [t.cpu().contiguous() for t in sl.get()]
+    assert sl.exchanges == steps + 1
+    sl.close()
+    parts = [[torch.empty_like(t) for _ in range(world)] if rank == 0 else None for t in mine]
+    for t, dst in zip(mine, parts):
+        dist.gather(t, dst, dst=0)
+    if rank == 0:
+        whole = clip.Clip.from_case(case, precision=64)
+        whole.step(steps)
+        ref = [t.cpu() for t in whole.get()]
+        whole.close()
+        got = [torch.cat(parts[0], 0), torch.cat(parts[1], 0), torch.cat(parts[2], 1)]
+        ok = ok and all(torch.equal(a, b) for a, b in zip(got, ref))
+flag = torch.tensor([1 if ok else 0])
+dist.broadcast(flag, 0)
+if rank == 0:
+    print(json.dumps(dict(ok=bool(flag.item()), world=world)))
+dist.destroy_process_group()
+"""
+
+
+@pytest.mark.parametrize("world,port", [(2, 29751), (3, 29752)])
+def test_slab_ranks_as_processes(tmp_path, world, port):
+    """The distributed code path itself (SlabClip.step -> halo_exchange -> torch.distributed P2P): `world` processes, one slab
+    each, sharing the one GPU (no kernel waits on another: the exchange is host-synchronous over gloo), periodic box and jet
+    replica; the gathered owned planes equal the undivided lattice bit for bit."""
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "slab_dist_worker.py"
+    script.write_text(_DIST_WORKER.format(root=root))
+    out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={world}",
+                          "--master-addr", "127.0.0.1", "--master-port", str(port), str(script)],
+                         capture_output=True, text=True, timeout=600, cwd=root)
+    assert out.returncode == 0, out.stderr[-3000:]
+    r = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert r == {"ok": True, "world": world}
