@@ -291,11 +291,13 @@ def run_slab(args):
     n, prec = args.n, args.precision
     dtype = torch.float32 if prec == 32 else torch.float64
     word = 4 if prec == 32 else 8
-    case = inputs.sweep_drops(shape=(n, n, n * world), seed=2505, ndrops=20 * world, precision=prec)   # same recipe, same drop density
+    planes = slab.slab_plane_index(n * world, rank, world, True)
+    # same recipe and drop density; every rank builds only its own planes (ghosts included) of the global field
+    case = inputs.sweep_drops(shape=(n, n, n * world), seed=2505, ndrops=20 * world, precision=prec, z_planes=planes)
     sl = slab.SlabClip(n, n, n * world, case["params"], rank, world, device=dev)
-    idx = torch.as_tensor(sl.planes)
-    phi0_h = torch.as_tensor(case["phi0"]).index_select(0, idx).to(dtype).pin_memory()
-    u0_h = torch.as_tensor(case["u0"]).index_select(1, idx).to(dtype).pin_memory()
+    assert sl.planes == planes
+    phi0_h = torch.as_tensor(case["phi0"]).to(dtype).pin_memory()
+    u0_h = torch.as_tensor(case["u0"]).to(dtype).pin_memory()
     del case
 
     def barrier():

@@ -139,11 +139,14 @@ def capillary_wave(L0=256, nu=0.005, sigma=1.0e-4, W=4.0, M=0.02, rho_h=1.0, rho
 
 
 def sweep_drops(n=64, seed=2505, ndrops=20, rmin=6.0, rmax=20.0, W=4.0, u_amp=0.01, precision=32,
-                shape=None):
+                shape=None, z_planes=None):
     """BASELINE.json configs[4]: periodic box with `ndrops` seeded spherical drops and i.i.d. uniform u0.
 
     phi0 = max_k [0.5 + 0.5 tanh(2 (R_k - d_k)/W)] with d_k the periodic minimum-image distance.
     `shape=(nx,ny,nz)` gives a non-cubic box (used by the odd-size parity case).
+    `z_planes` (list of global z indices; the z-slab bench of a lattice too large to build whole on every rank) returns only those
+    planes of phi0 / u0 (nz of the case stays the global one); u0 is then drawn plane by plane from PCG64([seed, z]) -- a different
+    but equally seeded field, the same on whichever rank asks for the plane.
     """
     nx, ny, nz = (n, n, n) if shape is None else shape
     rng = np.random.Generator(np.random.PCG64(seed))
@@ -151,15 +154,19 @@ def sweep_drops(n=64, seed=2505, ndrops=20, rmin=6.0, rmax=20.0, W=4.0, u_amp=0.
     rad = rng.uniform(rmin, rmax, size=ndrops)
     x = np.arange(nx, dtype=np.float64)[None, None, :]
     y = np.arange(ny, dtype=np.float64)[None, :, None]
-    z = np.arange(nz, dtype=np.float64)[:, None, None]
-    phi0 = np.zeros((nz, ny, nx))
+    z = (np.arange(nz, dtype=np.float64) if z_planes is None else np.asarray(z_planes, dtype=np.float64))[:, None, None]
+    phi0 = np.zeros((z.shape[0], ny, nx))
     for k in range(ndrops):
         dx = np.abs(x - cen[k, 0]); dx = np.minimum(dx, nx - dx)
         dy = np.abs(y - cen[k, 1]); dy = np.minimum(dy, ny - dy)
         dz = np.abs(z - cen[k, 2]); dz = np.minimum(dz, nz - dz)
         d = np.sqrt(dx * dx + dy * dy + dz * dz)
         np.maximum(phi0, 0.5 + 0.5 * np.tanh(2.0 * (rad[k] - d) / W), out=phi0)
-    u0 = rng.uniform(-u_amp, u_amp, size=(3, nz, ny, nx))
+    if z_planes is None:
+        u0 = rng.uniform(-u_amp, u_amp, size=(3, nz, ny, nx))
+    else:
+        u0 = np.stack([np.random.Generator(np.random.PCG64([seed, int(zz)])).uniform(-u_amp, u_amp, size=(3, ny, nx))
+                       for zz in z_planes], axis=1)
     p = default_params(precision=precision, rho_h=1.0, rho_l=1.0e-3, tau_h=0.8, tau_l=0.8, sigma=0.01,
                        W=W, M=0.1)
     return _case(nx, ny, nz, p, phi0, u0, f"sweep{nx}x{ny}x{nz}")

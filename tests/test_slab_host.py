@@ -120,3 +120,19 @@ def test_single_periodic_slab_is_its_own_neighbour():
     ra, rb = torch.zeros(4), torch.zeros(4)
     slab.exchange(a, b, ra, rb, 0, 1, True)
     assert torch.equal(ra, b) and torch.equal(rb, a)
+
+
+def test_bench_input_planes_match_the_whole_field():
+    """`inputs.sweep_drops(z_planes=...)` (each rank of the slab bench builds only its own planes): phi0 equals the planes of the
+    whole field, u0 of a plane does not depend on who asks for it."""
+    import numpy as np
+    from paper_2505_12205_b200 import inputs
+    whole = inputs.sweep_drops(shape=(16, 12, 24), ndrops=4, rmin=3, rmax=5)
+    planes = slab.slab_plane_index(24, 0, 3, True)
+    assert planes == [22, 23, 0, 1, 2, 3, 4, 5, 6, 7, 8, 9]
+    part = inputs.sweep_drops(shape=(16, 12, 24), ndrops=4, rmin=3, rmax=5, z_planes=planes)
+    assert part["nz"] == 24 and part["phi0"].shape == (12, 12, 16) and part["u0"].shape == (3, 12, 12, 16)
+    assert np.array_equal(part["phi0"], whole["phi0"][planes])
+    other = inputs.sweep_drops(shape=(16, 12, 24), ndrops=4, rmin=3, rmax=5, z_planes=slab.slab_plane_index(24, 1, 3, True))
+    assert np.array_equal(other["u0"][:, :4], part["u0"][:, 8:12])       # planes 6..9: ghosts of rank 1, owned by rank 0
+    assert np.abs(part["u0"]).max() <= 0.01
