@@ -38,7 +38,8 @@ struct Geo {
   int cym, cyp, czm, czp, cxm, cxp;
 };
 
-template <typename T, bool WALLS = false> __device__ __forceinline__ Geo make_geo(const KP<T>& P, int x0, int y, int z) {
+// WALLS: 0 = periodic code, 1 = any wall face, 2 = wall faces in x only (blocks away from the y / z faces of a lattice walled in x)
+template <typename T, int WALLS = 0> __device__ __forceinline__ Geo make_geo(const KP<T>& P, int x0, int y, int z) {
   Geo g;
   const int nxy = P.nx * P.ny;
   g.x0 = x0;
@@ -54,8 +55,10 @@ template <typename T, bool WALLS = false> __device__ __forceinline__ Geo make_ge
   g.bym = g.byp = g.bzm = g.bzp = g.bxm = g.bxp = false;
   if (WALLS) {
     g.bxm = g.wm && P.bc[0] != BC_PERIODIC; g.bxp = g.wp && P.bc[1] != BC_PERIODIC;
-    g.bym = (y == 0) && P.bc[2] != BC_PERIODIC; g.byp = (y == P.ny - 1) && P.bc[3] != BC_PERIODIC;
-    g.bzm = (z == 0) && P.bc[4] != BC_PERIODIC; g.bzp = (z == P.nz - 1) && P.bc[5] != BC_PERIODIC;
+    if (WALLS == 1) {
+      g.bym = (y == 0) && P.bc[2] != BC_PERIODIC; g.byp = (y == P.ny - 1) && P.bc[3] != BC_PERIODIC;
+      g.bzm = (z == 0) && P.bc[4] != BC_PERIODIC; g.bzp = (z == P.nz - 1) && P.bc[5] != BC_PERIODIC;
+    }
     if (g.bxm) g.cxm = 0;
     if (g.bxp) g.cxp = 1;
     if (g.bym) g.cym = 0;
@@ -83,14 +86,16 @@ template <typename T, int sy, int sz> __device__ __forceinline__ const T* pop_ro
 // NX > 0: nx known at compile time (component offsets become immediates); NX == 0: runtime nx.
 // WALLS: a link that crosses a wall face takes the opposite population of the node itself (B.10-B.11; any wall crossing
 // wins at edges and corners, R11).
-template <typename T, int a, int H, int NX, int SET, bool WALLS>
+template <typename T, int a, int H, int NX, int SET, int WALLS>
 __device__ __forceinline__ P2<T> pull2(const T* __restrict__ src, int nx_rt, const Geo& g) {
   const int nx = NX ? NX : nx_rt;
   const T* __restrict__ rp = pop_row<T, -cy(a), -cz(a)>(src, g) + (SET * Q + a) * nx;
   if (WALLS && a > 0) {
     const T* __restrict__ own = pop_row<T, 0, 0>(src, g) + (SET * Q + copp(a)) * nx;
-    const bool rb = (cy(a) == 1 && g.bym) || (cy(a) == -1 && g.byp) || (cz(a) == 1 && g.bzm) || (cz(a) == -1 && g.bzp);
-    if (rb) return ld_pair<T, H>(own);
+    if (WALLS == 1) {
+      const bool rb = (cy(a) == 1 && g.bym) || (cy(a) == -1 && g.byp) || (cz(a) == 1 && g.bzm) || (cz(a) == -1 && g.bzp);
+      if (rb) return ld_pair<T, H>(own);
+    }
     if (cx(a) == 1 && g.bxm) return P2<T>(ld_one<T, H>(own), ld_one<T, H>(rp));
     if (cx(a) == -1 && g.bxp) return P2<T>(ld_one<T, H>(rp + 1), ld_one<T, H>(own + 1));
   }
@@ -98,13 +103,13 @@ __device__ __forceinline__ P2<T> pull2(const T* __restrict__ src, int nx_rt, con
   if (cx(a) == 1) return P2<T>(g.wm ? ld_one<T, H>(rp + (nx - 1)) : ld_one<T, H>(rp - 1), ld_one<T, H>(rp));
   return P2<T>(ld_one<T, H>(rp + 1), g.wp ? ld_one<T, H>(rp + (2 - nx)) : ld_one<T, H>(rp + 2));
 }
-template <typename T, int H, int NX, int SET, bool WALLS, int a = 0> struct Pull2All {
+template <typename T, int H, int NX, int SET, int WALLS, int a = 0> struct Pull2All {
   static __device__ __forceinline__ void run(const T* __restrict__ src, int nx, const Geo& g, P2<T> (&v)[Q]) {
     v[a] = pull2<T, a, H, NX, SET, WALLS>(src, nx, g);
     Pull2All<T, H, NX, SET, WALLS, a + 1>::run(src, nx, g, v);
   }
 };
-template <typename T, int H, int NX, int SET, bool WALLS> struct Pull2All<T, H, NX, SET, WALLS, Q> {
+template <typename T, int H, int NX, int SET, int WALLS> struct Pull2All<T, H, NX, SET, WALLS, Q> {
   static __device__ __forceinline__ void run(const T* __restrict__, int, const Geo&, P2<T> (&)[Q]) {}
 };
 // stores of set SET into the node pair's own population row `rd` (= pointer to component 0 of node x0)
@@ -317,8 +322,14 @@ template <typename T> __device__ __forceinline__ bool block_touches_wall(const K
          (z == 0 && P.bc[4] != BC_PERIODIC) || (z == P.nz - 1 && P.bc[5] != BC_PERIODIC);
 }
 
+// Block-uniform: a y or z wall face next to the block (if not, a block of a walled lattice can only meet the x faces: WALLS = 2)
+template <typename T> __device__ __forceinline__ bool block_touches_yz_wall(const KP<T>& P, int y0, int rows, int z) {
+  return (y0 == 0 && P.bc[2] != BC_PERIODIC) || (y0 + rows >= P.ny && P.bc[3] != BC_PERIODIC) ||
+         (z == 0 && P.bc[4] != BC_PERIODIC) || (z == P.nz - 1 && P.bc[5] != BC_PERIODIC);
+}
+
 // phi(t+1) = sum_a g_a(x,t+1) (Eq. 38) of one node pair by pulling the post-collision g+(t).
-template <typename T, int HG, int NX, bool WALLS> __device__ __forceinline__ void phi_pair(const FP<T>& FPp, int x0, int y, int z) {
+template <typename T, int HG, int NX, int WALLS> __device__ __forceinline__ void phi_pair(const FP<T>& FPp, int x0, int y, int z) {
   const KP<T>& P = FPp.k;
   const Geo geo = make_geo<T, WALLS>(P, x0, y, z);
   P2<T> g[Q];
@@ -335,7 +346,7 @@ template <typename T, int HG, int NX, bool WALLS> __device__ __forceinline__ voi
 // macros and f+ are computed and stored.
 struct NoWait { __device__ __forceinline__ void operator()() const {} };
 struct NoAfter { template <typename T> __device__ __forceinline__ void operator()(const Geo&, const P2<T> (&)[Q]) const {} };
-template <typename T, int HL, int HP, int HS, int NX, bool WALLS, typename W, typename A = NoAfter>
+template <typename T, int HL, int HP, int HS, int NX, int WALLS, typename W, typename A = NoAfter>
 __device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z, W before_phi, A after = A()) {
   typedef P2<T> V;
   const KP<T>& P = FPp.k;
@@ -369,8 +380,9 @@ __device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z
 template <typename T, int NX, bool WALLS> __global__ void __launch_bounds__(256) k_phi2(const __grid_constant__ FP<T> FPp) {
   int x0, y, z;
   if (!pair_coords(FPp.k, x0, y, z)) return;
-  if (WALLS && !block_touches_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) phi_pair<T, LD_NC, NX, false>(FPp, x0, y, z);
-  else phi_pair<T, LD_NC, NX, WALLS>(FPp, x0, y, z);
+  if (WALLS && !block_touches_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) phi_pair<T, LD_NC, NX, 0>(FPp, x0, y, z);
+  else if (WALLS && !block_touches_yz_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) phi_pair<T, LD_NC, NX, 2>(FPp, x0, y, z);
+  else phi_pair<T, LD_NC, NX, WALLS ? 1 : 0>(FPp, x0, y, z);
 }
 // 128-thread blocks; fp32: 3 blocks per SM (<= 168 registers: all ~100 loads of a node pair in flight at once, measured
 // faster than 4 blocks at 128 registers), fp64: what 255 registers allow.
@@ -378,8 +390,9 @@ template <typename T, int NX, bool WALLS, int MINB>
 __global__ void __launch_bounds__(128, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
   int x0, y, z;
   if (!pair_coords(FPp.k, x0, y, z)) return;
-  if (WALLS && !block_touches_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) step_pair<T, LD_NC, LD_NC, ST_WB, NX, false>(FPp, x0, y, z, NoWait());
-  else step_pair<T, LD_NC, LD_NC, ST_WB, NX, WALLS>(FPp, x0, y, z, NoWait());
+  if (WALLS && !block_touches_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) step_pair<T, LD_NC, LD_NC, ST_WB, NX, 0>(FPp, x0, y, z, NoWait());
+  else if (WALLS && !block_touches_yz_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) step_pair<T, LD_NC, LD_NC, ST_WB, NX, 2>(FPp, x0, y, z, NoWait());
+  else step_pair<T, LD_NC, LD_NC, ST_WB, NX, WALLS ? 1 : 0>(FPp, x0, y, z, NoWait());
 }
 
 }  // namespace clip
