@@ -28,7 +28,8 @@ B_MIN_WORDS = 84  # f 19R+19W, g 19R+19W, phi 1R+1W, u 3R+3W
 # captures (profiles/r01_fused_256_fp32.md, profiles/r01_fast_256_fp32.md); reported as roofline.traffic when the run
 # matches that configuration.
 NCU_TRAFFIC = {("k_fused", 256, 32, "sweep"): 2.950e9 + 2.824e9, ("k_fused", 256, 64, "sweep"): 6.030e9 + 5.688e9,
-               ("k_step2", 256, 32, "sweep"): 2.821e9 + 2.698e9}
+               ("k_step2", 256, 32, "sweep"): 2.821e9 + 2.698e9,
+               ("k_step2", 256, 32, "jet"): 9.503e9 + 9.266e9}   # profiles/r01_jet_step2_fp32.md
 
 
 def measured_peak():
