@@ -14,8 +14,10 @@
  *
  * Readings of garbled / silent passages are marked [Gn]/[Rn] below.
  * Parity pins: see tests/test_oracle_pins.py, test_oracle_invariants.py (free-slip = mirror plane), test_oracle_physics.py.
- * "parity unpinned" items: R9 (phi ghost at walls / open faces),
- * R12 (outlet U_local from stored u(t)), R13 (lagged u inside the macro update's F_mu).
+ * "parity unpinned" items: R9 at OPEN faces (phi ghost; both readings available: open_ghost), R12's time level of U (the
+ * paper's two sentences disagree, PAPER.md:1107 vs :1117; both readings available: outlet_u_time), R13 (lagged u inside the
+ * macro update's F_mu).  The algebra of B.25 itself (constant lambda: first-order upwind response, growth factor 1/(1+lambda)
+ * per step, hence unstable for lambda < 0 without the clamp) is pinned in tests/test_oracle_outlet.py.
  */
 #include <math.h>
 #include <stdlib.h>
@@ -44,6 +46,17 @@ typedef struct clipo_params {
   int collision;           /* 0: WMRT, Eq. 27-28, 30; 1: BGK, Eq. 26, 29 */
   int phase_only;          /* 1: only the phase-field LBE (Eq. 33) is advanced; u is prescribed (clipo_set_u), f stays 0:
                               the set-up of the interface-in-shear-flow test, PAPER.md:675-713 (Sec. 5.4) */
+  int outlet_clamp;        /* 0: lambda = U dt/dy exactly as B.25 prints it; 1: lambda = max(0, U) -- B.21 is an
+                              OUTFLOW condition; for U < 0 the implicit upwind form B.23-B.25 amplifies chi(N) - chi(N-1) by
+                              1/(1 + lambda) > 1 per step (pinned), the clamp replaces that by chi(N,t+dt) = chi(N,t) [R12] */
+  int outlet_u_time;       /* which U enters lambda [R12]: 0: the stored macroscopic u_z(x,y,N-1,t) ("computed based on the
+                              distribution function from the previous time step"); 1: the first moment
+                              sum_a e_az f_a(x,y,N-1,t+dt) of the post-stream populations ("lambda = U(t+dt) dt/dy, determined after
+                              the streaming step in the (N-1)th layer"), without the half-force term (F needs
+                              grad phi(t+dt), which involves the outlet layer itself) */
+  int open_ghost;          /* ORACLE ONLY, sensitivity of reading R9 at the OPEN parts of the z faces (inlet disc, outlet): 0: clamp
+                              (zero gradient, the reading the product takes); 1: linear extrapolation phi(-1) = 2 phi(0) - phi(1);
+                              the plate around the nozzle is a wall and keeps the mirror value */
 } clipo_params;
 
 typedef struct clipo {
@@ -128,9 +141,15 @@ static int ghost(int i, int n, int bc_lo, int bc_hi) {
   if (i >= n) return bc_hi == BC_PERIODIC ? i - n : n - 1;
   return i;
 }
+static int in_disc(const clipo *h, int x, int y);
+static int is_open(int bc) { return bc == BC_INLET || bc == BC_OUTLET; }
 static double phi_at(const clipo *h, const double *phi, int x, int y, int z) {
   x = ghost(x, h->nx, h->p.bc[0], h->p.bc[1]);
   y = ghost(y, h->ny, h->p.bc[2], h->p.bc[3]);
+  if (h->p.open_ghost == 1 && h->nz >= 2) { /* sensitivity variant of [R9]: linear extrapolation through open z faces */
+    if (z < 0 && is_open(h->p.bc[4]) && (h->p.bc[4] != BC_INLET || in_disc(h, x, y))) return 2.0 * phi[IDX(h, x, y, 0)] - phi[IDX(h, x, y, 1)];
+    if (z >= h->nz && is_open(h->p.bc[5])) return 2.0 * phi[IDX(h, x, y, h->nz - 1)] - phi[IDX(h, x, y, h->nz - 2)];
+  }
   z = ghost(z, h->nz, h->p.bc[4], h->p.bc[5]);
   return phi[IDX(h, x, y, z)];
 }
@@ -209,40 +228,46 @@ static void total_force(const clipo *h, const double *f, double pstar, double ux
   }
 }
 
+/* Barred equilibria and forcing terms of one node state -- the lines the collision executes (also exported for pin P12):
+ * F_a Eq. 19, feq Eq. 17, feq_bar Eq. 16; F^phi_a Eq. 34, geq = phi Gamma_a Eq. 36, geq_bar Eq. 35. */
+static void node_terms(const clipo *h, double pstar, const double *u, double phi, const double *F, const double *nvec,
+                       double *feqbar, double *Fa, double *geqbar, double *Fphi) {
+  double rho = rho_of(h, phi);
+  double pref = (1.0 - 4.0 * (phi - 0.5) * (phi - 0.5)) / h->p.W;
+  for (int a = 0; a < Q; ++a) {
+    double Gam = Gamma(h, a, u[0], u[1], u[2]);
+    Fa[a] = h->w[a] * (EX[a] * F[0] + EY[a] * F[1] + EZ[a] * F[2]) / (rho * (1.0 / 3.0));   /* Eq. 19 */
+    feqbar[a] = pstar * h->w[a] + (Gam - h->w[a]) - 0.5 * Fa[a];                           /* Eq. 16-17 */
+    Fphi[a] = pref * h->w[a] * (EX[a] * nvec[0] + EY[a] * nvec[1] + EZ[a] * nvec[2]);       /* Eq. 34 */
+    geqbar[a] = phi * Gam - 0.5 * Fphi[a];                                                 /* Eq. 35-36 */
+  }
+}
+
 /* Steps 1-6 of SURVEY 8(c) for one node: Alg. 1.  fin/gin pre-collision, fout/gout post. */
 static void collide_node(const clipo *h, const double *phi_field, int x, int y, int z, const double *fin,
                          const double *gin, double ux, double uy, double uz, double *fout, double *gout) {
   double phi = phi_field[IDX(h, x, y, z)];
-  double G[3], L, F[3];
+  double G[3], L, F[3] = {0.0, 0.0, 0.0};
   stencils(h, phi_field, x, y, z, G, &L);
   double pstar = 0.0;
   for (int a = 0; a < Q; ++a) pstar += fin[a]; /* Eq. 31a */
+  if (!h->p.phase_only) total_force(h, fin, pstar, ux, uy, uz, phi, G, L, F);
+  double nrm = sqrt(G[0] * G[0] + G[1] * G[1] + G[2] * G[2]) + 1e-32; /* [R10] */
+  double u[3] = {ux, uy, uz}, nvec[3] = {G[0] / nrm, G[1] / nrm, G[2] / nrm};
+  double feqbar[Q], Fa[Q], geqbar[Q], Fphi[Q];
+  node_terms(h, pstar, u, phi, F, nvec, feqbar, Fa, geqbar, Fphi);
   if (h->p.phase_only) { /* prescribed u: the hydrodynamic populations are not advanced */
     for (int a = 0; a < Q; ++a) fout[a] = fin[a];
-  } else {
-    total_force(h, fin, pstar, ux, uy, uz, phi, G, L, F);
-    double rho = rho_of(h, phi), tau = tau_of(h, phi), s_nu = 1.0 / (tau + 0.5);
-    /* hydrodynamic collision: Eq. 13, 16, 17, 19, 27 */
-    double r[Q], t[Q], Fa[Q];
-    for (int a = 0; a < Q; ++a) {
-      double feq = pstar * h->w[a] + (Gamma(h, a, ux, uy, uz) - h->w[a]);
-      Fa[a] = h->w[a] * (EX[a] * F[0] + EY[a] * F[1] + EZ[a] * F[2]) / (rho * (1.0 / 3.0));
-      double feqbar = feq - 0.5 * Fa[a];
-      r[a] = fin[a] - feqbar;
-    }
+  } else { /* hydrodynamic collision: Eq. 13 with Eq. 27 (or Eq. 26) */
+    double tau = tau_of(h, phi), s_nu = 1.0 / (tau + 0.5);
+    double r[Q], t[Q];
+    for (int a = 0; a < Q; ++a) r[a] = fin[a] - feqbar[a];
     apply_collision(h, s_nu, r, t);
     for (int a = 0; a < Q; ++a) fout[a] = fin[a] - t[a] + Fa[a];
   }
-  /* phase-field collision: Eq. 33-36, tau_phi = M / c_s^2 (Eq. 37) */
+  /* phase-field collision: Eq. 33, tau_phi = M / c_s^2 (Eq. 37) */
   double tau_phi = 3.0 * h->p.M, om = 1.0 / (tau_phi + 0.5);
-  double nrm = sqrt(G[0] * G[0] + G[1] * G[1] + G[2] * G[2]) + 1e-32; /* [R10] */
-  double nxv = G[0] / nrm, nyv = G[1] / nrm, nzv = G[2] / nrm;
-  double pref = (1.0 - 4.0 * (phi - 0.5) * (phi - 0.5)) / h->p.W;
-  for (int a = 0; a < Q; ++a) {
-    double Fphi = pref * h->w[a] * (EX[a] * nxv + EY[a] * nyv + EZ[a] * nzv); /* Eq. 34 */
-    double geqbar = phi * Gamma(h, a, ux, uy, uz) - 0.5 * Fphi;              /* Eq. 35-36 */
-    gout[a] = gin[a] - om * (gin[a] - geqbar) + Fphi;                        /* Eq. 33 */
-  }
+  for (int a = 0; a < Q; ++a) gout[a] = gin[a] - om * (gin[a] - geqbar[a]) + Fphi[a];
 }
 
 /* Velocity inlet on one node, App. B.4 as read in [G6]: inward normal +z, unknown set =
@@ -396,25 +421,33 @@ static void step_once(clipo *h) {
       size_t i = IDX(h, x, y, 0);
       inlet_node(h, h->f2 + i * Q, h->g2 + i * Q);
     }
-  /* step 9: convective outlet on layer N = nz-1 (B.26-B.27), U_local = max(0, u_z(x,y,N-1,t)) [R12] */
+  /* step 9: convective outlet on layer N = nz-1 (B.26-B.27); lambda = U dt/dy with U one of
+   * the three schemes of B.22 built on the normal velocity of layer N-1 [R12: outlet_u_time, outlet_clamp] */
   if (bc[5] == BC_OUTLET) {
-    /* B.22: the plane-wide schemes take the mean / the maximum of the normal velocity over layer N-1 at the previous time */
-    double usum = 0.0, umax = h->uz[IDX(h, 0, 0, nz - 2)];
+    double *Ucol = (double *)malloc((size_t)nx * ny * sizeof(double));
+    double usum = 0.0, umax = 0.0;
     for (int y = 0; y < ny; ++y) for (int x = 0; x < nx; ++x) {
-      double v = h->uz[IDX(h, x, y, nz - 2)];
+      size_t iM = IDX(h, x, y, nz - 2);
+      double v;
+      if (h->p.outlet_u_time == 1 && !h->p.phase_only) { /* first moment of the post-stream f of layer N-1 at t+dt */
+        v = 0.0;
+        for (int a = 0; a < Q; ++a) v += EZ[a] * h->f2[iM * Q + a];
+      } else v = h->uz[iM];                               /* stored macroscopic velocity of the previous time step */
+      Ucol[(size_t)y * nx + x] = v;
       usum += v;
-      if (v > umax) umax = v;
+      if ((x == 0 && y == 0) || v > umax) umax = v;
     }
     double uplane = h->p.outlet_u_mode == 1 ? usum / ((double)nx * ny) : umax;
     for (int y = 0; y < ny; ++y) for (int x = 0; x < nx; ++x) {
       size_t iN = IDX(h, x, y, nz - 1), iM = IDX(h, x, y, nz - 2);
-      double U = h->p.outlet_u_mode == 0 ? h->uz[iM] : uplane;
-      double lam = U > 0.0 ? U : 0.0; /* [R12] */
+      double U = h->p.outlet_u_mode == 0 ? Ucol[(size_t)y * nx + x] : uplane;
+      double lam = (h->p.outlet_clamp && U < 0.0) ? 0.0 : U;
       for (int a = 0; a < Q; ++a) {
         h->f2[iN * Q + a] = (h->f[iN * Q + a] + lam * h->f2[iM * Q + a]) / (1.0 + lam);
         h->g2[iN * Q + a] = (h->g[iN * Q + a] + lam * h->g2[iM * Q + a]) / (1.0 + lam);
       }
     }
+    free(Ucol);
   }
   double *tf = h->f; h->f = h->f2; h->f2 = tf;
   double *tg = h->g; h->g = h->g2; h->g2 = tg;
@@ -481,18 +514,10 @@ void clipo_stencil_field(const clipo *h, const double *phi, double *G, double *L
     mu[i] = mu_phi_of(h, phi[i], l);
   }
 }
-/* barred equilibria and forcing terms of one node state (P12): outputs feqbar, Fa, geqbar, Fphi [19] each */
+/* barred equilibria and forcing terms of one node state (P12): the very function collide_node calls */
 void clipo_node_terms(const clipo *h, double pstar, const double *u, double phi, const double *F, const double *nvec,
                       double *feqbar, double *Fa, double *geqbar, double *Fphi) {
-  double rho = rho_of(h, phi);
-  double pref = (1.0 - 4.0 * (phi - 0.5) * (phi - 0.5)) / h->p.W;
-  for (int a = 0; a < Q; ++a) {
-    double Gam = Gamma(h, a, u[0], u[1], u[2]);
-    Fa[a] = h->w[a] * (EX[a] * F[0] + EY[a] * F[1] + EZ[a] * F[2]) / (rho * (1.0 / 3.0));
-    feqbar[a] = pstar * h->w[a] + (Gam - h->w[a]) - 0.5 * Fa[a];
-    Fphi[a] = pref * h->w[a] * (EX[a] * nvec[0] + EY[a] * nvec[1] + EZ[a] * nvec[2]);
-    geqbar[a] = phi * Gam - 0.5 * Fphi[a];
-  }
+  node_terms(h, pstar, u, phi, F, nvec, feqbar, Fa, geqbar, Fphi);
 }
 /* inlet rule on a caller-provided node (P13) */
 void clipo_inlet_node(const clipo *h, double *f, double *g) { inlet_node(h, f, g); }

@@ -10,7 +10,8 @@ Layout everywhere: phi0[z, y, x] (x fastest), u0[c, z, y, x].  Node j sits at co
 
 Parameter dictionary keys (both the oracle binding and the CUDA binding marshal these into their own structs):
   precision (32|64), rho_h, rho_l, tau_h, tau_l, sigma, W, M, g (3), rho_ref, bc (6: -x,+x,-y,+y,-z,+z),
-  inlet_u (3), inlet_phi, inlet_c (2), inlet_r, outlet_u_mode, visc_interp, collision (0 WMRT, 1 BGK), phase_only (1: prescribed u)
+  inlet_u (3), inlet_phi, inlet_c (2), inlet_r, outlet_u_mode, visc_interp, collision (0 WMRT, 1 BGK), phase_only (1: prescribed u),
+  outlet_clamp (0: lambda of B.25 as printed; 1: max(0, lambda)), outlet_u_time (0: stored u(t); 1: post-stream moment at t+dt)
 """
 from __future__ import annotations
 
@@ -30,6 +31,7 @@ def default_params(**kw) -> dict:
         inlet_u=(0.0, 0.0, 0.0), inlet_phi=1.0,
         inlet_c=(0.0, 0.0), inlet_r=0.0,
         outlet_u_mode=0, visc_interp=0, collision=0, phase_only=0,
+        outlet_clamp=0, outlet_u_time=0,
         path=0,  # libclip only: kernel path (include/clip.h); the oracle ignores it
     )
     p.update(kw)
@@ -119,7 +121,8 @@ def jet(nxy=192, nz=1536, r_nozzle=12.0, We=2.2, W=4.0, U=0.05, precision=32):
     p = default_params(precision=precision, rho_h=rho_h, rho_l=rho_l, tau_h=3 * nu_h, tau_l=3 * nu_l,
                        sigma=sigma, W=W, M=0.1,
                        bc=(WALL, WALL, WALL, WALL, INLET, OUTLET),
-                       inlet_u=(0.0, 0.0, U), inlet_phi=1.0, inlet_c=(c, c), inlet_r=r_nozzle)
+                       inlet_u=(0.0, 0.0, U), inlet_phi=1.0, inlet_c=(c, c), inlet_r=r_nozzle,
+                       outlet_clamp=1)   # quiescent gas at the outlet: u_z < 0 occurs, B.25 as printed then amplifies (R12)
     return _case(nx, ny, nz, p, phi0, u0, f"jet{nxy}x{nz}")
 
 
