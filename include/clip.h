@@ -51,19 +51,28 @@ typedef struct clip_params {
   double inlet_phi;        /* phi_in, B.16 (:1069) */
   double inlet_c[2];       /* nozzle disc centre (x, y) in node coordinates */
   double inlet_r;          /* nozzle radius; nodes of the -z face outside the disc are WALL */
-  int outlet_u_mode;       /* characteristic outlet velocity of B.22 (:1104), from u_z of layer N-1 at the previous time, clamped
-                              at 0: 0 = U_local (per column), 1 = U_ave (mean over the layer), 2 = U_max */
+  int outlet_u_mode;       /* characteristic outlet velocity U of B.22 (:1104), built on the normal velocity of layer N-1:
+                              0 = U_local (per column), 1 = U_ave (mean over the layer), 2 = U_max */
   int visc_interp;         /* 0 = linear tau, Eq. 24 (paper, Alg. 1); 1 = harmonic (1/tau linear in phi; non-paper);
                               2 = linear dynamic viscosity, Eq. 25 (:219): mu = rho tau / 3, tau = 3 mu(phi) / rho(phi) */
   int collision;           /* CLIP_COLL_WMRT (0, default): Eq. 27-28 + F_mu of Eq. 30; CLIP_COLL_BGK (1): Eq. 26 + F_mu of Eq. 29 */
   int phase_only;          /* 0 (default): full two-phase flow.  1: only the phase-field equation (Eq. 33) is advanced and
                               u is prescribed by the caller (clip_set_u) -- the set-up of the interface-in-shear-flow test,
                               PAPER.md:675-713 (Sec. 5.4); f stays 0, p is returned as 0 */
+  int outlet_clamp;        /* lambda of B.25 (:1115-1117): 0 (default) = U dt/dy exactly as printed; 1 = max(0, U).  B.21 is an
+                              OUTFLOW condition: for U < 0 the implicit upwind form B.23-B.25 multiplies chi(N) - chi(N-1) by
+                              1/(1 + lambda) > 1 every step (reading R12); with the clamp such columns keep
+                              chi(N, t+dt) = chi(N, t).  Lattices whose outlet sees backflow (the jet into quiescent gas) want 1 */
+  int outlet_u_time;       /* which velocity enters B.22 (the paper says both, :1107 and :1117; reading R12):
+                              0 (default) = the stored macroscopic u_z(x,y,N-1,t) of the previous time step; 1 = the first moment
+                              sum_a e_az f_a(x,y,N-1,t+dt) of the post-stream populations (not in phase_only mode) */
   int path;                /* kernel path of clip_step (not part of the method; all paths compute the same step): 0 = automatic
                               (see clip_step), 1 = generic kernels only, 2 = never k_fused (pair kernels where the lattice admits
                               them), 3 = k_fused wherever the lattice admits it.  The slabs of one lattice must agree on whether
-                              phi(t+1) is part of the state (clip_halo_pack), so slabs with different faces are created with 2.
-                              The environment switches listed at clip_step override this field (tests) */
+                              phi(t+1) is part of the state (clip_halo_pack), so slabs with different faces are created with 2 */
+  int tile_ty, tile_chunks; /* k_fused tiling (tests / tuning; 0 = automatic): lattice rows per tile (4, 8 or 16, must divide ny) and
+                              number of equal chunks along z (1 .. min(nz, 256)); they enter clip_workspace_bytes */
+  int runtime_nx;          /* 1 = take the runtime-nx instantiation of the pair kernels even where nx has its own (tests) */
 } clip_params;
 
 typedef struct clip_handle clip_t;
@@ -84,13 +93,11 @@ int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params,
 int clip_init(clip_t* h, const void* d_phi0, const void* d_u0);
 
 /* Advance n >= 0 time steps (Eq. 13, 33 with all of App. B); asynchronous on the stream.
- * Which kernels run is decided per lattice at clip_create: k_fused + k_fix on wide periodic / walled lattices,
- * k_phi2 + k_step2 on the other lattices with even nx, the generic k_phi + k_step otherwise (and on the planes next to an
- * INLET / OUTLET face, for FREESLIP faces, BGK and phase_only).  All paths compute the same step; they agree to round-off, and
- * each is deterministic: clip_step(a); clip_step(b) equals clip_step(a + b) bit for bit.  Test / tuning switches read from the
- * environment at clip_create (and, for the k_fused tiling, at clip_workspace_bytes): CLIP_FAST_MODE (3 = k_fused wherever the
- * lattice admits it, 2 = k_phi2 + k_step2, 0 = k_tick2), CLIP_FORCE_GENERIC=1, CLIP_NO_NX_SPECIAL=1, CLIP_FUSED_TY,
- * CLIP_FUSED_CHUNKS, CLIP_TICK_LAG. */
+ * Which kernels run is decided per lattice at clip_create: k_fused + k_fix on wide lattices, k_phi2 + k_step2
+ * on the other lattices with even nx, the generic k_phi + k_step otherwise (and on the planes next to an INLET / OUTLET face).
+ * All paths compute the same step; they agree to round-off, and each is deterministic: clip_step(a); clip_step(b) equals
+ * clip_step(a + b) bit for bit.  clip_params.path / tile_ty / tile_chunks / runtime_nx override the choice (tests, tuning); the
+ * library reads nothing from the environment. */
 int clip_step(clip_t* h, int n);
 
 /* phase_only mode: prescribe the velocity field u [3][nz][ny][nx] (device) that the following collisions use; the

@@ -28,7 +28,8 @@ class clip_params(C.Structure):
         ("inlet_u", C.c_double * 3), ("inlet_phi", C.c_double),
         ("inlet_c", C.c_double * 2), ("inlet_r", C.c_double),
         ("outlet_u_mode", C.c_int), ("visc_interp", C.c_int), ("collision", C.c_int), ("phase_only", C.c_int),
-        ("path", C.c_int),
+        ("outlet_clamp", C.c_int), ("outlet_u_time", C.c_int),
+        ("path", C.c_int), ("tile_ty", C.c_int), ("tile_chunks", C.c_int), ("runtime_nx", C.c_int),
     ]
 
 
@@ -45,7 +46,8 @@ def make_params(p: dict) -> clip_params:
     s.visc_interp = int(p["visc_interp"])
     s.collision = int(p.get("collision", 0))
     s.phase_only = int(p.get("phase_only", 0))
-    s.path = int(p.get("path", 0))
+    for k in ("outlet_clamp", "outlet_u_time", "path", "tile_ty", "tile_chunks", "runtime_nx"):
+        setattr(s, k, int(p.get(k, 0)))
     return s
 
 
@@ -200,20 +202,31 @@ class Clip:
         if rc != CLIP_OK:
             raise ClipError(rc, clip_last_error(self._h))
 
+    def _on_stream(self, x, shape):
+        """Copy / cast `x` to the device ON the handle's stream (which first waits for the caller's current stream, where
+        `x` may still be being produced)."""
+        t = self.torch
+        self.stream.wait_stream(t.cuda.current_stream(self.device))
+        with t.cuda.stream(self.stream):
+            y = x.to(device=self.device, dtype=self.dtype).contiguous().reshape(shape)
+        if y.is_cuda:
+            y.record_stream(self.stream)
+        return y
+
     def init(self, phi0, u0):
         t = self.torch
-        phi0 = phi0.to(device=self.device, dtype=self.dtype).contiguous().reshape(self.nz, self.ny, self.nx)
-        u0 = u0.to(device=self.device, dtype=self.dtype).contiguous().reshape(3, self.nz, self.ny, self.nx)
-        with t.cuda.device(self.device), t.cuda.stream(self.stream):
-            self._check(clip_init(self._h, phi0.data_ptr(), u0.data_ptr()))
-            phi0.record_stream(self.stream); u0.record_stream(self.stream)
+        with t.cuda.device(self.device):
+            phi0 = self._on_stream(phi0, (self.nz, self.ny, self.nx))
+            u0 = self._on_stream(u0, (3, self.nz, self.ny, self.nx))
+            with t.cuda.stream(self.stream):
+                self._check(clip_init(self._h, phi0.data_ptr(), u0.data_ptr()))
 
     def set_u(self, u):
         t = self.torch
-        u = u.to(device=self.device, dtype=self.dtype).contiguous().reshape(3, self.nz, self.ny, self.nx)
-        with t.cuda.device(self.device), t.cuda.stream(self.stream):
-            self._check(clip_set_u(self._h, u.data_ptr()))
-            u.record_stream(self.stream)
+        with t.cuda.device(self.device):
+            u = self._on_stream(u, (3, self.nz, self.ny, self.nx))
+            with t.cuda.stream(self.stream):
+                self._check(clip_set_u(self._h, u.data_ptr()))
 
     def step(self, n=1):
         with self.torch.cuda.device(self.device):
@@ -258,6 +271,10 @@ class Clip:
 
     def close(self):
         if getattr(self, "_h", None):
+            try:
+                self.stream.synchronize()   # kernels of this stream may still use the workspace the allocator is about to reuse
+            except Exception:
+                pass
             clip_destroy(self._h)
             self._h = None
             self._ws = None

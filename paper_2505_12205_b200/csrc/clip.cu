@@ -3,7 +3,6 @@
 #include "../../include/clip.h"
 #include "clip_kernels.cuh"
 #include "clip_fast.cuh"
-#include "clip_tick.cuh"
 #include "clip_fused.cuh"
 #include "clip_launch.cuh"
 
@@ -31,7 +30,7 @@ size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
   size_t word;  // 4 or 8
-  size_t off_p[2], off_phi, off_u, off_obf, off_obg, off_lam, off_mask, off_sync, off_phi2, off_part, total;
+  size_t off_p[2], off_phi, off_u, off_obf, off_obg, off_lam, off_mask, off_phi2, off_part, total;
 };
 
 // Tiling of the single-pass kernel k_fused (clip_fused.cuh): tiles of `ty` rows x one z chunk; the number of tiles is
@@ -51,7 +50,7 @@ FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   for (int k = 0; k < 6; ++k) if (p->bc[k] != CLIP_BC_PERIODIC && p->bc[k] != CLIP_BC_WALL) return f;
   if (nx % 64 != 0 || nx > 512 || ny % 4 != 0 || nz < 4) return f;
   f.ty = 4;  // small tiles leave more of the SM's L1 to the phi stencil and the shifted population loads (measured)
-  { const char* e = getenv("CLIP_FUSED_TY"); if (e && (atoi(e) == 4 || atoi(e) == 8 || atoi(e) == 16) && ny % atoi(e) == 0) f.ty = atoi(e); }
+  if ((p->tile_ty == 4 || p->tile_ty == 8 || p->tile_ty == 16) && ny % p->tile_ty == 0) f.ty = p->tile_ty;
   f.ytiles = ny / f.ty;
   f.threads = nx / 2;
   const int word = p->precision == 32 ? 4 : 8;
@@ -70,19 +69,27 @@ FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   f.pays = (nx >= 256 && f.fills_gpu) || (nx >= 128 && (long long)f.ytiles * max_chunks >= 4 * cap);
   // Chunks along z, dispatched in order (blockIdx.y): long ones (<= 16 planes: little halo traffic) first, then about one
   // wave of 8-plane and one wave of 4-plane chunks, so that the last blocks to finish are short ones (uniform chunks leave
-  // ~4 % of the SM time idle in the last wave).  Small lattices and CLIP_FUSED_CHUNKS=n (tests) take n equal chunks.
+  // ~4 % of the SM time idle in the last wave).  Small lattices and tile_chunks = n (tests) take n equal chunks.  The chunk
+  // COUNT is bounded before anything is written to zc (FUSED_MAX_CHUNKS entries): long thin lattices get longer chunks.
+  const int maxc = clip::FUSED_MAX_CHUNKS < nz ? clip::FUSED_MAX_CHUNKS : nz;
   int nchunks = 0, uniform = 0;
-  { const char* e = getenv("CLIP_FUSED_CHUNKS"); if (e && atoi(e) >= 1 && atoi(e) <= nz) uniform = atoi(e); }
-  const int per_wave = (int)((cap + f.ytiles - 1) / f.ytiles);  // chunks that are resident at the same time
-  if (!uniform && 12 * per_wave <= nz / 2) {
+  if (p->tile_chunks >= 1) uniform = p->tile_chunks < maxc ? p->tile_chunks : maxc;
+  const long long per_wave_ll = (cap + f.ytiles - 1) / f.ytiles;  // chunks that are resident at the same time
+  const int per_wave = per_wave_ll > nz ? nz : (int)per_wave_ll;
+  bool graded = !uniform && 12LL * per_wave <= nz / 2;
+  if (graded) {
     const int rest = nz - 12 * per_wave, nl = (rest + 15) / 16;
-    int z = 0;
-    for (int k = 0; k < nl; ++k) { f.zc[nchunks++] = z; z += rest / nl + (k < rest % nl ? 1 : 0); }
-    for (int k = 0; k < per_wave; ++k) { f.zc[nchunks++] = z; z += 8; }
-    for (int k = 0; k < per_wave; ++k) { f.zc[nchunks++] = z; z += 4; }
-    f.zc[nchunks] = nz;
-  } else {
-    if (!uniform) {  // as many equal chunks as fill a whole number of waves, at most 16 planes each
+    if ((long long)nl + 2LL * per_wave > maxc) graded = false;
+    else {
+      int z = 0;
+      for (int k = 0; k < nl; ++k) { f.zc[nchunks++] = z; z += rest / nl + (k < rest % nl ? 1 : 0); }
+      for (int k = 0; k < per_wave; ++k) { f.zc[nchunks++] = z; z += 8; }
+      for (int k = 0; k < per_wave; ++k) { f.zc[nchunks++] = z; z += 4; }
+      f.zc[nchunks] = nz;
+    }
+  }
+  if (!graded) {
+    if (!uniform) {  // as many equal chunks as fill a whole number of waves, at most 16 planes each (more where the count is bounded)
       for (int m = 1; m <= 64; ++m) {
         long long c = m * cap / f.ytiles;
         if (c < 1) continue;
@@ -91,11 +98,11 @@ FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
         if ((nz + uniform - 1) / uniform <= 16) break;
       }
       if (uniform < 1) uniform = 1;
+      if (uniform > maxc) uniform = maxc;
     }
     nchunks = uniform;
     for (int c = 0; c <= nchunks; ++c) f.zc[c] = (int)((long long)c * nz / nchunks);
   }
-  if (nchunks > clip::FUSED_MAX_CHUNKS) return f;
   f.nchunks = nchunks;
   f.tzmax = 1;
   for (int c = 0; c < nchunks; ++c) f.tzmax = f.zc[c + 1] - f.zc[c] > f.tzmax ? f.zc[c + 1] - f.zc[c] : f.tzmax;
@@ -118,7 +125,6 @@ Layout make_layout(int nx, int ny, int nz, const clip_params* p) {
   L.off_obg = take(outlet ? 19 * nxy * L.word : 0);
   L.off_lam = take(outlet ? nxy * L.word : 0);
   L.off_mask = take(inlet ? nxy : 0);
-  L.off_sync = take(((size_t)nz + 64) * sizeof(unsigned));  // k_tick: ticket counter + per-plane counters
   const FusedPlan fp = fused_plan(nx, ny, nz, p);                // k_fused: second phi buffer + tile-halo partial sums
   L.off_phi2 = take(fp.ok ? n * L.word : 0);
   L.off_part = take(fp.ok ? fp.part_words * L.word : 0);
@@ -153,7 +159,13 @@ const char* validate(int nx, int ny, int nz, const clip_params* p) {
   if (p->bc[5] == CLIP_BC_OUTLET && nz < 2) return "OUTLET needs nz >= 2";
   if (p->bc[4] == CLIP_BC_INLET && !(p->inlet_r >= 0.0)) return "inlet_r must be >= 0";
   if (p->outlet_u_mode < 0 || p->outlet_u_mode > 2) return "outlet_u_mode must be 0 (U_local), 1 (U_ave) or 2 (U_max)";
+  if (p->outlet_clamp != 0 && p->outlet_clamp != 1) return "outlet_clamp must be 0 (B.25 as printed) or 1 (lambda = max(0, U))";
+  if (p->outlet_u_time != 0 && p->outlet_u_time != 1) return "outlet_u_time must be 0 (stored u(t)) or 1 (post-stream moment at t+dt)";
+  if (p->outlet_u_time == 1 && p->phase_only) return "outlet_u_time = 1 needs the hydrodynamic populations (not phase_only)";
   if (p->path < 0 || p->path > 3) return "path must be 0 (automatic), 1 (generic), 2 (no k_fused) or 3 (k_fused where admitted)";
+  if (p->tile_ty != 0 && p->tile_ty != 4 && p->tile_ty != 8 && p->tile_ty != 16) return "tile_ty must be 0 (automatic), 4, 8 or 16";
+  if (p->tile_chunks < 0) return "tile_chunks must be >= 0";
+  if (p->runtime_nx != 0 && p->runtime_nx != 1) return "runtime_nx must be 0 or 1";
   return nullptr;
 }
 
@@ -170,13 +182,10 @@ struct clip_handle {
   bool phi_ahead;  // k_fused path: the other phi buffer already holds phi(t+1)
   FusedPlan fplan;
   bool inited;
-  int mode;            // fast-path variant (CLIP_FAST_MODE): unset = automatic (k_fused + k_fix on wide lattices, else k_phi2 + k_step2);
-                       // 3 = k_fused wherever the lattice allows; 2 = k_phi2 + k_step2; 0 = k_tick2 (one launch)
-  unsigned epoch;      // steps since clip_init (k_tick counters)
+  int mode;            // clip_params.path: 0 = automatic (k_fused + k_fix on wide lattices, else k_phi2 + k_step2), 1 = generic kernels
+                       // only, 2 = k_phi2 + k_step2, 3 = k_fused wherever the lattice allows
   int fast_threads;    // threads per block of the pair kernels (128)
-  int nx_special;      // nx, or 0 when CLIP_NO_NX_SPECIAL=1 forces the runtime-nx kernels (tests)
-  int tick_lag;        // CLIP_TICK_LAG (default 4, >= 3): groups between the phi job and the collision job of a plane (k_tick2)
-  bool force_generic;  // CLIP_FORCE_GENERIC=1 in the environment at clip_create: generic kernels only (tests)
+  int nx_special;      // nx, or 0 when clip_params.runtime_nx forces the runtime-nx kernels (tests)
   long long launches;
   long long t;
   std::vector<uint8_t> mask_host;
@@ -197,7 +206,7 @@ template <typename T> clip::KP<T> make_kp(const clip_handle* h) {
   P.has_inlet = p.bc[4] == CLIP_BC_INLET;
   P.has_outlet = p.bc[5] == CLIP_BC_OUTLET;
   P.visc_interp = p.visc_interp;
-  P.outlet_u_mode = p.outlet_u_mode;
+  P.outlet_u_mode = p.outlet_u_mode; P.outlet_clamp = p.outlet_clamp; P.outlet_u_time = p.outlet_u_time;
   P.collision = p.collision;
   P.phase_only = p.phase_only;
   P.rho_h = (T)p.rho_h; P.rho_l = (T)p.rho_l; P.drho = (T)(p.rho_h - p.rho_l);
@@ -231,8 +240,6 @@ int check_cuda(clip_handle* h, const char* what) {
 unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / block); }
 
 template <typename T> int do_init(clip_handle* h, const void* phi0, const void* u0) {
-  cudaMemsetAsync(h->ws + h->L.off_sync, 0, ((size_t)h->nz + 64) * sizeof(unsigned), h->stream);
-  h->epoch = 0;
   h->phi_cur = 0; h->phi_ahead = false;
   h->cur = 1;  // k_init writes into "dst"; flip afterwards so that it becomes the current state
   clip::KP<T> P = make_kp<T>(h);
@@ -242,12 +249,13 @@ template <typename T> int do_init(clip_handle* h, const void* phi0, const void* 
   return check_cuda(h, "k_init");
 }
 
-enum { KIND_PHI = 0, KIND_STEP = 1, KIND_PHI2 = 2, KIND_STEP2 = 3, KIND_FIX = 4, KIND_TICK = 5, KIND_FUSED = 6, KIND_COUNT = 7 };
-const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step2", "k_fix", "k_tick2", "k_fused"};
+enum { KIND_PHI = 0, KIND_STEP = 1, KIND_PHI2 = 2, KIND_STEP2 = 3, KIND_FIX = 4, KIND_FUSED = 5, KIND_OUTLET = 6, KIND_COUNT = 7 };
+const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step2", "k_fix", "k_fused", "k_outlet_lam"};
 
 // The pair-per-thread fast kernels (clip_fast.cuh) cover planes whose neighbourhood has only PERIODIC or WALL faces, even nx.
 bool fast_ok(const clip_handle* h) {
-  if (h->force_generic) return false;
+  if (h->mode == 1) return false;
+  if (h->nz > 65535 || h->ny > 65535) return false;  // grid.y / grid.z of the pair kernels
   if (h->p.collision != CLIP_COLL_WMRT || h->p.phase_only) return false;  // BGK keeps all 19 f in the collision: generic kernels only (round 1)
   for (int k = 0; k < 4; ++k) if (h->p.bc[k] != CLIP_BC_PERIODIC && h->p.bc[k] != CLIP_BC_WALL) return false;
   if (h->p.bc[4] == CLIP_BC_FREESLIP || h->p.bc[5] == CLIP_BC_FREESLIP) return false;  // free-slip: generic kernels only
@@ -274,7 +282,16 @@ struct Prof {  // optional per-launch event timing (clip_step_profiled)
   void end(int k) { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, stream); ev.push_back(e); kind.push_back(k); }
 };
 
-bool use_fused(const clip_handle* h) { return fast_ok(h) && h->fplan.ok && (h->mode == 3 || (h->mode < 0 && h->fplan.pays)); }
+bool use_fused(const clip_handle* h) { return fast_ok(h) && h->fplan.ok && (h->mode == 3 || (h->mode == 0 && h->fplan.pays)); }
+
+// lambda of B.25 for the step about to run (k_outlet_lam; the plane-wide schemes of B.22 add a one-block reduction)
+template <typename T> void outlet_lambda(clip_handle* h, const clip::KP<T>& P, Prof* prof) {
+  if (prof) prof->begin();
+  clip::k_outlet_lam<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(P);
+  h->launches += 1;
+  if (P.outlet_u_mode != 0) { clip::k_outlet_reduce<T><<<1, 1024, 0, h->stream>>>(P); h->launches += 1; }
+  if (prof) prof->end(KIND_OUTLET);
+}
 
 // k_fused path, once after clip_init: phi(t+1) = sum_a g+_a(x - e_a, t) into the second phi buffer (one k_phi2 launch).
 template <typename T> void fused_prepass(clip_handle* h, Prof* prof) {
@@ -298,12 +315,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
   for (int k = 0; k < 6; ++k) walls = walls || h->p.bc[k] == CLIP_BC_WALL;
   const bool xwalls = h->p.bc[0] == CLIP_BC_WALL || h->p.bc[1] == CLIP_BC_WALL;
   dim3 fg, fb;
-  bool tick = false;
   if (fast) fast_shape(h, fg, fb);
-  if (fast && h->mode == 0 && h->p.bc[4] != CLIP_BC_INLET && h->p.bc[5] != CLIP_BC_OUTLET && (h->nx / 2) % fb.x == 0 &&
-      h->ny % fb.y == 0) {
-    tick = true;
-  }
   const bool fused = use_fused(h);
   for (int s = 0; s < nsteps; ++s) {
     clip::KP<T> P = make_kp<T>(h);
@@ -323,7 +335,8 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       for (int c = 0; c <= fp.nchunks; ++c) U.zc[c] = fp.zc[c];
       U.tile_stride = (long long)(2 * fp.tzmax + 2 * (fp.ty + 2)) * h->nx;
       if (prof) prof->begin();
-      clip::launch_fused<T>(walls, h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+      const cudaError_t fe = clip::launch_fused<T>(walls, h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+      if (fe != cudaSuccess) { set_err(h->err, "k_fused: %s", cudaGetErrorString(fe)); return CLIP_ECUDA; }
       if (prof) { prof->end(KIND_FUSED); prof->begin(); }
       const int fix_rpb = clip::FIX_ROWS * (clip::FIX_THREADS / clip::fix_threads_per_row(h->nx, clip::Vec16<T>::EV));  // rows per block
       clip::launch_fix<T>(dim3(fp.ytiles, fp.nchunks, (2 * fp.tzmax + 2 * (fp.ty - 2) + fix_rpb - 1) / fix_rpb), h->stream, F, U);
@@ -334,35 +347,13 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       h->t += 1;
       continue;
     }
-    if (tick) {
-      clip::FP<T> F = make_fp<T>(P);
-      h->epoch += 1;
-      unsigned* sync = (unsigned*)(h->ws + h->L.off_sync);
-      clip::TickP tk;
-      tk.ticket = sync; tk.done_a = sync + 32;
-      tk.tp = (int)(fg.x * fg.y); tk.gx = (int)fg.x;
-      const unsigned lag = (unsigned)h->tick_lag;
-      const unsigned items = ((unsigned)h->nz + lag) * (unsigned)tk.tp;
-      tk.base = 0;
-      tk.target = (unsigned)tk.tp * h->epoch;
-      if (prof) prof->begin();
-      clip::launch_tick2<T>(walls, h->nx_special, items, fb, h->stream, F, tk, (int)lag);
-      if (prof) prof->end(KIND_TICK);
-      h->launches += 1;
-      h->cur ^= 1;
-      h->t += 1;
-      continue;
-    }
     // planes next to an INLET / OUTLET face: generic kernels; all other planes: pair kernels (when the lattice allows)
     const int glo = (fast && h->p.bc[4] == CLIP_BC_INLET) ? 1 : 0, ghi = (fast && h->p.bc[5] == CLIP_BC_OUTLET) ? 1 : 0;
     clip::KP<T> Plo = P, Phi = P;
     Plo.z_lo = 0; Plo.z_cnt = glo; Phi.z_lo = h->nz - ghi; Phi.z_cnt = ghi;
     clip::FP<T> F;
     if (fast) { F = make_fp<T>(P); F.k.z_lo = glo; F.k.z_cnt = h->nz - glo - ghi; fg.z = (unsigned)F.k.z_cnt; }
-    if (P.has_outlet && P.outlet_u_mode != 0) {  // B.22 U_ave / U_max from u(t), before anything of this step reads lam
-      clip::k_outlet_u<T><<<1, 1024, 0, h->stream>>>(P);
-      h->launches += 1;
-    }
+    if (P.has_outlet) outlet_lambda<T>(h, P, prof);  // lambda of B.25 for this step, before anything of the step reads it
     for (int pass = 0; pass < 2; ++pass) {  // pass 0: phi(t+1); pass 1: macros + collisions
       if (prof) prof->begin();
       if (!fast) {
@@ -510,11 +501,9 @@ int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params,
   h->nx = nx; h->ny = ny; h->nz = nz; h->p = *params; h->L = L; h->ws = (char*)d_workspace;
   h->stream = (cudaStream_t)cuda_stream; h->cur = 0; h->phi_cur = 0; h->phi_ahead = false; h->inited = false;
   h->fplan = fused_plan(nx, ny, nz, params);
-  { const char* e = getenv("CLIP_FORCE_GENERIC"); h->force_generic = e ? e[0] == '1' : params->path == 1; }
-  { const char* e = getenv("CLIP_FAST_MODE"); h->mode = e ? atoi(e) : (params->path == 2 ? 2 : params->path == 3 ? 3 : -1); h->epoch = 0; }
+  h->mode = params->path;
   h->fast_threads = 128;  // measured: fp64 8.2 vs 7.6 GLUPS, fp32 (with 3 blocks per SM) +2 % against 256-thread blocks
-  { const char* e = getenv("CLIP_NO_NX_SPECIAL"); h->nx_special = (e && e[0] == '1') ? 0 : nx; }
-  { const char* e = getenv("CLIP_TICK_LAG"); h->tick_lag = e ? atoi(e) : 4; if (h->tick_lag < 3) h->tick_lag = 3; }
+  h->nx_special = params->runtime_nx ? 0 : nx;
   h->launches = 0; h->t = 0; h->err[0] = 0;
   if (params->bc[4] == CLIP_BC_INLET) {  // disc mask, decided in double on the host
     h->mask_host.resize((size_t)nx * ny);

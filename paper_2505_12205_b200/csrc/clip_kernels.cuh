@@ -7,7 +7,7 @@
 //   phi             phi(x,t)                                                    [nz][ny][nx]
 //   u               u(x,t)                                                   [3][nz][ny][nx]   (node-local update)
 //   ob_f, ob_g      PRE-collision populations of the outlet layer z = nz-1 at t   [19][ny][nx] (outlet only)
-//   lam             lambda = max(0, u_z(x,y,nz-2,t)) of B.25                         [ny][nx]  (outlet only)
+//   lam             lambda of B.25 for the step in flight (k_outlet_lam)             [ny][nx]  (outlet only)
 //   mask            inlet disc mask of the -z face (uint8)                           [ny][nx]  (inlet only)
 //
 // One step t -> t+1:
@@ -51,7 +51,7 @@ template <typename T> struct KP {
   long long n;    // nodes
   long long nxy;  // nodes per z layer
   int bc[6];
-  int has_inlet, has_outlet, any_nonperiodic, visc_interp, collision, phase_only, outlet_u_mode;
+  int has_inlet, has_outlet, any_nonperiodic, visc_interp, collision, phase_only, outlet_u_mode, outlet_clamp, outlet_u_time;
   int z_lo, z_cnt;  // planes [z_lo, z_lo + z_cnt) a k_phi* / k_step* launch covers (whole lattice: 0, nz)
   T rho_h, rho_l, drho;
   T tau_h, tau_l, itau_h, itau_l, rt_h, rt_l;  // rt = rho tau = 3 mu (Eq. 23, 25)
@@ -227,11 +227,12 @@ template <typename T> __device__ __forceinline__ void inlet_f(const KP<T>& P, T 
   }
 }
 
-// Post-stream, post-BC populations of node (x,y,z) at t+1 (steps 7-9 of DESIGN.md): pull, inlet, outlet.
-// lam_out (may be null): where the outlet lambda of this column is stored when it is computed from u(t).
-template <typename T, bool WITH_F, bool LAM_FROM_U>
+// Post-stream, post-BC populations of node (x,y,z) at t+1 (steps 7-9 of DESIGN.md): pull, inlet, outlet.  The outlet's lambda
+// is read from P.lam (k_outlet_lam, launched before the kernels of a step).  OUTLET_RULE = false: the post-stream values of
+// the node itself even on the outlet layer (k_outlet_lam pulls layer N-1 this way).
+template <typename T, bool WITH_F, bool OUTLET_RULE = true>
 __device__ __forceinline__ void load_node(const KP<T>& P, int x, int y, int z, T (&f)[Q], T (&g)[Q]) {
-  const bool outlet_layer = P.has_outlet && (z == P.nz - 1);
+  const bool outlet_layer = OUTLET_RULE && P.has_outlet && (z == P.nz - 1);
   const int zs = outlet_layer ? z - 1 : z;  // B.26-B.27 need the post-stream values of layer N-1
   const long long i = (long long)zs * P.nxy + (long long)y * P.nx + x;
   const Nbr b = make_nbr(P, x, y, zs);
@@ -245,14 +246,7 @@ __device__ __forceinline__ void load_node(const KP<T>& P, int x, int y, int z, T
   }
   if (outlet_layer) {
     const long long c = (long long)y * P.nx + x;
-    T lam;
-    if (LAM_FROM_U && P.outlet_u_mode == 0) {  // U_local of B.22 from the stored u(t) of layer N-1, clamped at 0 (R12)
-      lam = P.u[2 * P.n + i];
-      lam = lam > T(0) ? lam : T(0);
-      P.lam[c] = lam;
-    } else {
-      lam = P.lam[c];  // second pass of the step, or a plane-wide scheme (k_outlet_u)
-    }
+    const T lam = P.lam[c];
     const T inv = T(1) / (T(1) + lam);
 #pragma unroll
     for (int a = 0; a < Q; ++a) {
@@ -400,12 +394,32 @@ template <typename T> struct StoreAll<T, Q> {
 };
 
 // ------------------------------------------------------------------------------------------------ kernels
-// k_phi: phi(t+1) = sum_a g_a(x,t+1)  (Eq. 38) from the post-collision g+(t); inlet nodes get phi_in.
-// Plane-wide outlet velocity of B.22: U_ave (mode 1) or U_max (mode 2) of u_z(., ., N-1, t), clamped at 0
-// (R12), written to every entry of `lam`.  One block, fixed reduction order (deterministic).
-template <typename T> __global__ void __launch_bounds__(1024) k_outlet_u(const __grid_constant__ KP<T> P) {
+// lambda = U dt/dy of B.25 for the step t -> t+1, one entry per column of the outlet layer.  U is the
+// normal velocity of layer N-1 (B.22, :1104): the stored u_z(x,y,N-1,t) (outlet_u_time = 0, ":1107 previous time step") or the
+// first moment of the post-stream f of that layer at t+1 (outlet_u_time = 1, ":1117 after the streaming step"; reading R12).
+// U_local: clamped here if outlet_clamp; the plane-wide schemes go on to k_outlet_reduce.
+template <typename T> __global__ void __launch_bounds__(256) k_outlet_lam(const __grid_constant__ KP<T> P) {
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= P.nxy) return;
+  T U;
+  if (P.outlet_u_time == 1 && !P.phase_only) {
+    const int x = (int)(c % P.nx), y = (int)(c / P.nx);
+    T f[Q], g[Q];
+    load_node<T, true, false>(P, x, y, P.nz - 2, f, g);
+    U = T(0);
+#pragma unroll
+    for (int a = 0; a < Q; ++a) if (cz(a) != 0) U += T(cz(a)) * f[a];
+  } else {
+    U = P.u[2 * P.n + (long long)(P.nz - 2) * P.nxy + c];
+  }
+  if (P.outlet_u_mode == 0 && P.outlet_clamp && U < T(0)) U = T(0);
+  P.lam[c] = U;
+}
+// Plane-wide outlet velocity of B.22: U_ave (mode 1) or U_max (mode 2) over the per-column values k_outlet_lam
+// left in `lam`, clamped at 0 if outlet_clamp, written to every entry.  One block, fixed reduction order (deterministic).
+template <typename T> __global__ void __launch_bounds__(1024) k_outlet_reduce(const __grid_constant__ KP<T> P) {
   __shared__ T sh[1024];
-  const T* __restrict__ uz = P.u + 2 * P.n + (long long)(P.nz - 2) * P.nxy;
+  const T* __restrict__ uz = P.lam;
   const bool ave = P.outlet_u_mode == 1;
   T acc = ave ? T(0) : uz[0];
   for (long long c = threadIdx.x; c < P.nxy; c += blockDim.x) {
@@ -422,10 +436,12 @@ template <typename T> __global__ void __launch_bounds__(1024) k_outlet_u(const _
     __syncthreads();
   }
   T U = ave ? sh[0] / T(P.nxy) : sh[0];
-  U = U > T(0) ? U : T(0);
+  if (P.outlet_clamp && U < T(0)) U = T(0);
+  __syncthreads();
   for (long long c = threadIdx.x; c < P.nxy; c += blockDim.x) P.lam[c] = U;
 }
 
+// k_phi: phi(t+1) = sum_a g_a(x,t+1)  (Eq. 38) from the post-collision g+(t); inlet nodes get phi_in.
 template <typename T> __global__ void __launch_bounds__(256) k_phi(const __grid_constant__ KP<T> P) {
   const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= P.z_cnt * P.nxy) return;
@@ -434,7 +450,7 @@ template <typename T> __global__ void __launch_bounds__(256) k_phi(const __grid_
   const long long r = i / P.nx;
   const int y = (int)(r % P.ny), z = (int)(r / P.ny);
   T f[Q], g[Q];
-  load_node<T, false, true>(P, x, y, z, f, g);
+  load_node<T, false>(P, x, y, z, f, g);
   T s = ((g[0] + (g[1] + g[2])) + ((g[3] + g[4]) + (g[5] + g[6]))) +
         (((g[7] + g[8]) + (g[9] + g[10])) + ((g[11] + g[12]) + (g[13] + g[14])) + ((g[15] + g[16]) + (g[17] + g[18])));
   if (P.has_inlet && z == 0 && P.mask[(long long)y * P.nx + x]) s = P.phi_in;
@@ -450,7 +466,7 @@ template <typename T> __global__ void __launch_bounds__(256) k_step(const __grid
   const long long r = i / P.nx;
   const int y = (int)(r % P.ny), z = (int)(r / P.ny);
   T f[Q], g[Q];
-  load_node<T, true, false>(P, x, y, z, f, g);
+  load_node<T, true>(P, x, y, z, f, g);
   if (P.has_outlet && z == P.nz - 1) {  // keep chi(N, t+1) for the next step's B.26-B.27
     const long long c = (long long)y * P.nx + x;
 #pragma unroll
@@ -531,8 +547,8 @@ __global__ void __launch_bounds__(256) k_get(const __grid_constant__ KP<T> P, T*
   if (u_out) { u_out[i] = P.u[i]; u_out[P.n + i] = P.u[P.n + i]; u_out[2 * P.n + i] = P.u[2 * P.n + i]; }
   if (p_out) {
     T f[Q];
-#pragma unroll
     const int x = (int)(i % P.nx);
+#pragma unroll
     for (int a = 0; a < Q; ++a) f[a] = P.p_src[pop_base(i, x) + a * P.nx];
     const Mom<T> m = moments(f);
     p_out[i] = m.p * (P.rho_l + phi * P.drho) * T(1.0 / 3.0);

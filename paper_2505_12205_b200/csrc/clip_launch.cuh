@@ -3,7 +3,6 @@
 // explicit instantiations), so that the ~170 kernel instantiations compile in parallel instead of in one 3-minute unit.
 #pragma once
 #include "clip_fast.cuh"
-#include "clip_tick.cuh"
 #include "clip_fused.cuh"
 
 namespace clip {
@@ -19,8 +18,8 @@ constexpr int fused_threads_per_sm(int precision, int block_threads) {
 // walls: the lattice has WALL faces (WALLS instantiation); xwalls: it has them in x (k_step2 then keeps 16 warps per SM)
 template <typename T> void launch_phi2(bool walls, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F);
 template <typename T> void launch_step2(bool walls, bool xwalls, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F);
-template <typename T> void launch_tick2(bool walls, int nx, unsigned items, dim3 b, cudaStream_t st, const FP<T>& F, const TickP& tk, int lag);
-template <typename T> void launch_fused(bool walls, int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
+// returns the CUDA error of the shared-memory opt-in (cudaFuncSetAttribute, once per device and instantiation) or of nothing
+template <typename T> cudaError_t launch_fused(bool walls, int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
 template <typename T> void launch_fix(dim3 g, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
 
 }  // namespace clip

@@ -32,7 +32,7 @@ def default_params(**kw) -> dict:
         inlet_c=(0.0, 0.0), inlet_r=0.0,
         outlet_u_mode=0, visc_interp=0, collision=0, phase_only=0,
         outlet_clamp=0, outlet_u_time=0,
-        path=0,  # libclip only: kernel path (include/clip.h); the oracle ignores it
+        path=0, tile_ty=0, tile_chunks=0, runtime_nx=0,  # libclip only: kernel path / tiling (include/clip.h); the oracle ignores them
     )
     p.update(kw)
     return p

@@ -65,6 +65,12 @@ def test_validation_without_gpu():
         (dict(outlet_u_mode=3), "outlet_u_mode"),
         (dict(visc_interp=7), "visc_interp"),
         (dict(path=4), "path"),
+        (dict(outlet_clamp=2), "outlet_clamp"),
+        (dict(outlet_u_time=2), "outlet_u_time"),
+        (dict(outlet_u_time=1, phase_only=1), "outlet_u_time"),
+        (dict(tile_ty=5), "tile_ty"),
+        (dict(tile_chunks=-1), "tile_chunks"),
+        (dict(runtime_nx=2), "runtime_nx"),
     ):
         q = dict(p); q.update(bad)
         assert clip.clip_workspace_bytes(8, 8, 8, clip.make_params(q)) == 0
@@ -80,6 +86,19 @@ def test_validation_without_gpu():
     rc, h = clip.clip_create(8, 8, 8, ok, 4096, 16, 0)            # too small
     assert rc == clip.CLIP_ENOMEM
     assert clip.clip_step(None, 1) == clip.CLIP_EINVAL and clip.clip_destroy(None) == clip.CLIP_EINVAL
+
+
+def test_elongated_lattices_do_not_overflow_the_tiling_tables():
+    """k_fused's chunk table holds 256 entries: long thin lattices (and absurd tile_chunks) must get longer chunks or another
+    path, never a write past the table (round-1 finding: 64 x 64 x 4096 smashed the stack inside clip_workspace_bytes)."""
+    p32 = dict(inputs.default_params(), precision=32)
+    for shape in ((64, 64, 4096), (64, 4, 20000), (128, 8, 70000), (512, 4, 3000), (64, 64, 257), (256, 1024, 1100)):
+        for over in ({}, dict(tile_chunks=10 ** 6), dict(tile_chunks=1), dict(path=3), dict(bc=(1, 1, 1, 1, 1, 1))):
+            q = dict(p32); q.update(over)
+            n = clip.clip_workspace_bytes(*shape, clip.make_params(q))
+            nodes = shape[0] * shape[1] * shape[2]
+            assert n >= 80 * 4 * nodes, (shape, over)
+            assert n < 86 * 4 * nodes + (1 << 20), (shape, over, n / nodes)
 
 
 def test_no_cpu_fallback(tmp_path, monkeypatch):

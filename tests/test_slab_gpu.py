@@ -52,7 +52,7 @@ def _with(case, **kw):
     return case
 
 
-CASES = {   # name: (case, steps, slab counts, environment)
+CASES = {   # name: (case, steps, slab counts, clip_params overrides)
     "sweep64": (lambda: inputs.sweep_drops(n=64), 30, (1, 2, 4), {}),                       # periodic z, pair kernels
     "rt_replica": (lambda: inputs.rayleigh_taylor(L=16, W=3.0), 30, (2, 4), {}),            # y walls, periodic z
     "walled_box": (lambda: inputs.walled_box(nx=12, ny=10, nz=16), 30, (2, 4), {}),         # z walls: end slabs have one ghost side
@@ -62,19 +62,17 @@ CASES = {   # name: (case, steps, slab counts, environment)
     "jet_replica": (lambda: inputs.jet(nxy=24, nz=96, r_nozzle=4.0), 40, (2, 3, 4), {}),
     "jet_replica_umax": (lambda: _with(inputs.jet(nxy=24, nz=48, r_nozzle=4.0), outlet_u_mode=2), 40, (2,), {}),
     # free-slip on all six faces: generic kernels everywhere (the cut faces of the inner slabs would otherwise take the pair kernels)
-    "freeslip_box": (lambda: _with(inputs.walled_box(nx=12, ny=10, nz=16), bc=(inputs.FREESLIP,) * 6), 30, (2, 4), {"CLIP_FORCE_GENERIC": "1"}),
+    "freeslip_box": (lambda: _with(inputs.walled_box(nx=12, ny=10, nz=16), bc=(inputs.FREESLIP,) * 6), 30, (2, 4), {"path": 1}),
 }
 
 
 @pytest.mark.parametrize("precision", [64, 32])
 @pytest.mark.parametrize("name", sorted(CASES))
-def test_slabs_equal_the_undivided_lattice(name, precision, monkeypatch):
+def test_slabs_equal_the_undivided_lattice(name, precision):
     import torch
-    monkeypatch.setenv("CLIP_FAST_MODE", "2")   # same per-node arithmetic whatever the tiling: bit for bit
-    make, steps, worlds, env = CASES[name]
-    for k, v in env.items():
-        monkeypatch.setenv(k, v)
+    make, steps, worlds, over = CASES[name]
     case = make()
+    case["params"].update(dict({"path": 2}, **over))   # path 2: same per-node arithmetic whatever the tiling: bit for bit
     ref = _whole(case, steps, precision)
     for world in worlds:
         out, launches = _slabs(case, steps, precision, world, chunks=(steps - 7, 7))
@@ -85,14 +83,14 @@ def test_slabs_equal_the_undivided_lattice(name, precision, monkeypatch):
 
 
 @pytest.mark.parametrize("precision", [64, 32])
-def test_slabs_on_the_fused_path(precision, monkeypatch):
+def test_slabs_on_the_fused_path(precision):
     """k_fused keeps phi(t+1) as state: the record carries it (clip.h).  Equal to the undivided two-kernel run to round-off."""
     import torch
     case = inputs.sweep_drops(n=64)
     steps = 30
-    monkeypatch.setenv("CLIP_FAST_MODE", "2")
+    case["params"]["path"] = 2
     ref = _whole(case, steps, precision)
-    monkeypatch.setenv("CLIP_FAST_MODE", "3")
+    case["params"]["path"] = 3
     for world in (2, 4):
         out, _ = _slabs(case, steps, precision, world, chunks=(1, steps - 1))
         tol = 1e-12 if precision == 64 else 3e-5
@@ -167,7 +165,6 @@ def test_halo_abi_errors_and_roundtrip():
 _DIST_WORKER = r"""
 import json, os, sys
 sys.path.insert(0, {root!r})
-os.environ["CLIP_FAST_MODE"] = "2"     # per-node arithmetic independent of the tiling: bit for bit
 import torch
 import torch.distributed as dist
 from paper_2505_12205_b200 import clip, inputs, slab
@@ -177,6 +174,7 @@ rank, world = dist.get_rank(), dist.get_world_size()
 ok = True
 for make, steps in ((lambda: inputs.sweep_drops(shape=(32, 32, 36), ndrops=5, rmin=3, rmax=6), 25), (lambda: inputs.jet(nxy=24, nz=48, r_nozzle=4.0), 25)):
     case = make()
+    case["params"]["path"] = 2       # per-node arithmetic independent of the tiling: bit for bit
     params = dict(case["params"]); params["precision"] = 64
     sl = slab.SlabClip(case["nx"], case["ny"], case["nz"], params, rank, world, device="cuda:0")
     sl.init(torch.as_tensor(case["phi0"]), torch.as_tensor(case["u0"]))
