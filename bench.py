@@ -177,9 +177,10 @@ def run_ours(args):
     if args.workload == "rt":  # BASELINE configs[2]: Rayleigh-Taylor 128 x 512 x 128, walls in y (not the headline workload)
         case = inputs.rayleigh_taylor(L=n // 2, precision=prec)
     elif args.workload == "jet":  # BASELINE configs[3]: liquid jet 192 x 192 x 1536, inlet disc, convective outlet, side walls
-        case = inputs.jet(nxy=3 * n // 4, nz=6 * n, r_nozzle=12.0 * n / 256, precision=prec)
+        case = inputs.jet(nxy=3 * n // 4, nz=args.nz or 6 * n, r_nozzle=12.0 * n / 256, precision=prec)
     else:
         case = inputs.sweep_drops(n=n, seed=rank_seed(rank), precision=prec)
+    case["params"]["path"] = args.path
     nxl, nyl, nzl = case["nx"], case["ny"], case["nz"]
     nodes = nxl * nyl * nzl
     sim = clip.Clip(nxl, nyl, nzl, case["params"], device=dev)
@@ -365,6 +366,89 @@ def run_slab(args):
         dist.destroy_process_group()
 
 
+def run_long(args):
+    """`--long-run rt|jet`: BASELINE configs[2] / configs[3] at FULL LENGTH on the GPU (the CPU oracle would need
+    days), with the checks the survey lists: finite fields, drift of sum(phi), x <-> z symmetry (RT: the initial condition is
+    symmetric under the swap), inflow mass balance d(sum phi)/dt against the nozzle's flux (jet, before the liquid reaches the
+    outlet), range of phi, max |u|.  Prints ONE JSON line with the time series; diagnostics are torch reductions on the device
+    between clip_step calls (measurement, not the path)."""
+    import torch
+    import __graft_entry__ as g
+    g.build()
+    from paper_2505_12205_b200 import clip, inputs
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    prec = args.precision
+    if args.long_run == "rt":
+        case = inputs.rayleigh_taylor(L=args.n // 2, precision=prec)
+        total = args.steps if args.steps_given else 20000
+    else:
+        case = inputs.jet(nxy=3 * args.n // 4, nz=6 * args.n, r_nozzle=12.0 * args.n / 256, We=args.we, precision=prec)
+        total = args.steps if args.steps_given else 50000
+    every = max(1, total // 50)
+    case["params"]["path"] = args.path
+    sim = clip.Clip.from_case(case, precision=prec)
+    pr = case["params"]
+    nx, ny, nz = case["nx"], case["ny"], case["nz"]
+    phi0 = torch.as_tensor(case["phi0"]).to(dev)
+    s0 = float(phi0.double().sum())
+    disc = None
+    if args.long_run == "jet":
+        yy, xx = torch.meshgrid(torch.arange(ny, dtype=torch.float64), torch.arange(nx, dtype=torch.float64), indexing="ij")
+        disc = int((((xx - pr["inlet_c"][0]) ** 2 + (yy - pr["inlet_c"][1]) ** 2) <= pr["inlet_r"] ** 2).sum())
+    series, first_bad = [], None
+    t0 = time.perf_counter()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    gpu_ms = 0.0
+    done = 0
+    while done < total:
+        n = min(every, total - done)
+        e0.record(sim.stream)
+        sim.step(n)
+        e1.record(sim.stream)
+        done += n
+        phi, p, u = sim.get()
+        torch.cuda.synchronize()
+        gpu_ms += e0.elapsed_time(e1)
+        finite = bool(torch.isfinite(phi).all() and torch.isfinite(u).all() and torch.isfinite(p).all())
+        rec = {"t": done, "finite": finite}
+        if finite:
+            rec.update(sum_phi=float(phi.double().sum()), phi_min=float(phi.min()), phi_max=float(phi.max()), u_max=float(u.abs().max()))
+            if args.long_run == "rt":
+                rec["xz_asym"] = float((phi - phi.transpose(0, 2)).abs().max())
+                rec["y_front_heavy"] = int((phi[:, :, :] > 0.5).any(dim=2).any(dim=0).nonzero().min())   # lowest row the heavy fluid has reached
+            else:
+                col = (phi[:, ny // 2, nx // 2] > 0.5).nonzero()
+                rec["tip_z"] = int(col.max()) if col.numel() else -1
+                rec["outlet_phi_max"] = float(phi[-1].max())
+        elif first_bad is None:
+            first_bad = done
+        series.append(rec)
+        if not finite:
+            break
+    wall = time.perf_counter() - t0
+    last = series[-1]
+    out = {"long_run": args.long_run, "lattice": [nx, ny, nz], "precision": prec, "steps_requested": total, "steps_done": done,
+           "stable": first_bad is None, "first_non_finite_step_at_or_before": first_bad,
+           "params": {k: (list(v) if isinstance(v, tuple) else v) for k, v in pr.items()},
+           "sum_phi_0": s0, "mlups": nx * ny * nz * done / (gpu_ms * 1e-3) / 1e6, "gpu_ms_per_step": gpu_ms / max(done, 1), "wall_s": wall,
+           "series": series}
+    if first_bad is None:
+        if args.long_run == "rt":
+            out["sum_phi_rel_drift"] = (last["sum_phi"] - s0) / s0
+            out["xz_asym_max"] = max(r["xz_asym"] for r in series)
+        else:
+            # inflow mass balance while the liquid is far from the outlet: d(sum phi)/dt against (disc nodes) x U x phi_in
+            pre = [r for r in series if r["outlet_phi_max"] < 0.01]
+            if len(pre) >= 2:
+                rate = (pre[-1]["sum_phi"] - pre[0]["sum_phi"]) / (pre[-1]["t"] - pre[0]["t"])
+                out["inflow"] = {"d_sum_phi_dt": rate, "disc_nodes_x_U": disc * pr["inlet_u"][2] * pr["inlet_phi"],
+                                 "pi_R2_U": 3.141592653589793 * pr["inlet_r"] ** 2 * pr["inlet_u"][2], "disc_nodes": disc,
+                                 "window": [pre[0]["t"], pre[-1]["t"]]}
+    print(json.dumps(out))
+    sim.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -378,7 +462,16 @@ def main():
                     help="sweep = BASELINE configs[4] (headline); rt = configs[2] lattice (n/2 x 2n x n/2), walls in y; jet = configs[3] lattice (3n/4 x 3n/4 x 6n)")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replica per GPU (default) or one lattice n x n x (n N) cut into z slabs with halo exchange")
+    ap.add_argument("--nz", type=int, default=0, help="jet workload only: planes along the jet (default 6 n = 1536; shorter for profiling runs)")
+    ap.add_argument("--path", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="clip_params.path: 0 automatic (default), 1 generic kernels, 2 pair kernels (k_phi2 + k_step2), 3 k_fused wherever admitted")
+    ap.add_argument("--long-run", default=None, choices=["rt", "jet"],
+                    help="run BASELINE configs[2] (rt, 20000 steps) or configs[3] (jet, 50000 steps) at full length with diagnostics; one JSON line")
+    ap.add_argument("--we", type=float, default=2.2, help="Weber number of the jet (--long-run jet)")
     args = ap.parse_args()
+    args.steps_given = any(a == "--steps" or a.startswith("--steps=") for a in sys.argv[1:])
+    if args.long_run:
+        return run_long(args)
     if args.impl == "reference":
         run_reference(args)
     elif args.decomp == "slab":

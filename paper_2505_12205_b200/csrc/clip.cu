@@ -47,7 +47,11 @@ constexpr int B200_SMS = 148;
 FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   FusedPlan f{};
   if (p->collision != CLIP_COLL_WMRT || p->phase_only) return f;
-  for (int k = 0; k < 6; ++k) if (p->bc[k] != CLIP_BC_PERIODIC && p->bc[k] != CLIP_BC_WALL) return f;
+  for (int k = 0; k < 4; ++k) if (p->bc[k] != CLIP_BC_PERIODIC && p->bc[k] != CLIP_BC_WALL) return f;
+  if (p->bc[4] == CLIP_BC_FREESLIP || p->bc[5] == CLIP_BC_FREESLIP) return f;
+  // an INLET / OUTLET plane is stepped by the generic kernels; k_fused covers the planes [zlo, zlo + nz) in between
+  const int zlo = p->bc[4] == CLIP_BC_INLET ? 1 : 0;
+  nz -= zlo + (p->bc[5] == CLIP_BC_OUTLET ? 1 : 0);
   if (nx % 64 != 0 || nx > 512 || ny % 4 != 0 || nz < 4) return f;
   f.ty = 4;  // small tiles leave more of the SM's L1 to the phi stencil and the shifted population loads (measured)
   if ((p->tile_ty == 4 || p->tile_ty == 8 || p->tile_ty == 16) && ny % p->tile_ty == 0) f.ty = p->tile_ty;
@@ -103,6 +107,7 @@ FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
     nchunks = uniform;
     for (int c = 0; c <= nchunks; ++c) f.zc[c] = (int)((long long)c * nz / nchunks);
   }
+  for (int c = 0; c <= nchunks; ++c) f.zc[c] += zlo;
   f.nchunks = nchunks;
   f.tzmax = 1;
   for (int c = 0; c < nchunks; ++c) f.tzmax = f.zc[c + 1] - f.zc[c] > f.tzmax ? f.zc[c + 1] - f.zc[c] : f.tzmax;
@@ -293,19 +298,43 @@ template <typename T> void outlet_lambda(clip_handle* h, const clip::KP<T>& P, P
   if (prof) prof->end(KIND_OUTLET);
 }
 
-// k_fused path, once after clip_init: phi(t+1) = sum_a g+_a(x - e_a, t) into the second phi buffer (one k_phi2 launch).
+// k_fused path on a lattice with an INLET / OUTLET z face, from the state (f+, g+, u) at the current time t: lambda of B.25 for the
+// step t -> t+1 and phi(t+1) of the planes the single-pass kernel cannot complete -- the open planes themselves (inlet rule,
+// B.26-B.27) and their neighbours, which receive g+ from them -- by the generic k_phi, into the phi(t+1) buffer.
+template <typename T> void fused_open_planes(clip_handle* h, Prof* prof) {
+  const int glo = h->p.bc[4] == CLIP_BC_INLET ? 1 : 0, ghi = h->p.bc[5] == CLIP_BC_OUTLET ? 1 : 0;
+  if (!glo && !ghi) return;
+  clip::KP<T> P = make_kp<T>(h);
+  P.phi = (T*)(h->ws + (h->phi_cur ? h->L.off_phi : h->L.off_phi2));
+  if (P.has_outlet) outlet_lambda<T>(h, P, prof);
+  for (int side = 0; side < 2; ++side) {
+    if (!(side ? ghi : glo)) continue;
+    clip::KP<T> Q = P;
+    Q.z_lo = side ? h->nz - 2 : 0; Q.z_cnt = 2;
+    if (prof) prof->begin();
+    clip::k_phi<T><<<grid_for(2 * P.nxy, 256), 256, 0, h->stream>>>(Q);
+    if (prof) prof->end(KIND_PHI);
+    h->launches += 1;
+  }
+}
+
+// k_fused path, once after clip_init: phi(t+1) = sum_a g+_a(x - e_a, t) into the second phi buffer (one k_phi2 launch, plus the
+// generic kernel on the planes next to an open face).
 template <typename T> void fused_prepass(clip_handle* h, Prof* prof) {
   if (h->phi_ahead) return;
   bool walls = false;
   for (int k = 0; k < 6; ++k) walls = walls || h->p.bc[k] == CLIP_BC_WALL;
+  const int glo = h->p.bc[4] == CLIP_BC_INLET ? 1 : 0, ghi = h->p.bc[5] == CLIP_BC_OUTLET ? 1 : 0;
   dim3 fg, fb;
   fast_shape(h, fg, fb);
   clip::FP<T> F = make_fp<T>(make_kp<T>(h));
   F.k.phi = (T*)(h->ws + (h->phi_cur ? h->L.off_phi : h->L.off_phi2));
+  F.k.z_lo = glo; F.k.z_cnt = h->nz - glo - ghi; fg.z = (unsigned)F.k.z_cnt;
   if (prof) prof->begin();
   clip::launch_phi2<T>(walls, h->nx_special, fg, fb, h->stream, F);
   if (prof) prof->end(KIND_PHI2);
   h->launches += 1;
+  fused_open_planes<T>(h, prof);
   h->phi_ahead = true;
 }
 
@@ -328,7 +357,17 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       T* const phi_next = (T*)(h->ws + (h->phi_cur ? h->L.off_phi : h->L.off_phi2));
       F.k.phi = phi_next;
       fused_prepass<T>(h, prof);
+      for (int side = 0; side < 2; ++side) {  // the INLET / OUTLET plane: generic kernel, phi(t+1) and lambda are in place
+        if (!(side ? h->p.bc[5] == CLIP_BC_OUTLET : h->p.bc[4] == CLIP_BC_INLET)) continue;
+        clip::KP<T> Q = F.k;
+        Q.z_lo = side ? h->nz - 1 : 0; Q.z_cnt = 1;
+        if (prof) prof->begin();
+        clip::k_step<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Q);
+        if (prof) prof->end(KIND_STEP);
+        h->launches += 1;
+      }
       clip::FusedP<T> U;
+      U.z_wrap = h->p.bc[4] == CLIP_BC_PERIODIC ? 1 : 0;
       U.phi_dst = phi_now;  // becomes phi(t+2); phi(t) is no longer needed once the time is t+1
       U.part = (T*)(h->ws + h->L.off_part);
       U.ty = fp.ty; U.ytiles = fp.ytiles; U.nchunks = fp.nchunks; U.tzmax = fp.tzmax;
@@ -345,6 +384,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       h->cur ^= 1;
       h->phi_cur ^= 1;
       h->t += 1;
+      fused_open_planes<T>(h, prof);  // open z faces: lambda and the boundary planes of phi(t+2), from the new state
       continue;
     }
     // planes next to an INLET / OUTLET face: generic kernels; all other planes: pair kernels (when the lattice allows)
@@ -355,24 +395,24 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
     if (fast) { F = make_fp<T>(P); F.k.z_lo = glo; F.k.z_cnt = h->nz - glo - ghi; fg.z = (unsigned)F.k.z_cnt; }
     if (P.has_outlet) outlet_lambda<T>(h, P, prof);  // lambda of B.25 for this step, before anything of the step reads it
     for (int pass = 0; pass < 2; ++pass) {  // pass 0: phi(t+1); pass 1: macros + collisions
-      if (prof) prof->begin();
       if (!fast) {
+        if (prof) prof->begin();
         if (pass == 0) clip::k_phi<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
         else clip::k_step<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
         h->launches += 1;
         if (prof) prof->end(pass == 0 ? KIND_PHI : KIND_STEP);
         continue;
       }
-      if (glo) {
-        if (pass == 0) clip::k_phi<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Plo);
-        else clip::k_step<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Plo);
+      for (int side = 0; side < 2; ++side) {
+        if (!(side ? ghi : glo)) continue;
+        const clip::KP<T>& Q = side ? Phi : Plo;
+        if (prof) prof->begin();
+        if (pass == 0) clip::k_phi<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Q);
+        else clip::k_step<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Q);
         h->launches += 1;
+        if (prof) prof->end(pass == 0 ? KIND_PHI : KIND_STEP);
       }
-      if (ghi) {
-        if (pass == 0) clip::k_phi<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Phi);
-        else clip::k_step<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Phi);
-        h->launches += 1;
-      }
+      if (prof) prof->begin();
       if (pass == 0) {
         clip::launch_phi2<T>(walls, h->nx_special, fg, fb, h->stream, F);
       } else {

@@ -32,6 +32,7 @@ template <typename T> struct FusedP {
   int ty, ytiles, nchunks, tzmax;
   int zc[FUSED_MAX_CHUNKS + 1];  // chunk c covers the planes zc[c] .. zc[c+1]-1 (sizes <= tzmax; clip.cu: fused_plan)
   long long tile_stride;  // elements of `part` per tile
+  int z_wrap;             // the z faces are PERIODIC: the first and the last chunk are neighbours (k_fix)
 };
 // rows of a tile's slab in `part`
 __host__ __device__ __forceinline__ int slot_ym(int k) { return k; }
@@ -45,7 +46,8 @@ template <typename T> __device__ __forceinline__ T shfl_dn1(T v) { return __shfl
 // Accumulation of one source row into the ring.  Column-private shared memory: acc[(slot * rows + j) * nx + x0 .. +1].
 // The nine contributions are formed in registers first; the shared-memory read-modify-writes are then issued as one
 // batch of loads followed by one batch of stores (the rows are distinct, which the compiler cannot know).
-template <typename T, bool WALLS> struct Scatter {
+// WALLS: 0 = periodic code, 1 = any wall face next to the row, 2 = wall faces in x only (as in clip_fast.cuh)
+template <typename T, int WALLS> struct Scatter {
   typedef P2<T> V;
   T* ring;     // ring base
   T* edge_p;   // [slots * rows][nwarps]: lane 31's +x sends (land in the next warp's first column)
@@ -57,7 +59,7 @@ template <typename T, bool WALLS> struct Scatter {
   template <int dz> __device__ __forceinline__ int slot() const { return dz < 0 ? sm : (dz > 0 ? sp : sc); }
   template <int dy, int dz> __device__ __forceinline__ bool behind_wall(const Geo& geo) const {
     // the row (dy, dz) lies behind a wall: everything returns to the sender (B.10-B.11)
-    return WALLS && ((dy > 0 && geo.byp) || (dy < 0 && geo.bym) || (dz > 0 && geo.bzp) || (dz < 0 && geo.bzm));
+    return WALLS == 1 && ((dy > 0 && geo.byp) || (dy < 0 && geo.bym) || (dz > 0 && geo.bzp) || (dz < 0 && geo.bzm));
   }
   // target row (dy, dz) with the three directions a0 (e_x = 0), ap (e_x = +1), am (e_x = -1): c = what lands in this
   // thread's columns, ep / em = what lane 31 / lane 0 sends across the warp edge; bounced links go to `own`
@@ -153,7 +155,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP
   for (int i = threadIdx.x; i < nslots * rows * (nx + 2 * nwarps); i += blockDim.x) ring[i] = T(0);
   __syncthreads();
   T* const slab = U.part + (long long)(c * U.ytiles + iy) * U.tile_stride;
-  Scatter<T, WALLS> sc;
+  Scatter<T, WALLS ? 1 : 0> sc;
   sc.ring = ring; sc.edge_p = edge_p; sc.edge_m = edge_m; sc.nx = nx; sc.rows = rows; sc.nwarps = nwarps; sc.warp = warp; sc.lane = lane;
   // flush of plane k (-1 .. tz) of the tile, held in ring slot (k + 1) % slots
   auto flush = [&](int k) {
@@ -181,19 +183,25 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP
     for (int ly = 0; ly < U.ty; ++ly) {
       const int y = y0 + ly;
       sc.j = ly + 1;
-      bool wall_row = false;
-      if (WALLS) {
-        wall_row = P.bc[0] != BC_PERIODIC || P.bc[1] != BC_PERIODIC || (y == 0 && P.bc[2] != BC_PERIODIC) ||
-                   (y == P.ny - 1 && P.bc[3] != BC_PERIODIC) || (z == 0 && P.bc[4] != BC_PERIODIC) ||
-                   (z == P.nz - 1 && P.bc[5] != BC_PERIODIC);
+      int wall_row = 0;  // 1: a y / z wall face next to the row; 2: only the x faces are walls (two tests per link instead of six)
+      if constexpr (WALLS) {
+        const bool yz = (y == 0 && P.bc[2] != BC_PERIODIC) || (y == P.ny - 1 && P.bc[3] != BC_PERIODIC) ||
+                        (z == 0 && P.bc[4] != BC_PERIODIC) || (z == P.nz - 1 && P.bc[5] != BC_PERIODIC);
+        wall_row = yz ? 1 : ((P.bc[0] != BC_PERIODIC || P.bc[1] != BC_PERIODIC) ? 2 : 0);
+        if (wall_row == 1) {
+          step_pair<T, LD_NC, LD_NC, ST_WB, NX, 1>(FPp, x0, y, z, NoWait(), sc);
+        } else if (wall_row == 2) {
+          Scatter<T, 2> sx;
+          sx.ring = ring; sx.edge_p = edge_p; sx.edge_m = edge_m; sx.nx = nx; sx.rows = rows; sx.nwarps = nwarps; sx.warp = warp; sx.lane = lane;
+          sx.sm = sc.sm; sx.sc = sc.sc; sx.sp = sc.sp; sx.j = sc.j;
+          step_pair<T, LD_NC, LD_NC, ST_WB, NX, 2>(FPp, x0, y, z, NoWait(), sx);
+        }
       }
-      if (WALLS && wall_row) {
-        step_pair<T, LD_NC, LD_NC, ST_WB, NX, true>(FPp, x0, y, z, NoWait(), sc);
-      } else {
-        Scatter<T, false> sp;
+      if (wall_row == 0) {
+        Scatter<T, 0> sp;
         sp.ring = ring; sp.edge_p = edge_p; sp.edge_m = edge_m; sp.nx = nx; sp.rows = rows; sp.nwarps = nwarps; sp.warp = warp; sp.lane = lane;
         sp.sm = sc.sm; sp.sc = sc.sc; sp.sp = sc.sp; sp.j = sc.j;
-        step_pair<T, LD_NC, LD_NC, ST_WB, NX, false>(FPp, x0, y, z, NoWait(), sp);
+        step_pair<T, LD_NC, LD_NC, ST_WB, NX, 0>(FPp, x0, y, z, NoWait(), sp);
       }
     }
     __syncthreads();  // also keeps the block's warps on the same plane: without it the kernel is 4 % slower (L1 reuse)
@@ -246,7 +254,10 @@ template <typename T> __global__ void __launch_bounds__(FIX_THREADS) k_fix(const
       if (s >= U.ty - 2 && tz == 1) continue;
     }
     const int y = iy * U.ty + ly;
-    const bool ylo = ly == 0, yhi = ly == U.ty - 1, zlo = lz == 0, zhi = lz == tz - 1;
+    // without z periodicity nothing arrives from beyond the first / the last chunk (walls send nothing there; next to an INLET /
+    // OUTLET plane the generic kernels redo the plane, clip.cu)
+    const bool ylo = ly == 0, yhi = ly == U.ty - 1;
+    const bool zlo = lz == 0 && (U.z_wrap || c > 0), zhi = lz == tz - 1 && (U.z_wrap || c < U.nchunks - 1);
     const T* src[8];
     int ns = 0;
     if (ylo) src[ns++] = slab(c, iym, slot_yp(lz, U.tzmax));
