@@ -86,22 +86,28 @@ template <typename T, int sy, int sz> __device__ __forceinline__ const T* pop_ro
 // NX > 0: nx known at compile time (component offsets become immediates); NX == 0: runtime nx.
 // WALLS: a link that crosses a wall face takes the opposite population of the node itself (B.10-B.11; any wall crossing
 // wins at edges and corners, R11).
+// Every variant is straight-line code: wrap-around and bounce-back SELECT the address of a load, they do not branch around
+// it, so that all loads of a node pair can be issued back to back whatever the lattice's faces are.
 template <typename T, int a, int H, int NX, int SET, int WALLS>
 __device__ __forceinline__ P2<T> pull2(const T* __restrict__ src, int nx_rt, const Geo& g) {
   const int nx = NX ? NX : nx_rt;
   const T* __restrict__ rp = pop_row<T, -cy(a), -cz(a)>(src, g) + (SET * Q + a) * nx;
-  if (WALLS && a > 0) {
-    const T* __restrict__ own = pop_row<T, 0, 0>(src, g) + (SET * Q + copp(a)) * nx;
-    if (WALLS == 1) {
-      const bool rb = (cy(a) == 1 && g.bym) || (cy(a) == -1 && g.byp) || (cz(a) == 1 && g.bzm) || (cz(a) == -1 && g.bzp);
-      if (rb) return ld_pair<T, H>(own);
-    }
-    if (cx(a) == 1 && g.bxm) return P2<T>(ld_one<T, H>(own), ld_one<T, H>(rp));
-    if (cx(a) == -1 && g.bxp) return P2<T>(ld_one<T, H>(rp + 1), ld_one<T, H>(own + 1));
+  if (a == 0) return ld_pair<T, H>(rp);
+  const T* __restrict__ own = pop_row<T, 0, 0>(src, g) + (SET * Q + copp(a)) * nx;
+  bool rb = false;  // the link crosses a y / z wall: both nodes of the pair take their own opposite population
+  if (WALLS == 1) rb = (cy(a) == 1 && g.bym) || (cy(a) == -1 && g.byp) || (cz(a) == 1 && g.bzm) || (cz(a) == -1 && g.bzp);
+  if (cx(a) == 0) return ld_pair<T, H>((WALLS == 1 && rb) ? own : rp);
+  const T* __restrict__ plo;
+  const T* __restrict__ phi;
+  if (cx(a) == 1) {
+    plo = rp + (g.wm ? nx - 1 : -1); phi = rp;
+    if (WALLS && g.bxm) plo = own;
+  } else {
+    plo = rp + 1; phi = rp + (g.wp ? 2 - nx : 2);
+    if (WALLS && g.bxp) phi = own + 1;
   }
-  if (cx(a) == 0) return ld_pair<T, H>(rp);
-  if (cx(a) == 1) return P2<T>(g.wm ? ld_one<T, H>(rp + (nx - 1)) : ld_one<T, H>(rp - 1), ld_one<T, H>(rp));
-  return P2<T>(ld_one<T, H>(rp + 1), g.wp ? ld_one<T, H>(rp + (2 - nx)) : ld_one<T, H>(rp + 2));
+  if (WALLS == 1 && rb) { plo = own; phi = own + 1; }
+  return P2<T>(ld_one<T, H>(plo), ld_one<T, H>(phi));
 }
 template <typename T, int H, int NX, int SET, int WALLS, int a = 0> struct Pull2All {
   static __device__ __forceinline__ void run(const T* __restrict__ src, int nx, const Geo& g, P2<T> (&v)[Q]) {

@@ -11,7 +11,7 @@ namespace clip {
 // 12 warps with every load of a row in flight beat 16 warps at 128 registers, measured 17.3 vs 16.8 GLUPS at 256^3),
 // except 256-thread blocks (nx = 512 and the runtime-nx form), which keep 2 blocks; fp64 256 (255 registers).
 constexpr int fused_threads_per_sm(int precision, int block_threads) {
-  return precision == 32 ? (block_threads >= 256 ? 512 : 384) : 256;
+  return precision == 32 ? (block_threads >= 256 ? 512 : (block_threads == 96 ? 480 : 384)) : 256;
 }
 
 
