@@ -296,7 +296,8 @@ def run_slab(args):
     planes = slab.slab_plane_index(n * world, rank, world, True)
     # same recipe and drop density; every rank builds only its own planes (ghosts included) of the global field
     case = inputs.sweep_drops(shape=(n, n, n * world), seed=2505, ndrops=20 * world, precision=prec, z_planes=planes)
-    sl = slab.SlabClip(n, n, n * world, case["params"], rank, world, device=dev)
+    case["params"]["path"] = args.path
+    sl = slab.SlabClip(n, n, n * world, case["params"], rank, world, device=dev, overlap=not args.no_overlap)
     assert sl.planes == planes
     phi0_h = torch.as_tensor(case["phi0"]).to(dtype).pin_memory()
     u0_h = torch.as_tensor(case["u0"]).to(dtype).pin_memory()
@@ -337,6 +338,9 @@ def run_slab(args):
         o.copy_(d, non_blocking=True)
     barrier()
     e2e_s = time.perf_counter() - t0
+    # per-kernel durations of the slab's own step (CUDA events around every launch; no exchange in between: timing only)
+    prof = sl.sim.step_profiled(10)
+    kernels_ms = {k: v[0] / 10 for k, v in prof.items() if v[1]}
     ms, e2e_s, finite = reduce_over_ranks(ms, e2e_s, finite, world, dev)
     if rank == 0:
         peak, peak_src = measured_peak()
@@ -350,18 +354,35 @@ def run_slab(args):
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
             "config": {"workload": f"BASELINE configs[4] recipe on ONE periodic lattice {n}x{n}x{n * world} cut into {world} z slab(s), fp{prec}",
-                       "lattice": [n, n, n * world], "parallelism": f"z slabs, {slab.HALO} ghost planes per cut, neighbour send/recv after every step",
+                       "lattice": [n, n, n * world], "parallelism": f"z slabs, {slab.HALO} ghost plane per cut, neighbour send/recv of one 12-word record per face node after every step",
                        "halo_bytes_sent_per_rank_per_step": sl.halo_bytes_per_step, "local_planes": sl.nz_local,
                        "l2": f"state {sl.sim.workspace_bytes / 1e9:.2f} GB >> 126 MB L2, no flush needed", "finite_after_run": finite},
             "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
-                         "peak_source": peak_src, "kernel": "whole step incl. ghost planes and halo copies",
+                         "peak_source": peak_src, "kernel": "whole step incl. halo pack / exchange / unpack", "kernels_ms_per_step": kernels_ms,
+                         "overlap": sl.halo is not None,
                          "note": "achieved = 84 words/LU x OWNED nodes / step time (CUDA events around the timed steps)"},
             "e2e": {"value": world * nodes * args.steps / e2e_s / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": h2d / args.steps,
                     "d2h_bytes_per_step": d2h / args.steps,
                     "job": "pinned host slab -> H2D -> clip_init -> K x (clip_step(1) + halo exchange) -> clip_get -> D2H, wall clock"},
             "clocks": clocks}))
     sl.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_plumbing(args):
+    """`--plumbing-only`: the launch / rendezvous / reduction path of a multi-rank run without any GPU work (CPU test)."""
+    import torch
+    import torch.distributed as dist
+    world, rank = int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    ms, e2e, finite = reduce_over_ranks(1.0 + rank, 2.0 + rank, True, world, torch.device("cpu"))
+    if rank == 0:
+        decomp = args.decomp or ("slab" if world > 1 else "replicas")
+        print(json.dumps({"plumbing_only": True, "n_gpus": world, "gpus_requested": args.gpus, "decomp": decomp, "max_ms": ms, "max_e2e_s": e2e,
+                          "finite": finite}))
     if world > 1:
         dist.destroy_process_group()
 
@@ -460,8 +481,12 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--workload", default="sweep", choices=["sweep", "rt", "jet"],
                     help="sweep = BASELINE configs[4] (headline); rt = configs[2] lattice (n/2 x 2n x n/2), walls in y; jet = configs[3] lattice (3n/4 x 3n/4 x 6n)")
-    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
-                    help="N > 1: independent replica per GPU (default) or one lattice n x n x (n N) cut into z slabs with halo exchange")
+    ap.add_argument("--decomp", default=None, choices=["replicas", "slab"],
+                    help="slab (default for N > 1): ONE lattice n x n x (n N) cut into N z slabs with a halo exchange per step -- the path's "
+                         "own sharding (SURVEY.md 8(e)); replicas: an independent lattice per GPU.  N = 1 default: the undivided lattice")
+    ap.add_argument("--no-overlap", action="store_true", help="slab decomposition: plain sequence step; pack; exchange; unpack on one stream")
+    ap.add_argument("--plumbing-only", action="store_true",
+                    help="no GPU work: start the ranks, rendezvous (gloo), reduce dummy timings and print the line's skeleton (CPU test of --gpus N)")
     ap.add_argument("--nz", type=int, default=0, help="jet workload only: planes along the jet (default 6 n = 1536; shorter for profiling runs)")
     ap.add_argument("--path", type=int, default=0, choices=[0, 1, 2, 3],
                     help="clip_params.path: 0 automatic (default), 1 generic kernels, 2 pair kernels (k_phi2 + k_step2), 3 k_fused wherever admitted")
@@ -472,9 +497,21 @@ def main():
     args.steps_given = any(a == "--steps" or a.startswith("--steps=") for a in sys.argv[1:])
     if args.long_run:
         return run_long(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` without a launcher: start the N ranks ourselves (one process per GPU), same command line
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+        raise SystemExit(subprocess.call(cmd))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.plumbing_only:
+        return run_plumbing(args)
     if args.impl == "reference":
         run_reference(args)
-    elif args.decomp == "slab":
+    elif args.decomp == "slab" or (args.decomp is None and world > 1):
         run_slab(args)
     else:
         run_ours(args)

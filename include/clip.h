@@ -35,7 +35,10 @@ enum { CLIP_OK = 0, CLIP_EINVAL = -1, CLIP_ENOMEM = -2, CLIP_ESTATE = -3, CLIP_E
  * App. B.5 (:1094-1129), only on the +z face.  FREESLIP: specular reflection half a cell outside the last node, App. B.2
  * (B.8-B.9, :1017-1026): zero normal velocity, free tangential velocity; where a link also crosses a WALL face the
  * bounce-back wins.  The phi stencils (Eq. 40) take the mirror value behind WALL, FREESLIP, INLET and OUTLET faces. */
-enum { CLIP_BC_PERIODIC = 0, CLIP_BC_WALL = 1, CLIP_BC_INLET = 2, CLIP_BC_OUTLET = 3, CLIP_BC_FREESLIP = 4 };
+enum { CLIP_BC_PERIODIC = 0, CLIP_BC_WALL = 1, CLIP_BC_INLET = 2, CLIP_BC_OUTLET = 3, CLIP_BC_FREESLIP = 4, CLIP_BC_HALO = 5 };
+/* CLIP_BC_HALO (z faces only): the cut face of a z slab of a larger lattice.  The first / last plane of such a
+ * lattice is a GHOST plane -- an image of the neighbouring slab's outermost owned plane, refreshed by clip_halo_unpack after every
+ * step -- and clip_step advances the owned planes only.  See clip_halo_pack. */
 
 /* Hydrodynamic collision operator: weighted MRT (the paper's choice for 3-D, :849) or BGK. */
 enum { CLIP_COLL_WMRT = 0, CLIP_COLL_BGK = 1 };
@@ -69,7 +72,7 @@ typedef struct clip_params {
   int path;                /* kernel path of clip_step (not part of the method; all paths compute the same step): 0 = automatic
                               (see clip_step), 1 = generic kernels only, 2 = never k_fused (pair kernels where the lattice admits
                               them), 3 = k_fused wherever the lattice admits it.  The slabs of one lattice must agree on whether
-                              phi(t+1) is part of the state (clip_halo_pack), so slabs with different faces are created with 2 */
+                              phi(t+1) is kept in a second buffer */
   int tile_ty, tile_chunks; /* k_fused tiling (tests / tuning; 0 = automatic): lattice rows per tile (4, 8 or 16, must divide ny) and
                               number of equal chunks along z (1 .. min(nz, 256)); they enter clip_workspace_bytes */
   int runtime_nx;          /* 1 = take the runtime-nx instantiation of the pair kernels even where nx has its own (tests) */
@@ -110,26 +113,46 @@ int clip_set_u(clip_t* h, const void* d_u);
  * (device; any may be NULL); asynchronous on the stream. */
 int clip_get(clip_t* h, void* d_phi, void* d_p, void* d_u);
 
-/* z-slab decomposition over several GPUs.  Streaming pulls every population from a neighbour at most one
- * plane away (Eq. 13, 33; Alg. 2 :432-459) and the stencils of Eq. 40 (:309-331) read phi(t+1) = sum_a g+_a(x - e_a, t)
- * one further plane away, so a slab that carries TWO ghost planes beyond each interior cut, refreshed after every step with the
- * neighbour's outermost owned planes, computes its owned planes exactly as the undivided lattice does (the ghost planes
- * themselves come out wrong and are overwritten).  clip_halo_pack copies the complete state of the planes [z0, z0 + nplanes)
- * -- post-collision populations, phi(t), on the k_fused path also phi(t+1), u(t) -- into `d_buf` (device, 16-byte aligned,
- * clip_halo_bytes(h, nplanes) bytes); clip_halo_unpack writes such a record, packed by a handle of the same nx, ny, precision,
- * parameters and kernel path at the same time step, over the planes [z0, z0 + nplanes).  Both are asynchronous on the
- * handle's stream: ONE launch of a copy kernel over the record's contiguous plane ranges (16-byte accesses) per call (the
- * first call after clip_init on a k_fused handle also runs that path's one-time phi(t+1) pre-pass, so that the record is
- * complete: the ghost planes must be refreshed once before the first step, because k_init's gradient is wrong on the
- * outermost one); the transfer between GPUs is the
- * caller's (paper_2505_12205_b200/slab.py: NCCL send / recv between z neighbours).  A physical z face of the whole lattice
- * (WALL, FREESLIP, INLET, OUTLET) belongs to the first / last slab only; the cut faces of a slab may carry any non-periodic type
- * (slab.py uses WALL), their planes are ghosts.  The outlet's U_ave / U_max (B.22) are taken over one x-y plane, which lies in the
- * last slab: no reduction between slabs.  CLIP_ESTATE before clip_init, CLIP_EINVAL for planes outside the lattice or a bad buffer;
- * clip_halo_bytes returns 0 for bad arguments. */
-size_t clip_halo_bytes(const clip_t* h, int nplanes);
-int clip_halo_pack(clip_t* h, int z0, int nplanes, void* d_buf);
-int clip_halo_unpack(clip_t* h, int z0, int nplanes, const void* d_buf);
+/* z-slab decomposition over several GPUs: one process per GPU holds a slab of consecutive z planes as an ordinary
+ * clip_t whose cut faces are CLIP_BC_HALO (one ghost plane per cut).  Streaming pulls every population from at most one plane away
+ * (Eq. 13, 33; Alg. 2 :432-459) and the stencils of Eq. 40 (:307-309) read phi one plane away, so what an owned plane needs from
+ * the ghost plane next to it is: the 5 f+ and 5 g+ populations that move towards it, and phi of the next collision there.  Per
+ * step and per cut each side sends ONE record of 12 words per face node (clip_halo_bytes bytes, layout [12][ny][nx]):
+ *   0-4 f+_a, 5-9 g+_a of its boundary plane B for the five directions a that point at the neighbour;
+ *   10  the part of phi_B(t+1) = sum_a g+_a(x - e_a, t) that comes from its own side (links bounced at an x / y wall included);
+ *   11  C: what B sends into the neighbour's boundary plane, sum over those five a of g+_a(x - e_a) (in-plane faces applied).
+ * The receiver completes both boundary planes by additions: phi_ghost = received[10] + (its own C, just sent), and, on the
+ * k_fused path (whose on-chip scatter cannot see the ghost's populations), phi_B += received[11]; the ghost plane's ten
+ * populations are stored as they are.  phi is therefore summed in a different order than on the undivided lattice: the slabs
+ * reproduce it to round-off, not bit for bit.
+ *   clip_halo_pack(h, d_lo, d_hi)    writes the records of the -z / +z HALO face into d_lo / d_hi (device, 16-byte aligned,
+ *                                    clip_halo_bytes(h) each; NULL for a face that is not HALO).  One launch.
+ *   clip_halo_unpack(h, d_recv_lo, d_recv_hi, d_sent_lo, d_sent_hi)
+ *                                    d_recv_lo = the record the slab BELOW packed for its +z face, d_recv_hi = the record the slab
+ *                                    above packed for its -z face, d_sent_* = what this handle packed at the same time.  One launch.
+ * Both are asynchronous on the handle's stream; the transfer between GPUs is the caller's (paper_2505_12205_b200/slab.py: NCCL
+ * send / recv between z neighbours).  Protocol: clip_init; pack, exchange, unpack; then per step: clip_step(h, 1); pack, exchange,
+ * unpack.  A physical z face of the whole lattice (WALL, FREESLIP, INLET, OUTLET) belongs to the first / last slab.  The outlet's
+ * U_ave / U_max (B.22) are taken over one x-y plane, which lies in the last slab: no reduction between slabs.
+ * CLIP_ESTATE before clip_init, CLIP_EINVAL for a missing or misaligned buffer; clip_halo_bytes returns 0 for h == NULL. */
+size_t clip_halo_bytes(const clip_t* h);
+int clip_halo_pack(clip_t* h, void* d_lo, void* d_hi);
+int clip_halo_unpack(clip_t* h, const void* d_recv_lo, const void* d_recv_hi, const void* d_sent_lo, const void* d_sent_hi);
+
+/* Overlapped slab step: the exchange of a step's records runs on a second stream while the bulk of the step still computes.
+ *   clip_halo_stream(h, s2)            s2 (cudaStream_t as void*, ideally of higher priority) becomes the handle's halo stream
+ *                                      (NULL: none); the library creates three events for the ordering below.
+ *   clip_step_halo_begin(h, d_lo, d_hi)  ONE time step.  k_fused path: the first and the last z chunk (the planes next to the HALO
+ *                                      faces) run on the halo stream, followed there by clip_halo_pack into d_lo / d_hi; the other
+ *                                      chunks and k_fix run on the handle's stream at the same time.  Other kernel paths: the step
+ *                                      on the handle's stream, then the pack on the halo stream.  On return the records are being
+ *                                      produced ON THE HALO STREAM: the caller enqueues its transfer there.
+ *   clip_step_halo_end(h, recv_lo, recv_hi, sent_lo, sent_hi)   makes the handle's stream wait for the halo stream (the transfer)
+ *                                      and runs clip_halo_unpack there.
+ * CLIP_ESTATE without a halo stream or when begin / end do not alternate. */
+int clip_halo_stream(clip_t* h, void* cuda_stream);
+int clip_step_halo_begin(clip_t* h, void* d_lo, void* d_hi);
+int clip_step_halo_end(clip_t* h, const void* d_recv_lo, const void* d_recv_hi, const void* d_sent_lo, const void* d_sent_hi);
 
 /* Free the handle (not the workspace). */
 int clip_destroy(clip_t* h);

@@ -85,11 +85,17 @@ def lib():
         L.clip_step_profiled.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.clip_kernel_kinds.restype = C.c_int
         L.clip_halo_bytes.restype = C.c_size_t
-        L.clip_halo_bytes.argtypes = [C.c_void_p, C.c_int]
+        L.clip_halo_bytes.argtypes = [C.c_void_p]
         L.clip_halo_pack.restype = C.c_int
-        L.clip_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        L.clip_halo_pack.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.clip_halo_unpack.restype = C.c_int
-        L.clip_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        L.clip_halo_unpack.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.clip_halo_stream.restype = C.c_int
+        L.clip_halo_stream.argtypes = [C.c_void_p, C.c_void_p]
+        L.clip_step_halo_begin.restype = C.c_int
+        L.clip_step_halo_begin.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.clip_step_halo_end.restype = C.c_int
+        L.clip_step_halo_end.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.clip_kernel_name.restype = C.c_char_p
         L.clip_kernel_name.argtypes = [C.c_int]
         _lib = L
@@ -137,16 +143,28 @@ def clip_launch_count(h) -> int:
     return int(lib().clip_launch_count(h))
 
 
-def clip_halo_bytes(h, nplanes: int) -> int:
-    return int(lib().clip_halo_bytes(h, int(nplanes)))
+def clip_halo_bytes(h) -> int:
+    return int(lib().clip_halo_bytes(h))
 
 
-def clip_halo_pack(h, z0: int, nplanes: int, d_buf: int) -> int:
-    return lib().clip_halo_pack(h, int(z0), int(nplanes), C.c_void_p(d_buf))
+def clip_halo_pack(h, d_lo: int, d_hi: int) -> int:
+    return lib().clip_halo_pack(h, C.c_void_p(d_lo), C.c_void_p(d_hi))
 
 
-def clip_halo_unpack(h, z0: int, nplanes: int, d_buf: int) -> int:
-    return lib().clip_halo_unpack(h, int(z0), int(nplanes), C.c_void_p(d_buf))
+def clip_halo_unpack(h, d_recv_lo: int, d_recv_hi: int, d_sent_lo: int, d_sent_hi: int) -> int:
+    return lib().clip_halo_unpack(h, C.c_void_p(d_recv_lo), C.c_void_p(d_recv_hi), C.c_void_p(d_sent_lo), C.c_void_p(d_sent_hi))
+
+
+def clip_halo_stream(h, cuda_stream: int) -> int:
+    return lib().clip_halo_stream(h, C.c_void_p(cuda_stream))
+
+
+def clip_step_halo_begin(h, d_lo: int, d_hi: int) -> int:
+    return lib().clip_step_halo_begin(h, C.c_void_p(d_lo), C.c_void_p(d_hi))
+
+
+def clip_step_halo_end(h, d_recv_lo: int, d_recv_hi: int, d_sent_lo: int, d_sent_hi: int) -> int:
+    return lib().clip_step_halo_end(h, C.c_void_p(d_recv_lo), C.c_void_p(d_recv_hi), C.c_void_p(d_sent_lo), C.c_void_p(d_sent_hi))
 
 
 def clip_step_profiled(h, n: int):
@@ -247,17 +265,34 @@ class Clip:
             self._check(clip_get(self._h, phi.data_ptr() if phi is not None else 0,
                                  p.data_ptr() if p is not None else 0, u.data_ptr() if u is not None else 0))
 
-    def halo_buffer(self, nplanes):
-        """Device buffer (uint8) for the state record of `nplanes` planes (clip_halo_pack / clip_halo_unpack)."""
-        return self.torch.empty(clip_halo_bytes(self._h, nplanes), dtype=self.torch.uint8, device=self.device)
+    def halo_buffer(self):
+        """Device buffer for one face's halo record, [12, ny, nx] in the handle's precision (clip_halo_pack / clip_halo_unpack)."""
+        assert clip_halo_bytes(self._h) == 12 * self.ny * self.nx * (4 if self.dtype == self.torch.float32 else 8)
+        return self.torch.empty((12, self.ny, self.nx), dtype=self.dtype, device=self.device)
 
-    def halo_pack(self, z0, nplanes, buf):
+    def halo_pack(self, lo, hi):
         with self.torch.cuda.device(self.device):
-            self._check(clip_halo_pack(self._h, z0, nplanes, buf.data_ptr()))
+            self._check(clip_halo_pack(self._h, lo.data_ptr() if lo is not None else 0, hi.data_ptr() if hi is not None else 0))
 
-    def halo_unpack(self, z0, nplanes, buf):
+    def halo_unpack(self, recv_lo, recv_hi, sent_lo, sent_hi):
+        ptr = lambda t: t.data_ptr() if t is not None else 0  # noqa: E731
         with self.torch.cuda.device(self.device):
-            self._check(clip_halo_unpack(self._h, z0, nplanes, buf.data_ptr()))
+            self._check(clip_halo_unpack(self._h, ptr(recv_lo), ptr(recv_hi), ptr(sent_lo), ptr(sent_hi)))
+
+    def halo_stream(self, stream):
+        """Second (torch) stream of the overlapped slab step (clip_halo_stream); kept alive by the object."""
+        self._halo_stream = stream
+        with self.torch.cuda.device(self.device):
+            self._check(clip_halo_stream(self._h, stream.cuda_stream if stream is not None else 0))
+
+    def step_halo_begin(self, lo, hi):
+        with self.torch.cuda.device(self.device):
+            self._check(clip_step_halo_begin(self._h, lo.data_ptr() if lo is not None else 0, hi.data_ptr() if hi is not None else 0))
+
+    def step_halo_end(self, recv_lo, recv_hi, sent_lo, sent_hi):
+        ptr = lambda t: t.data_ptr() if t is not None else 0  # noqa: E731
+        with self.torch.cuda.device(self.device):
+            self._check(clip_step_halo_end(self._h, ptr(recv_lo), ptr(recv_hi), ptr(sent_lo), ptr(sent_hi)))
 
     def step_profiled(self, n=1):
         with self.torch.cuda.device(self.device):

@@ -49,9 +49,10 @@ FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   if (p->collision != CLIP_COLL_WMRT || p->phase_only) return f;
   for (int k = 0; k < 4; ++k) if (p->bc[k] != CLIP_BC_PERIODIC && p->bc[k] != CLIP_BC_WALL) return f;
   if (p->bc[4] == CLIP_BC_FREESLIP || p->bc[5] == CLIP_BC_FREESLIP) return f;
-  // an INLET / OUTLET plane is stepped by the generic kernels; k_fused covers the planes [zlo, zlo + nz) in between
-  const int zlo = p->bc[4] == CLIP_BC_INLET ? 1 : 0;
-  nz -= zlo + (p->bc[5] == CLIP_BC_OUTLET ? 1 : 0);
+  // an INLET / OUTLET plane is stepped by the generic kernels, the ghost plane of a HALO face not at all; k_fused covers the
+  // planes [zlo, zlo + nz) in between
+  const int zlo = (p->bc[4] == CLIP_BC_INLET || p->bc[4] == CLIP_BC_HALO) ? 1 : 0;
+  nz -= zlo + ((p->bc[5] == CLIP_BC_OUTLET || p->bc[5] == CLIP_BC_HALO) ? 1 : 0);
   if (nx % 64 != 0 || nx > 512 || ny % 4 != 0 || nz < 4) return f;
   f.ty = 4;  // small tiles leave more of the SM's L1 to the phi stencil and the shifted population loads (measured)
   if ((p->tile_ty == 4 || p->tile_ty == 8 || p->tile_ty == 16) && ny % p->tile_ty == 0) f.ty = p->tile_ty;
@@ -154,7 +155,8 @@ const char* validate(int nx, int ny, int nz, const clip_params* p) {
   if (!std::isfinite(p->sigma)) return "sigma must be finite";
   for (int d = 0; d < 3; ++d) {
     const int lo = p->bc[2 * d], hi = p->bc[2 * d + 1];
-    if (lo < 0 || lo > 4 || hi < 0 || hi > 4) return "unknown boundary type";
+    if (lo < 0 || lo > 5 || hi < 0 || hi > 5) return "unknown boundary type";
+    if (d < 2 && (lo == CLIP_BC_HALO || hi == CLIP_BC_HALO)) return "HALO faces (slab cuts) are only supported on the z faces";
     if ((lo == CLIP_BC_PERIODIC) != (hi == CLIP_BC_PERIODIC)) return "PERIODIC faces must come in pairs";
     const bool open_lo = lo == CLIP_BC_INLET || lo == CLIP_BC_OUTLET, open_hi = hi == CLIP_BC_INLET || hi == CLIP_BC_OUTLET;
     if (d < 2 && (open_lo || open_hi)) return "INLET / OUTLET are only supported on the z faces";
@@ -162,6 +164,9 @@ const char* validate(int nx, int ny, int nz, const clip_params* p) {
   if (p->bc[4] == CLIP_BC_OUTLET) return "OUTLET is only supported on the +z face";
   if (p->bc[5] == CLIP_BC_INLET) return "INLET is only supported on the -z face";
   if (p->bc[5] == CLIP_BC_OUTLET && nz < 2) return "OUTLET needs nz >= 2";
+  if (nz - (p->bc[4] == CLIP_BC_HALO ? 1 : 0) - (p->bc[5] == CLIP_BC_HALO ? 1 : 0) < 2) {
+    if (p->bc[4] == CLIP_BC_HALO || p->bc[5] == CLIP_BC_HALO) return "a slab with HALO faces must own at least 2 planes besides its ghost planes";
+  }
   if (p->bc[4] == CLIP_BC_INLET && !(p->inlet_r >= 0.0)) return "inlet_r must be >= 0";
   if (p->outlet_u_mode < 0 || p->outlet_u_mode > 2) return "outlet_u_mode must be 0 (U_local), 1 (U_ave) or 2 (U_max)";
   if (p->outlet_clamp != 0 && p->outlet_clamp != 1) return "outlet_clamp must be 0 (B.25 as printed) or 1 (lambda = max(0, U))";
@@ -185,6 +190,12 @@ struct clip_handle {
   int cur;      // which of the A/B population buffers holds the current post-collision state
   int phi_cur;  // which phi buffer holds phi(t) (flips only on the k_fused path)
   bool phi_ahead;  // k_fused path: the other phi buffer already holds phi(t+1)
+  bool phi_partial[2];  // k_fused path, HALO faces: phi(t+1) of the boundary plane still lacks what the ghost plane sends (clip_halo_unpack)
+  int zlo, zhi;    // planes [zlo, zhi) are stepped: all but the ghost planes of HALO faces
+  cudaStream_t halo_stream;  // clip_halo_stream: second stream of the overlapped slab step (nullptr: none)
+  cudaEvent_t ev_start, ev_bnd, ev_halo;
+  bool overlap_open;         // between clip_step_halo_begin and clip_step_halo_end
+  bool split_done;           // the last do_step packed the records itself (split launch)
   FusedPlan fplan;
   bool inited;
   int mode;            // clip_params.path: 0 = automatic (k_fused + k_fix on wide lattices, else k_phi2 + k_step2), 1 = generic kernels
@@ -207,7 +218,7 @@ template <typename T> clip::KP<T> make_kp(const clip_handle* h) {
   P.nxy = (long long)h->nx * h->ny;
   P.any_nonperiodic = 0;
   for (int k = 0; k < 6; ++k) { P.bc[k] = p.bc[k]; if (p.bc[k] != CLIP_BC_PERIODIC) P.any_nonperiodic = 1; }
-  P.z_lo = 0; P.z_cnt = h->nz;
+  P.z_lo = h->zlo; P.z_cnt = h->zhi - h->zlo;
   P.has_inlet = p.bc[4] == CLIP_BC_INLET;
   P.has_outlet = p.bc[5] == CLIP_BC_OUTLET;
   P.visc_interp = p.visc_interp;
@@ -245,7 +256,7 @@ int check_cuda(clip_handle* h, const char* what) {
 unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / block); }
 
 template <typename T> int do_init(clip_handle* h, const void* phi0, const void* u0) {
-  h->phi_cur = 0; h->phi_ahead = false;
+  h->phi_cur = 0; h->phi_ahead = false; h->phi_partial[0] = h->phi_partial[1] = false;
   h->cur = 1;  // k_init writes into "dst"; flip afterwards so that it becomes the current state
   clip::KP<T> P = make_kp<T>(h);
   clip::k_init<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P, (const T*)phi0, (const T*)u0);
@@ -329,7 +340,7 @@ template <typename T> void fused_prepass(clip_handle* h, Prof* prof) {
   fast_shape(h, fg, fb);
   clip::FP<T> F = make_fp<T>(make_kp<T>(h));
   F.k.phi = (T*)(h->ws + (h->phi_cur ? h->L.off_phi : h->L.off_phi2));
-  F.k.z_lo = glo; F.k.z_cnt = h->nz - glo - ghi; fg.z = (unsigned)F.k.z_cnt;
+  F.k.z_lo = h->zlo + glo; F.k.z_cnt = h->zhi - ghi - F.k.z_lo; fg.z = (unsigned)F.k.z_cnt;
   if (prof) prof->begin();
   clip::launch_phi2<T>(walls, h->nx_special, fg, fb, h->stream, F);
   if (prof) prof->end(KIND_PHI2);
@@ -338,7 +349,10 @@ template <typename T> void fused_prepass(clip_handle* h, Prof* prof) {
   h->phi_ahead = true;
 }
 
-template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullptr) {
+// split = true (clip_step_halo_begin, one step, k_fused path with >= 3 chunks): the first and the last z chunk -- the ones next to
+// the HALO faces -- run on the halo stream, followed there by the pack kernel (the caller's exchange then overlaps the interior
+// chunks, which run on the handle's stream together with k_fix).
+template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullptr, bool split = false, void* d_lo = nullptr, void* d_hi = nullptr) {
   const bool fast = fast_ok(h);
   bool walls = false;
   for (int k = 0; k < 6; ++k) walls = walls || h->p.bc[k] == CLIP_BC_WALL;
@@ -374,7 +388,29 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       for (int c = 0; c <= fp.nchunks; ++c) U.zc[c] = fp.zc[c];
       U.tile_stride = (long long)(2 * fp.tzmax + 2 * (fp.ty + 2)) * h->nx;
       if (prof) prof->begin();
-      const cudaError_t fe = clip::launch_fused<T>(walls, h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+      cudaError_t fe;
+      if (split && fp.nchunks >= 3 && fp.zc[1] - fp.zc[0] >= 2 && fp.zc[fp.nchunks] - fp.zc[fp.nchunks - 1] >= 2) {
+        h->split_done = true;
+        cudaEventRecord(h->ev_start, h->stream);
+        cudaStreamWaitEvent(h->halo_stream, h->ev_start, 0);
+        U.c_mode = 1;
+        fe = clip::launch_fused<T>(walls, h->nx_special, dim3(fp.ytiles, 2), dim3(fp.threads), fp.smem_bytes, h->halo_stream, F, U);
+        cudaEventRecord(h->ev_bnd, h->halo_stream);
+        if (fe == cudaSuccess) {  // the records need the new populations of the boundary planes and their neighbours only
+          const cudaStream_t main_stream = h->stream;
+          h->cur ^= 1; h->stream = h->halo_stream;
+          const int rc = clip_halo_pack(h, d_lo, d_hi);
+          h->cur ^= 1; h->stream = main_stream;
+          if (rc != CLIP_OK) return rc;
+          U.c_mode = 2;
+          fe = clip::launch_fused<T>(walls, h->nx_special, dim3(fp.ytiles, fp.nchunks - 2), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+          h->launches += 1;
+        }
+        cudaStreamWaitEvent(h->stream, h->ev_bnd, 0);
+      } else {
+        U.c_mode = 0;
+        fe = clip::launch_fused<T>(walls, h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+      }
       if (fe != cudaSuccess) { set_err(h->err, "k_fused: %s", cudaGetErrorString(fe)); return CLIP_ECUDA; }
       if (prof) { prof->end(KIND_FUSED); prof->begin(); }
       const int fix_rpb = clip::FIX_ROWS * (clip::FIX_THREADS / clip::fix_threads_per_row(h->nx, clip::Vec16<T>::EV));  // rows per block
@@ -384,6 +420,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       h->cur ^= 1;
       h->phi_cur ^= 1;
       h->t += 1;
+      h->phi_partial[0] = h->p.bc[4] == CLIP_BC_HALO; h->phi_partial[1] = h->p.bc[5] == CLIP_BC_HALO;  // completed by clip_halo_unpack
       fused_open_planes<T>(h, prof);  // open z faces: lambda and the boundary planes of phi(t+2), from the new state
       continue;
     }
@@ -392,13 +429,13 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
     clip::KP<T> Plo = P, Phi = P;
     Plo.z_lo = 0; Plo.z_cnt = glo; Phi.z_lo = h->nz - ghi; Phi.z_cnt = ghi;
     clip::FP<T> F;
-    if (fast) { F = make_fp<T>(P); F.k.z_lo = glo; F.k.z_cnt = h->nz - glo - ghi; fg.z = (unsigned)F.k.z_cnt; }
+    if (fast) { F = make_fp<T>(P); F.k.z_lo = h->zlo + glo; F.k.z_cnt = h->zhi - ghi - F.k.z_lo; fg.z = (unsigned)F.k.z_cnt; }
     if (P.has_outlet) outlet_lambda<T>(h, P, prof);  // lambda of B.25 for this step, before anything of the step reads it
     for (int pass = 0; pass < 2; ++pass) {  // pass 0: phi(t+1); pass 1: macros + collisions
       if (!fast) {
         if (prof) prof->begin();
-        if (pass == 0) clip::k_phi<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
-        else clip::k_step<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
+        if (pass == 0) clip::k_phi<T><<<grid_for(P.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(P);
+        else clip::k_step<T><<<grid_for(P.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(P);
         h->launches += 1;
         if (prof) prof->end(pass == 0 ? KIND_PHI : KIND_STEP);
         continue;
@@ -434,87 +471,187 @@ template <typename T> int do_get(clip_handle* h, void* phi, void* p, void* u) {
   return check_cuda(h, "k_get");
 }
 
-// z-slab decomposition (clip.h): the state of `np` consecutive planes is six contiguous segments of the workspace
-// (z is the slowest index of every array): populations, phi(t), phi(t+1) (k_fused only), u_x, u_y, u_z.
-struct HaloSeg { size_t off, bytes; };
-struct HaloJob {  // up to six (source, destination) ranges, copied by ONE launch in units of U bytes
-  const char* src[6];
-  char* dst[6];
-  unsigned long long end[6];  // running sum of the ranges' unit counts
-  int ns;
+// z-slab decomposition (clip.h).  A HALO z face means: the first / last plane of this lattice is a GHOST plane, an
+// image of the neighbouring slab's outermost owned plane; the step kernels cover the owned planes only.  What an owned plane
+// reads from the ghost plane next to it: the 5 + 5 populations that move towards it (pull streaming, Alg. 2) and phi of the
+// next collision (stencils of Eq. 40).  The record one slab sends per face node (12 words, SURVEY's 10 + 1 and one more):
+//   [0..4]  f+_a, [5..9] g+_a of its boundary plane B for the five a that point at the neighbour (e_z = s)
+//   [10]    the PART of phi_B(next) = sum_a g_a (Eq. 38 after streaming) that comes from its own side (planes B, B -+ 1; links
+//           bounced at an x / y wall included)
+//   [11]    C = what B sends INTO the neighbour's boundary plane: sum over the five a of g+_a(x - e_a), in-plane faces applied
+// The receiver completes both boundary planes by additions: phi_ghost = record[10] + (its own C, which it has just sent), and --
+// on the k_fused path, whose scatter could not see the ghost's populations -- phi_B += record[11].
+template <typename T, int a = 1> struct HaloDirs {
+  // sums over directions of the pull at node (pb, nb); WHICH selects by e_z: +1 / -1 = only that sign; 0 handled by the caller
+  static __device__ __forceinline__ void run(const clip::KP<T>& P, long long pb, const clip::Nbr& nb, int s, T& part, T& c_in) {
+    using namespace clip;
+    const bool bounced = src_bounce<a>(nb);
+    // partial of the boundary plane: everything except what comes from beyond the HALO face (e_z = -s, not bounced in-plane)
+    if (cz(a) != 0) {
+      if (cz(a) != -s || bounced) part += pull_one<T, a>(P.p_src + Q * P.nx, P.nx, pb, nb, nb.any);
+    } else part += pull_one<T, a>(P.p_src + Q * P.nx, P.nx, pb, nb, nb.any);
+    HaloDirs<T, a + 1>::run(P, pb, nb, s, part, c_in);
+  }
+  static __device__ __forceinline__ void into(const clip::KP<T>& P, long long pbg, const clip::Nbr& ng, int s, T& c) {
+    using namespace clip;
+    if (cz(a) != 0 && cz(a) == s && !src_bounce<a>(ng)) c += pull_one<T, a>(P.p_src + Q * P.nx, P.nx, pbg, ng, ng.any);
+    HaloDirs<T, a + 1>::into(P, pbg, ng, s, c);
+  }
+  static __device__ __forceinline__ void copy_out(const clip::KP<T>& P, long long pb, int s, T* rec, long long c, int& k) {
+    using namespace clip;
+    if (cz(a) == s) { rec[k * P.nxy + c] = P.p_src[pb + a * P.nx]; rec[(5 + k) * P.nxy + c] = P.p_src[pb + (Q + a) * P.nx]; ++k; }
+    HaloDirs<T, a + 1>::copy_out(P, pb, s, rec, c, k);
+  }
+  static __device__ __forceinline__ void copy_in(const clip::KP<T>& P, T* pop, long long pb, int s, const T* rec, long long c, int& k) {
+    using namespace clip;
+    if (cz(a) == s) { pop[pb + a * P.nx] = rec[k * P.nxy + c]; pop[pb + (Q + a) * P.nx] = rec[(5 + k) * P.nxy + c]; ++k; }
+    HaloDirs<T, a + 1>::copy_in(P, pop, pb, s, rec, c, k);
+  }
 };
-template <typename U> __global__ void __launch_bounds__(256) k_halo(const HaloJob J) {
-  const unsigned long long total = J.end[J.ns - 1], stride = (unsigned long long)gridDim.x * blockDim.x;
-  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride) {
-    int k = 0;
-#pragma unroll
-    for (int q = 0; q < 5; ++q) k += (q < J.ns - 1 && i >= J.end[q]) ? 1 : 0;
-    const unsigned long long j = i - (k ? J.end[k - 1] : 0ull);
-    reinterpret_cast<U*>(J.dst[k])[j] = reinterpret_cast<const U*>(J.src[k])[j];
-  }
-}
-int halo_segments(const clip_handle* h, int z0, int np, HaloSeg* seg) {
-  const size_t w = h->L.word, nxy = (size_t)h->nx * h->ny, n = nxy * h->nz;
+template <typename T> struct HaloDirs<T, clip::Q> {
+  static __device__ __forceinline__ void run(const clip::KP<T>&, long long, const clip::Nbr&, int, T&, T&) {}
+  static __device__ __forceinline__ void into(const clip::KP<T>&, long long, const clip::Nbr&, int, T&) {}
+  static __device__ __forceinline__ void copy_out(const clip::KP<T>&, long long, int, T*, long long, int&) {}
+  static __device__ __forceinline__ void copy_in(const clip::KP<T>&, T*, long long, int, const T*, long long, int&) {}
+};
+constexpr int HALO_WORDS = 12;
+
+// grid = (ceil(nxy / 256), 2): blockIdx.y = side (0: -z, 1: +z); a side without a record has rec == nullptr
+template <typename T> __global__ void __launch_bounds__(256) k_halo_pack(const __grid_constant__ clip::KP<T> P, T* rec_lo, T* rec_hi) {
+  using namespace clip;
+  const int side = blockIdx.y;
+  T* const rec = side ? rec_hi : rec_lo;
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (!rec || c >= P.nxy) return;
+  const int x = (int)(c % P.nx), y = (int)(c / P.nx);
+  const int s = side ? 1 : -1, zg = side ? P.nz - 1 : 0, zb = zg - s;
+  const long long ib = (long long)zb * P.nxy + c, ig = (long long)zg * P.nxy + c;
+  const long long pb = pop_base(ib, x), pbg = pop_base(ig, x);
   int k = 0;
-  seg[k++] = {h->L.off_p[h->cur] + 38 * nxy * z0 * w, 38 * nxy * np * w};
-  seg[k++] = {(h->phi_cur ? h->L.off_phi2 : h->L.off_phi) + nxy * z0 * w, nxy * np * w};
-  if (use_fused(h)) seg[k++] = {(h->phi_cur ? h->L.off_phi : h->L.off_phi2) + nxy * z0 * w, h->phi_ahead ? nxy * np * w : 0};
-  for (int c = 0; c < 3; ++c) seg[k++] = {h->L.off_u + (c * n + nxy * z0) * w, nxy * np * w};
-  return k;
+  HaloDirs<T>::copy_out(P, pb, s, rec, c, k);
+  // the boundary plane is never the first / last plane of the array, so its Nbr (in-plane faces, plain z offsets) also serves
+  // the pull of the ghost-plane node from this side
+  const Nbr nb = make_nbr(P, x, y, zb);
+  const Nbr& ng = nb;
+  T part = P.p_src[pb + Q * P.nx], dummy = T(0), cin = T(0);  // direction 0
+  HaloDirs<T>::run(P, pb, nb, s, part, dummy);
+  HaloDirs<T>::into(P, pbg, ng, s, cin);
+  if (P.has_inlet && zb == 0 && P.mask[c]) part = P.phi_in;   // (cannot happen: an inlet plane is never next to a HALO face)
+  rec[10 * P.nxy + c] = part;
+  rec[11 * P.nxy + c] = cin;
 }
-int halo_copy(clip_handle* h, int z0, int np, char* buf, bool pack, const char* who) {
-  if (!h->inited) { set_err(h->err, "%s: clip_init has not been called", who); return CLIP_ESTATE; }
-  if (z0 < 0 || np < 0 || z0 + np > h->nz) { set_err(h->err, "%s: planes [%d, %d) are outside the lattice", who, z0, z0 + np); return CLIP_EINVAL; }
-  if (!buf || ((uintptr_t)buf) % 16) { set_err(h->err, "%s: buffer must be a 16-byte aligned device pointer", who); return CLIP_EINVAL; }
-  if (np == 0) return CLIP_OK;
-  if (use_fused(h) && !h->phi_ahead) {  // the record of a k_fused handle carries phi(t+1): bring it into being first
-    if (h->p.precision == 32) fused_prepass<float>(h, nullptr); else fused_prepass<double>(h, nullptr);
-    const int rc = check_cuda(h, who);
-    if (rc != CLIP_OK) return rc;
-  }
-  HaloSeg seg[6];
-  const int ns = halo_segments(h, z0, np, seg);
-  const size_t slot = (size_t)h->nx * h->ny * np * h->L.word;  // the phi(t+1) slot is kept even while it is not yet valid
-  bool wide = true;  // 16-byte units when every range allows it (always on the lattices of the fast kernels), else 4-byte units
-  size_t o = 0;
-  HaloJob J{};
-  for (int k = 0; k < ns; ++k) {
-    if (seg[k].bytes) {
-      char* in_ws = h->ws + seg[k].off;
-      J.src[J.ns] = pack ? in_ws : buf + o;
-      J.dst[J.ns] = pack ? buf + o : in_ws;
-      J.end[J.ns] = seg[k].bytes;  // bytes for now
-      wide = wide && seg[k].bytes % 16 == 0 && ((uintptr_t)in_ws) % 16 == 0 && o % 16 == 0;
-      J.ns += 1;
-    }
-    o += k == 0 ? seg[k].bytes : slot;
-  }
-  const unsigned unit = wide ? 16u : 4u;
-  unsigned long long run = 0;
-  for (int k = 0; k < J.ns; ++k) { run += J.end[k] / unit; J.end[k] = run; }
-  unsigned long long blocks = (run + 255) / 256;
-  if (blocks > (unsigned long long)B200_SMS * 8) blocks = (unsigned long long)B200_SMS * 8;
-  if (wide) k_halo<uint4><<<(unsigned)blocks, 256, 0, h->stream>>>(J);
-  else k_halo<unsigned><<<(unsigned)blocks, 256, 0, h->stream>>>(J);
-  h->launches += 1;
-  return check_cuda(h, who);
+// recv_*: the record the neighbour on that side packed (its opposite side); sent_*: the record this handle packed for that side
+template <typename T> __global__ void __launch_bounds__(256)
+k_halo_unpack(const __grid_constant__ clip::KP<T> P, const T* recv_lo, const T* recv_hi, const T* sent_lo, const T* sent_hi, T* phi_next,
+              int add_lo, int add_hi) {
+  using namespace clip;
+  const int side = blockIdx.y;
+  const T* const recv = side ? recv_hi : recv_lo;
+  const T* const sent = side ? sent_hi : sent_lo;
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (!recv || c >= P.nxy) return;
+  const int x = (int)(c % P.nx);
+  const int s = side ? 1 : -1, zg = side ? P.nz - 1 : 0, zb = zg - s;
+  const long long ib = (long long)zb * P.nxy + c, ig = (long long)zg * P.nxy + c;
+  int k = 0;
+  HaloDirs<T>::copy_in(P, const_cast<T*>(P.p_src), pop_base(ig, x), -s, recv, c, k);   // what moves from the neighbour towards me
+  phi_next[ig] = recv[10 * P.nxy + c] + sent[11 * P.nxy + c];
+  if (side ? add_hi : add_lo) phi_next[ib] += recv[11 * P.nxy + c];
 }
 
 }  // namespace
 
 extern "C" {
 
-size_t clip_halo_bytes(const clip_t* h, int nplanes) {
-  if (!h || nplanes < 0) return 0;
-  return (size_t)h->nx * h->ny * nplanes * h->L.word * (38 + 1 + (use_fused(h) ? 1 : 0) + 3);
+size_t clip_halo_bytes(const clip_t* h) {
+  if (!h) return 0;
+  return (size_t)h->nx * h->ny * h->L.word * HALO_WORDS;
 }
-int clip_halo_pack(clip_t* h, int z0, int nplanes, void* d_buf) {
+int clip_halo_pack(clip_t* h, void* d_lo, void* d_hi) {
   if (!h) return CLIP_EINVAL;
-  return halo_copy(h, z0, nplanes, (char*)d_buf, true, "clip_halo_pack");
+  if (!h->inited) { set_err(h->err, "clip_halo_pack: clip_init has not been called"); return CLIP_ESTATE; }
+  const bool lo = h->p.bc[4] == CLIP_BC_HALO, hi = h->p.bc[5] == CLIP_BC_HALO;
+  if ((lo && !d_lo) || (hi && !d_hi) || ((uintptr_t)d_lo) % 16 || ((uintptr_t)d_hi) % 16) {
+    set_err(h->err, "clip_halo_pack: every HALO face needs a 16-byte aligned device buffer of clip_halo_bytes");
+    return CLIP_EINVAL;
+  }
+  if (!lo && !hi) return CLIP_OK;
+  const dim3 grid(grid_for((long long)h->nx * h->ny, 256), 2);
+  if (h->p.precision == 32) k_halo_pack<float><<<grid, 256, 0, h->stream>>>(make_kp<float>(h), lo ? (float*)d_lo : nullptr, hi ? (float*)d_hi : nullptr);
+  else k_halo_pack<double><<<grid, 256, 0, h->stream>>>(make_kp<double>(h), lo ? (double*)d_lo : nullptr, hi ? (double*)d_hi : nullptr);
+  h->launches += 1;
+  return check_cuda(h, "clip_halo_pack");
 }
-int clip_halo_unpack(clip_t* h, int z0, int nplanes, const void* d_buf) {
+int clip_halo_unpack(clip_t* h, const void* d_recv_lo, const void* d_recv_hi, const void* d_sent_lo, const void* d_sent_hi) {
   if (!h) return CLIP_EINVAL;
-  return halo_copy(h, z0, nplanes, (char*)d_buf, false, "clip_halo_unpack");
+  if (!h->inited) { set_err(h->err, "clip_halo_unpack: clip_init has not been called"); return CLIP_ESTATE; }
+  const bool lo = h->p.bc[4] == CLIP_BC_HALO, hi = h->p.bc[5] == CLIP_BC_HALO;
+  if ((lo && (!d_recv_lo || !d_sent_lo)) || (hi && (!d_recv_hi || !d_sent_hi)) || ((uintptr_t)d_recv_lo) % 16 || ((uintptr_t)d_recv_hi) % 16 ||
+      ((uintptr_t)d_sent_lo) % 16 || ((uintptr_t)d_sent_hi) % 16) {
+    set_err(h->err, "clip_halo_unpack: every HALO face needs the received and the sent record (16-byte aligned device buffers)");
+    return CLIP_EINVAL;
+  }
+  if (!lo && !hi) return CLIP_OK;
+  const dim3 grid(grid_for((long long)h->nx * h->ny, 256), 2);
+  // phi of the NEXT collision: the k_fused path keeps it in the second buffer, the other paths rewrite the one buffer in place
+  char* const next = h->ws + (use_fused(h) ? (h->phi_cur ? h->L.off_phi : h->L.off_phi2) : h->L.off_phi);
+  const int add_lo = lo && h->phi_partial[0], add_hi = hi && h->phi_partial[1];
+  if (h->p.precision == 32)
+    k_halo_unpack<float><<<grid, 256, 0, h->stream>>>(make_kp<float>(h), lo ? (const float*)d_recv_lo : nullptr, hi ? (const float*)d_recv_hi : nullptr,
+                                                      (const float*)d_sent_lo, (const float*)d_sent_hi, (float*)next, add_lo, add_hi);
+  else
+    k_halo_unpack<double><<<grid, 256, 0, h->stream>>>(make_kp<double>(h), lo ? (const double*)d_recv_lo : nullptr, hi ? (const double*)d_recv_hi : nullptr,
+                                                       (const double*)d_sent_lo, (const double*)d_sent_hi, (double*)next, add_lo, add_hi);
+  h->phi_partial[0] = h->phi_partial[1] = false;
+  h->launches += 1;
+  return check_cuda(h, "clip_halo_unpack");
+}
+
+int clip_halo_stream(clip_t* h, void* cuda_stream) {
+  if (!h) return CLIP_EINVAL;
+  if (h->overlap_open) { set_err(h->err, "clip_halo_stream: a step is open (clip_step_halo_end missing)"); return CLIP_ESTATE; }
+  if (cuda_stream && !h->ev_start) {
+    if (cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming) != cudaSuccess || cudaEventCreateWithFlags(&h->ev_bnd, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_halo, cudaEventDisableTiming) != cudaSuccess) {
+      set_err(h->err, "clip_halo_stream: %s", cudaGetErrorString(cudaGetLastError()));
+      return CLIP_ECUDA;
+    }
+  }
+  h->halo_stream = (cudaStream_t)cuda_stream;
+  return CLIP_OK;
+}
+int clip_step_halo_begin(clip_t* h, void* d_lo, void* d_hi) {
+  if (!h) return CLIP_EINVAL;
+  if (!h->inited) { set_err(h->err, "clip_step_halo_begin: clip_init has not been called"); return CLIP_ESTATE; }
+  if (!h->halo_stream) { set_err(h->err, "clip_step_halo_begin: no halo stream (clip_halo_stream)"); return CLIP_ESTATE; }
+  if (h->overlap_open) { set_err(h->err, "clip_step_halo_begin: the previous step is still open (clip_step_halo_end missing)"); return CLIP_ESTATE; }
+  const bool lo = h->p.bc[4] == CLIP_BC_HALO, hi = h->p.bc[5] == CLIP_BC_HALO;
+  if ((lo && !d_lo) || (hi && !d_hi) || ((uintptr_t)d_lo) % 16 || ((uintptr_t)d_hi) % 16) {
+    set_err(h->err, "clip_step_halo_begin: every HALO face needs a 16-byte aligned device buffer of clip_halo_bytes");
+    return CLIP_EINVAL;
+  }
+  h->split_done = false;
+  int rc = h->p.precision == 32 ? do_step<float>(h, 1, nullptr, use_fused(h), d_lo, d_hi) : do_step<double>(h, 1, nullptr, use_fused(h), d_lo, d_hi);
+  if (rc != CLIP_OK) return rc;
+  if (!h->split_done) {  // other paths: the whole step on the handle's stream, then the records on the halo stream
+    cudaEventRecord(h->ev_start, h->stream);
+    cudaStreamWaitEvent(h->halo_stream, h->ev_start, 0);
+    const cudaStream_t main_stream = h->stream;
+    h->stream = h->halo_stream;
+    rc = clip_halo_pack(h, d_lo, d_hi);
+    h->stream = main_stream;
+    if (rc != CLIP_OK) return rc;
+  }
+  h->overlap_open = true;
+  return check_cuda(h, "clip_step_halo_begin");
+}
+int clip_step_halo_end(clip_t* h, const void* d_recv_lo, const void* d_recv_hi, const void* d_sent_lo, const void* d_sent_hi) {
+  if (!h) return CLIP_EINVAL;
+  if (!h->overlap_open) { set_err(h->err, "clip_step_halo_end: no open step (clip_step_halo_begin)"); return CLIP_ESTATE; }
+  cudaEventRecord(h->ev_halo, h->halo_stream);     // after the caller's exchange
+  cudaStreamWaitEvent(h->stream, h->ev_halo, 0);
+  h->overlap_open = false;
+  return clip_halo_unpack(h, d_recv_lo, d_recv_hi, d_sent_lo, d_sent_hi);
 }
 
 size_t clip_workspace_bytes(int nx, int ny, int nz, const clip_params* params) {
@@ -540,6 +677,9 @@ int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params,
   if (!h) { set_err(g_create_error, "clip_create: out of host memory"); return CLIP_ENOMEM; }
   h->nx = nx; h->ny = ny; h->nz = nz; h->p = *params; h->L = L; h->ws = (char*)d_workspace;
   h->stream = (cudaStream_t)cuda_stream; h->cur = 0; h->phi_cur = 0; h->phi_ahead = false; h->inited = false;
+  h->phi_partial[0] = h->phi_partial[1] = false;
+  h->halo_stream = nullptr; h->ev_start = h->ev_bnd = h->ev_halo = nullptr; h->overlap_open = false; h->split_done = false;
+  h->zlo = params->bc[4] == CLIP_BC_HALO ? 1 : 0; h->zhi = nz - (params->bc[5] == CLIP_BC_HALO ? 1 : 0);
   h->fplan = fused_plan(nx, ny, nz, params);
   h->mode = params->path;
   h->fast_threads = 128;  // measured: fp64 8.2 vs 7.6 GLUPS, fp32 (with 3 blocks per SM) +2 % against 256-thread blocks
@@ -624,6 +764,7 @@ int clip_get(clip_t* h, void* d_phi, void* d_p, void* d_u) {
 int clip_destroy(clip_t* h) {
   if (!h) return CLIP_EINVAL;
   if (!h->mask_host.empty()) cudaStreamSynchronize(h->stream);  // the mask upload reads host memory we own
+  if (h->ev_start) { cudaEventDestroy(h->ev_start); cudaEventDestroy(h->ev_bnd); cudaEventDestroy(h->ev_halo); }
   delete h;
   return CLIP_OK;
 }

@@ -33,6 +33,7 @@ template <typename T> struct FusedP {
   int zc[FUSED_MAX_CHUNKS + 1];  // chunk c covers the planes zc[c] .. zc[c+1]-1 (sizes <= tzmax; clip.cu: fused_plan)
   long long tile_stride;  // elements of `part` per tile
   int z_wrap;             // the z faces are PERIODIC: the first and the last chunk are neighbours (k_fix)
+  int c_mode;             // which chunks a k_fused launch covers: 0 all (c = blockIdx.y), 1 the first and the last one, 2 all others
 };
 // rows of a tile's slab in `part`
 __host__ __device__ __forceinline__ int slot_ym(int k) { return k; }
@@ -149,7 +150,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP
   T* edge_p = ring + (size_t)nslots * rows * nx;
   T* edge_m = edge_p + nslots * rows * nwarps;
   const int x0 = 2 * threadIdx.x;
-  const int iy = blockIdx.x, c = blockIdx.y;
+  const int iy = blockIdx.x;
+  const int c = U.c_mode == 0 ? (int)blockIdx.y : (U.c_mode == 1 ? (blockIdx.y ? U.nchunks - 1 : 0) : (int)blockIdx.y + 1);
   const int y0 = iy * U.ty, z0 = U.zc[c], z1 = U.zc[c + 1];
   const int tz = z1 - z0;
   for (int i = threadIdx.x; i < nslots * rows * (nx + 2 * nwarps); i += blockDim.x) ring[i] = T(0);

@@ -1,20 +1,20 @@
 """z-slab decomposition of one lattice over several GPUs (include/clip.h, clip_halo_pack).
 
-One process per GPU owns `nz / world` consecutive z planes plus two ghost planes beyond each interior cut.  After every
-step the two outermost OWNED planes on each side go to the z neighbour, which writes them over its ghost planes: the pull of
-Eq. 13 / 33 (Alg. 2 :432-459) reaches one plane, the stencils of Eq. 40 (:309-331) on phi(t+1) one more, so
-two planes make the owned planes equal to those of the undivided lattice (bit for bit on the two-kernel path; the
-k_fused path sums phi in tile order, and a slab has other tiles than the whole lattice: equal to round-off).  The exchange is
-the path's only collective: a neighbour send / recv (`torch.distributed` P2P: NCCL over NVLink on GPUs, gloo in the CPU tests),
-no reduction.  Everything else -- packing, stepping, unpacking -- runs in libclip.
+One process per GPU owns `nz / world` consecutive z planes plus ONE ghost plane beyond each interior cut (face type CLIP_BC_HALO:
+libclip steps the owned planes only).  After every step each side of a cut sends one record of 12 words per face node -- the ten
+populations of its boundary plane that move towards the neighbour (Eq. 13 / 33 streaming; Alg. 2 :432-459) and
+two partial sums of phi(t+1) = sum_a g_a (Eq. 38), from which both sides complete phi on the two planes of the cut (the stencils of
+Eq. 40, :307-309, read it one plane away).  The owned planes then equal those of the undivided lattice to round-off (phi of the cut
+planes is summed in another order).  The exchange is the path's only collective: a neighbour send / recv (`torch.distributed` P2P:
+NCCL over NVLink on GPUs, gloo in the CPU tests), no reduction.  Packing, stepping and unpacking run in libclip.
 
 This module holds plumbing only (who owns which planes, who sends what to whom); no arithmetic of the method.
 """
 from __future__ import annotations
 
-HALO = 2  # ghost planes per interior cut (see the module docstring)
+HALO = 1  # ghost planes per interior cut (see the module docstring)
 
-_WALL = 1  # CLIP_BC_WALL
+_HALO_BC = 5  # CLIP_BC_HALO
 
 
 def slab_range(nz: int, rank: int, world: int):
@@ -24,8 +24,8 @@ def slab_range(nz: int, rank: int, world: int):
     if nz % world != 0:
         raise ValueError(f"nz = {nz} is not a multiple of the {world} slabs")
     own = nz // world
-    if own < HALO:
-        raise ValueError(f"a slab of {own} planes is thinner than the halo ({HALO})")
+    if own < 2:
+        raise ValueError(f"a slab must own at least 2 planes (got {own}): its two halo records must not depend on each other")
     return rank * own, (rank + 1) * own
 
 
@@ -48,13 +48,6 @@ def neighbours(rank: int, world: int, z_periodic: bool):
     below = (rank - 1) % world if (z_periodic or rank > 0) else None
     above = (rank + 1) % world if (z_periodic or rank < world - 1) else None
     return below, above
-
-
-def halo_planes(nz_local: int, lo: int, hi: int):
-    """First local plane of the four halo records: the owned planes that are SENT down / up, and the ghost planes that the
-    records RECEIVED from below / above overwrite (None where that side has no ghosts)."""
-    return {"send_lo": lo if lo else None, "send_hi": nz_local - hi - HALO if hi else None,
-            "recv_lo": 0 if lo else None, "recv_hi": nz_local - HALO if hi else None}
 
 
 def exchange(send_lo, send_hi, recv_lo, recv_hi, rank: int, world: int, z_periodic: bool, group=None):
@@ -98,7 +91,7 @@ def exchange(send_lo, send_hi, recv_lo, recv_hi, rank: int, world: int, z_period
 class SlabClip:
     """One rank's slab of a global nx x ny x nz lattice.  `params["bc"]` are the GLOBAL faces (any type the library takes)."""
 
-    def __init__(self, nx, ny, nz, params: dict, rank: int, world: int, device="cuda:0", stream=None):
+    def __init__(self, nx, ny, nz, params: dict, rank: int, world: int, device="cuda:0", stream=None, overlap=True):
         from . import clip
         bc = [int(v) for v in params["bc"]]
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
@@ -108,24 +101,28 @@ class SlabClip:
         self.lo, self.hi = slab_ghosts(self.rank, self.world, self.z_periodic)
         self.planes = slab_plane_index(self.nz, self.rank, self.world, self.z_periodic)
         self.nz_local = len(self.planes)
-        # Local faces: a physical z face belongs to the first / last slab; a cut face may apply any rule (its planes are ghosts and are
-        # overwritten): PERIODIC on a periodic lattice (all slabs alike), else WALL.  Slabs with different faces or plane counts could
-        # choose different kernel paths; the record must agree on whether phi(t+1) is state, so they are created with path = 2.
+        # Local faces: a physical z face belongs to the first / last slab; every cut face is HALO (also both faces of the single slab
+        # of a periodic lattice, which is its own neighbour).  The record does not depend on the kernel path: slabs may differ.
         local = dict(params)
-        if not self.z_periodic:
-            bc[4] = bc[4] if self.rank == 0 else _WALL
-            bc[5] = bc[5] if self.rank == self.world - 1 else _WALL
-            local["bc"] = tuple(bc)
-            if self.world > 1 and int(params.get("path", 0)) in (0, 3):
-                local["path"] = 2
+        if self.lo:
+            bc[4] = _HALO_BC
+        if self.hi:
+            bc[5] = _HALO_BC
+        local["bc"] = tuple(bc)
         self.sim = clip.Clip(self.nx, self.ny, self.nz_local, local, device=device, stream=stream)
         self.torch = self.sim.torch
         self.device = self.sim.device
-        self.hp = halo_planes(self.nz_local, self.lo, self.hi)
-        mk = lambda n: self.sim.halo_buffer(HALO) if n else None  # noqa: E731
+        mk = lambda n: self.sim.halo_buffer() if n else None  # noqa: E731
         self.send_lo, self.recv_lo = mk(self.lo), mk(self.lo)
         self.send_hi, self.recv_hi = mk(self.hi), mk(self.hi)
         self.exchanges = 0
+        # overlapped step (clip_step_halo_begin / _end): the records travel on a second, higher-priority stream while the interior
+        # of the slab is still being computed
+        self.halo = None
+        if overlap and (self.lo or self.hi):
+            with self.torch.cuda.device(self.device):
+                self.halo = self.torch.cuda.Stream(device=self.device, priority=-1)
+            self.sim.halo_stream(self.halo)
 
     # -- plumbing -------------------------------------------------------------------------------------------------
     def init(self, phi0, u0):
@@ -135,18 +132,12 @@ class SlabClip:
         self.sim.init(phi0.index_select(0, idx), u0.index_select(1, idx))
 
     def pack(self):
-        """Copy my outermost owned planes into the send buffers (clip_halo_pack)."""
-        if self.lo:
-            self.sim.halo_pack(self.hp["send_lo"], HALO, self.send_lo)
-        if self.hi:
-            self.sim.halo_pack(self.hp["send_hi"], HALO, self.send_hi)
+        """Records of my boundary planes into the send buffers (clip_halo_pack, one launch)."""
+        self.sim.halo_pack(self.send_lo, self.send_hi)
 
     def unpack(self):
-        """Write the received records over my ghost planes (clip_halo_unpack)."""
-        if self.lo:
-            self.sim.halo_unpack(self.hp["recv_lo"], HALO, self.recv_lo)
-        if self.hi:
-            self.sim.halo_unpack(self.hp["recv_hi"], HALO, self.recv_hi)
+        """Complete the two planes of each cut from the received records (clip_halo_unpack, one launch)."""
+        self.sim.halo_unpack(self.recv_lo, self.recv_hi, self.send_lo, self.send_hi)
         self.exchanges += 1
 
     def halo_exchange(self, group=None):
@@ -154,17 +145,33 @@ class SlabClip:
         t = self.torch
         with t.cuda.device(self.device), t.cuda.stream(self.sim.stream):
             self.pack()
+            if self.world == 1:   # a single periodic slab is its own neighbour: unpack straight from what was packed
+                if self.lo:
+                    self.sim.halo_unpack(self.send_hi, self.send_lo, self.send_lo, self.send_hi)
+                self.exchanges += 1
+                return
             exchange(self.send_lo, self.send_hi, self.recv_lo, self.recv_hi, self.rank, self.world, self.z_periodic, group)
             self.unpack()
 
     def step(self, n=1, group=None):
-        """n time steps of the global lattice: clip_step(1) on the slab, then the halo exchange, n times.
-        The first call also refreshes the ghosts of the initial state (k_init's gradient is wrong on the outermost plane)."""
+        """n time steps of the global lattice: clip_step(1) on the slab, then the halo exchange, n times; nothing here waits for
+        the GPU.  The first call also exchanges the records of the initial state."""
+        t = self.torch
         if self.exchanges == 0:
             self.halo_exchange(group)
         for _ in range(int(n)):
-            self.sim.step(1)
-            self.halo_exchange(group)
+            if self.halo is None:
+                self.sim.step(1)
+                self.halo_exchange(group)
+                continue
+            self.sim.step_halo_begin(self.send_lo, self.send_hi)      # records are produced on the halo stream ...
+            if self.world == 1:
+                self.sim.step_halo_end(self.send_hi, self.send_lo, self.send_lo, self.send_hi)
+            else:
+                with t.cuda.device(self.device), t.cuda.stream(self.halo):   # ... and travel on it while the interior computes
+                    exchange(self.send_lo, self.send_hi, self.recv_lo, self.recv_hi, self.rank, self.world, self.z_periodic, group)
+                self.sim.step_halo_end(self.recv_lo, self.recv_hi, self.send_lo, self.send_hi)
+            self.exchanges += 1
 
     def get(self):
         """phi, p [own, ny, nx] and u [3, own, ny, nx] of the OWNED planes z0 .. z1-1."""
@@ -175,7 +182,7 @@ class SlabClip:
     @property
     def halo_bytes_per_step(self):
         """Bytes this rank sends per step."""
-        return sum(b.numel() for b in (self.send_lo, self.send_hi) if b is not None)
+        return sum(b.numel() * b.element_size() for b in (self.send_lo, self.send_hi) if b is not None)
 
     def close(self):
         self.sim.close()
@@ -183,20 +190,19 @@ class SlabClip:
 
 def step_group(slabs, n=1):
     """All slabs of a lattice held by ONE process (tests; several slabs on one GPU, stepped one after the other -- no kernel waits on
-    another): step each, then hand every record to its neighbour by a device copy."""
+    another): step each, then hand every record to its neighbour (the neighbour unpacks straight from the sender's buffer)."""
     world = len(slabs)
 
     def swap():
         for s in slabs:
             s.pack()
+        s0 = slabs[0]
+        s0.torch.cuda.synchronize()   # the slabs may sit on different streams
         for s in slabs:
             below, above = neighbours(s.rank, world, s.z_periodic)
-            if below is not None:
-                s.recv_lo.copy_(slabs[below].send_hi)
-            if above is not None:
-                s.recv_hi.copy_(slabs[above].send_lo)
-        for s in slabs:
-            s.unpack()
+            s.sim.halo_unpack(slabs[below].send_hi if below is not None else None, slabs[above].send_lo if above is not None else None,
+                              s.send_lo, s.send_hi)
+            s.exchanges += 1
 
     if slabs[0].exchanges == 0:
         swap()

@@ -56,7 +56,9 @@ def test_validation_without_gpu():
         (dict(precision=16), "precision"),
         (dict(bc=(0, 1, 0, 0, 0, 0)), "PERIODIC"),
         (dict(bc=(2, 3, 0, 0, 0, 0)), "z faces"),
-        (dict(bc=(5, 5, 0, 0, 0, 0)), "unknown boundary"),
+        (dict(bc=(6, 6, 0, 0, 0, 0)), "unknown boundary"),
+        (dict(bc=(5, 5, 0, 0, 0, 0)), "HALO"),
+        (dict(bc=(0, 0, 0, 0, 5, 0)), "PERIODIC"),
         (dict(bc=(4, 0, 0, 0, 0, 0)), "PERIODIC"),
         (dict(rho_l=0.0), "densit"),
         (dict(W=0.0), "W"),
@@ -152,3 +154,18 @@ def test_reference_arm_other_ranks_do_nothing():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0"],
                          capture_output=True, text=True, timeout=120, env=env, cwd=ROOT)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_bench_gpus_n_starts_n_ranks():
+    """`python bench.py --gpus 2` with no launcher around it starts two ranks itself and defaults to the slab decomposition (the
+    path's own sharding); checked on CPU through --plumbing-only (gloo rendezvous, max-over-ranks reduction, no GPU work)."""
+    import json
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--plumbing-only"], capture_output=True, text=True,
+                         timeout=300, env=env, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    r = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert r["n_gpus"] == 2 and r["gpus_requested"] == 2 and r["decomp"] == "slab" and r["max_ms"] == 2.0 and r["max_e2e_s"] == 3.0
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--plumbing-only"], capture_output=True, text=True, timeout=120, env=env, cwd=ROOT)
+    r = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert r["n_gpus"] == 1 and r["decomp"] == "replicas"
