@@ -178,6 +178,9 @@ def run_ours(args):
         case = inputs.rayleigh_taylor(L=n // 2, precision=prec)
     elif args.workload == "jet":  # BASELINE configs[3]: liquid jet 192 x 192 x 1536, inlet disc, convective outlet, side walls
         case = inputs.jet(nxy=3 * n // 4, nz=args.nz or 6 * n, r_nozzle=12.0 * n / 256, precision=prec)
+    elif args.workload == "jetfs":  # the paper's own jet set-up: free-slip side walls (Sec. 6)
+        case = inputs.jet(nxy=3 * n // 4, nz=args.nz or 6 * n, r_nozzle=12.0 * n / 256, precision=prec)
+        case["params"]["bc"] = (inputs.FREESLIP,) * 4 + (inputs.INLET, inputs.OUTLET)
     else:
         case = inputs.sweep_drops(n=n, seed=rank_seed(rank), precision=prec)
     case["params"]["path"] = args.path
@@ -244,6 +247,7 @@ def run_ours(args):
             "vs_baseline": None, "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
             "config": {"workload": (f"BASELINE configs[2] Rayleigh-Taylor {nxl}x{nyl}x{nzl}, walls in y, fp{prec}" if args.workload == "rt" else
                                     f"BASELINE configs[3] liquid jet {nxl}x{nyl}x{nzl}, inlet disc + convective outlet + side walls, fp{prec}" if args.workload == "jet" else
+                                    f"the paper's jet set-up {nxl}x{nyl}x{nzl}: inlet disc + convective outlet + FREE-SLIP sides (PAPER.md Sec. 6), fp{prec}" if args.workload == "jetfs" else
                                     f"BASELINE configs[4] throughput sweep at {n}^3: periodic two-phase box, 20 seeded drops, "
                                     f"rho ratio 1000, fp{prec} (north_star target lattice)"),
                        "lattice": [nxl, nyl, nzl], "l2": f"state {sim.workspace_bytes / 1e9:.2f} GB >> 126 MB L2, no flush needed",
@@ -252,7 +256,7 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "effective_gbs": mlups * 1e6 * B_MIN_WORDS * word / 1e9 / world,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC.get((dom, n, prec, args.workload)), "peak_source": peak_src,
+                         "traffic": NCU_TRAFFIC.get((dom, n, prec, args.workload)) if not args.nz else None, "peak_source": peak_src,
                          "kernel": dom, "algorithmic_bytes_per_step": step_bytes,
                          "note": "achieved = 84 words/LU x nodes / (sum of the step's kernel durations, CUDA events per launch)",
                          "kernels_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
@@ -479,7 +483,7 @@ def main():
     ap.add_argument("--n", type=int, default=256)
     ap.add_argument("--precision", type=int, default=32, choices=[32, 64])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
-    ap.add_argument("--workload", default="sweep", choices=["sweep", "rt", "jet"],
+    ap.add_argument("--workload", default="sweep", choices=["sweep", "rt", "jet", "jetfs"],
                     help="sweep = BASELINE configs[4] (headline); rt = configs[2] lattice (n/2 x 2n x n/2), walls in y; jet = configs[3] lattice (3n/4 x 3n/4 x 6n)")
     ap.add_argument("--decomp", default=None, choices=["replicas", "slab"],
                     help="slab (default for N > 1): ONE lattice n x n x (n N) cut into N z slabs with a halo exchange per step -- the path's "

@@ -47,7 +47,7 @@ constexpr int B200_SMS = 148;
 FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   FusedPlan f{};
   if (p->collision != CLIP_COLL_WMRT || p->phase_only) return f;
-  for (int k = 0; k < 4; ++k) if (p->bc[k] != CLIP_BC_PERIODIC && p->bc[k] != CLIP_BC_WALL) return f;
+  for (int k = 0; k < 4; ++k) if (p->bc[k] != CLIP_BC_PERIODIC && p->bc[k] != CLIP_BC_WALL && p->bc[k] != CLIP_BC_FREESLIP) return f;
   if (p->bc[4] == CLIP_BC_FREESLIP || p->bc[5] == CLIP_BC_FREESLIP) return f;
   // an INLET / OUTLET plane is stepped by the generic kernels, the ghost plane of a HALO face not at all; k_fused covers the
   // planes [zlo, zlo + nz) in between
@@ -253,6 +253,14 @@ int check_cuda(clip_handle* h, const char* what) {
   return CLIP_OK;
 }
 
+// 0 = all faces PERIODIC (or open / HALO in z only), 1 = WALL faces, 2 = FREESLIP faces in x / y (instantiations of the pair kernels)
+int face_mode(const clip_handle* h) {
+  int m = 0;
+  for (int k = 0; k < 6; ++k) if (h->p.bc[k] == CLIP_BC_WALL) m = 1;
+  for (int k = 0; k < 4; ++k) if (h->p.bc[k] == CLIP_BC_FREESLIP) m = 2;
+  return m;
+}
+
 unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / block); }
 
 template <typename T> int do_init(clip_handle* h, const void* phi0, const void* u0) {
@@ -273,8 +281,7 @@ bool fast_ok(const clip_handle* h) {
   if (h->mode == 1) return false;
   if (h->nz > 65535 || h->ny > 65535) return false;  // grid.y / grid.z of the pair kernels
   if (h->p.collision != CLIP_COLL_WMRT || h->p.phase_only) return false;  // BGK keeps all 19 f in the collision: generic kernels only (round 1)
-  for (int k = 0; k < 4; ++k) if (h->p.bc[k] != CLIP_BC_PERIODIC && h->p.bc[k] != CLIP_BC_WALL) return false;
-  if (h->p.bc[4] == CLIP_BC_FREESLIP || h->p.bc[5] == CLIP_BC_FREESLIP) return false;  // free-slip: generic kernels only
+  if (h->p.bc[4] == CLIP_BC_FREESLIP || h->p.bc[5] == CLIP_BC_FREESLIP) return false;  // free-slip in z: generic kernels only
   // an INLET (-z) / OUTLET (+z) face is served by the generic kernels on its own plane (hybrid launches, do_step)
   return h->nx % 2 == 0 && h->nz >= 4;
 }
@@ -333,8 +340,7 @@ template <typename T> void fused_open_planes(clip_handle* h, Prof* prof) {
 // generic kernel on the planes next to an open face).
 template <typename T> void fused_prepass(clip_handle* h, Prof* prof) {
   if (h->phi_ahead) return;
-  bool walls = false;
-  for (int k = 0; k < 6; ++k) walls = walls || h->p.bc[k] == CLIP_BC_WALL;
+  const int faces = face_mode(h);
   const int glo = h->p.bc[4] == CLIP_BC_INLET ? 1 : 0, ghi = h->p.bc[5] == CLIP_BC_OUTLET ? 1 : 0;
   dim3 fg, fb;
   fast_shape(h, fg, fb);
@@ -342,7 +348,7 @@ template <typename T> void fused_prepass(clip_handle* h, Prof* prof) {
   F.k.phi = (T*)(h->ws + (h->phi_cur ? h->L.off_phi : h->L.off_phi2));
   F.k.z_lo = h->zlo + glo; F.k.z_cnt = h->zhi - ghi - F.k.z_lo; fg.z = (unsigned)F.k.z_cnt;
   if (prof) prof->begin();
-  clip::launch_phi2<T>(walls, h->nx_special, fg, fb, h->stream, F);
+  clip::launch_phi2<T>(faces, h->nx_special, fg, fb, h->stream, F);
   if (prof) prof->end(KIND_PHI2);
   h->launches += 1;
   fused_open_planes<T>(h, prof);
@@ -354,9 +360,8 @@ template <typename T> void fused_prepass(clip_handle* h, Prof* prof) {
 // chunks, which run on the handle's stream together with k_fix).
 template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullptr, bool split = false, void* d_lo = nullptr, void* d_hi = nullptr) {
   const bool fast = fast_ok(h);
-  bool walls = false;
-  for (int k = 0; k < 6; ++k) walls = walls || h->p.bc[k] == CLIP_BC_WALL;
-  const bool xwalls = h->p.bc[0] == CLIP_BC_WALL || h->p.bc[1] == CLIP_BC_WALL;
+  const int faces = face_mode(h);
+  const bool xwalls = h->p.bc[0] != CLIP_BC_PERIODIC;
   dim3 fg, fb;
   if (fast) fast_shape(h, fg, fb);
   const bool fused = use_fused(h);
@@ -394,7 +399,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
         cudaEventRecord(h->ev_start, h->stream);
         cudaStreamWaitEvent(h->halo_stream, h->ev_start, 0);
         U.c_mode = 1;
-        fe = clip::launch_fused<T>(walls, h->nx_special, dim3(fp.ytiles, 2), dim3(fp.threads), fp.smem_bytes, h->halo_stream, F, U);
+        fe = clip::launch_fused<T>(faces, h->nx_special, dim3(fp.ytiles, 2), dim3(fp.threads), fp.smem_bytes, h->halo_stream, F, U);
         cudaEventRecord(h->ev_bnd, h->halo_stream);
         if (fe == cudaSuccess) {  // the records need the new populations of the boundary planes and their neighbours only
           const cudaStream_t main_stream = h->stream;
@@ -403,13 +408,13 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
           h->cur ^= 1; h->stream = main_stream;
           if (rc != CLIP_OK) return rc;
           U.c_mode = 2;
-          fe = clip::launch_fused<T>(walls, h->nx_special, dim3(fp.ytiles, fp.nchunks - 2), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+          fe = clip::launch_fused<T>(faces, h->nx_special, dim3(fp.ytiles, fp.nchunks - 2), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
           h->launches += 1;
         }
         cudaStreamWaitEvent(h->stream, h->ev_bnd, 0);
       } else {
         U.c_mode = 0;
-        fe = clip::launch_fused<T>(walls, h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+        fe = clip::launch_fused<T>(faces, h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
       }
       if (fe != cudaSuccess) { set_err(h->err, "k_fused: %s", cudaGetErrorString(fe)); return CLIP_ECUDA; }
       if (prof) { prof->end(KIND_FUSED); prof->begin(); }
@@ -451,9 +456,9 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       }
       if (prof) prof->begin();
       if (pass == 0) {
-        clip::launch_phi2<T>(walls, h->nx_special, fg, fb, h->stream, F);
+        clip::launch_phi2<T>(faces, h->nx_special, fg, fb, h->stream, F);
       } else {
-        clip::launch_step2<T>(walls, xwalls, h->nx_special, fg, fb, h->stream, F);
+        clip::launch_step2<T>(faces, xwalls, h->nx_special, fg, fb, h->stream, F);
       }
       h->launches += 1;
       if (prof) prof->end(pass == 0 ? KIND_PHI2 : KIND_STEP2);

@@ -34,11 +34,14 @@ struct Geo {
   // walls (WALLS instantiations only): links of this pair that cross a halfway bounce-back face (B.10-B.11) ...
   bool bym, byp, bzm, bzp;  // ... towards y-1, y+1, z-1, z+1 (both nodes of the pair)
   bool bxm, bxp;            // ... towards x0-1 (node x0 only) and towards x0+2 (node x0+1 only)
+  // free-slip faces in x / y (WALLS = 3, 4 only; B.8-B.9 :1017-1026): links that are reflected specularly there
+  bool sxm, sxp, sym, syp;
   // ... and the phi ghost rule there (clamp = mirror across the wall, R9): plain offsets for the stencil rows / columns
   int cym, cyp, czm, czp, cxm, cxp;
 };
 
-// WALLS: 0 = periodic code, 1 = any wall face, 2 = wall faces in x only (blocks away from the y / z faces of a lattice walled in x)
+// WALLS: 0 = periodic code, 1 = any wall face, 2 = wall faces in x only (blocks away from the y / z faces of a lattice walled in x);
+// 3 / 4 = the same two for lattices that (also) have FREESLIP faces in x or y
 template <typename T, int WALLS = 0> __device__ __forceinline__ Geo make_geo(const KP<T>& P, int x0, int y, int z) {
   Geo g;
   const int nxy = P.nx * P.ny;
@@ -53,16 +56,28 @@ template <typename T, int WALLS = 0> __device__ __forceinline__ Geo make_geo(con
   g.xp = g.wp ? 2 - P.nx : 2;
   g.cym = g.dym; g.cyp = g.dyp; g.czm = g.dzm; g.czp = g.dzp; g.cxm = g.xm; g.cxp = g.xp;
   g.bym = g.byp = g.bzm = g.bzp = g.bxm = g.bxp = false;
-  if (WALLS) {
+  g.sxm = g.sxp = g.sym = g.syp = false;
+  if (WALLS == 1 || WALLS == 2) {
     g.bxm = g.wm && P.bc[0] != BC_PERIODIC; g.bxp = g.wp && P.bc[1] != BC_PERIODIC;
     if (WALLS == 1) {
       g.bym = (y == 0) && P.bc[2] != BC_PERIODIC; g.byp = (y == P.ny - 1) && P.bc[3] != BC_PERIODIC;
       g.bzm = (z == 0) && P.bc[4] != BC_PERIODIC; g.bzp = (z == P.nz - 1) && P.bc[5] != BC_PERIODIC;
     }
-    if (g.bxm) g.cxm = 0;
-    if (g.bxp) g.cxp = 1;
-    if (g.bym) g.cym = 0;
-    if (g.byp) g.cyp = 0;
+  }
+  if (WALLS >= 3) {
+    g.bxm = g.wm && P.bc[0] == BC_WALL; g.bxp = g.wp && P.bc[1] == BC_WALL;
+    g.sxm = g.wm && P.bc[0] == BC_FREESLIP; g.sxp = g.wp && P.bc[1] == BC_FREESLIP;
+    if (WALLS == 3) {
+      g.bym = (y == 0) && P.bc[2] == BC_WALL; g.byp = (y == P.ny - 1) && P.bc[3] == BC_WALL;
+      g.sym = (y == 0) && P.bc[2] == BC_FREESLIP; g.syp = (y == P.ny - 1) && P.bc[3] == BC_FREESLIP;
+      g.bzm = (z == 0) && P.bc[4] != BC_PERIODIC; g.bzp = (z == P.nz - 1) && P.bc[5] != BC_PERIODIC;
+    }
+  }
+  if (WALLS) {  // phi ghost = mirror value behind walls and free-slip faces alike (R9)
+    if (g.bxm || g.sxm) g.cxm = 0;
+    if (g.bxp || g.sxp) g.cxp = 1;
+    if (g.bym || g.sym) g.cym = 0;
+    if (g.byp || g.syp) g.cyp = 0;
     if (g.bzm) g.czm = 0;
     if (g.bzp) g.czp = 0;
   }
@@ -95,18 +110,31 @@ __device__ __forceinline__ P2<T> pull2(const T* __restrict__ src, int nx_rt, con
   if (a == 0) return ld_pair<T, H>(rp);
   const T* __restrict__ own = pop_row<T, 0, 0>(src, g) + (SET * Q + copp(a)) * nx;
   bool rb = false;  // the link crosses a y / z wall: both nodes of the pair take their own opposite population
-  if (WALLS == 1) rb = (cy(a) == 1 && g.bym) || (cy(a) == -1 && g.byp) || (cz(a) == 1 && g.bzm) || (cz(a) == -1 && g.bzp);
-  if (cx(a) == 0) return ld_pair<T, H>((WALLS == 1 && rb) ? own : rp);
+  if (WALLS == 1 || WALLS == 3) rb = (cy(a) == 1 && g.bym) || (cy(a) == -1 && g.byp) || (cz(a) == 1 && g.bzm) || (cz(a) == -1 && g.bzp);
+  // Free-slip (B.8-B.9, pull form, as clip::pull_reflected): a link that crosses a free-slip face was sent with that velocity
+  // component reversed by the node that has the SAME coordinate in that dimension; a wall crossing anywhere on the link wins.
+  const T* __restrict__ srx = rp;  // source of an x-reflected link: direction (-cx, cy, cz) of the same row
+  if (WALLS >= 3) {
+    srx = pop_row<T, -cy(a), -cz(a)>(src, g) + (SET * Q + dir_of(-cx(a), cy(a), cz(a))) * nx;
+    if (WALLS == 3 && cy(a) != 0) {
+      const bool ry = (cy(a) == 1 && g.sym) || (cy(a) == -1 && g.syp);
+      const T* __restrict__ r0 = pop_row<T, 0, -cz(a)>(src, g);
+      if (ry) { rp = r0 + (SET * Q + dir_of(cx(a), -cy(a), cz(a))) * nx; srx = r0 + (SET * Q + dir_of(-cx(a), -cy(a), cz(a))) * nx; }
+    }
+  }
+  if (cx(a) == 0) return ld_pair<T, H>(rb ? own : rp);
   const T* __restrict__ plo;
   const T* __restrict__ phi;
   if (cx(a) == 1) {
     plo = rp + (g.wm ? nx - 1 : -1); phi = rp;
+    if (WALLS >= 3 && g.sxm) plo = srx;
     if (WALLS && g.bxm) plo = own;
   } else {
     plo = rp + 1; phi = rp + (g.wp ? 2 - nx : 2);
+    if (WALLS >= 3 && g.sxp) phi = srx + 1;
     if (WALLS && g.bxp) phi = own + 1;
   }
-  if (WALLS == 1 && rb) { plo = own; phi = own + 1; }
+  if (rb) { plo = own; phi = own + 1; }
   return P2<T>(ld_one<T, H>(plo), ld_one<T, H>(phi));
 }
 template <typename T, int H, int NX, int SET, int WALLS, int a = 0> struct Pull2All {
@@ -383,22 +411,23 @@ __device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z
   after(geo, g);
 }
 
-template <typename T, int NX, bool WALLS> __global__ void __launch_bounds__(256) k_phi2(const __grid_constant__ FP<T> FPp) {
+// WALLS (kernel level): 0 = periodic lattice, 1 = lattice with WALL faces, 2 = lattice with FREESLIP (and maybe WALL) faces in x / y
+template <typename T, int NX, int WALLS> __global__ void __launch_bounds__(256) k_phi2(const __grid_constant__ FP<T> FPp) {
   int x0, y, z;
   if (!pair_coords(FPp.k, x0, y, z)) return;
   if (WALLS && !block_touches_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) phi_pair<T, LD_NC, NX, 0>(FPp, x0, y, z);
-  else if (WALLS && !block_touches_yz_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) phi_pair<T, LD_NC, NX, 2>(FPp, x0, y, z);
-  else phi_pair<T, LD_NC, NX, WALLS ? 1 : 0>(FPp, x0, y, z);
+  else if (WALLS && !block_touches_yz_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) phi_pair<T, LD_NC, NX, WALLS == 2 ? 4 : 2>(FPp, x0, y, z);
+  else phi_pair<T, LD_NC, NX, WALLS == 2 ? 3 : (WALLS ? 1 : 0)>(FPp, x0, y, z);
 }
 // 128-thread blocks; fp32: 3 blocks per SM (<= 168 registers: all ~100 loads of a node pair in flight at once, measured
 // faster than 4 blocks at 128 registers), fp64: what 255 registers allow.
-template <typename T, int NX, bool WALLS, int MINB>
+template <typename T, int NX, int WALLS, int MINB>
 __global__ void __launch_bounds__(128, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
   int x0, y, z;
   if (!pair_coords(FPp.k, x0, y, z)) return;
   if (WALLS && !block_touches_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) step_pair<T, LD_NC, LD_NC, ST_WB, NX, 0>(FPp, x0, y, z, NoWait());
-  else if (WALLS && !block_touches_yz_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) step_pair<T, LD_NC, LD_NC, ST_WB, NX, 2>(FPp, x0, y, z, NoWait());
-  else step_pair<T, LD_NC, LD_NC, ST_WB, NX, WALLS ? 1 : 0>(FPp, x0, y, z, NoWait());
+  else if (WALLS && !block_touches_yz_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) step_pair<T, LD_NC, LD_NC, ST_WB, NX, WALLS == 2 ? 4 : 2>(FPp, x0, y, z, NoWait());
+  else step_pair<T, LD_NC, LD_NC, ST_WB, NX, WALLS == 2 ? 3 : (WALLS ? 1 : 0)>(FPp, x0, y, z, NoWait());
 }
 
 }  // namespace clip

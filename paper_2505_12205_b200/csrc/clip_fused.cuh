@@ -47,7 +47,10 @@ template <typename T> __device__ __forceinline__ T shfl_dn1(T v) { return __shfl
 // Accumulation of one source row into the ring.  Column-private shared memory: acc[(slot * rows + j) * nx + x0 .. +1].
 // The nine contributions are formed in registers first; the shared-memory read-modify-writes are then issued as one
 // batch of loads followed by one batch of stores (the rows are distinct, which the compiler cannot know).
-// WALLS: 0 = periodic code, 1 = any wall face next to the row, 2 = wall faces in x only (as in clip_fast.cuh)
+// WALLS: 0 = periodic code, 1 = any wall face next to the row, 2 = wall faces in x only, 3 / 4 = the same two on lattices that
+// (also) have FREESLIP faces in x / y (as in clip_fast.cuh).  Where a population lands (which direction it then has does not
+// matter for phi = sum_a g_a): a link that crosses a WALL face returns to the sender (B.10-B.11); a link that crosses a free-slip
+// face keeps its tangential displacement and drops the normal one (B.8-B.9 :1017-1026); a wall crossing anywhere wins.
 template <typename T, int WALLS> struct Scatter {
   typedef P2<T> V;
   T* ring;     // ring base
@@ -56,47 +59,64 @@ template <typename T, int WALLS> struct Scatter {
   int nx, rows, nwarps, warp, lane;
   int sm, sc, sp;  // ring slots of the planes z-1, z, z+1
   int j;           // ring row of the source row (ly + 1)
+  static constexpr bool YZ = WALLS == 1 || WALLS == 3;   // y / z faces next to the row
+  static constexpr bool FS = WALLS >= 3;
 
-  template <int dz> __device__ __forceinline__ int slot() const { return dz < 0 ? sm : (dz > 0 ? sp : sc); }
+  struct Tri { V v0, vp, vm; };  // what one source pair sends to a target row with e_x = 0, +1, -1
   template <int dy, int dz> __device__ __forceinline__ bool behind_wall(const Geo& geo) const {
     // the row (dy, dz) lies behind a wall: everything returns to the sender (B.10-B.11)
-    return WALLS == 1 && ((dy > 0 && geo.byp) || (dy < 0 && geo.bym) || (dz > 0 && geo.bzp) || (dz < 0 && geo.bzm));
+    return YZ && ((dy > 0 && geo.byp) || (dy < 0 && geo.bym) || (dz > 0 && geo.bzp) || (dz < 0 && geo.bzm));
   }
-  // target row (dy, dz) with the three directions a0 (e_x = 0), ap (e_x = +1), am (e_x = -1): c = what lands in this
-  // thread's columns, ep / em = what lane 31 / lane 0 sends across the warp edge; bounced links go to `own`
-  template <int dy, int dz, int a0, int ap, int am>
-  __device__ __forceinline__ void xrow(const Geo& geo, const V (&g)[Q], V& own, V& c, T& ep, T& em) const {
-    V v0 = g[a0], vp = g[ap], vm = g[am];
-    if (WALLS) {
-      if (behind_wall<dy, dz>(geo)) { own = own + ((v0 + vp) + vm); v0 = V(T(0)); vp = V(T(0)); vm = V(T(0)); }
-      else {  // x walls: node x0+1 sending +x through the +x face / node x0 sending -x through the -x face
-        if (geo.bxp) { own = own + V(T(0), vp.hi()); vp = V(vp.lo(), T(0)); }
-        if (geo.bxm) { own = own + V(vm.lo(), T(0)); vm = V(T(0), vm.hi()); }
-      }
+  template <int dy> __device__ __forceinline__ bool behind_slip(const Geo& geo) const {
+    return WALLS == 3 && ((dy > 0 && geo.syp) || (dy < 0 && geo.sym));
+  }
+  template <int dy, int dz, int a0, int ap, int am> __device__ __forceinline__ Tri take(const Geo& geo, const V (&g)[Q], V& own) const {
+    Tri t; t.v0 = g[a0]; t.vp = g[ap]; t.vm = g[am];
+    if (behind_wall<dy, dz>(geo)) { own = own + ((t.v0 + t.vp) + t.vm); t.v0 = V(T(0)); t.vp = V(T(0)); t.vm = V(T(0)); }
+    return t;
+  }
+  // the diagonal rows (dy, dz = +-1) carry one direction each; behind a free-slip y face it lands in the row (0, dz)
+  template <int dy, int dz, int a0> __device__ __forceinline__ V take_diag(const Geo& geo, const V (&g)[Q], V& own, Tri& row0dz) const {
+    V c = g[a0];
+    if (behind_wall<dy, dz>(geo)) { own = own + c; c = V(T(0)); }
+    else if (behind_slip<dy>(geo)) { row0dz.v0 = row0dz.v0 + c; c = V(T(0)); }
+    return c;
+  }
+  // x faces, then the three directions of a target row are combined: c = what lands in this thread's columns, ep / em = what
+  // lane 31 / lane 0 sends across the warp edge
+  __device__ __forceinline__ void finish(const Geo& geo, Tri t, V& own, V& c, T& ep, T& em) const {
+    if (WALLS) {  // node x0+1 sending +x through the +x face / node x0 sending -x through the -x face
+      if (geo.bxp) { own = own + V(T(0), t.vp.hi()); t.vp = V(t.vp.lo(), T(0)); }
+      if (geo.bxm) { own = own + V(t.vm.lo(), T(0)); t.vm = V(T(0), t.vm.hi()); }
+      if (FS && geo.sxp) { t.v0 = t.v0 + V(T(0), t.vp.hi()); t.vp = V(t.vp.lo(), T(0)); }
+      if (FS && geo.sxm) { t.v0 = t.v0 + V(t.vm.lo(), T(0)); t.vm = V(T(0), t.vm.hi()); }
     }
-    T up = shfl_up1(vp.hi()), dn = shfl_dn1(vm.lo());  // executed by every lane (wall rows are uniform over the block)
+    T up = shfl_up1(t.vp.hi()), dn = shfl_dn1(t.vm.lo());  // executed by every lane (wall rows are uniform over the block)
     if (lane == 0) up = T(0);
     if (lane == 31) dn = T(0);
-    c = (v0 + V(up, vp.lo())) + V(vm.hi(), dn);
-    ep = vp.hi(); em = vm.lo();
-  }
-  template <int dy, int dz, int a0> __device__ __forceinline__ void diag(const Geo& geo, const V (&g)[Q], V& own, V& c) const {
-    c = g[a0];
-    if (WALLS && behind_wall<dy, dz>(geo)) { own = own + c; c = V(T(0)); }
+    c = (t.v0 + V(up, t.vp.lo())) + V(t.vm.hi(), dn);
+    ep = t.vp.hi(); em = t.vm.lo();
   }
   __device__ __forceinline__ void operator()(const Geo& geo, const V (&g)[Q]) const {
     typedef typename PairOf<T>::type U;
     V own(T(0)), c[9];
     T ep[5], em[5];
-    xrow<1, 0, 3, 7, 10>(geo, g, own, c[0], ep[0], em[0]);
-    xrow<-1, 0, 4, 9, 8>(geo, g, own, c[1], ep[1], em[1]);
-    xrow<0, 1, 5, 11, 14>(geo, g, own, c[2], ep[2], em[2]);
-    xrow<0, -1, 6, 13, 12>(geo, g, own, c[3], ep[3], em[3]);
-    diag<1, 1, 15>(geo, g, own, c[5]);
-    diag<-1, -1, 16>(geo, g, own, c[6]);
-    diag<1, -1, 17>(geo, g, own, c[7]);
-    diag<-1, 1, 18>(geo, g, own, c[8]);
-    xrow<0, 0, 0, 1, 2>(geo, g, own, c[4], ep[4], em[4]);  // own row last: with walls it also collects what bounced back
+    Tri yp = take<1, 0, 3, 7, 10>(geo, g, own), ym = take<-1, 0, 4, 9, 8>(geo, g, own);
+    Tri zp = take<0, 1, 5, 11, 14>(geo, g, own), zm = take<0, -1, 6, 13, 12>(geo, g, own);
+    Tri me = take<0, 0, 0, 1, 2>(geo, g, own);
+    c[5] = take_diag<1, 1, 15>(geo, g, own, zp);
+    c[6] = take_diag<-1, -1, 16>(geo, g, own, zm);
+    c[7] = take_diag<1, -1, 17>(geo, g, own, zm);
+    c[8] = take_diag<-1, 1, 18>(geo, g, own, zp);
+    if (WALLS == 3) {  // the in-plane rows behind a free-slip y face land in the sender's own row, x displacement kept
+      if (geo.syp) { me.v0 = me.v0 + yp.v0; me.vp = me.vp + yp.vp; me.vm = me.vm + yp.vm; yp.v0 = V(T(0)); yp.vp = V(T(0)); yp.vm = V(T(0)); }
+      if (geo.sym) { me.v0 = me.v0 + ym.v0; me.vp = me.vp + ym.vp; me.vm = me.vm + ym.vm; ym.v0 = V(T(0)); ym.vp = V(T(0)); ym.vm = V(T(0)); }
+    }
+    finish(geo, yp, own, c[0], ep[0], em[0]);
+    finish(geo, ym, own, c[1], ep[1], em[1]);
+    finish(geo, zp, own, c[2], ep[2], em[2]);
+    finish(geo, zm, own, c[3], ep[3], em[3]);
+    finish(geo, me, own, c[4], ep[4], em[4]);  // own row last: with walls it also collects what bounced back
     c[4] = c[4] + own;
     const int r[9] = {sc * rows + j + 1, sc * rows + j - 1, sp * rows + j, sm * rows + j, sc * rows + j,
                       sp * rows + j + 1, sm * rows + j - 1, sm * rows + j + 1, sp * rows + j - 1};
@@ -138,7 +158,8 @@ __device__ __forceinline__ void flush_slot(T* ring, T* edge_p, T* edge_m, int nx
 }
 
 // grid = (ytiles, nchunks); block = nx/2 threads (nx % 64 == 0); dynamic shared memory = ring + edges.
-template <typename T, int NX, bool WALLS, int MAXT, int MINB>
+// WALLS (kernel level): 0 = periodic lattice, 1 = lattice with WALL faces, 2 = lattice with FREESLIP (and maybe WALL) faces in x / y
+template <typename T, int NX, int WALLS, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP<T> FPp, const FusedP<T> U) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const KP<T>& P = FPp.k;
@@ -157,7 +178,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP
   for (int i = threadIdx.x; i < nslots * rows * (nx + 2 * nwarps); i += blockDim.x) ring[i] = T(0);
   __syncthreads();
   T* const slab = U.part + (long long)(c * U.ytiles + iy) * U.tile_stride;
-  Scatter<T, WALLS ? 1 : 0> sc;
+  Scatter<T, WALLS == 2 ? 3 : (WALLS ? 1 : 0)> sc;
   sc.ring = ring; sc.edge_p = edge_p; sc.edge_m = edge_m; sc.nx = nx; sc.rows = rows; sc.nwarps = nwarps; sc.warp = warp; sc.lane = lane;
   // flush of plane k (-1 .. tz) of the tile, held in ring slot (k + 1) % slots
   auto flush = [&](int k) {
@@ -191,12 +212,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP
                         (z == 0 && P.bc[4] != BC_PERIODIC) || (z == P.nz - 1 && P.bc[5] != BC_PERIODIC);
         wall_row = yz ? 1 : ((P.bc[0] != BC_PERIODIC || P.bc[1] != BC_PERIODIC) ? 2 : 0);
         if (wall_row == 1) {
-          step_pair<T, LD_NC, LD_NC, ST_WB, NX, 1>(FPp, x0, y, z, NoWait(), sc);
+          step_pair<T, LD_NC, LD_NC, ST_WB, NX, WALLS == 2 ? 3 : 1>(FPp, x0, y, z, NoWait(), sc);
         } else if (wall_row == 2) {
-          Scatter<T, 2> sx;
+          Scatter<T, WALLS == 2 ? 4 : 2> sx;
           sx.ring = ring; sx.edge_p = edge_p; sx.edge_m = edge_m; sx.nx = nx; sx.rows = rows; sx.nwarps = nwarps; sx.warp = warp; sx.lane = lane;
           sx.sm = sc.sm; sx.sc = sc.sc; sx.sp = sc.sp; sx.j = sc.j;
-          step_pair<T, LD_NC, LD_NC, ST_WB, NX, 2>(FPp, x0, y, z, NoWait(), sx);
+          step_pair<T, LD_NC, LD_NC, ST_WB, NX, WALLS == 2 ? 4 : 2>(FPp, x0, y, z, NoWait(), sx);
         }
       }
       if (wall_row == 0) {

@@ -15,11 +15,12 @@ constexpr int fused_threads_per_sm(int precision, int block_threads) {
 }
 
 
-// walls: the lattice has WALL faces (WALLS instantiation); xwalls: it has them in x (k_step2 then keeps 16 warps per SM)
-template <typename T> void launch_phi2(bool walls, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F);
-template <typename T> void launch_step2(bool walls, bool xwalls, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F);
+// faces: 0 = all PERIODIC, 1 = the lattice has WALL faces, 2 = it has FREESLIP faces in x / y (and maybe walls); xwalls: non-periodic
+// faces in x (k_step2 then keeps 16 warps per SM)
+template <typename T> void launch_phi2(int faces, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F);
+template <typename T> void launch_step2(int faces, bool xwalls, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F);
 // returns the CUDA error of the shared-memory opt-in (cudaFuncSetAttribute, once per device and instantiation) or of nothing
-template <typename T> cudaError_t launch_fused(bool walls, int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
+template <typename T> cudaError_t launch_fused(int faces, int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
 template <typename T> void launch_fix(dim3 g, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
 
 }  // namespace clip

@@ -9,7 +9,7 @@
 
 namespace clip {
 
-template <typename T, bool W> void launch_phi2_w(int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F) {
+template <typename T, int W> void launch_phi2_w(int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F) {
   switch (nx) {
 #define X(N) case N: k_phi2<T, N, W><<<g, b, 0, st>>>(F); break;
     CLIP_NX_LIST(X)
@@ -17,7 +17,7 @@ template <typename T, bool W> void launch_phi2_w(int nx, dim3 g, dim3 b, cudaStr
     default: k_phi2<T, 0, W><<<g, b, 0, st>>>(F);
   }
 }
-template <typename T, bool W, int MB> void launch_step2_w(int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F) {
+template <typename T, int W, int MB> void launch_step2_w(int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F) {
   switch (nx) {
 #define X(N) case N: k_step2<T, N, W, MB><<<g, b, 0, st>>>(F); break;
     CLIP_NX_LIST(X)
@@ -33,7 +33,7 @@ template <> struct StepMinBlocksXWalls<double> { static constexpr int value = 1;
 // The opt-in to > 48 KB of dynamic shared memory is a per-DEVICE attribute of the kernel: set it once per device and
 // instantiation (a process may drive several GPUs), and report its error.
 constexpr int MAX_DEVICES = 64;
-template <typename T, int NX, bool W> cudaError_t launch_fused_nx(dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
+template <typename T, int NX, int W> cudaError_t launch_fused_nx(dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
   constexpr int MAXT = NX ? NX / 2 : 256;
   constexpr int TPSM = fused_threads_per_sm(sizeof(T) == 4 ? 32 : 64, MAXT);
   constexpr int MINB = TPSM / MAXT > 0 ? TPSM / MAXT : 1;
@@ -50,7 +50,7 @@ template <typename T, int NX, bool W> cudaError_t launch_fused_nx(dim3 g, dim3 b
   kern<<<g, b, smem, st>>>(F, U);
   return cudaSuccess;
 }
-template <typename T, bool W> cudaError_t launch_fused_w(int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
+template <typename T, int W> cudaError_t launch_fused_w(int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
   switch (nx) {
 #define X(N) case N: return launch_fused_nx<T, N, W>(g, b, smem, st, F, U);
     CLIP_NX_LIST(X)
@@ -60,18 +60,27 @@ template <typename T, bool W> cudaError_t launch_fused_w(int nx, dim3 g, dim3 b,
 }
 
 
-template <typename T> void launch_phi2(bool walls, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F) {
-  if (walls) launch_phi2_w<T, true>(nx, g, b, st, F);
-  else launch_phi2_w<T, false>(nx, g, b, st, F);
+// Lattices with FREESLIP faces in x / y (faces = 2): their own instantiations only for the runtime-nx form and nx = 192 (the
+// paper's jet has free-slip side walls); other widths take the runtime-nx kernel.
+template <typename T> void launch_phi2(int faces, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F) {
+  if (faces == 2) {
+    if (nx == 192) k_phi2<T, 192, 2><<<g, b, 0, st>>>(F);
+    else k_phi2<T, 0, 2><<<g, b, 0, st>>>(F);
+  } else if (faces) launch_phi2_w<T, 1>(nx, g, b, st, F);
+  else launch_phi2_w<T, 0>(nx, g, b, st, F);
 }
-template <typename T> void launch_step2(bool walls, bool xwalls, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F) {
-  // walls in x: most blocks run the branchy wall code, which wants warps more than registers (jet lattice: +6 %)
-  if (walls && xwalls) launch_step2_w<T, true, StepMinBlocksXWalls<T>::value>(nx, g, b, st, F);
-  else if (walls) launch_step2_w<T, true, StepMinBlocks<T>::value>(nx, g, b, st, F);
-  else launch_step2_w<T, false, StepMinBlocks<T>::value>(nx, g, b, st, F);
+template <typename T> void launch_step2(int faces, bool xwalls, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F) {
+  // walls in x: most blocks run the wall code, which wants warps more than registers (jet lattice: +6 %)
+  if (faces == 2) {
+    if (nx == 192) k_step2<T, 192, 2, StepMinBlocksXWalls<T>::value><<<g, b, 0, st>>>(F);
+    else k_step2<T, 0, 2, StepMinBlocksXWalls<T>::value><<<g, b, 0, st>>>(F);
+  } else if (faces && xwalls) launch_step2_w<T, 1, StepMinBlocksXWalls<T>::value>(nx, g, b, st, F);
+  else if (faces) launch_step2_w<T, 1, StepMinBlocks<T>::value>(nx, g, b, st, F);
+  else launch_step2_w<T, 0, StepMinBlocks<T>::value>(nx, g, b, st, F);
 }
-template <typename T> cudaError_t launch_fused(bool walls, int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
-  return walls ? launch_fused_w<T, true>(nx, g, b, smem, st, F, U) : launch_fused_w<T, false>(nx, g, b, smem, st, F, U);
+template <typename T> cudaError_t launch_fused(int faces, int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
+  if (faces == 2) return nx == 192 ? launch_fused_nx<T, 192, 2>(g, b, smem, st, F, U) : launch_fused_nx<T, 0, 2>(g, b, smem, st, F, U);  // as launch_step2
+  return faces ? launch_fused_w<T, 1>(nx, g, b, smem, st, F, U) : launch_fused_w<T, 0>(nx, g, b, smem, st, F, U);
 }
 template <typename T> void launch_fix(dim3 g, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
   k_fix<T><<<g, FIX_THREADS, 0, st>>>(F, U);

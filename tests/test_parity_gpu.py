@@ -83,6 +83,10 @@ CASES = {
     "freeslip_mixed": (lambda: _with(inputs.walled_box(nx=14, ny=12, nz=10), bc=(inputs.FREESLIP, inputs.WALL, inputs.WALL, inputs.FREESLIP, inputs.FREESLIP, inputs.FREESLIP)), 100),
     "freeslip_channel": (lambda: _with(inputs.rayleigh_taylor(L=16, W=3.0), bc=(inputs.PERIODIC, inputs.PERIODIC, inputs.FREESLIP, inputs.FREESLIP, inputs.PERIODIC, inputs.PERIODIC)), 100),
     "jet_freeslip_sides": (lambda: _with(inputs.jet(nxy=24, nz=48, r_nozzle=4.0), bc=(inputs.FREESLIP,) * 4 + (inputs.INLET, inputs.OUTLET)), 100),
+    # free-slip in x / y on the pair kernels (pull2 selects the reflected source): with walls in z, with a wall sharing an edge,
+    # periodic z
+    "freeslip_xy_zwall": (lambda: _with(inputs.walled_box(nx=14, ny=12, nz=10), bc=(inputs.FREESLIP, inputs.WALL, inputs.WALL, inputs.FREESLIP, inputs.WALL, inputs.WALL)), 100),
+    "freeslip_xy_periodic_z": (lambda: _with(inputs.walled_box(nx=16, ny=8, nz=12), bc=(inputs.FREESLIP,) * 4 + (inputs.PERIODIC,) * 2), 100),
     "sweep64_linear_mu": (lambda: _with(inputs.sweep_drops(n=64), visc_interp=2, tau_l=0.3), 100),   # fused-free fast path
     "rt_replica_linear_mu": (lambda: _with(inputs.rayleigh_taylor(L=16, W=3.0), visc_interp=2), 100),
     "jet_replica_uave": (lambda: _with(inputs.jet(nxy=24, nz=48, r_nozzle=4.0), outlet_u_mode=1), 150),   # B.22 U_ave
@@ -338,12 +342,43 @@ def test_jet_lattice_width_against_the_oracle(over, precision):
             assert err <= (FP32_PHI if name == "phi" else FP32_U) * np.abs(b).max(), (name, err, ran)
 
 
+def test_jet_with_free_slip_sides_at_its_own_width():
+    """The paper's jet set-up proper (free-slip side walls, Sec. 6) at nx = ny = 192 -- the free-slip
+    instantiation of the pair kernels -- directly against the oracle: 192 x 192 x 24, 16 steps, fp64 and fp32."""
+    import torch
+    from paper_2505_12205_b200 import clip
+    case = inputs.jet(nxy=192, nz=24, r_nozzle=12.0)
+    case["params"]["bc"] = (inputs.FREESLIP,) * 4 + (inputs.INLET, inputs.OUTLET)
+    steps = 16
+    ref = _oracle(case, steps)
+    for precision in (64, 32):
+        sim = clip.Clip.from_case(case, precision=precision)
+        sim.step(steps)
+        got = [t.double().cpu().numpy() for t in sim.get()]
+        ran = {k for k, v in sim.step_profiled(1).items() if v[1]}
+        torch.cuda.synchronize()
+        sim.close()
+        assert "k_step2" in ran or "k_fused" in ran, ran      # not the generic kernels
+        for name, a, b in zip(("phi", "p", "u"), got, ref):
+            err = np.abs(a - b).max()
+            if precision == 64:
+                assert err <= FP64_ABS, (name, err)
+            elif name != "p":
+                assert err <= (FP32_PHI if name == "phi" else FP32_U) * np.abs(b).max(), (name, err)
+
+
 FUSED_LATTICES = {
     "periodic_128x24x20": lambda: inputs.sweep_drops(shape=(128, 24, 20), ndrops=6, rmin=3, rmax=6),
     "periodic_64x4x5": lambda: inputs.sweep_drops(shape=(64, 4, 5), ndrops=2, rmin=2, rmax=3),      # one y tile: the halo wraps onto the tile itself
     "walled_64x12x9": lambda: inputs.walled_box(nx=64, ny=12, nz=9),
     "walled_128x8x17": lambda: inputs.walled_box(nx=128, ny=8, nz=17),
     "rt_64": lambda: inputs.rayleigh_taylor(L=64, W=3.0),                                       # y walls, x / z periodic
+    # free-slip faces in x / y: the scatter drops the normal displacement and keeps the tangential one
+    "freeslip_xy_64x12x9": lambda: _with(inputs.walled_box(nx=64, ny=12, nz=9), bc=(inputs.FREESLIP,) * 4 + (inputs.WALL, inputs.WALL)),
+    "freeslip_mixed_64x8x10": lambda: _with(inputs.walled_box(nx=64, ny=8, nz=10), bc=(inputs.FREESLIP, inputs.WALL, inputs.WALL, inputs.FREESLIP, inputs.PERIODIC, inputs.PERIODIC)),
+    "freeslip_192x8x6": lambda: _with(inputs.walled_box(nx=192, ny=8, nz=6), bc=(inputs.FREESLIP,) * 4 + (inputs.PERIODIC, inputs.PERIODIC)),
+    "jet_freeslip_64x64x24": lambda: _with(inputs.jet(nxy=64, nz=24, r_nozzle=6.0), bc=(inputs.FREESLIP,) * 4 + (inputs.INLET, inputs.OUTLET)),
+    "jet_64x64x24": lambda: inputs.jet(nxy=64, nz=24, r_nozzle=6.0),
 }
 
 
@@ -421,8 +456,12 @@ def test_fused_path_time_semantics():
 def test_walled_fast_paths(precision):
     """Walls in the pair-per-thread kernels (bounce-back of either node of a pair in x, of both in y / z, edges and
     corners, clamped phi ghosts): close to the generic thread-per-node kernels."""
+    FS, WL, PE = inputs.FREESLIP, inputs.WALL, inputs.PERIODIC
     for case in (inputs.walled_box(), inputs.rayleigh_taylor(L=16, W=3.0), inputs.poiseuille(nx=4, ny=32, nz=4),
-                 inputs.jet(nxy=24, nz=32, r_nozzle=4.0)):  # jet: inlet / outlet planes by the generic kernels (hybrid)
+                 inputs.jet(nxy=24, nz=32, r_nozzle=4.0),   # jet: inlet / outlet planes by the generic kernels (hybrid)
+                 _with(inputs.jet(nxy=24, nz=32, r_nozzle=4.0), bc=(FS,) * 4 + (inputs.INLET, inputs.OUTLET)),   # the paper's jet: free-slip sides
+                 _with(inputs.walled_box(nx=64, ny=12, nz=9), bc=(FS, WL, WL, FS, WL, WL)),
+                 _with(inputs.walled_box(nx=192, ny=8, nz=6), bc=(FS, FS, FS, FS, PE, PE))):   # nx = 192: its own free-slip instantiation
         a = _gpu_p(case, 40, precision, path=1)
         b = _gpu_p(case, 40, precision, path=2)
         tol = 1e-12 if precision == 64 else 5e-5
