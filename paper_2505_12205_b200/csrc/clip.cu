@@ -280,7 +280,8 @@ const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step
 bool fast_ok(const clip_handle* h) {
   if (h->mode == 1) return false;
   if (h->nz > 65535 || h->ny > 65535) return false;  // grid.y / grid.z of the pair kernels
-  if (h->p.collision != CLIP_COLL_WMRT || h->p.phase_only) return false;  // BGK keeps all 19 f in the collision: generic kernels only (round 1)
+  if (h->p.phase_only) return false;
+  if (h->p.collision != CLIP_COLL_WMRT && face_mode(h) == 2) return false;  // BGK with free-slip faces: generic kernels
   if (h->p.bc[4] == CLIP_BC_FREESLIP || h->p.bc[5] == CLIP_BC_FREESLIP) return false;  // free-slip in z: generic kernels only
   // an INLET (-z) / OUTLET (+z) face is served by the generic kernels on its own plane (hybrid launches, do_step)
   return h->nx % 2 == 0 && h->nz >= 4;

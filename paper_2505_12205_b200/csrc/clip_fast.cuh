@@ -236,7 +236,8 @@ template <typename T> __device__ __forceinline__ Mom2<T> moments2(const P2<T> (&
 }
 
 // Total force (Eq. 20) and D = dev(Pi^neq); same closed forms as clip::total_force.
-template <typename T>
+// BGK: the trace of Pi^neq relaxes at s_nu too (Eq. 29); WMRT: at rate 1 (Eq. 30)
+template <typename T, bool BGK = false>
 __device__ __forceinline__ void total_force2(const KP<T>& P, const Mom2<T>& m, const Mat2<T>& mat, P2<T> ux, P2<T> uy,
                                              P2<T> uz, const P2<T> (&G)[3], P2<T> (&F)[3], P2<T> (&D)[6]) {
   typedef P2<T> V;
@@ -246,7 +247,8 @@ __device__ __forceinline__ void total_force2(const KP<T>& P, const Mom2<T>& m, c
   const V tr3 = ((nxx + nyy) + nzz) * V(T(1.0 / 3.0));
   D[0] = nxx - tr3; D[1] = nyy - tr3; D[2] = nzz - tr3; D[3] = nxy; D[4] = nyz; D[5] = nxz;
   const V s = mat.s_nu;
-  const V Sxx = fma2(s, D[0], tr3), Syy = fma2(s, D[1], tr3), Szz = fma2(s, D[2], tr3);
+  const V trs = BGK ? s * tr3 : tr3;
+  const V Sxx = fma2(s, D[0], trs), Syy = fma2(s, D[1], trs), Szz = fma2(s, D[2], trs);
   const V Sxy = s * D[3], Syz = s * D[4], Sxz = s * D[5];
   const V cmu = -(mat.tau * V(P.drho));
   const V cs = mat.mu - p3 * V(P.drho);
@@ -269,6 +271,14 @@ struct Coll2 {
     f[a] = w * (A + ev);
     f[a + 1] = w * (A - ev);
   }
+  // BGK, Eq. 26: f+ = (1 - s) f + s feq_bar + F_a = (1 - s) f + w [s (p* + Gamma'/w) +- e.(3 s u + (2 - s) 1.5 F/rho)];
+  // here k = s_nu, c0 = -1.5 u.u, om1 = 1 - s_nu
+  template <int a> __device__ __forceinline__ void pair_f_bgk(V eu, V eb, V (&f)[Q]) const {
+    const V w(cw<T>(a));
+    const V A = k * (p + q(eu));
+    f[a] = fma2(om1, f[a], w * (A + eb));
+    f[a + 1] = fma2(om1, f[a + 1], w * (A - eb));
+  }
   template <int a> __device__ __forceinline__ void pair_g(V eu, V em, V (&g)[Q]) const {
     const V w(cw<T>(a));
     const V C = fma2(omphi, q(eu), omphi);
@@ -281,12 +291,12 @@ template <typename T> struct GCtx { Coll2<T> c; P2<T> ux, uy, uz, mx, my, mz, us
 
 // f collision (Alg. 1) of a node pair: f+ out (a function of the moments only, because the 14 non-shear moments relax at
 // rate 1, G2); fills the context of the g collision.
-template <typename T>
+template <typename T, bool BGK = false>
 __device__ __forceinline__ void collide2_f(const KP<T>& P, const Mom2<T>& m, const Mat2<T>& mat, P2<T> phi, const P2<T> (&G)[3],
                                            P2<T> ux, P2<T> uy, P2<T> uz, P2<T> (&f)[Q], GCtx<T>& x) {
   typedef P2<T> V;
   V F[3], D[6];
-  total_force2(P, m, mat, ux, uy, uz, G, F, D);
+  total_force2<T, BGK>(P, m, mat, ux, uy, uz, G, F, D);
   const V usq15 = V(T(1.5)) * fma2(ux, ux, fma2(uy, uy, uz * uz));
   const V ir15 = V(T(1.5)) * mat.inv_rho;
   // v = 3u + 1.5 F/rho
@@ -302,6 +312,23 @@ __device__ __forceinline__ void collide2_f(const KP<T>& P, const Mom2<T>& m, con
   const V o3 = V(T(3)) * c.omphi;
   x.mx = fma2(o3, ux, cn * G[0]); x.my = fma2(o3, uy, cn * G[1]); x.mz = fma2(o3, uz, cn * G[2]);
   x.ux = ux; x.uy = uy; x.uz = uz; x.usq15 = usq15;
+  if (BGK) {  // f is relaxed, not replaced: all 19 pre-collision values are still needed here
+    Coll2<T> b;
+    b.p = m.p; b.c0 = -usq15; b.k = mat.s_nu; b.om1 = V(T(1)) - mat.s_nu;
+    const V s3 = V(T(3)) * mat.s_nu, s2 = V(T(2)) - mat.s_nu;
+    const V bx = fma2(s3, ux, s2 * (F[0] * ir15)), by = fma2(s3, uy, s2 * (F[1] * ir15)), bz = fma2(s3, uz, s2 * (F[2] * ir15));
+    f[0] = fma2(b.om1, f[0], V(cw<T>(0)) * (mat.s_nu * (m.p - usq15)));
+    b.template pair_f_bgk<1>(ux, bx, f);
+    b.template pair_f_bgk<3>(uy, by, f);
+    b.template pair_f_bgk<5>(uz, bz, f);
+    b.template pair_f_bgk<7>(ux + uy, bx + by, f);
+    b.template pair_f_bgk<9>(ux - uy, bx - by, f);
+    b.template pair_f_bgk<11>(ux + uz, bx + bz, f);
+    b.template pair_f_bgk<13>(ux - uz, bx - bz, f);
+    b.template pair_f_bgk<15>(uy + uz, by + bz, f);
+    b.template pair_f_bgk<17>(uy - uz, by - bz, f);
+    return;
+  }
   f[0] = V(cw<T>(0)) * (m.p - usq15);
   const V Dxy2 = D[3] + D[3], Dyz2 = D[4] + D[4], Dxz2 = D[5] + D[5];
   const V sxy = D[0] + D[1], sxz = D[0] + D[2], syz = D[1] + D[2];
@@ -380,7 +407,7 @@ template <typename T, int HG, int NX, int WALLS> __device__ __forceinline__ void
 // macros and f+ are computed and stored.
 struct NoWait { __device__ __forceinline__ void operator()() const {} };
 struct NoAfter { template <typename T> __device__ __forceinline__ void operator()(const Geo&, const P2<T> (&)[Q]) const {} };
-template <typename T, int HL, int HP, int HS, int NX, int WALLS, typename W, typename A = NoAfter>
+template <typename T, int HL, int HP, int HS, int NX, int WALLS, typename W, typename A = NoAfter, bool BGK = false>
 __device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z, W before_phi, A after = A()) {
   typedef P2<T> V;
   const KP<T>& P = FPp.k;
@@ -397,13 +424,13 @@ __device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z
   const Mat2<T> mat = materials2<T>(P, phi, L);
   {  // macros, Alg. 3: F from (new p*, new phi, lagged u, R13), then Eq. 31b
     V F[3], D[6];
-    total_force2(P, m, mat, ux, uy, uz, G, F, D);
+    total_force2<T, BGK>(P, m, mat, ux, uy, uz, G, F, D);
     const V h = V(T(0.5)) * mat.inv_rho;
     ux = fma2(h, F[0], m.mx); uy = fma2(h, F[1], m.my); uz = fma2(h, F[2], m.mz);
   }
   st_pair<T, HS>(P.u + geo.rc, ux); st_pair<T, HS>(P.u + P.n + geo.rc, uy); st_pair<T, HS>(P.u + 2 * P.n + geo.rc, uz);
   GCtx<T> gx;
-  collide2_f<T>(P, m, mat, phi, G, ux, uy, uz, f, gx);
+  collide2_f<T, BGK>(P, m, mat, phi, G, ux, uy, uz, f, gx);
   T* const rd = const_cast<T*>(pop_row<T, 0, 0>(P.p_dst, geo));
   Store2All<T, HS, NX, 0>::run(rd, P.nx, f);
   collide2_g<T>(gx, g);
@@ -421,6 +448,14 @@ template <typename T, int NX, int WALLS> __global__ void __launch_bounds__(256) 
 }
 // 128-thread blocks; fp32: 3 blocks per SM (<= 168 registers: all ~100 loads of a node pair in flight at once, measured
 // faster than 4 blocks at 128 registers), fp64: what 255 registers allow.
+// BGK collision (Eq. 26, 29) on the pair kernels: runtime-nx form, periodic / walled lattices (the generic kernels take the rest)
+template <typename T, int WALLS, int MINB>
+__global__ void __launch_bounds__(128, MINB) k_step2_bgk(const __grid_constant__ FP<T> FPp) {
+  int x0, y, z;
+  if (!pair_coords(FPp.k, x0, y, z)) return;
+  if (WALLS && !block_touches_wall(FPp.k, y - threadIdx.y, blockDim.y, z)) step_pair<T, LD_NC, LD_NC, ST_WB, 0, 0, NoWait, NoAfter, true>(FPp, x0, y, z, NoWait());
+  else step_pair<T, LD_NC, LD_NC, ST_WB, 0, WALLS ? 1 : 0, NoWait, NoAfter, true>(FPp, x0, y, z, NoWait());
+}
 template <typename T, int NX, int WALLS, int MINB>
 __global__ void __launch_bounds__(128, MINB) k_step2(const __grid_constant__ FP<T> FPp) {
   int x0, y, z;

@@ -27,6 +27,8 @@ template <typename T, int W, int MB> void launch_step2_w(int nx, dim3 g, dim3 b,
 }
 template <typename T> struct StepMinBlocks { static constexpr int value = 3; };  // k_step2 (128-thread blocks)
 template <> struct StepMinBlocks<double> { static constexpr int value = 1; };
+template <typename T> struct StepMinBlocksBgk { static constexpr int value = 2; };  // all 19 f stay live: 255 registers
+template <> struct StepMinBlocksBgk<double> { static constexpr int value = 1; };
 template <typename T> struct StepMinBlocksXWalls { static constexpr int value = 4; };  // 128 registers, 16 warps
 template <> struct StepMinBlocksXWalls<double> { static constexpr int value = 1; };
 
@@ -70,6 +72,11 @@ template <typename T> void launch_phi2(int faces, int nx, dim3 g, dim3 b, cudaSt
   else launch_phi2_w<T, 0>(nx, g, b, st, F);
 }
 template <typename T> void launch_step2(int faces, bool xwalls, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F) {
+  if (F.k.collision == 1) {  // BGK: runtime-nx kernels (clip.cu admits it on periodic / walled lattices only)
+    if (faces) k_step2_bgk<T, 1, StepMinBlocksBgk<T>::value><<<g, b, 0, st>>>(F);
+    else k_step2_bgk<T, 0, StepMinBlocksBgk<T>::value><<<g, b, 0, st>>>(F);
+    return;
+  }
   // walls in x: most blocks run the wall code, which wants warps more than registers (jet lattice: +6 %)
   if (faces == 2) {
     if (nx == 192) k_step2<T, 192, 2, StepMinBlocksXWalls<T>::value><<<g, b, 0, st>>>(F);

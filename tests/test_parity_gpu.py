@@ -342,6 +342,28 @@ def test_jet_lattice_width_against_the_oracle(over, precision):
             assert err <= (FP32_PHI if name == "phi" else FP32_U) * np.abs(b).max(), (name, err, ran)
 
 
+@pytest.mark.parametrize("precision", [64, 32])
+def test_bgk_runs_on_the_pair_kernels(precision):
+    """BGK collision (Eq. 26, 29) on the pair kernels (k_step2_bgk keeps all 19 f through the collision): the
+    automatic path of a periodic and of a walled lattice is k_phi2 + k_step2, and agrees with the generic kernels to round-off (both
+    are tied to the oracle by test_parity[drop32_bgk / jet_replica_bgk])."""
+    import torch
+    from paper_2505_12205_b200 import clip
+    for case in (_with(inputs.sweep_drops(shape=(64, 16, 12), ndrops=4, rmin=3, rmax=5), collision=1, tau_l=0.3),
+                 _with(inputs.walled_box(nx=24, ny=10, nz=8), collision=1)):
+        a = _gpu_p(case, 40, precision, path=1)
+        sim = clip.Clip.from_case(case, precision=precision)
+        sim.step(40)
+        b = [t.double().cpu().numpy() for t in sim.get()]
+        ran = {k for k, v in sim.step_profiled(1).items() if v[1]}
+        torch.cuda.synchronize()
+        sim.close()
+        assert "k_step2" in ran and "k_step" not in ran, ran
+        tol = 1e-12 if precision == 64 else 5e-5
+        for x, y in zip(a, b):
+            assert np.abs(x - y).max() <= tol * max(1.0, np.abs(x).max()), case["name"]
+
+
 def test_jet_with_free_slip_sides_at_its_own_width():
     """The paper's jet set-up proper (free-slip side walls, Sec. 6) at nx = ny = 192 -- the free-slip
     instantiation of the pair kernels -- directly against the oracle: 192 x 192 x 24, 16 steps, fp64 and fp32."""
