@@ -7,6 +7,8 @@
  * shares no code, header, table or constant generator with the CUDA path (paper_2505_12205_b200/csrc).
  *
  * Build:  gcc -O3 -ffp-contract=off -shared -fPIC -o libclip_oracle.so clip_oracle.c -lm
+ *         gcc ... -DCLIPO_D2Q9 -o libclip_oracle_d2q9.so clip_oracle.c -lm     (the 2-D lattice of the paper's 2-D benchmarks,
+ *         same equations, D2Q9 velocities and weights, nz = 1, faces PERIODIC / WALL / FREESLIP in x and y)
  *
  * Storage follows the paper as written: populations f[index][a], g[index][a] (Alg. 1-3),
  * index = x + nx*(y + ny*z) (Fig. 4b), two full population buffers (the in-place Alg. 2 is a data
@@ -23,14 +25,32 @@
 #include <stdlib.h>
 #include <string.h>
 
+#ifdef CLIPO_D2Q9
+#define Q 9
+#else
 #define Q 19
+#endif
 enum { BC_PERIODIC = 0, BC_WALL = 1, BC_INLET = 2, BC_OUTLET = 3, BC_FREESLIP = 4 };
 
+#ifdef CLIPO_D2Q9
+/* D2Q9 (Fig. B.24 :969): rest, 4 axis and 4 diagonal velocities, weights 4/9, 1/9, 1/36; opposite pairs adjacent.
+ * The ordering is immaterial [G1] (the 2-D inlet of :1044 is not built). */
+static const int EX[Q] = {0, 1, -1, 0, 0, 1, -1, 1, -1};
+static const int EY[Q] = {0, 0, 0, 1, -1, 1, -1, -1, 1};
+static const int EZ[Q] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+static double weight_of(int a) { return a == 0 ? 4.0 / 9.0 : (a < 5 ? 1.0 / 9.0 : 1.0 / 36.0); }
+#define SHEAR_LO 3 /* rows of the traceless second-order moments in the basis below: e_x e_y, e_x^2 - e_y^2 */
+#define SHEAR_HI 4
+#else
 /* D3Q19 velocities, Eq. 14, in the ordering consistent with the inlet set {1,7,9,11,13} being
  * the +x-pointing directions [G1]; opposite pairs adjacent. */
 static const int EX[Q] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
 static const int EY[Q] = {0, 0, 0, 1, -1, 0, 0, 1, -1, -1, 1, 0, 0, 0, 0, 1, -1, 1, -1};
 static const int EZ[Q] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, -1, -1, 1, 1, -1, -1, 1};
+static double weight_of(int a) { return a == 0 ? 1.0 / 3.0 : (a < 7 ? 1.0 / 18.0 : 1.0 / 36.0); } /* Eq. 15 */
+#define SHEAR_LO 4 /* rows of the 5 traceless second-order moments in the basis below */
+#define SHEAR_HI 8
+#endif
 static int opp(int a) { return a == 0 ? 0 : ((a & 1) ? a + 1 : a - 1); }
 
 typedef struct clipo_params {
@@ -76,6 +96,12 @@ static void build_basis(clipo *h) {
   double poly[Q][Q];
   for (int a = 0; a < Q; ++a) {
     double x = EX[a], y = EY[a], z = EZ[a], e2 = x * x + y * y + z * z;
+#ifdef CLIPO_D2Q9
+    (void)z; /* 9 polynomials of rank 9 on D2Q9; rows 3, 4 = the traceless second-order moments [G2 in two dimensions] */
+    poly[0][a] = 1.0; poly[1][a] = x; poly[2][a] = y;
+    poly[3][a] = x * y; poly[4][a] = x * x - y * y;
+    poly[5][a] = e2; poly[6][a] = x * e2; poly[7][a] = y * e2; poly[8][a] = e2 * e2;
+#else
     poly[0][a] = 1.0;
     poly[1][a] = x; poly[2][a] = y; poly[3][a] = z;
     poly[4][a] = x * y; poly[5][a] = y * z; poly[6][a] = x * z;          /* the 5 traceless 2nd-order moments */
@@ -85,6 +111,7 @@ static void build_basis(clipo *h) {
     poly[11][a] = x * e2; poly[12][a] = y * e2; poly[13][a] = z * e2;
     poly[14][a] = (x * x - y * y) * e2; poly[15][a] = (x * x + y * y - 2.0 * z * z) * e2;
     poly[16][a] = x * (y * y - z * z); poly[17][a] = y * (z * z - x * x); poly[18][a] = z * (x * x - y * y);
+#endif
   }
   for (int k = 0; k < Q; ++k) {
     double v[Q];
@@ -106,8 +133,8 @@ static void build_basis(clipo *h) {
 }
 
 /* S-hat of Eq. 28 read as: rate s_nu on the 5 traceless second-order moments (rows 4..8), rate 1
- * on the other 14 [G2]. */
-static double S_of(int k, double s_nu) { return (k >= 4 && k <= 8) ? s_nu : 1.0; }
+ * on the others [G2] (D2Q9: the 2 traceless second-order moments, the other 7 at rate 1). */
+static double S_of(int k, double s_nu) { return (k >= SHEAR_LO && k <= SHEAR_HI) ? s_nu : 1.0; }
 
 /* Collision operator applied to r = f - feq_bar (or f - feq in the viscous force):
  * WMRT: M^-1 S M r (Eq. 27);  BGK: r / (tau + 1/2) (Eq. 26; the same factor multiplies the stress in Eq. 29). */
@@ -323,9 +350,13 @@ static void macros(clipo *h) {
 /* ---------------------------------------------------------------- C ABI ---------------------------------- */
 clipo *clipo_create(int nx, int ny, int nz, const clipo_params *p) {
   if (nx < 1 || ny < 1 || nz < 1 || !p) return NULL;
+#ifdef CLIPO_D2Q9
+  if (nz != 1 || p->bc[4] != BC_PERIODIC || p->bc[5] != BC_PERIODIC) return NULL; /* 2-D: one plane, nothing happens in z */
+  for (int k = 0; k < 4; ++k) if (p->bc[k] == BC_INLET || p->bc[k] == BC_OUTLET) return NULL;
+#endif
   clipo *h = (clipo *)calloc(1, sizeof(clipo));
   h->nx = nx; h->ny = ny; h->nz = nz; h->n = (size_t)nx * ny * nz; h->p = *p;
-  for (int a = 0; a < Q; ++a) h->w[a] = a == 0 ? 1.0 / 3.0 : (a < 7 ? 1.0 / 18.0 : 1.0 / 36.0); /* Eq. 15 */
+  for (int a = 0; a < Q; ++a) h->w[a] = weight_of(a);
   build_basis(h);
   size_t nq = h->n * Q;
   h->f = calloc(nq, 8); h->g = calloc(nq, 8); h->f2 = calloc(nq, 8); h->g2 = calloc(nq, 8);
@@ -527,3 +558,4 @@ void clipo_total_force(const clipo *h, const double *f, double pstar, const doub
   total_force(h, f, pstar, u[0], u[1], u[2], phi, G, L, F);
 }
 long clipo_time(const clipo *h) { return h->t; }
+int clipo_q(void) { return Q; }

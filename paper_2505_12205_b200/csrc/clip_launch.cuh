@@ -9,7 +9,8 @@ namespace clip {
 
 // Resident threads per SM the k_fused instantiations are compiled for (__launch_bounds__): fp32 384 (<= 168 registers;
 // 12 warps with every load of a row in flight beat 16 warps at 128 registers, measured 17.3 vs 16.8 GLUPS at 256^3),
-// except 256-thread blocks (nx = 512 and the runtime-nx form), which keep 2 blocks; fp64 256 (255 registers).
+// re-measured in round 2 after the branch-free pull: 17.75 vs 16.81), except 256-thread blocks (nx = 512 and the runtime-nx form),
+// which keep 2 blocks, and 96-thread blocks (nx = 192: 5 blocks = 15 warps at 128 registers: the jet lattice); fp64 256 (255 registers).
 constexpr int fused_threads_per_sm(int precision, int block_threads) {
   return precision == 32 ? (block_threads >= 256 ? 512 : (block_threads == 96 ? 480 : 384)) : 256;
 }

@@ -11,7 +11,8 @@ Layout everywhere: phi0[z, y, x] (x fastest), u0[c, z, y, x].  Node j sits at co
 Parameter dictionary keys (both the oracle binding and the CUDA binding marshal these into their own structs):
   precision (32|64), rho_h, rho_l, tau_h, tau_l, sigma, W, M, g (3), rho_ref, bc (6: -x,+x,-y,+y,-z,+z),
   inlet_u (3), inlet_phi, inlet_c (2), inlet_r, outlet_u_mode, visc_interp, collision (0 WMRT, 1 BGK), phase_only (1: prescribed u),
-  outlet_clamp (0: lambda of B.25 as printed; 1: max(0, lambda)), outlet_u_time (0: stored u(t); 1: post-stream moment at t+dt)
+  outlet_clamp (0: lambda of B.25 as printed; 1: max(0, lambda)), outlet_u_time (0: stored u(t); 1: post-stream moment at t+dt),
+  lattice (0: D3Q19, 1: D2Q9)
 """
 from __future__ import annotations
 
@@ -32,6 +33,7 @@ def default_params(**kw) -> dict:
         inlet_c=(0.0, 0.0), inlet_r=0.0,
         outlet_u_mode=0, visc_interp=0, collision=0, phase_only=0,
         outlet_clamp=0, outlet_u_time=0,
+        lattice=0,  # 0 = D3Q19; 1 = D2Q9 (nz = 1, z faces PERIODIC): the lattice of the paper's 2-D benchmarks
         path=0, tile_ty=0, tile_chunks=0, runtime_nx=0,  # libclip only: kernel path / tiling (include/clip.h); the oracle ignores them
     )
     p.update(kw)
@@ -185,3 +187,31 @@ def walled_box(nx=12, ny=10, nz=14, seed=7, precision=64):
     p = default_params(precision=precision, rho_h=1.0, rho_l=0.1, tau_h=0.6, tau_l=0.3, sigma=0.005, W=3.0,
                        M=0.05, g=(0.0, 0.0, -1.0e-5), bc=(WALL,) * 6)
     return _case(nx, ny, nz, p, phi0, u0, f"walled{nx}x{ny}x{nz}")
+
+
+# ---- two-dimensional cases on the D2Q9 lattice ("For 2D problems, the D2Q9 lattice model is utilized"): nz = 1
+def drop2d(n=64, R=16.0, W=4.0, sigma=0.01, rho_ratio=1000.0, tau=0.8, M=0.1, precision=64):
+    """Stationary 2-D drop (a cylinder) in a periodic square: the 2-D Laplace law dp = sigma / R (Eq. 44 as printed)."""
+    x, y, z = _grid(n, n, 1)
+    c = 0.5 * (n - 1)
+    r = np.sqrt((x - c) ** 2 + (y - c) ** 2)
+    phi0 = 0.5 + 0.5 * np.tanh(2.0 * (R - r) / W)
+    p = default_params(precision=precision, rho_h=1.0, rho_l=1.0 / rho_ratio, tau_h=tau, tau_l=tau, sigma=sigma, W=W, M=M, lattice=1)
+    return _case(n, n, 1, p, phi0, np.zeros((3, 1, n, n)), f"drop2d_{n}")
+
+
+def poiseuille2d(nx=4, ny=64, **kw):
+    """The paper's own layered Poiseuille set-up (Sec. 5.3: 2-D, 64 nodes across) on D2Q9; arguments as poiseuille()."""
+    case = poiseuille(nx=nx, ny=ny, nz=1, **kw)
+    case["params"]["lattice"] = 1
+    case["name"] = f"poiseuille2d_{nx}x{ny}"
+    return case
+
+
+def sweep2d(nx=128, ny=96, seed=2505, ndrops=8, rmin=5.0, rmax=12.0, W=4.0, u_amp=0.01, precision=32, bc=(PERIODIC,) * 6):
+    """2-D analogue of configs[4]: seeded discs in a box, i.i.d. uniform in-plane u0 (u_z = 0), density ratio 1000, D2Q9."""
+    case = sweep_drops(shape=(nx, ny, 1), seed=seed, ndrops=ndrops, rmin=rmin, rmax=rmax, W=W, u_amp=u_amp, precision=precision)
+    case["u0"][2] = 0.0
+    case["params"].update(lattice=1, bc=tuple(bc))
+    case["name"] = f"sweep2d_{nx}x{ny}"
+    return case
