@@ -181,6 +181,8 @@ def run_ours(args):
     elif args.workload == "jetfs":  # the paper's own jet set-up: free-slip side walls (Sec. 6)
         case = inputs.jet(nxy=3 * n // 4, nz=args.nz or 6 * n, r_nozzle=12.0 * n / 256, precision=prec)
         case["params"]["bc"] = (inputs.FREESLIP,) * 4 + (inputs.INLET, inputs.OUTLET)
+    elif args.workload == "d2q9":  # 2-D lattice 16 n x 16 n on D2Q9 (Table 2 :561 times a 256 x 64 D2Q9 case)
+        case = inputs.sweep2d(nx=16 * n, ny=16 * n, seed=rank_seed(rank), ndrops=20 * n // 16, rmin=6.0, rmax=20.0, precision=prec)
     else:
         case = inputs.sweep_drops(n=n, seed=rank_seed(rank), precision=prec)
     case["params"]["path"] = args.path
@@ -239,7 +241,8 @@ def run_ours(args):
         peak, peak_src = measured_peak()
         mlups = whole_job_mlups(nodes, args.steps, ms, world)
         e2e_mlups = world * nodes * args.steps / e2e_s / 1e6
-        step_bytes = B_MIN_WORDS * word * nodes
+        b_min = 42 if args.workload == "d2q9" else B_MIN_WORDS   # D2Q9: f 9R+9W, g 9R+9W, phi 1R+1W, u 2R+2W
+        step_bytes = b_min * word * nodes
         achieved = step_bytes / (step_ms_prof * 1e-3) / 1e9
         line = {
             "metric": "MLUPS", "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
@@ -247,6 +250,7 @@ def run_ours(args):
             "vs_baseline": None, "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
             "config": {"workload": (f"BASELINE configs[2] Rayleigh-Taylor {nxl}x{nyl}x{nzl}, walls in y, fp{prec}" if args.workload == "rt" else
                                     f"BASELINE configs[3] liquid jet {nxl}x{nyl}x{nzl}, inlet disc + convective outlet + side walls, fp{prec}" if args.workload == "jet" else
+                                    f"2-D periodic two-phase lattice {nxl}x{nyl} on D2Q9 (PAPER.md:568), seeded discs, rho ratio 1000, fp{prec}; B_min = 42 words/LU" if args.workload == "d2q9" else
                                     f"the paper's jet set-up {nxl}x{nyl}x{nzl}: inlet disc + convective outlet + FREE-SLIP sides (PAPER.md Sec. 6), fp{prec}" if args.workload == "jetfs" else
                                     f"BASELINE configs[4] throughput sweep at {n}^3: periodic two-phase box, 20 seeded drops, "
                                     f"rho ratio 1000, fp{prec} (north_star target lattice)"),
@@ -254,11 +258,11 @@ def run_ours(args):
                        "parallelism": "independent replica per GPU" if world > 1 else "single GPU",
                        "finite_after_run": finite},
             "gpu_launches": int(launches),
-            "effective_gbs": mlups * 1e6 * B_MIN_WORDS * word / 1e9 / world,
+            "effective_gbs": mlups * 1e6 * b_min * word / 1e9 / world,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": NCU_TRAFFIC.get((dom, n, prec, args.workload)) if not args.nz else None, "peak_source": peak_src,
                          "kernel": dom, "algorithmic_bytes_per_step": step_bytes,
-                         "note": "achieved = 84 words/LU x nodes / (sum of the step's kernel durations, CUDA events per launch)",
+                         "note": f"achieved = {b_min} words/LU x nodes / (sum of the step's kernel durations, CUDA events per launch)",
                          "kernels_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
                          "frac_of_nominal_8TBs": achieved / 8000.0},
             "e2e": {"value": e2e_mlups, "unit": "MLUPS", "h2d_bytes_per_step": h2d / args.steps,
@@ -483,7 +487,7 @@ def main():
     ap.add_argument("--n", type=int, default=256)
     ap.add_argument("--precision", type=int, default=32, choices=[32, 64])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
-    ap.add_argument("--workload", default="sweep", choices=["sweep", "rt", "jet", "jetfs"],
+    ap.add_argument("--workload", default="sweep", choices=["sweep", "rt", "jet", "jetfs", "d2q9"],
                     help="sweep = BASELINE configs[4] (headline); rt = configs[2] lattice (n/2 x 2n x n/2), walls in y; jet = configs[3] lattice (3n/4 x 3n/4 x 6n)")
     ap.add_argument("--decomp", default=None, choices=["replicas", "slab"],
                     help="slab (default for N > 1): ONE lattice n x n x (n N) cut into N z slabs with a halo exchange per step -- the path's "

@@ -76,6 +76,9 @@ typedef struct clip_params {
   int tile_ty, tile_chunks; /* k_fused tiling (tests / tuning; 0 = automatic): lattice rows per tile (4, 8 or 16, must divide ny) and
                               number of equal chunks along z (1 .. min(nz, 256)); they enter clip_workspace_bytes */
   int runtime_nx;          /* 1 = take the runtime-nx instantiation of the pair kernels even where nx has its own (tests) */
+  int lattice;             /* velocity set: 0 (default) = D3Q19, Eq. 14-15 (:169-176); 1 = D2Q9, the lattice of the paper's 2-D benchmarks
+                              (:568): nz must be 1, the z faces PERIODIC, the x / y faces PERIODIC, WALL or FREESLIP; u_z is returned as
+                              given to clip_init (0).  Thread-per-node kernels (k_phi9 + k_step9) */
 } clip_params;
 
 typedef struct clip_handle clip_t;

@@ -4,6 +4,7 @@
 #include "clip_kernels.cuh"
 #include "clip_fast.cuh"
 #include "clip_fused.cuh"
+#include "clip_d2q9.cuh"
 #include "clip_launch.cuh"
 
 #include <cmath>
@@ -46,7 +47,7 @@ constexpr int B200_SMS = 148;
 
 FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   FusedPlan f{};
-  if (p->collision != CLIP_COLL_WMRT || p->phase_only) return f;
+  if (p->collision != CLIP_COLL_WMRT || p->phase_only || p->lattice != 0) return f;
   for (int k = 0; k < 4; ++k) if (p->bc[k] != CLIP_BC_PERIODIC && p->bc[k] != CLIP_BC_WALL && p->bc[k] != CLIP_BC_FREESLIP) return f;
   if (p->bc[4] == CLIP_BC_FREESLIP || p->bc[5] == CLIP_BC_FREESLIP) return f;
   // an INLET / OUTLET plane is stepped by the generic kernels, the ghost plane of a HALO face not at all; k_fused covers the
@@ -123,7 +124,8 @@ Layout make_layout(int nx, int ny, int nz, const clip_params* p) {
   const size_t n = (size_t)nx * ny * nz, nxy = (size_t)nx * ny;
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t r = o; o += align_up(bytes); return r; };
-  L.off_p[0] = take(38 * n * L.word); L.off_p[1] = take(38 * n * L.word);
+  const size_t npop = p->lattice == 1 ? 18 : 38;  // f and g of D2Q9 / D3Q19
+  L.off_p[0] = take(npop * n * L.word); L.off_p[1] = take(npop * n * L.word);
   L.off_phi = take(n * L.word);
   L.off_u = take(3 * n * L.word);
   const bool outlet = p->bc[5] == CLIP_BC_OUTLET, inlet = p->bc[4] == CLIP_BC_INLET;
@@ -176,6 +178,12 @@ const char* validate(int nx, int ny, int nz, const clip_params* p) {
   if (p->tile_ty != 0 && p->tile_ty != 4 && p->tile_ty != 8 && p->tile_ty != 16) return "tile_ty must be 0 (automatic), 4, 8 or 16";
   if (p->tile_chunks < 0) return "tile_chunks must be >= 0";
   if (p->runtime_nx != 0 && p->runtime_nx != 1) return "runtime_nx must be 0 or 1";
+  if (p->lattice != 0 && p->lattice != 1) return "lattice must be 0 (D3Q19) or 1 (D2Q9)";
+  if (p->lattice == 1) {
+    if (nz != 1 || p->bc[4] != CLIP_BC_PERIODIC || p->bc[5] != CLIP_BC_PERIODIC) return "D2Q9 needs nz = 1 and PERIODIC z faces";
+    for (int k = 0; k < 4; ++k)
+      if (p->bc[k] != CLIP_BC_PERIODIC && p->bc[k] != CLIP_BC_WALL && p->bc[k] != CLIP_BC_FREESLIP) return "D2Q9 takes PERIODIC, WALL or FREESLIP faces in x and y";
+  }
   return nullptr;
 }
 
@@ -267,7 +275,8 @@ template <typename T> int do_init(clip_handle* h, const void* phi0, const void* 
   h->phi_cur = 0; h->phi_ahead = false; h->phi_partial[0] = h->phi_partial[1] = false;
   h->cur = 1;  // k_init writes into "dst"; flip afterwards so that it becomes the current state
   clip::KP<T> P = make_kp<T>(h);
-  clip::k_init<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P, (const T*)phi0, (const T*)u0);
+  if (h->p.lattice == 1) clip::d2q9::k_init9<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P, (const T*)phi0, (const T*)u0);
+  else clip::k_init<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P, (const T*)phi0, (const T*)u0);
   h->launches += 1;
   h->cur = 0;
   return check_cuda(h, "k_init");
@@ -278,7 +287,7 @@ const char* const KIND_NAMES[KIND_COUNT] = {"k_phi", "k_step", "k_phi2", "k_step
 
 // The pair-per-thread fast kernels (clip_fast.cuh) cover planes whose neighbourhood has only PERIODIC or WALL faces, even nx.
 bool fast_ok(const clip_handle* h) {
-  if (h->mode == 1) return false;
+  if (h->mode == 1 || h->p.lattice != 0) return false;
   if (h->nz > 65535 || h->ny > 65535) return false;  // grid.y / grid.z of the pair kernels
   if (h->p.phase_only) return false;
   if (h->p.collision != CLIP_COLL_WMRT && face_mode(h) == 2) return false;  // BGK with free-slip faces: generic kernels
@@ -440,7 +449,10 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
     for (int pass = 0; pass < 2; ++pass) {  // pass 0: phi(t+1); pass 1: macros + collisions
       if (!fast) {
         if (prof) prof->begin();
-        if (pass == 0) clip::k_phi<T><<<grid_for(P.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(P);
+        if (h->p.lattice == 1) {  // D2Q9 (clip_d2q9.cuh)
+          if (pass == 0) clip::d2q9::k_phi9<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
+          else clip::d2q9::k_step9<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
+        } else if (pass == 0) clip::k_phi<T><<<grid_for(P.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(P);
         else clip::k_step<T><<<grid_for(P.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(P);
         h->launches += 1;
         if (prof) prof->end(pass == 0 ? KIND_PHI : KIND_STEP);
@@ -472,7 +484,8 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
 
 template <typename T> int do_get(clip_handle* h, void* phi, void* p, void* u) {
   clip::KP<T> P = make_kp<T>(h);
-  clip::k_get<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P, (T*)phi, (T*)p, (T*)u);
+  if (h->p.lattice == 1) clip::d2q9::k_get9<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P, (T*)phi, (T*)p, (T*)u);
+  else clip::k_get<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P, (T*)phi, (T*)p, (T*)u);
   h->launches += 1;
   return check_cuda(h, "k_get");
 }

@@ -1,0 +1,217 @@
+// clip_d2q9.cuh -- the same time step on the D2Q9 lattice, the lattice of the paper's 2-D benchmarks ("For 2D
+// problems, the D2Q9 lattice model is utilized"; capillary wave :570-596, layered Poiseuille :647-669, interface in shear flow
+// :675-713; Table 2 :561 times a 256 x 64 D2Q9 case).  Equations, readings and the lean arithmetic are those of clip_kernels.cuh with
+// the two-dimensional velocity set: weights 4/9, 1/9, 1/36, c_s^2 = 1/3, and the TWO traceless second-order moments
+// {e_x e_y, e_x^2 - e_y^2} relaxing at s_nu (G2 in two dimensions), so that
+//   M^-1 S M = I - (1 - s_nu) P,  P_ab = w_a / (2 c_s^4) Q_a : dev2(Q_b),  dev2 = traceless part of a 2 x 2 tensor
+//   f+_a = w_a [p* + 3 e.u + 4.5 (e.u)^2 - 1.5 u.u + 1.5 e.F / rho + 4.5 (1 - s_nu) e^T D e],  D = dev2(Pi^neq)
+//   F_mu = -tau (rho_h - rho_l) [s_nu D + tr(Pi^neq)/2 I] . grad phi   (BGK: s_nu on the trace as well, Eq. 29)
+// Thread per node, scalar, two kernels per step (k_phi9: phi(t+1) = sum_a g_a after streaming; k_step9: the rest), the design "D0"
+// of DESIGN.md: 2-D lattices are small, the 3-D lattices carry the throughput work.  Faces: PERIODIC, WALL (halfway bounce-back),
+// FREESLIP in x and y; nz = 1.  State: pop [ny][18][nx] (A/B), phi [ny][nx], u [3][ny][nx] (u_z == 0, never touched by a step).
+#pragma once
+#include "clip_kernels.cuh"
+
+namespace clip {
+namespace d2q9 {
+
+constexpr int Q9 = 9;
+constexpr int NC9 = 2 * Q9;
+// rest; (+-1, 0); (0, +-1); (1,1), (-1,-1); (1,-1), (-1,1): opposite directions adjacent (a odd -> a + 1)
+__host__ __device__ constexpr int ex(int a) { return (a == 1 || a == 5 || a == 7) ? 1 : ((a == 2 || a == 6 || a == 8) ? -1 : 0); }
+__host__ __device__ constexpr int ey(int a) { return (a == 3 || a == 5 || a == 8) ? 1 : ((a == 4 || a == 6 || a == 7) ? -1 : 0); }
+__host__ __device__ constexpr int opp9(int a) { return a == 0 ? 0 : ((a & 1) ? a + 1 : a - 1); }
+template <typename T> __host__ __device__ constexpr T w9(int a) { return a == 0 ? T(4.0 / 9.0) : (a < 5 ? T(1.0 / 9.0) : T(1.0 / 36.0)); }
+__host__ __device__ constexpr int dir9(int x, int y) {
+  for (int a = 0; a < Q9; ++a) if (ex(a) == x && ey(a) == y) return a;
+  return 0;
+}
+
+__device__ __forceinline__ long long pidx(int nx, int y, int c, int x) { return ((long long)y * NC9 + c) * nx + x; }
+
+// Streaming (pull; Alg. 2, B.3-B.6) of direction a of set `set` (0: f, 1: g) at node (x, y): periodic wrap, halfway bounce-back
+// (B.10-B.11; a wall crossing wins at corners, R11), specular reflection at free-slip faces (B.8-B.9, pull form).
+template <typename T, int a> __device__ __forceinline__ T pull9(const KP<T>& P, int set, int x, int y) {
+  const T* __restrict__ src = P.p_src;
+  if (a == 0) return __ldg(src + pidx(P.nx, y, set * Q9, x));
+  int sx = x - ex(a), sy = y - ey(a), fx = ex(a), fy = ey(a);
+  bool bounce = false;
+  if (ex(a) != 0 && (sx < 0 || sx >= P.nx)) {
+    const int bc = P.bc[sx < 0 ? 0 : 1];
+    if (bc == BC_PERIODIC) sx = sx < 0 ? P.nx - 1 : 0;
+    else if (bc == BC_FREESLIP) { sx = x; fx = -fx; }
+    else bounce = true;
+  }
+  if (ey(a) != 0 && (sy < 0 || sy >= P.ny)) {
+    const int bc = P.bc[sy < 0 ? 2 : 3];
+    if (bc == BC_PERIODIC) sy = sy < 0 ? P.ny - 1 : 0;
+    else if (bc == BC_FREESLIP) { sy = y; fy = -fy; }
+    else bounce = true;
+  }
+  if (bounce) return __ldg(src + pidx(P.nx, y, set * Q9 + opp9(a), x));
+  const int as = (fx == ex(a) && fy == ey(a)) ? a : dir9(fx, fy);
+  return __ldg(src + pidx(P.nx, sy, set * Q9 + as, sx));
+}
+template <typename T, int a = 0> struct Pull9 {
+  static __device__ __forceinline__ void run(const KP<T>& P, int set, int x, int y, T (&v)[Q9]) {
+    v[a] = pull9<T, a>(P, set, x, y);
+    Pull9<T, a + 1>::run(P, set, x, y, v);
+  }
+};
+template <typename T> struct Pull9<T, Q9> { static __device__ __forceinline__ void run(const KP<T>&, int, int, int, T (&)[Q9]) {} };
+
+// Eq. 40a/b with the D2Q9 weights on differences d_a = phi(x + e_a) - phi(x); ghost rule: wrap or clamp (R9)
+template <typename T> __device__ __forceinline__ void stencil9(const KP<T>& P, const T* __restrict__ phi, int x, int y, T pc, T (&G)[3], T& L) {
+  const int xm = x > 0 ? x - 1 : (P.bc[0] == BC_PERIODIC ? P.nx - 1 : 0), xp = x < P.nx - 1 ? x + 1 : (P.bc[1] == BC_PERIODIC ? 0 : P.nx - 1);
+  const int ym = y > 0 ? y - 1 : (P.bc[2] == BC_PERIODIC ? P.ny - 1 : 0), yp = y < P.ny - 1 ? y + 1 : (P.bc[3] == BC_PERIODIC ? 0 : P.ny - 1);
+  const T* __restrict__ r0 = phi + (long long)y * P.nx;
+  const T* __restrict__ rm = phi + (long long)ym * P.nx;
+  const T* __restrict__ rp = phi + (long long)yp * P.nx;
+  const T d1 = r0[xp] - pc, d2 = r0[xm] - pc, d3 = rp[x] - pc, d4 = rm[x] - pc;
+  const T d5 = rp[xp] - pc, d6 = rm[xm] - pc, d7 = rm[xp] - pc, d8 = rp[xm] - pc;
+  L = T(6) * (T(1.0 / 9.0) * ((d1 + d2) + (d3 + d4)) + T(1.0 / 36.0) * ((d5 + d6) + (d7 + d8)));
+  G[0] = T(3) * (T(1.0 / 9.0) * (d1 - d2) + T(1.0 / 36.0) * ((d5 - d6) + (d7 - d8)));
+  G[1] = T(3) * (T(1.0 / 9.0) * (d3 - d4) + T(1.0 / 36.0) * ((d5 - d6) - (d7 - d8)));
+  G[2] = T(0);
+}
+
+template <typename T> struct Mom9 { T p, mx, my, xx, yy, xy; };
+template <typename T> __device__ __forceinline__ Mom9<T> moments9(const T (&f)[Q9]) {
+  Mom9<T> m;
+  const T s12 = f[1] + f[2], s34 = f[3] + f[4], s56 = f[5] + f[6], s78 = f[7] + f[8];
+  const T d12 = f[1] - f[2], d34 = f[3] - f[4], d56 = f[5] - f[6], d78 = f[7] - f[8];
+  m.p = (f[0] + (s12 + s34)) + (s56 + s78);
+  m.mx = d12 + (d56 + d78);
+  m.my = d34 + (d56 - d78);
+  m.xx = s12 + (s56 + s78);
+  m.yy = s34 + (s56 + s78);
+  m.xy = s56 - s78;
+  return m;
+}
+// Total force (Eq. 20) and D = dev2(Pi^neq) = (Dxx, Dxy), Dyy = -Dxx
+template <typename T>
+__device__ __forceinline__ void force9(const KP<T>& P, const Mom9<T>& m, const Mat<T>& mat, T ux, T uy, const T (&G)[3], T (&F)[2], T (&D)[2]) {
+  const T p3 = m.p * T(1.0 / 3.0);
+  const T nxx = m.xx - (p3 + ux * ux), nyy = m.yy - (p3 + uy * uy), nxy = m.xy - ux * uy;
+  const T tr2 = T(0.5) * (nxx + nyy);
+  D[0] = nxx - tr2; D[1] = nxy;
+  const T s = mat.s_nu;
+  const T trs = P.collision == 1 ? s * tr2 : tr2;   // BGK relaxes the trace at s_nu too (Eq. 29); WMRT at rate 1 (Eq. 30)
+  const T Sxx = s * D[0] + trs, Syy = trs - s * D[0], Sxy = s * D[1];
+  const T cmu = -mat.tau * P.drho;
+  const T cs = mat.mu - p3 * P.drho;                 // F_s + F_p
+  const T rb = mat.rho - P.rho_ref;
+  F[0] = cs * G[0] + rb * P.gx + cmu * (Sxx * G[0] + Sxy * G[1]);
+  F[1] = cs * G[1] + rb * P.gy + cmu * (Sxy * G[0] + Syy * G[1]);
+}
+// Both collisions of one node (Alg. 1): in f, g pre-collision; out post-collision in place.
+template <typename T>
+__device__ __forceinline__ void collide9(const KP<T>& P, const Mom9<T>& m, const Mat<T>& mat, T phi, const T (&G)[3], T ux, T uy,
+                                         T (&f)[Q9], T (&g)[Q9]) {
+  T F[2] = {T(0), T(0)}, D[2] = {T(0), T(0)};
+  if (!P.phase_only) force9(P, m, mat, ux, uy, G, F, D);
+  const T usq15 = T(1.5) * (ux * ux + uy * uy);
+  const T hx = T(1.5) * F[0] * mat.inv_rho, hy = T(1.5) * F[1] * mat.inv_rho;
+  const T k = T(4.5) * (T(1) - mat.s_nu);
+  const T gn = sqrt_(G[0] * G[0] + G[1] * G[1]) + T(1e-32);   // R10
+  const T pref = (T(1) - T(4) * (phi - T(0.5)) * (phi - T(0.5))) * P.inv_W;
+  const T om = P.om_phi;
+  const T cphi = (T(1) - T(0.5) * om) * pref / gn;
+  const T nx_ = G[0] * cphi, ny_ = G[1] * cphi;
+  const T omphi = om * phi, om1 = T(1) - om;
+#pragma unroll
+  for (int a = 0; a < Q9; ++a) {
+    const T cx_ = T(ex(a)), cy_ = T(ey(a));
+    const T eu = cx_ * ux + cy_ * uy;
+    const T gam = T(3) * eu + T(4.5) * eu * eu - usq15;
+    const T eDe = (cx_ * cx_ - cy_ * cy_) * D[0] + T(2) * cx_ * cy_ * D[1];
+    if (P.phase_only) f[a] = T(0);
+    else if (P.collision == 1) f[a] = (T(1) - mat.s_nu) * f[a] + w9<T>(a) * (mat.s_nu * (m.p + gam) + (T(2) - mat.s_nu) * (cx_ * hx + cy_ * hy));
+    else f[a] = w9<T>(a) * ((m.p + gam) + (cx_ * hx + cy_ * hy) + k * eDe);
+    g[a] = om1 * g[a] + w9<T>(a) * (omphi * (T(1) + gam) + (cx_ * nx_ + cy_ * ny_));
+  }
+}
+template <typename T> __device__ __forceinline__ void store9(const KP<T>& P, int x, int y, const T (&f)[Q9], const T (&g)[Q9]) {
+#pragma unroll
+  for (int a = 0; a < Q9; ++a) { P.p_dst[pidx(P.nx, y, a, x)] = f[a]; P.p_dst[pidx(P.nx, y, Q9 + a, x)] = g[a]; }
+}
+
+template <typename T> __global__ void __launch_bounds__(256) k_phi9(const __grid_constant__ KP<T> P) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= P.n) return;
+  const int x = (int)(i % P.nx), y = (int)(i / P.nx);
+  T g[Q9];
+  Pull9<T>::run(P, 1, x, y, g);
+  P.phi[i] = (g[0] + ((g[1] + g[2]) + (g[3] + g[4]))) + ((g[5] + g[6]) + (g[7] + g[8]));
+}
+template <typename T> __global__ void __launch_bounds__(256) k_step9(const __grid_constant__ KP<T> P) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= P.n) return;
+  const int x = (int)(i % P.nx), y = (int)(i / P.nx);
+  T f[Q9], g[Q9];
+  Pull9<T>::run(P, 0, x, y, f);
+  Pull9<T>::run(P, 1, x, y, g);
+  const T phi = P.phi[i];
+  T G[3], L;
+  stencil9(P, P.phi, x, y, phi, G, L);
+  const Mat<T> mat = materials(P, phi, L);
+  const Mom9<T> m = moments9(f);
+  T ux = P.u[i], uy = P.u[P.n + i];
+  if (!P.phase_only) {  // macros, Alg. 3: F from (new p*, new phi, lagged u, R13), then Eq. 31b
+    T F[2], D[2];
+    force9(P, m, mat, ux, uy, G, F, D);
+    const T h = T(0.5) * mat.inv_rho;
+    ux = m.mx + h * F[0]; uy = m.my + h * F[1];
+    P.u[i] = ux; P.u[P.n + i] = uy;
+  }
+  collide9(P, m, mat, phi, G, ux, uy, f, g);
+  store9(P, x, y, f, g);
+}
+// I1-I4 of DESIGN.md (R8), then the first collision
+template <typename T> __global__ void __launch_bounds__(256) k_init9(const __grid_constant__ KP<T> P, const T* __restrict__ phi0, const T* __restrict__ u0) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= P.n) return;
+  const int x = (int)(i % P.nx), y = (int)(i / P.nx);
+  const T phi = phi0[i], ux = u0[i], uy = u0[P.n + i];
+  T G[3], L;
+  stencil9(P, phi0, x, y, phi, G, L);
+  const Mat<T> mat = materials(P, phi, L);
+  const T rb = mat.rho - P.rho_ref;
+  const T F0 = mat.mu * G[0] + rb * P.gx, F1 = mat.mu * G[1] + rb * P.gy;   // I3: F = F_s + F_b (p* = 0, F_mu = 0)
+  const T usq15 = T(1.5) * (ux * ux + uy * uy);
+  const T gn = sqrt_(G[0] * G[0] + G[1] * G[1]) + T(1e-32);
+  const T pref = (T(1) - T(4) * (phi - T(0.5)) * (phi - T(0.5))) * P.inv_W / gn;
+  T f[Q9], g[Q9];
+#pragma unroll
+  for (int a = 0; a < Q9; ++a) {
+    const T cx_ = T(ex(a)), cy_ = T(ey(a));
+    const T eu = cx_ * ux + cy_ * uy;
+    const T gam = T(3) * eu + T(4.5) * eu * eu - usq15;
+    f[a] = P.phase_only ? T(0) : w9<T>(a) * (gam - T(0.5) * (T(3) * (cx_ * F0 + cy_ * F1) * mat.inv_rho));   // I4
+    g[a] = w9<T>(a) * (phi * (T(1) + gam) - T(0.5) * (pref * (cx_ * G[0] + cy_ * G[1])));
+  }
+  P.phi[i] = phi;
+  P.u[i] = ux; P.u[P.n + i] = uy; P.u[2 * P.n + i] = T(0);
+  const Mom9<T> m = moments9(f);
+  collide9(P, m, mat, phi, G, ux, uy, f, g);
+  store9(P, x, y, f, g);
+}
+// phi, p = p* rho c_s^2 with p* = sum_a f+_a, u
+template <typename T>
+__global__ void __launch_bounds__(256) k_get9(const __grid_constant__ KP<T> P, T* __restrict__ phi_out, T* __restrict__ p_out, T* __restrict__ u_out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= P.n) return;
+  const int x = (int)(i % P.nx), y = (int)(i / P.nx);
+  const T phi = P.phi[i];
+  if (phi_out) phi_out[i] = phi;
+  if (u_out) { u_out[i] = P.u[i]; u_out[P.n + i] = P.u[P.n + i]; u_out[2 * P.n + i] = P.u[2 * P.n + i]; }
+  if (p_out) {
+    T f[Q9];
+#pragma unroll
+    for (int a = 0; a < Q9; ++a) f[a] = P.p_src[pidx(P.nx, y, a, x)];
+    p_out[i] = moments9(f).p * (P.rho_l + phi * P.drho) * T(1.0 / 3.0);
+  }
+}
+
+}  // namespace d2q9
+}  // namespace clip

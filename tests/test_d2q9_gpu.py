@@ -1,0 +1,113 @@
+"""GPU parity on the D2Q9 lattice (clip_params.lattice = 1): libclip through the C ABI against
+the D2Q9 build of the oracle, element by element on the same seeded inputs, north_star tolerances."""
+import numpy as np
+import pytest
+
+from paper_2505_12205_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FP64_ABS, FP32_PHI, FP32_U = 1e-10, 1e-4, 1e-3
+P_, WL, FS = inputs.PERIODIC, inputs.WALL, inputs.FREESLIP
+
+
+def _with(case, **kw):
+    case["params"].update(kw)
+    return case
+
+
+def _capwave2d():
+    case = inputs.capillary_wave(L0=32, sigma=5e-3)     # Sec. 5.1 set-up at reduced size: free-slip sides, no-slip top / bottom
+    case["params"]["lattice"] = 1
+    return case
+
+
+# The cases avoid ONE thing on purpose: a drop at rest at density ratio 1000.  The interface normal n = grad phi / |grad phi| (Eq. 34) is
+# ill-conditioned on the plateau inside a drop, where phi overshoots 1 by ~1e-3 during the start-up transient; in two dimensions this
+# amplifies round-off so strongly that two fp64 runs of the ORACLE whose inputs differ by 6e-8 relative are 6e-5 .. 1e-3 apart in phi
+# after 100 steps (drop2d R = 16, rho* = 1000; 3-D configs[0]: 3e-9) -- DESIGN.md reading G21.  The cases below have that factor <= 2e-7.
+CASES = {
+    "sweep2d_periodic": (lambda: _with(inputs.sweep2d(nx=128, ny=96), rho_l=0.01), 100),       # seeded discs, rho ratio 100
+    "sweep2d_walls": (lambda: _with(inputs.sweep2d(nx=67, ny=50, ndrops=4), bc=(WL,) * 4 + (P_, P_), g=(1e-5, -2e-5, 0.0), rho_l=0.05, sigma=0.002), 100),
+    "sweep2d_freeslip_mixed": (lambda: _with(inputs.sweep2d(nx=40, ny=36, ndrops=3, rmin=4, rmax=6), bc=(FS, WL, FS, FS, P_, P_), rho_l=0.1), 100),
+    "poiseuille2d": (lambda: inputs.poiseuille2d(nx=4, ny=32), 1000),
+    "poiseuille2d_rho10_mu": (lambda: inputs.poiseuille2d(nx=4, ny=64, tau_a=5.0, tau_b=0.5, rho_a=10.0, rho_b=1.0, gx=1e-7, visc_interp=2), 500),
+    "capwave2d": (_capwave2d, 200),
+    "sweep2d_bgk": (lambda: _with(inputs.sweep2d(nx=64, ny=48, ndrops=3), rho_l=0.01, collision=1, tau_l=0.3), 100),
+    "drop2d_rho1000_20_steps": (lambda: inputs.drop2d(n=64, R=16.0), 20),       # the resting drop itself, before the amplification sets in
+}
+_ref = {}
+
+
+@pytest.mark.parametrize("name", list(CASES))
+@pytest.mark.parametrize("precision", [64, 32])
+def test_parity_d2q9(name, precision):
+    import torch
+    from oracle.clip_oracle import Oracle
+    from paper_2505_12205_b200 import clip
+    mk, steps = CASES[name]
+    if name not in _ref:
+        case = mk()
+        o = Oracle.from_case(case)
+        assert o.Q == 9
+        o.step(steps)
+        _ref[name] = (case, o.get())
+    case, (rphi, rp, ru) = _ref[name]
+    sim = clip.Clip.from_case(case, precision=precision)
+    sim.step(steps)
+    phi, p, u = (t.double().cpu().numpy() for t in sim.get())
+    torch.cuda.synchronize()
+    sim.close()
+    assert np.isfinite(phi).all() and np.isfinite(p).all() and np.isfinite(u).all() and np.abs(u[2]).max() == 0.0
+    if precision == 64:
+        e = [np.abs(a - b).max() for a, b in ((phi, rphi), (p, rp), (u, ru))]
+        print(f"{name} fp64: max-abs phi {e[0]:.2e} p {e[1]:.2e} u {e[2]:.2e}")
+        assert max(e) <= FP64_ABS
+    else:
+        ephi = np.abs(phi - rphi).max() / np.abs(rphi).max()
+        eu = np.abs(u - ru).max() / max(np.abs(ru).max(), 1e-30)
+        print(f"{name} fp32: field-rel phi {ephi:.2e} u {eu:.2e}")
+        assert ephi <= FP32_PHI and eu <= FP32_U
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_phase_only_d2q9(precision):
+    """The set-up of Sec. 5.4 (2-D, D2Q9, prescribed reversing shear flow) at reduced size: clip_set_u + clip_step
+    against the D2Q9 oracle.  The GPU stores post-collision populations, so it takes u(k+1) before step k+1."""
+    import torch
+    from oracle.clip_oracle import Oracle
+    from paper_2505_12205_b200 import clip
+    n, U0, W, steps = 48, 0.04, 3.0, 150
+    p = inputs.default_params(W=W, M=U0 * W / 600.0, sigma=0.0, rho_h=1.0, rho_l=1.0, phase_only=1, lattice=1, precision=precision)
+    y, x = np.meshgrid(np.arange(n, dtype=float), np.arange(n, dtype=float), indexing="ij")
+    phi0 = (0.5 + 0.5 * np.tanh(2.0 * (n / 5 - np.sqrt((x - 0.5 * n) ** 2 + (y - 0.3 * n) ** 2)) / W))[None]
+
+    def vel(t):
+        c = U0 * np.cos(np.pi * t / 300.0)
+        return np.stack([c * np.sin(np.pi * x / n) ** 2 * np.sin(2 * np.pi * y / n), -c * np.sin(np.pi * y / n) ** 2 * np.sin(2 * np.pi * x / n),
+                         np.zeros_like(x)])[:, None]
+    o = Oracle(n, n, 1, p)
+    o.init(phi0, vel(0))
+    for k in range(steps):
+        o.set_u(vel(k)); o.step(1)
+    rphi = o.get()[0]
+    sim = clip.Clip(n, n, 1, p)
+    sim.init(torch.as_tensor(phi0), torch.as_tensor(vel(0)))
+    for k in range(steps):
+        sim.set_u(torch.as_tensor(vel(k + 1))); sim.step(1)
+    phi, pr, u = (t.double().cpu().numpy() for t in sim.get())
+    sim.close()
+    err = np.abs(phi - rphi).max()
+    assert np.abs(pr).max() == 0.0 and np.abs(rphi - phi0).max() > 0.2
+    assert err <= (FP64_ABS if precision == 64 else FP32_PHI), err
+
+
+def test_d2q9_abi():
+    from paper_2505_12205_b200 import clip
+    p = inputs.default_params(lattice=1)
+    n2 = clip.clip_workspace_bytes(64, 64, 1, clip.make_params(p))
+    n3 = clip.clip_workspace_bytes(64, 64, 1, clip.make_params(dict(p, lattice=0)))
+    assert 0 < n2 < n3 and n2 >= (4 * 9 + 4) * 64 * 64 * 8
+    assert clip.clip_workspace_bytes(64, 64, 2, clip.make_params(p)) == 0 and "D2Q9" in clip.clip_last_error(None)
+    assert clip.clip_workspace_bytes(64, 64, 1, clip.make_params(dict(p, bc=(0, 0, 0, 0, 1, 1)))) == 0
+    assert clip.clip_workspace_bytes(64, 64, 1, clip.make_params(dict(p, lattice=2))) == 0
