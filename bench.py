@@ -411,10 +411,13 @@ def run_long(args):
     if args.long_run == "rt":
         case = inputs.rayleigh_taylor(L=args.n // 2, precision=prec)
         total = args.steps if args.steps_given else 20000
+    elif args.long_run == "jetpaper":   # the paper's own set-up (Sec. 6.1, Table 6 row --case): 6 D x 6 D x 20 D, free-slip sides, gravity
+        case = inputs.jet_paper(case=args.case, D=args.n // 8, precision=prec)
+        total = args.steps if args.steps_given else 40000
     else:
         case = inputs.jet(nxy=3 * args.n // 4, nz=6 * args.n, r_nozzle=12.0 * args.n / 256, We=args.we, precision=prec)
         total = args.steps if args.steps_given else 50000
-    every = max(1, total // 50)
+    every = max(1, total // (200 if args.long_run == "jetpaper" else 50))
     case["params"]["path"] = args.path
     sim = clip.Clip.from_case(case, precision=prec)
     pr = case["params"]
@@ -422,7 +425,7 @@ def run_long(args):
     phi0 = torch.as_tensor(case["phi0"]).to(dev)
     s0 = float(phi0.double().sum())
     disc = None
-    if args.long_run == "jet":
+    if args.long_run in ("jet", "jetpaper"):
         yy, xx = torch.meshgrid(torch.arange(ny, dtype=torch.float64), torch.arange(nx, dtype=torch.float64), indexing="ij")
         disc = int((((xx - pr["inlet_c"][0]) ** 2 + (yy - pr["inlet_c"][1]) ** 2) <= pr["inlet_r"] ** 2).sum())
     series, first_bad = [], None
@@ -447,8 +450,11 @@ def run_long(args):
                 rec["xz_asym"] = float((phi - phi.transpose(0, 2)).abs().max())
                 rec["y_front_heavy"] = int((phi[:, :, :] > 0.5).any(dim=2).any(dim=0).nonzero().min())   # lowest row the heavy fluid has reached
             else:
-                col = (phi[:, ny // 2, nx // 2] > 0.5).nonzero()
+                axis = phi[:, ny // 2, nx // 2] > 0.5
+                col = axis.nonzero()
                 rec["tip_z"] = int(col.max()) if col.numel() else -1
+                gaps = (~axis).nonzero()
+                rec["attached_len"] = int(gaps.min()) if gaps.numel() else nz      # length of the liquid column still attached to the nozzle
                 rec["outlet_phi_max"] = float(phi[-1].max())
         elif first_bad is None:
             first_bad = done
@@ -468,6 +474,15 @@ def run_long(args):
             out["xz_asym_max"] = max(r["xz_asym"] for r in series)
         else:
             # inflow mass balance while the liquid is far from the outlet: d(sum phi)/dt against (disc nodes) x U x phi_in
+            if args.long_run == "jetpaper":
+                # breakup length (Fig. 18c): the attached column grows until a drop pinches off; L_b = its length just
+                # before each pinch-off (local maxima of the attached length followed by a drop of more than D / 2)
+                D = 2.0 * pr["inlet_r"]
+                al = [r["attached_len"] for r in series]
+                peaks = [al[k] for k in range(1, len(al) - 1) if al[k] >= al[k - 1] and al[k + 1] < al[k] - 0.5 * D]
+                out["breakup"] = {"D": D, "pinch_offs": len(peaks), "L_b_over_D": [v / D for v in peaks],
+                                  "L_b_over_D_mean": (sum(peaks) / len(peaks) / D) if peaks else None, "t_star_end": done * pr["inlet_u"][2] / D,
+                                  "case": args.case, "Re_We_Fr": inputs.JET_TABLE6[args.case]}
             pre = [r for r in series if r["outlet_phi_max"] < 0.01]
             if len(pre) >= 2:
                 rate = (pre[-1]["sum_phi"] - pre[0]["sum_phi"]) / (pre[-1]["t"] - pre[0]["t"])
@@ -498,7 +513,8 @@ def main():
     ap.add_argument("--nz", type=int, default=0, help="jet workload only: planes along the jet (default 6 n = 1536; shorter for profiling runs)")
     ap.add_argument("--path", type=int, default=0, choices=[0, 1, 2, 3],
                     help="clip_params.path: 0 automatic (default), 1 generic kernels, 2 pair kernels (k_phi2 + k_step2), 3 k_fused wherever admitted")
-    ap.add_argument("--long-run", default=None, choices=["rt", "jet"],
+    ap.add_argument("--case", default="l", help="--long-run jetpaper: row of the paper's Table 6 (a .. l)")
+    ap.add_argument("--long-run", default=None, choices=["rt", "jet", "jetpaper"],
                     help="run BASELINE configs[2] (rt, 20000 steps) or configs[3] (jet, 50000 steps) at full length with diagnostics; one JSON line")
     ap.add_argument("--we", type=float, default=2.2, help="Weber number of the jet (--long-run jet)")
     args = ap.parse_args()

@@ -128,6 +128,36 @@ def jet(nxy=192, nz=1536, r_nozzle=12.0, We=2.2, W=4.0, U=0.05, precision=32):
     return _case(nx, ny, nz, p, phi0, u0, f"jet{nxy}x{nz}")
 
 
+# Table 6: Re, We, Fr of the paper's twelve jet cases; rho* = 814, mu* = 55, Oh = sqrt(We) / Re = 4.4e-3
+JET_TABLE6 = {"a": (151, 0.44, 2.60), "b": (211, 0.88, 3.65), "c": (228, 1.03, 3.94), "d": (302, 1.79, 5.22), "e": (332, 2.17, 5.74),
+              "f": (340, 2.27, 5.87), "g": (347, 2.37, 6.01), "h": (362, 2.58, 6.26), "i": (397, 3.10, 6.86), "j": (408, 3.27, 7.05),
+              "k": (423, 3.52, 7.31), "l": (454, 4.05, 7.84)}
+
+
+def jet_paper(case="l", D=32, W=4.0, precision=32, nz=None):
+    """The paper's own jet set-up (Sec. 6.1, Fig. 18; Eq. 58-59; Table 6): domain 6 D x 6 D x 20 D, circular inlet of
+    diameter D with uniform velocity u_j = 0.05 and rho_j = 1 (:849), FREE-SLIP side walls, convective outlet, gravity along the jet
+    with F_g = (rho - rho_L) g (Eq. 58: rho_ref = rho_l), rho* = 814, mu* = 55, and (Re, We, Fr) of the named row of Table 6
+    (Eq. 59: sigma = rho_j u_j^2 D / We, nu_j = u_j D / Re, g = u_j^2 / (Fr^2 D)).  The jet runs along +z here (the paper's y).
+    D = 32 gives 192 x 192 x 640; D = 4 the parity replica 24 x 24 x 80."""
+    Re, We, Fr = JET_TABLE6[case]
+    U = 0.05
+    nxy, nz = 6 * D, (20 * D if nz is None else nz)
+    x, y, z = _grid(nxy, nxy, nz)
+    c = 0.5 * (nxy - 1)
+    r_n = 0.5 * D
+    rxy = np.sqrt((x - c) ** 2 + (y - c) ** 2)
+    phi0 = 0.5 + 0.5 * np.tanh(2.0 * np.minimum(r_n - rxy, r_n - z) / W)          # a liquid stub in front of the nozzle
+    u0 = np.zeros((3, nz, nxy, nxy))
+    rho_h, rho_l = 1.0, 1.0 / 814.0
+    nu_h = U * D / Re
+    nu_l = nu_h * 814.0 / 55.0                                                    # mu* = 55
+    p = default_params(precision=precision, rho_h=rho_h, rho_l=rho_l, tau_h=3 * nu_h, tau_l=3 * nu_l, sigma=rho_h * U * U * D / We, W=W, M=0.1,
+                       g=(0.0, 0.0, U * U / (Fr * Fr * D)), rho_ref=rho_l,
+                       bc=(FREESLIP,) * 4 + (INLET, OUTLET), inlet_u=(0.0, 0.0, U), inlet_phi=1.0, inlet_c=(c, c), inlet_r=r_n, outlet_clamp=1)
+    return _case(nxy, nxy, nz, p, phi0, u0, f"jet_paper_{case}_D{D}")
+
+
 def capillary_wave(L0=256, nu=0.005, sigma=1.0e-4, W=4.0, M=0.02, rho_h=1.0, rho_l=0.1, eta0_rel=0.02, precision=64):
     """PAPER.md Sec. 5.1 (:559-595, Fig. 7): L0 x 2 L0 (x 1) box, free-slip faces in x, no-slip walls in y; heavy fluid
     below the interface y = L0 + eta0 cos(2 pi x / L0), eta0 = 0.02 L0; equal kinematic viscosity nu in both fluids;

@@ -87,6 +87,8 @@ CASES = {
     # periodic z
     "freeslip_xy_zwall": (lambda: _with(inputs.walled_box(nx=14, ny=12, nz=10), bc=(inputs.FREESLIP, inputs.WALL, inputs.WALL, inputs.FREESLIP, inputs.WALL, inputs.WALL)), 100),
     "freeslip_xy_periodic_z": (lambda: _with(inputs.walled_box(nx=16, ny=8, nz=12), bc=(inputs.FREESLIP,) * 4 + (inputs.PERIODIC,) * 2), 100),
+    # the paper's jet set-up proper (Sec. 6.1: free-slip sides, gravity with Eq. 58, Table 6 row l: Re 454, We 4.05, Fr 7.84) as a replica
+    "jet_paper_replica": (lambda: inputs.jet_paper(case="l", D=4, W=3.0, nz=48), 150),
     "sweep64_linear_mu": (lambda: _with(inputs.sweep_drops(n=64), visc_interp=2, tau_l=0.3), 100),   # fused-free fast path
     "rt_replica_linear_mu": (lambda: _with(inputs.rayleigh_taylor(L=16, W=3.0), visc_interp=2), 100),
     "jet_replica_uave": (lambda: _with(inputs.jet(nxy=24, nz=48, r_nozzle=4.0), outlet_u_mode=1), 150),   # B.22 U_ave
