@@ -24,12 +24,18 @@ if ROOT not in sys.path:
 
 B_MIN_WORDS = 84  # f 19R+19W, g 19R+19W, phi 1R+1W, u 3R+3W
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
-# captures (profiles/r01_fused_256_fp32.md, profiles/r01_fast_256_fp32.md); reported as roofline.traffic when the run
-# matches that configuration.
-NCU_TRAFFIC = {("k_fused", 256, 32, "sweep"): 2.950e9 + 2.824e9, ("k_fused", 256, 64, "sweep"): 6.030e9 + 5.688e9,
-               ("k_step2", 256, 32, "sweep"): 2.821e9 + 2.698e9,
-               ("k_step2", 256, 32, "jet"): 9.503e9 + 9.266e9}   # profiles/r01_jet_step2_fp32.md
+def ncu_traffic(kernel, workload, n, precision):
+    """roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu
+    --set full captures (profiles/r02_traffic.csv, written from the .ncu-rep files named there; commands in profiles/r02_traffic.md).
+    None when no capture matches this run's kernel / workload / size / precision."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "r02_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    for row in csv.DictReader(open(path)):
+        if (row["kernel"], row["workload"], int(row["n"]), int(row["precision"])) == (kernel, workload, int(n), int(precision)):
+            return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
+    return None
 
 
 def measured_peak():
@@ -260,7 +266,7 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "effective_gbs": mlups * 1e6 * b_min * word / 1e9 / world,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC.get((dom, n, prec, args.workload)) if not args.nz else None, "peak_source": peak_src,
+                         "traffic": ncu_traffic(dom, args.workload, n, prec) if not args.nz else None, "peak_source": peak_src,
                          "kernel": dom, "algorithmic_bytes_per_step": step_bytes,
                          "note": f"achieved = {b_min} words/LU x nodes / (sum of the step's kernel durations, CUDA events per launch)",
                          "kernels_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
