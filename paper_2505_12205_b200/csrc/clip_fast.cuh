@@ -174,15 +174,22 @@ template <typename T, int H> __device__ __forceinline__ Row3<T> ld_row3(const T*
   return r;
 }
 
-// Eq. 40a/b on differences d = phi(x+e) - phi(x) (exact zero on a uniform field).
-template <typename T, int H = LD_NC>
-__device__ __forceinline__ void stencil2(const T* __restrict__ phi, const Geo& g, P2<T>& pc, P2<T> (&G)[3], P2<T>& L) {
+// Eq. 40a/b on differences d = phi(x+e) - phi(x) (exact zero on a uniform field).  Split into the loads
+// (StRaw: the 19-point neighbourhood of a node pair) and the arithmetic, so that a kernel may fetch a row ahead (k_fused_tma).
+template <typename T> struct StRaw { Row3<T> c, yp, ym, zp, zm; P2<T> ypzp, ymzm, ypzm, ymzp; };
+template <typename T, int H = LD_NC> __device__ __forceinline__ StRaw<T> stencil2_load(const T* __restrict__ phi, const Geo& g) {
+  StRaw<T> r;
+  r.c = ld_row3<T, H>(phi, phi_row_of<0, 0>(g), g);
+  r.yp = ld_row3<T, H>(phi, phi_row_of<1, 0>(g), g); r.ym = ld_row3<T, H>(phi, phi_row_of<-1, 0>(g), g);
+  r.zp = ld_row3<T, H>(phi, phi_row_of<0, 1>(g), g); r.zm = ld_row3<T, H>(phi, phi_row_of<0, -1>(g), g);
+  r.ypzp = ld_pair<T, H>(phi + phi_row_of<1, 1>(g)); r.ymzm = ld_pair<T, H>(phi + phi_row_of<-1, -1>(g));
+  r.ypzm = ld_pair<T, H>(phi + phi_row_of<1, -1>(g)); r.ymzp = ld_pair<T, H>(phi + phi_row_of<-1, 1>(g));
+  return r;
+}
+template <typename T> __device__ __forceinline__ void stencil2_eval(const StRaw<T>& r, P2<T>& pc, P2<T> (&G)[3], P2<T>& L) {
   typedef P2<T> V;
-  const Row3<T> c = ld_row3<T, H>(phi, phi_row_of<0, 0>(g), g);
-  const Row3<T> yp = ld_row3<T, H>(phi, phi_row_of<1, 0>(g), g), ym = ld_row3<T, H>(phi, phi_row_of<-1, 0>(g), g);
-  const Row3<T> zp = ld_row3<T, H>(phi, phi_row_of<0, 1>(g), g), zm = ld_row3<T, H>(phi, phi_row_of<0, -1>(g), g);
-  const V ypzp = ld_pair<T, H>(phi + phi_row_of<1, 1>(g)), ymzm = ld_pair<T, H>(phi + phi_row_of<-1, -1>(g));
-  const V ypzm = ld_pair<T, H>(phi + phi_row_of<1, -1>(g)), ymzp = ld_pair<T, H>(phi + phi_row_of<-1, 1>(g));
+  const Row3<T>&c = r.c, &yp = r.yp, &ym = r.ym, &zp = r.zp, &zm = r.zm;
+  const V ypzp = r.ypzp, ymzm = r.ymzm, ypzm = r.ypzm, ymzp = r.ymzp;
   pc = c.C;
   const V d1 = c.R - pc, d2 = c.L - pc, d3 = yp.C - pc, d4 = ym.C - pc, d5 = zp.C - pc, d6 = zm.C - pc;
   const V d7 = yp.R - pc, d8 = ym.L - pc, d9 = ym.R - pc, d10 = yp.L - pc;
@@ -195,6 +202,10 @@ __device__ __forceinline__ void stencil2(const T* __restrict__ phi, const Geo& g
   G[0] = fma2(V(T(1.0 / 6.0)), d1 - d2, V(T(1.0 / 12.0)) * ((e78 + e910) + (e1112 + e1314)));
   G[1] = fma2(V(T(1.0 / 6.0)), d3 - d4, V(T(1.0 / 12.0)) * ((e78 - e910) + (e1516 + e1718)));
   G[2] = fma2(V(T(1.0 / 6.0)), d5 - d6, V(T(1.0 / 12.0)) * ((e1112 - e1314) + (e1516 - e1718)));
+}
+template <typename T, int H = LD_NC>
+__device__ __forceinline__ void stencil2(const T* __restrict__ phi, const Geo& g, P2<T>& pc, P2<T> (&G)[3], P2<T>& L) {
+  stencil2_eval<T>(stencil2_load<T, H>(phi, g), pc, G, L);
 }
 
 template <typename T> struct Mat2 { P2<T> rho, inv_rho, tau, s_nu, mu; };
@@ -406,21 +417,35 @@ template <typename T, int HG, int NX, int WALLS> __device__ __forceinline__ void
 // issued as soon as f has been reduced to its 10 moments and phi to (grad, laplacian), and stay in flight while the
 // macros and f+ are computed and stored.
 struct NoWait { __device__ __forceinline__ void operator()() const {} };
+// Where the streamed populations of a node pair come from: global memory (pull2, every kernel but k_fused_tma) ...
+struct GlobalPull {
+  static constexpr bool F_FIRST = true;   // issue the f loads before u and phi (all of them stay in flight together)
+  template <typename T, int HL, int NX, int SET, int WALLS>
+  __device__ __forceinline__ void run(const KP<T>& P, const Geo& geo, P2<T> (&v)[Q]) const { Pull2All<T, HL, NX, SET, WALLS>::run(P.p_src, P.nx, geo, v); }
+  template <typename T, int HL> __device__ __forceinline__ void load_u(const KP<T>& P, const Geo& geo, P2<T>& ux, P2<T>& uy, P2<T>& uz) const {
+    ux = ld_pair<T, HL>(P.u + geo.rc); uy = ld_pair<T, HL>(P.u + P.n + geo.rc); uz = ld_pair<T, HL>(P.u + 2 * P.n + geo.rc);
+  }
+  template <typename T, int HP> __device__ __forceinline__ void stencil(const KP<T>& P, const Geo& geo, P2<T>& phi, P2<T> (&G)[3], P2<T>& L) const {
+    stencil2<T, HP>(P.phi, geo, phi, G, L);
+  }
+};
 struct NoAfter { template <typename T> __device__ __forceinline__ void operator()(const Geo&, const P2<T> (&)[Q]) const {} };
-template <typename T, int HL, int HP, int HS, int NX, int WALLS, typename W, typename A = NoAfter, bool BGK = false>
-__device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z, W before_phi, A after = A()) {
+template <typename T, int HL, int HP, int HS, int NX, int WALLS, typename W, typename A = NoAfter, bool BGK = false, typename PL = GlobalPull>
+__device__ __forceinline__ void step_pair(const FP<T>& FPp, int x0, int y, int z, W before_phi, A after = A(), PL pl = PL()) {
   typedef P2<T> V;
   const KP<T>& P = FPp.k;
   const Geo geo = make_geo<T, WALLS>(P, x0, y, z);
   V f[Q], g[Q];
-  Pull2All<T, HL, NX, 0, WALLS>::run(P.p_src, P.nx, geo, f);
-  V ux = ld_pair<T, HL>(P.u + geo.rc), uy = ld_pair<T, HL>(P.u + P.n + geo.rc), uz = ld_pair<T, HL>(P.u + 2 * P.n + geo.rc);
+  if (PL::F_FIRST) pl.template run<T, HL, NX, 0, WALLS>(P, geo, f);
+  V ux, uy, uz;
+  pl.template load_u<T, HL>(P, geo, ux, uy, uz);
   before_phi();
   V phi, G[3], L;
-  stencil2<T, HP>(P.phi, geo, phi, G, L);
+  pl.template stencil<T, HP>(P, geo, phi, G, L);
+  if (!PL::F_FIRST) pl.template run<T, HL, NX, 0, WALLS>(P, geo, f);   // staged source: u and phi are already on their way
   const Mom2<T> m = moments2<T>(f);
   CLIP_LOAD_FENCE();
-  Pull2All<T, HL, NX, 1, WALLS>::run(P.p_src, P.nx, geo, g);
+  pl.template run<T, HL, NX, 1, WALLS>(P, geo, g);
   const Mat2<T> mat = materials2<T>(P, phi, L);
   {  // macros, Alg. 3: F from (new p*, new phi, lagged u, R13), then Eq. 31b
     V F[3], D[6];

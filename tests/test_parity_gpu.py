@@ -426,6 +426,32 @@ def test_fused_single_pass_path(name, precision):
             assert np.abs(a - b).max() <= tol * max(1.0, np.abs(a).max()), (name, env)
 
 
+@pytest.mark.parametrize("precision", [64, 32])
+def test_fused_tma_path(precision):
+    """k_fused_tma (path 4: the 38 population rows of a lattice row arrive in shared memory by bulk-async copies, one row ahead;
+    x / y faces PERIODIC) against k_phi2 + k_step2: round-off only; several tilings; periodic z, walled z and an inlet / outlet pair."""
+    import torch
+    from paper_2505_12205_b200 import clip
+    P_, WL = inputs.PERIODIC, inputs.WALL
+    cases = [inputs.sweep_drops(shape=(128, 24, 20), ndrops=6, rmin=3, rmax=6), inputs.sweep_drops(shape=(64, 4, 5), ndrops=2, rmin=2, rmax=3),
+             inputs.sweep_drops(shape=(256, 8, 9), ndrops=3, rmin=3, rmax=4),
+             _with(inputs.sweep_drops(shape=(128, 8, 12), ndrops=3, rmin=3, rmax=4), bc=(P_,) * 4 + (WL, WL), g=(0.0, 0.0, -1e-5)),
+             _with(inputs.jet(nxy=64, nz=20, r_nozzle=6.0), bc=(P_,) * 4 + (inputs.INLET, inputs.OUTLET))]
+    tol = 1e-12 if precision == 64 else 3e-5
+    for case in cases:
+        ref = _gpu_p(case, 25, precision, path=2)
+        for over in ({}, {"tile_chunks": 1}, {"tile_chunks": case["nz"]}):
+            c = dict(case, params=dict(case["params"], path=4, **over))
+            sim = clip.Clip.from_case(c, precision=precision)
+            sim.step(25)
+            out = [t.double().cpu().numpy() for t in sim.get()]
+            torch.cuda.synchronize()
+            sim.close()
+            for a, b in zip(ref, out):
+                assert np.isfinite(b).all()
+                assert np.abs(a - b).max() <= tol * max(1.0, np.abs(a).max()), (case["name"], over)
+
+
 def test_fused_path_is_deterministic_at_full_size():
     """k_fused keeps phi's partial sums in a shared-memory ring that warps of a block fill and flush at different times
     (one barrier per plane, warp-edge sends through side arrays) and hands tile halos over through `part`: any race would
