@@ -191,6 +191,7 @@ def run_ours(args):
     else:
         case = inputs.sweep_drops(n=n, seed=rank_seed(rank), precision=prec)
     case["params"]["path"] = args.path
+    case["params"]["tile_ty"], case["params"]["tile_chunks"] = args.tile_ty, args.tile_chunks
     nxl, nyl, nzl = case["nx"], case["ny"], case["nz"]
     nodes = nxl * nyl * nzl
     sim = clip.Clip(nxl, nyl, nzl, case["params"], device=dev)
@@ -519,6 +520,8 @@ def main():
     ap.add_argument("--path", type=int, default=0, choices=[0, 1, 2, 3, 4],
                     help="clip_params.path: 0 automatic (default), 1 generic kernels, 2 pair kernels (k_phi2 + k_step2), 3 k_fused wherever admitted")
     ap.add_argument("--case", default="l", help="--long-run jetpaper: row of the paper's Table 6 (a .. l)")
+    ap.add_argument("--tile-ty", type=int, default=0, help="clip_params.tile_ty (k_fused rows per tile: 0 automatic, 4, 8, 16)")
+    ap.add_argument("--tile-chunks", type=int, default=0, help="clip_params.tile_chunks (k_fused: number of equal z chunks, 0 automatic)")
     ap.add_argument("--long-run", default=None, choices=["rt", "jet", "jetpaper"],
                     help="run BASELINE configs[2] (rt, 20000 steps) or configs[3] (jet, 50000 steps) at full length with diagnostics; one JSON line")
     ap.add_argument("--we", type=float, default=2.2, help="Weber number of the jet (--long-run jet)")

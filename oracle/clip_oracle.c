@@ -74,6 +74,9 @@ typedef struct clipo_params {
                               sum_a e_az f_a(x,y,N-1,t+dt) of the post-stream populations ("lambda = U(t+dt) dt/dy, determined after
                               the streaming step in the (N-1)th layer"), without the half-force term (F needs
                               grad phi(t+dt), which involves the outlet layer itself) */
+  int macro_u_refine;      /* ORACLE ONLY, sensitivity of reading R13 (Alg. 3 evaluates F_mu with the velocity of the PREVIOUS step,
+                              PAPER.md:501, before u is updated): 0: as printed (lagged u, one evaluation); 1: one fixed-point refinement,
+                              F is evaluated again with the u just obtained and u = sum f e + F / 2 rho is redone */
   int open_ghost;          /* ORACLE ONLY, sensitivity of reading R9 at the OPEN parts of the z faces (inlet disc, outlet): 0: clamp
                               (zero gradient, the reading the product takes); 1: linear extrapolation phi(-1) = 2 phi(0) - phi(1);
                               the plate around the nozzle is a wall and keeps the mirror value */
@@ -343,6 +346,10 @@ static void macros(clipo *h) {
       h->ux[i] = h->p.inlet_u[0]; h->uy[i] = h->p.inlet_u[1]; h->uz[i] = h->p.inlet_u[2];
     } else { /* Eq. 31b */
       h->ux[i] = mx + 0.5 * F[0] / rho; h->uy[i] = my + 0.5 * F[1] / rho; h->uz[i] = mz + 0.5 * F[2] / rho;
+      if (h->p.macro_u_refine == 1) { /* sensitivity variant of [R13] */
+        total_force(h, f, pstar, h->ux[i], h->uy[i], h->uz[i], h->phi[i], G, L, F);
+        h->ux[i] = mx + 0.5 * F[0] / rho; h->uy[i] = my + 0.5 * F[1] / rho; h->uz[i] = mz + 0.5 * F[2] / rho;
+      }
     }
   }
 }

@@ -37,7 +37,7 @@ class _Params(C.Structure):
         ("inlet_u", C.c_double * 3), ("inlet_phi", C.c_double), ("inlet_c", C.c_double * 2),
         ("inlet_r", C.c_double),
         ("outlet_u_mode", C.c_int), ("visc_interp", C.c_int), ("collision", C.c_int), ("phase_only", C.c_int),
-        ("outlet_clamp", C.c_int), ("outlet_u_time", C.c_int), ("open_ghost", C.c_int),
+        ("outlet_clamp", C.c_int), ("outlet_u_time", C.c_int), ("macro_u_refine", C.c_int), ("open_ghost", C.c_int),
     ]
 
 
@@ -56,6 +56,7 @@ def _marshal(p: dict) -> _Params:
     s.outlet_clamp = int(p.get("outlet_clamp", 0))
     s.outlet_u_time = int(p.get("outlet_u_time", 0))
     s.open_ghost = int(p.get("open_ghost", 0))   # oracle only (sensitivity of reading R9)
+    s.macro_u_refine = int(p.get("macro_u_refine", 0))   # oracle only (sensitivity of reading R13)
     return s
 
 

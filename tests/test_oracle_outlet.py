@@ -132,26 +132,34 @@ def test_recurrence_tells_the_two_time_levels_of_U_apart(when, clamp):
     assert seen_back
 
 
+def _sens_run(kw):
+    """One oracle run of the jet replica with parameter overrides (top level: runs in a process pool)."""
+    case = inputs.jet(nxy=24, nz=48, r_nozzle=4.0)
+    case["params"].update(kw)
+    o = Oracle.from_case(case)
+    o.step(200)
+    phi, p, u = o.get()
+    return phi, u / case["params"]["inlet_u"][2]
+
+
 def test_sensitivity_of_the_unpinned_readings_on_the_jet_replica():
-    """What the readings the paper cannot pin are worth (recorded in DESIGN.md, readings R9 and R12): jet replica 24 x 24 x 48,
+    """What the readings the paper cannot pin are worth (recorded in DESIGN.md, readings R9, R12, R13): jet replica 24 x 24 x 48,
     nozzle radius 4, 200 steps; max |d phi| and max |d u| / U_in against the default readings for
-      (a) R9 at the open faces: linear extrapolation of phi through the inlet / outlet instead of the clamp (oracle only);
+      (a) R9 at the open faces: linear extrapolation of phi through the inlet disc / outlet instead of the clamp (oracle only);
       (b) R12: U of B.22 from the post-stream moment at t + dt instead of the stored u(t);
-      (c) R12: B.25 as printed (no clamp) instead of lambda = max(0, U).
+      (c) R12: B.25 as printed (no clamp) instead of lambda = max(0, U);
+      (d) R13: F_mu of the macro update re-evaluated once with the new u instead of the lagged one alone (oracle only).
     Not a pin: the differences are reported and only bounded loosely (each reading changes the fields near the face it acts on)."""
-    def run(**kw):
-        case = inputs.jet(nxy=24, nz=48, r_nozzle=4.0)
-        case["params"].update(kw)
-        o = Oracle.from_case(case)
-        o.step(200)
-        phi, p, u = o.get()
-        return phi, u / case["params"]["inlet_u"][2]
-    base = run()
+    from concurrent.futures import ProcessPoolExecutor
+    variants = (("R9 open faces: linear extrapolation", dict(open_ghost=1)),
+                ("R12: U(t+dt) from the post-stream moment", dict(outlet_u_time=1)),
+                ("R12: B.25 without the clamp", dict(outlet_clamp=0)),
+                ("R13: one refinement of u in the macro update", dict(macro_u_refine=1)))
+    with ProcessPoolExecutor(max_workers=5) as ex:
+        runs = list(ex.map(_sens_run, [dict()] + [kw for _, kw in variants]))
+    base = runs[0]
     out = {}
-    for name, kw in (("R9 open faces: linear extrapolation", dict(open_ghost=1)),
-                     ("R12: U(t+dt) from the post-stream moment", dict(outlet_u_time=1)),
-                     ("R12: B.25 without the clamp", dict(outlet_clamp=0))):
-        phi, u = run(**kw)
+    for (name, kw), (phi, u) in zip(variants, runs[1:]):
         dphi, du = np.abs(phi - base[0]), np.abs(u - base[1]).max(axis=0)
         zphi, zu = np.unravel_index(dphi.argmax(), dphi.shape)[0], np.unravel_index(du.argmax(), du.shape)[0]
         out[name] = (dphi.max(), du.max())

@@ -310,6 +310,15 @@ def test_full_size_lattices_against_the_oracle(lattice, precision):
         _tiled_against_oracle(inputs.sweep_drops(n=64), (r, r, r), precision, 20, "k_fused")
 
 
+@pytest.mark.parametrize("n", [256, 384, 512])
+def test_fused_tma_full_size_against_the_oracle(n):
+    """k_fused_tma (path 4) at the sizes profiles/r02_experiments.md quotes for it (its nx = 256 / 384 / 512 instantiations, fp32),
+    against the tiled oracle cell like the default path."""
+    r = n // 64
+    ran = _tiled_against_oracle(inputs.sweep_drops(n=64), (r, r, r), 32, 20, "k_fused", path=4)
+    assert "k_step2" not in ran
+
+
 _jet192_ref = {}
 
 
