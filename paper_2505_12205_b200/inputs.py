@@ -192,11 +192,14 @@ def sweep_drops(n=64, seed=2505, ndrops=20, rmin=6.0, rmax=20.0, W=4.0, u_amp=0.
     z = (np.arange(nz, dtype=np.float64) if z_planes is None else np.asarray(z_planes, dtype=np.float64))[:, None, None]
     phi0 = np.zeros((z.shape[0], ny, nx))
     for k in range(ndrops):
+        dz = np.abs(z - cen[k, 2]); dz = np.minimum(dz, nz - dz)
+        near = dz[:, 0, 0] <= rad[k] + 10.0 * W      # beyond that tanh(2 (R - d) / W) == -1 exactly in fp64: the drop adds exactly 0
+        if not near.any():
+            continue
         dx = np.abs(x - cen[k, 0]); dx = np.minimum(dx, nx - dx)
         dy = np.abs(y - cen[k, 1]); dy = np.minimum(dy, ny - dy)
-        dz = np.abs(z - cen[k, 2]); dz = np.minimum(dz, nz - dz)
-        d = np.sqrt(dx * dx + dy * dy + dz * dz)
-        np.maximum(phi0, 0.5 + 0.5 * np.tanh(2.0 * (rad[k] - d) / W), out=phi0)
+        d = np.sqrt(dx * dx + dy * dy + dz[near] * dz[near])
+        phi0[near] = np.maximum(phi0[near], 0.5 + 0.5 * np.tanh(2.0 * (rad[k] - d) / W))
     if z_planes is None:
         u0 = rng.uniform(-u_amp, u_amp, size=(3, nz, ny, nx))
     else:

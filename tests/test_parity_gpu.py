@@ -606,3 +606,29 @@ def test_capillary_wave_against_prosperetti():
     assert abs(num.min() - ref.min()) < 0.05             # depth of the first trough (damping): measured -0.662 vs -0.681
     zc = lambda v: next(ts[i] + (ts[i + 1] - ts[i]) * v[i] / (v[i] - v[i + 1]) for i in range(len(v) - 1) if v[i] > 0 >= v[i + 1])
     assert abs(zc(num) / zc(ref) - 1) < 0.05             # first zero crossing (frequency): measured +3 %
+
+
+@pytest.mark.parametrize("which,extra", [("rt", ["--n", "64", "--steps", "400"]), ("jet", ["--n", "64", "--steps", "600"]),
+                                         ("jetpaper", ["--n", "64", "--case", "l", "--steps", "400"])])
+def test_long_run_diagnostics_at_reduced_size(which, extra):
+    """`bench.py --long-run` (the full-length runs of BASELINE configs[2] / configs[3] and of the paper's jet set-up recorded in
+    profiles/r02_long_runs.md) at a reduced size: the run stays finite, sum(phi) is conserved (RT) / grows by the nozzle's flux
+    (jet: d(sum phi)/dt within 2 % of disc nodes x U), and the diagnostics are there."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--long-run", which, *extra], capture_output=True, text=True,
+                         timeout=600, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    r = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert r["stable"] and r["steps_done"] == int(extra[-1]) and all(s["finite"] for s in r["series"])
+    if which == "rt":
+        assert abs(r["sum_phi_rel_drift"]) < 1e-4 and r["xz_asym_max"] < 0.05 and r["series"][-1]["u_max"] > 0
+    else:
+        f = r["inflow"]
+        assert abs(f["d_sum_phi_dt"] / f["disc_nodes_x_U"] - 1) < 0.02, f
+        assert r["series"][-1]["tip_z"] > 0
+        if which == "jetpaper":
+            assert r["breakup"]["case"] == "l" and r["params"]["g"][2] > 0 and r["params"]["bc"][:4] == [4, 4, 4, 4]
