@@ -632,3 +632,40 @@ def test_long_run_diagnostics_at_reduced_size(which, extra):
         assert r["series"][-1]["tip_z"] > 0
         if which == "jetpaper":
             assert r["breakup"]["case"] == "l" and r["params"]["g"][2] > 0 and r["params"]["bc"][:4] == [4, 4, 4, 4]
+
+
+def test_laplace_table3_on_the_gpu():
+    """The paper's stationary-drop test itself (Sec. 5.2, Table 3 :626-635) ON THE PRODUCT: 100^3 periodic, tau_d = tau_g
+    = 0.5, xi = 4, rho_d / rho_g = 1000, 50 000 iterations, fp64 (the oracle would need 14 h per case; the CUDA path is tied to it by
+    test_parity[drop32]).  Error of dp = p_in - p_out against 2 sigma / R (Eq. 44 in its 3-D form, reading G5), R from the drop volume, next
+    to the percentages the paper prints (tests/golden/paper_table3_laplace.txt).  The paper does not say how it measured p_in, p_out and R
+    (nor its mobility), so this is a RECORD with a loose gate, not a pin: measured 0.7-0.8 % at sigma = 0.01 (paper 0.33-1.04 %) and
+    1.9-2.7 % at sigma = 0.001 (paper 0.31-0.91 %; the runs are stationary: the same values at 200 000 steps), dp below 2 sigma / R."""
+    import os
+    import torch
+    from paper_2505_12205_b200 import clip
+    gold = {}
+    for line in open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_table3_laplace.txt")):
+        if not line.startswith("#"):
+            v = line.split()
+            gold[int(v[0])] = dict(zip((0.001, 0.005, 0.010), map(float, v[1:])))
+    n, W = 100, 4.0
+    z, y, x = np.meshgrid(*[np.arange(n, dtype=float)] * 3, indexing="ij")
+    r = np.sqrt((x - 49.5) ** 2 + (y - 49.5) ** 2 + (z - 49.5) ** 2)
+    errs = {}
+    for R in (15, 25, 35):
+        for sigma in (0.001, 0.010):
+            case = inputs.drop(n=n, R=float(R), W=W, sigma=sigma, rho_ratio=1000.0, tau=0.5, M=0.1)
+            sim = clip.Clip.from_case(case, precision=64)
+            sim.step(50000)
+            phi, p, u = (t.cpu().numpy() for t in sim.get())
+            torch.cuda.synchronize()
+            sim.close()
+            assert np.isfinite(p).all() and np.abs(u).max() < 1e-3
+            R_eff = (3 * phi.sum() / (4 * np.pi)) ** (1 / 3)
+            dp = p[r < R / 2].mean() - p[r > R + 2 * W].mean()
+            errs[(R, sigma)] = 100 * abs(dp / (2 * sigma / R_eff) - 1)
+            print(f"Laplace 100^3 R = {R} sigma = {sigma}: E = {errs[(R, sigma)]:.2f} % (paper {gold[R][sigma]:.2f} %), R_eff = {R_eff:.3f}, max |u| = {np.abs(u).max():.1e}")
+    for (R, sigma), e in errs.items():
+        assert e < 3.0, (R, sigma, e)                              # Laplace's law within 3 % at the paper's resolution
+        assert abs(e - gold[R][sigma]) < 2.5, (R, sigma, e)        # percentage points from the printed value
