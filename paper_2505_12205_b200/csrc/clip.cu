@@ -734,6 +734,11 @@ int clip_init(clip_t* h, const void* d_phi0, const void* d_u0) {
   if (!h) return CLIP_EINVAL;
   if (!d_phi0 || !d_u0) { set_err(h->err, "clip_init: NULL input"); return CLIP_EINVAL; }
   if (((uintptr_t)d_phi0) % 16 || ((uintptr_t)d_u0) % 16) { set_err(h->err, "clip_init: inputs must be 16-byte aligned"); return CLIP_EINVAL; }
+  if (h->overlap_open) {  // a step left open on the halo stream: order the new state after it
+    cudaEventRecord(h->ev_halo, h->halo_stream);
+    cudaStreamWaitEvent(h->stream, h->ev_halo, 0);
+    h->overlap_open = false;
+  }
   int rc = h->p.precision == 32 ? do_init<float>(h, d_phi0, d_u0) : do_init<double>(h, d_phi0, d_u0);
   if (rc == CLIP_OK) { h->inited = true; h->t = 0; }
   return rc;
@@ -754,6 +759,7 @@ int clip_step(clip_t* h, int n) {
   if (!h) return CLIP_EINVAL;
   if (!h->inited) { set_err(h->err, "clip_step: clip_init has not been called"); return CLIP_ESTATE; }
   if (n < 0) { set_err(h->err, "clip_step: n must be >= 0"); return CLIP_EINVAL; }
+  if (h->overlap_open) { set_err(h->err, "clip_step: an overlapped step is open (clip_step_halo_end missing)"); return CLIP_ESTATE; }
   return h->p.precision == 32 ? do_step<float>(h, n) : do_step<double>(h, n);
 }
 

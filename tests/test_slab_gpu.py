@@ -131,9 +131,17 @@ def test_overlapped_slab_step_equals_the_plain_sequence(precision):
             sl.close()
         for a, b in zip(*outs):
             assert torch.isfinite(a).all() and torch.equal(a, b), (path, shape)
+    case = inputs.sweep_drops(shape=(64, 16, 12), ndrops=3, rmin=3, rmax=4)
     sl = slab.SlabClip(64, 16, 12, dict(case["params"], precision=precision), 0, 1)
     from paper_2505_12205_b200 import clip
     assert clip.clip_step_halo_end(sl.sim._h, 0, 0, 0, 0) == clip.CLIP_ESTATE      # no open step
+    sl.init(torch.as_tensor(case["phi0"]), torch.as_tensor(case["u0"]))
+    sl.sim.step_halo_begin(sl.send_lo, sl.send_hi)
+    assert clip.clip_step(sl.sim._h, 1) == clip.CLIP_ESTATE                          # a step is open
+    assert clip.clip_step_halo_begin(sl.sim._h, sl.send_lo.data_ptr(), sl.send_hi.data_ptr()) == clip.CLIP_ESTATE
+    sl.sim.step_halo_end(sl.send_hi, sl.send_lo, sl.send_lo, sl.send_hi)
+    sl.sim.step(0)
+    torch.cuda.synchronize()
     sl.close()
 
 
