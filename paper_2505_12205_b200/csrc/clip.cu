@@ -152,6 +152,7 @@ const char* validate(int nx, int ny, int nz, const clip_params* p) {
   if (!p) return "params is NULL";
   if (nx < 1 || ny < 1 || nz < 1) return "nx, ny, nz must be >= 1";
   if ((double)nx * ny * nz > 2.0e9) return "lattice too large (nx*ny*nz must stay below 2e9)";
+  if (p && p->lattice == 1 && ny > 65535) return "D2Q9: ny must stay below 65536 (grid.y of the pair kernels)";
   if (p->precision != 32 && p->precision != 64) return "precision must be 32 or 64";
   if (!(p->rho_h > 0.0) || !(p->rho_l > 0.0)) return "densities must be positive";
   if (!(p->tau_h + 0.5 > 0.0) || !(p->tau_l + 0.5 > 0.0)) return "tau + 1/2 must be positive";
@@ -457,7 +458,13 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
     for (int pass = 0; pass < 2; ++pass) {  // pass 0: phi(t+1); pass 1: macros + collisions
       if (!fast) {
         if (prof) prof->begin();
-        if (h->p.lattice == 1) {  // D2Q9 (clip_d2q9.cuh)
+        if (h->p.lattice == 1 && h->nx % 2 == 0 && h->mode != 1) {  // D2Q9, pair-per-thread packed kernels (clip_d2q9.cuh)
+          int bx = 1;
+          while (bx < h->nx / 2 && bx < 128) bx *= 2;
+          const dim3 g9((h->nx / 2 + bx - 1) / bx, h->ny);
+          if (pass == 0) clip::d2q9::k_phi9p<T><<<g9, bx, 0, h->stream>>>(P);
+          else clip::d2q9::k_step9p<T><<<g9, bx, 0, h->stream>>>(P);
+        } else if (h->p.lattice == 1) {  // D2Q9, thread per node (odd nx, path 1)
           if (pass == 0) clip::d2q9::k_phi9<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
           else clip::d2q9::k_step9<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
         } else if (pass == 0) clip::k_phi<T><<<grid_for(P.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(P);

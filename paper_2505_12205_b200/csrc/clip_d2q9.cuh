@@ -215,3 +215,212 @@ __global__ void __launch_bounds__(256) k_get9(const __grid_constant__ KP<T> P, T
 
 }  // namespace d2q9
 }  // namespace clip
+
+// ------------------------------------------------------------------------------------------------------------------------------
+// Pair-per-thread D2Q9 kernels (even nx): one thread owns the node pair (x0, x0 + 1) of a row, two-lane packed arithmetic
+// (clip_pack.cuh: FFMA2 / FADD2 / FMUL2 in fp32), every wrap / bounce-back / free-slip case SELECTS the address of a load (as pull2 of
+// clip_fast.cuh).  Same two-kernel step as k_phi9 + k_step9; odd nx and `path = 1` keep the scalar kernels.
+#include "clip_pack.cuh"
+
+namespace clip {
+namespace d2q9 {
+
+struct Geo9 {
+  int x0, nx;
+  long long r0, rm, rp;     // population-row starts (element index of component 0, column 0) of the rows y, y-1, y+1 (periodic wrap)
+  int p0, pm, pp;           // phi-row starts of y and of the ghost-rule rows y-1, y+1 (wrap or clamp)
+  bool wm, wp;              // x0-1 / x0+2 wrap around
+  bool bxm, bxp, bym, byp;  // links that cross a WALL face
+  bool sxm, sxp, sym, syp;  // links that cross a FREESLIP face
+  int cxm, cxp;             // phi column offsets from x0 to x0-1 and x0+2 under the ghost rule
+};
+template <typename T> __device__ __forceinline__ Geo9 make_geo9(const KP<T>& P, int x0, int y) {
+  Geo9 g;
+  g.x0 = x0; g.nx = P.nx;
+  const int ym = y > 0 ? y - 1 : P.ny - 1, yp = y < P.ny - 1 ? y + 1 : 0;
+  g.r0 = (long long)y * NC9 * P.nx; g.rm = (long long)ym * NC9 * P.nx; g.rp = (long long)yp * NC9 * P.nx;
+  g.wm = x0 == 0; g.wp = x0 + 2 == P.nx;
+  g.bxm = g.wm && P.bc[0] == BC_WALL; g.sxm = g.wm && P.bc[0] == BC_FREESLIP;
+  g.bxp = g.wp && P.bc[1] == BC_WALL; g.sxp = g.wp && P.bc[1] == BC_FREESLIP;
+  g.bym = y == 0 && P.bc[2] == BC_WALL; g.sym = y == 0 && P.bc[2] == BC_FREESLIP;
+  g.byp = y == P.ny - 1 && P.bc[3] == BC_WALL; g.syp = y == P.ny - 1 && P.bc[3] == BC_FREESLIP;
+  g.p0 = y * P.nx;
+  g.pm = ((y == 0 && P.bc[2] != BC_PERIODIC) ? y : ym) * P.nx;
+  g.pp = ((y == P.ny - 1 && P.bc[3] != BC_PERIODIC) ? y : yp) * P.nx;
+  g.cxm = g.wm ? (P.bc[0] == BC_PERIODIC ? P.nx - 1 : 0) : -1;
+  g.cxp = g.wp ? (P.bc[1] == BC_PERIODIC ? 2 - P.nx : 1) : 2;
+  return g;
+}
+template <typename T, int a, int SET> __device__ __forceinline__ P2<T> pull9p(const T* __restrict__ src, const Geo9& g) {
+  const int nx = g.nx;
+  const long long rs = ey(a) == 1 ? g.rm : (ey(a) == -1 ? g.rp : g.r0);   // the row the population comes from
+  const T* __restrict__ rp = src + rs + (SET * Q9 + a) * nx + g.x0;
+  if (a == 0) return ld_pair<T>(rp);
+  const T* __restrict__ own = src + g.r0 + (SET * Q9 + opp9(a)) * nx + g.x0;
+  const bool rb = (ey(a) == 1 && g.bym) || (ey(a) == -1 && g.byp);
+  const bool ry = (ey(a) == 1 && g.sym) || (ey(a) == -1 && g.syp);
+  const T* __restrict__ srx = src + rs + (SET * Q9 + dir9(-ex(a), ey(a))) * nx + g.x0;   // x-reflected source
+  if (ey(a) != 0 && ry) {
+    rp = src + g.r0 + (SET * Q9 + dir9(ex(a), -ey(a))) * nx + g.x0;
+    srx = src + g.r0 + (SET * Q9 + dir9(-ex(a), -ey(a))) * nx + g.x0;
+  }
+  if (ex(a) == 0) return ld_pair<T>(rb ? own : rp);
+  const T* __restrict__ plo;
+  const T* __restrict__ phi;
+  if (ex(a) == 1) {
+    plo = rp + (g.wm ? nx - 1 : -1); phi = rp;
+    if (g.sxm) plo = srx;
+    if (g.bxm) plo = own;
+  } else {
+    plo = rp + 1; phi = rp + (g.wp ? 2 - nx : 2);
+    if (g.sxp) phi = srx + 1;
+    if (g.bxp) phi = own + 1;
+  }
+  if (rb) { plo = own; phi = own + 1; }
+  return P2<T>(ld_one<T>(plo), ld_one<T>(phi));
+}
+template <typename T, int SET, int a = 0> struct Pull9p {
+  static __device__ __forceinline__ void run(const T* __restrict__ src, const Geo9& g, P2<T> (&v)[Q9]) {
+    v[a] = pull9p<T, a, SET>(src, g);
+    Pull9p<T, SET, a + 1>::run(src, g, v);
+  }
+};
+template <typename T, int SET> struct Pull9p<T, SET, Q9> { static __device__ __forceinline__ void run(const T* __restrict__, const Geo9&, P2<T> (&)[Q9]) {} };
+
+template <typename T> struct Row3p { P2<T> L, C, R; };
+template <typename T> __device__ __forceinline__ Row3p<T> ld_row3p(const T* __restrict__ phi, int row, const Geo9& g) {
+  Row3p<T> r;
+  r.C = ld_pair<T>(phi + row + g.x0);
+  const T m = ld_one<T>(phi + row + g.x0 + g.cxm), p = ld_one<T>(phi + row + g.x0 + g.cxp);
+  r.L = P2<T>(m, r.C.lo());
+  r.R = P2<T>(r.C.hi(), p);
+  return r;
+}
+template <typename T> __device__ __forceinline__ void stencil9p(const T* __restrict__ phi, const Geo9& g, P2<T>& pc, P2<T> (&G)[2], P2<T>& L) {
+  typedef P2<T> V;
+  const Row3p<T> c = ld_row3p<T>(phi, g.p0, g), yp = ld_row3p<T>(phi, g.pp, g), ym = ld_row3p<T>(phi, g.pm, g);
+  pc = c.C;
+  const V d1 = c.R - pc, d2 = c.L - pc, d3 = yp.C - pc, d4 = ym.C - pc;
+  const V d5 = yp.R - pc, d6 = ym.L - pc, d7 = ym.R - pc, d8 = yp.L - pc;
+  L = fma2(V(T(6.0 / 9.0)), (d1 + d2) + (d3 + d4), V(T(6.0 / 36.0)) * ((d5 + d6) + (d7 + d8)));
+  G[0] = fma2(V(T(3.0 / 9.0)), d1 - d2, V(T(3.0 / 36.0)) * ((d5 - d6) + (d7 - d8)));
+  G[1] = fma2(V(T(3.0 / 9.0)), d3 - d4, V(T(3.0 / 36.0)) * ((d5 - d6) - (d7 - d8)));
+}
+
+template <typename T> struct Mom9p { P2<T> p, mx, my, xx, yy, xy; };
+template <typename T> __device__ __forceinline__ Mom9p<T> moments9p(const P2<T> (&f)[Q9]) {
+  typedef P2<T> V;
+  Mom9p<T> m;
+  const V s12 = f[1] + f[2], s34 = f[3] + f[4], s56 = f[5] + f[6], s78 = f[7] + f[8];
+  const V d12 = f[1] - f[2], d34 = f[3] - f[4], d56 = f[5] - f[6], d78 = f[7] - f[8];
+  m.p = (f[0] + (s12 + s34)) + (s56 + s78);
+  m.mx = d12 + (d56 + d78);
+  m.my = d34 + (d56 - d78);
+  m.xx = s12 + (s56 + s78);
+  m.yy = s34 + (s56 + s78);
+  m.xy = s56 - s78;
+  return m;
+}
+template <typename T> struct Mat9p { P2<T> rho, inv_rho, tau, s_nu, mu; };
+template <typename T> __device__ __forceinline__ Mat9p<T> materials9p(const KP<T>& P, P2<T> phi, P2<T> L) {
+  typedef P2<T> V;
+  Mat9p<T> m;
+  m.rho = fma2(phi, V(P.drho), V(P.rho_l));
+  m.inv_rho = rcp2(m.rho);
+  if (P.visc_interp == 1) m.tau = rcp2(fma2(phi, V(P.itau_h - P.itau_l), V(P.itau_l)));
+  else if (P.visc_interp == 2) m.tau = fma2(phi, V(P.rt_h - P.rt_l), V(P.rt_l)) * m.inv_rho;
+  else m.tau = fma2(phi, V(P.tau_h - P.tau_l), V(P.tau_l));
+  m.s_nu = rcp2(m.tau + V(T(0.5)));
+  m.mu = fms2(V(P.beta4) * phi, (phi - V(T(1))) * (phi - V(T(0.5))), V(P.kappa) * L);
+  return m;
+}
+template <typename T>
+__device__ __forceinline__ void force9p(const KP<T>& P, const Mom9p<T>& m, const Mat9p<T>& mat, P2<T> ux, P2<T> uy, const P2<T> (&G)[2],
+                                        P2<T> (&F)[2], P2<T> (&D)[2]) {
+  typedef P2<T> V;
+  const V p3 = m.p * V(T(1.0 / 3.0));
+  const V nxx = m.xx - fma2(ux, ux, p3), nyy = m.yy - fma2(uy, uy, p3), nxy = m.xy - ux * uy;
+  const V tr2 = V(T(0.5)) * (nxx + nyy);
+  D[0] = nxx - tr2; D[1] = nxy;
+  const V s = mat.s_nu;
+  const V trs = P.collision == 1 ? s * tr2 : tr2;
+  const V Sxx = fma2(s, D[0], trs), Syy = trs - s * D[0], Sxy = s * D[1];
+  const V cmu = -(mat.tau * V(P.drho));
+  const V cs = mat.mu - p3 * V(P.drho);
+  const V rb = mat.rho - V(P.rho_ref);
+  F[0] = fma2(cs, G[0], fma2(rb, V(P.gx), cmu * fma2(Sxx, G[0], Sxy * G[1])));
+  F[1] = fma2(cs, G[1], fma2(rb, V(P.gy), cmu * fma2(Sxy, G[0], Syy * G[1])));
+}
+template <typename T>
+__device__ __forceinline__ void collide9p(const KP<T>& P, const Mom9p<T>& m, const Mat9p<T>& mat, P2<T> phi, const P2<T> (&G)[2], P2<T> ux,
+                                          P2<T> uy, P2<T> (&f)[Q9], P2<T> (&g)[Q9]) {
+  typedef P2<T> V;
+  V F[2] = {V(T(0)), V(T(0))}, D[2] = {V(T(0)), V(T(0))};
+  if (!P.phase_only) force9p(P, m, mat, ux, uy, G, F, D);
+  const V usq15 = V(T(1.5)) * fma2(ux, ux, uy * uy);
+  const V ir15 = V(T(1.5)) * mat.inv_rho;
+  const V hx = F[0] * ir15, hy = F[1] * ir15;
+  const V k = V(T(4.5)) * (V(T(1)) - mat.s_nu);
+  const V gn = sqrt2(fma2(G[0], G[0], G[1] * G[1])) + V(T(1e-32));
+  const V ph = phi - V(T(0.5));
+  const V pref = fma2(V(T(-4)) * ph, ph, V(T(1))) * V(P.inv_W);
+  const V cphi = (V(T(1) - T(0.5) * P.om_phi) * pref) * rcp2(gn);
+  const V nx_ = G[0] * cphi, ny_ = G[1] * cphi;
+  const V omphi = V(P.om_phi) * phi, om1 = V(T(1) - P.om_phi);
+#pragma unroll
+  for (int a = 0; a < Q9; ++a) {
+    const V cx_ = V(T(ex(a))), cy_ = V(T(ey(a)));
+    const V eu = fma2(cx_, ux, cy_ * uy);
+    const V gam = fma2(V(T(4.5)) * eu, eu, fma2(V(T(3)), eu, -usq15));
+    const V eDe = fma2(V(T(ex(a) * ex(a) - ey(a) * ey(a))), D[0], V(T(2 * ex(a) * ey(a))) * D[1]);
+    const V eh = fma2(cx_, hx, cy_ * hy);
+    const V w(w9<T>(a));
+    if (P.phase_only) f[a] = V(T(0));
+    else if (P.collision == 1) f[a] = fma2(V(T(1)) - mat.s_nu, f[a], w * fma2(mat.s_nu, m.p + gam, (V(T(2)) - mat.s_nu) * eh));
+    else f[a] = w * ((m.p + gam) + fma2(k, eDe, eh));
+    g[a] = fma2(om1, g[a], w * fma2(omphi, V(T(1)) + gam, fma2(cx_, nx_, cy_ * ny_)));
+  }
+}
+template <typename T> __device__ __forceinline__ bool pair9_coords(const KP<T>& P, int& x0, int& y) {
+  x0 = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
+  y = blockIdx.y;
+  return x0 < P.nx;
+}
+// grid = (ceil(nx / 2 / blockDim.x), ny)
+template <typename T> __global__ void __launch_bounds__(128) k_phi9p(const __grid_constant__ KP<T> P) {
+  int x0, y;
+  if (!pair9_coords(P, x0, y)) return;
+  const Geo9 g = make_geo9(P, x0, y);
+  P2<T> v[Q9];
+  Pull9p<T, 1>::run(P.p_src, g, v);
+  st_pair<T>(P.phi + g.p0 + x0, (v[0] + ((v[1] + v[2]) + (v[3] + v[4]))) + ((v[5] + v[6]) + (v[7] + v[8])));
+}
+template <typename T> __global__ void __launch_bounds__(128) k_step9p(const __grid_constant__ KP<T> P) {
+  typedef P2<T> V;
+  int x0, y;
+  if (!pair9_coords(P, x0, y)) return;
+  const Geo9 geo = make_geo9(P, x0, y);
+  V f[Q9], g[Q9];
+  Pull9p<T, 0>::run(P.p_src, geo, f);
+  Pull9p<T, 1>::run(P.p_src, geo, g);
+  const int i = geo.p0 + x0;
+  V ux = ld_pair<T>(P.u + i), uy = ld_pair<T>(P.u + P.n + i);
+  V phi, G[2], L;
+  stencil9p<T>(P.phi, geo, phi, G, L);
+  const Mat9p<T> mat = materials9p<T>(P, phi, L);
+  const Mom9p<T> m = moments9p<T>(f);
+  if (!P.phase_only) {  // macros, Alg. 3 (lagged u, R13), then Eq. 31b
+    V F[2], D[2];
+    force9p(P, m, mat, ux, uy, G, F, D);
+    const V h = V(T(0.5)) * mat.inv_rho;
+    ux = fma2(h, F[0], m.mx); uy = fma2(h, F[1], m.my);
+    st_pair<T>(P.u + i, ux); st_pair<T>(P.u + P.n + i, uy);
+  }
+  collide9p<T>(P, m, mat, phi, G, ux, uy, f, g);
+  T* const rd = P.p_dst + geo.r0 + x0;
+#pragma unroll
+  for (int a = 0; a < Q9; ++a) { st_pair<T>(rd + a * P.nx, f[a]); st_pair<T>(rd + (Q9 + a) * P.nx, g[a]); }
+}
+
+}  // namespace d2q9
+}  // namespace clip
