@@ -383,6 +383,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
   dim3 fg, fb;
   if (fast) fast_shape(h, fg, fb);
   const bool fused = use_fused(h);
+  const bool plain = h->p.collision == CLIP_COLL_WMRT && !h->p.phase_only;   // k_step<T, true>: no mode tests in the direction loop
   for (int s = 0; s < nsteps; ++s) {
     clip::KP<T> P = make_kp<T>(h);
     if (fused) {  // one pass over f and g (clip_fused.cuh) + the tile-surface fix-up of phi(t+2)
@@ -399,7 +400,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
         clip::KP<T> Q = F.k;
         Q.z_lo = side ? h->nz - 1 : 0; Q.z_cnt = 1;
         if (prof) prof->begin();
-        clip::k_step<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Q);
+        clip::k_step<T, true><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Q);   // the k_fused path is WMRT, two-phase
         if (prof) prof->end(KIND_STEP);
         h->launches += 1;
       }
@@ -468,6 +469,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
           if (pass == 0) clip::d2q9::k_phi9<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
           else clip::d2q9::k_step9<T><<<grid_for(P.n, 256), 256, 0, h->stream>>>(P);
         } else if (pass == 0) clip::k_phi<T><<<grid_for(P.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(P);
+        else if (plain) clip::k_step<T, true><<<grid_for(P.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(P);
         else clip::k_step<T><<<grid_for(P.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(P);
         h->launches += 1;
         if (prof) prof->end(pass == 0 ? KIND_PHI : KIND_STEP);
@@ -478,6 +480,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
         const clip::KP<T>& Q = side ? Phi : Plo;
         if (prof) prof->begin();
         if (pass == 0) clip::k_phi<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Q);
+        else if (plain) clip::k_step<T, true><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Q);
         else clip::k_step<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Q);
         h->launches += 1;
         if (prof) prof->end(pass == 0 ? KIND_PHI : KIND_STEP);

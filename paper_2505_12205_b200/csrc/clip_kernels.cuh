@@ -351,11 +351,12 @@ __device__ __forceinline__ void total_force(const KP<T>& P, const Mom<T>& m, con
 }
 
 // Both collisions of one node (Alg. 1): in f, g pre-collision; out post-collision in place.
-template <typename T>
+// PLAIN: the caller guarantees WMRT collision and the full two-phase mode (no runtime mode tests inside the direction loop)
+template <typename T, bool PLAIN = false>
 __device__ __forceinline__ void collide(const KP<T>& P, const Mom<T>& m, const Mat<T>& mat, T phi, const T (&G)[3], T ux,
                                         T uy, T uz, T (&f)[Q], T (&g)[Q]) {
   T F[3] = {T(0), T(0), T(0)}, D[6] = {T(0), T(0), T(0), T(0), T(0), T(0)};
-  if (!P.phase_only) total_force(P, m, mat, ux, uy, uz, G, F, D);
+  if (PLAIN || !P.phase_only) total_force(P, m, mat, ux, uy, uz, G, F, D);
   const T usq15 = T(1.5) * (ux * ux + uy * uy + uz * uz);
   const T hx = T(1.5) * F[0] * mat.inv_rho, hy = T(1.5) * F[1] * mat.inv_rho, hz = T(1.5) * F[2] * mat.inv_rho;
   const T k = T(4.5) * (T(1) - mat.s_nu);
@@ -373,9 +374,9 @@ __device__ __forceinline__ void collide(const KP<T>& P, const Mom<T>& m, const M
     const T eu = ex * ux + ey * uy + ez * uz;
     const T gam = T(3) * eu + T(4.5) * eu * eu - usq15;  // Gamma_a / w_a - 1
     const T eDe = ex * ex * D[0] + ey * ey * D[1] + ez * ez * D[2] + T(2) * (ex * ey * D[3] + ey * ez * D[4] + ex * ez * D[5]);
-    if (P.phase_only)  // prescribed u (Sec. 5.4): the hydrodynamic populations are not advanced
+    if (!PLAIN && P.phase_only)  // prescribed u (Sec. 5.4): the hydrodynamic populations are not advanced
       f[a] = T(0);
-    else if (P.collision == 1)  // BGK, Eq. 26: f+ = (1 - s) f + s feq_bar + F_a
+    else if (!PLAIN && P.collision == 1)  // BGK, Eq. 26: f+ = (1 - s) f + s feq_bar + F_a
       f[a] = (T(1) - mat.s_nu) * f[a] + cw<T>(a) * (mat.s_nu * (m.p + gam) + (T(2) - mat.s_nu) * (ex * hx + ey * hy + ez * hz));
     else
       f[a] = cw<T>(a) * ((m.p + gam) + (ex * hx + ey * hy + ez * hz) + k * eDe);
@@ -458,7 +459,7 @@ template <typename T> __global__ void __launch_bounds__(256) k_phi(const __grid_
 }
 
 // k_step: the fused stream -> BC -> macro -> collide kernel.
-template <typename T> __global__ void __launch_bounds__(256) k_step(const __grid_constant__ KP<T> P) {
+template <typename T, bool PLAIN = false> __global__ void __launch_bounds__(256) k_step(const __grid_constant__ KP<T> P) {
   const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= P.z_cnt * P.nxy) return;
   const long long i = j + P.z_lo * P.nxy;
@@ -479,7 +480,7 @@ template <typename T> __global__ void __launch_bounds__(256) k_step(const __grid
   const Mom<T> m = moments(f);
   // macros, Alg. 3: F from (new p*, new phi, lagged u), then Eq. 31b
   T ux = P.u[i], uy = P.u[P.n + i], uz = P.u[2 * P.n + i];
-  if (!P.phase_only) {
+  if (PLAIN || !P.phase_only) {
     T F[3], D[6];
     total_force(P, m, mat, ux, uy, uz, G, F, D);
     const T h = T(0.5) * mat.inv_rho;
@@ -487,7 +488,7 @@ template <typename T> __global__ void __launch_bounds__(256) k_step(const __grid
   }
   if (P.has_inlet && z == 0 && P.mask[(long long)y * P.nx + x]) { ux = P.uin[0]; uy = P.uin[1]; uz = P.uin[2]; }
   P.u[i] = ux; P.u[P.n + i] = uy; P.u[2 * P.n + i] = uz;
-  collide(P, m, mat, phi, G, ux, uy, uz, f, g);
+  collide<T, PLAIN>(P, m, mat, phi, G, ux, uy, uz, f, g);
   StoreAll<T>::run(P.p_dst, P.nx, pop_base(i, x), f);
   StoreAll<T>::run(P.p_dst + Q * P.nx, P.nx, pop_base(i, x), g);
 }
