@@ -486,7 +486,19 @@ def run_long(args):
                 D = 2.0 * pr["inlet_r"]
                 al = [r["attached_len"] for r in series]
                 peaks = [al[k] for k in range(1, len(al) - 1) if al[k] >= al[k - 1] and al[k + 1] < al[k] - 0.5 * D]
-                out["breakup"] = {"D": D, "pinch_offs": len(peaks), "L_b_over_D": [v / D for v in peaks],
+                # drop sizes ("equilibrium droplet diameter d_e", Fig. 18c): connected components of phi > 1/2 in the final field
+                # that do not touch the inlet plane; d_e = (6 V / pi)^(1/3), V = sum of phi over the component (host side, scipy)
+                drops = []
+                try:
+                    from scipy import ndimage
+                    ph = phi.float().cpu().numpy()
+                    lab, ncomp = ndimage.label(ph > 0.5)
+                    attached = set(lab[0][lab[0] > 0].ravel().tolist())
+                    vol = ndimage.sum_labels(ph, lab, index=range(1, ncomp + 1))
+                    drops = sorted(((6.0 * float(v) / 3.141592653589793) ** (1.0 / 3.0) / D for k, v in enumerate(vol, start=1) if k not in attached and v > 30.0), reverse=True)
+                except Exception as e:  # diagnostics only
+                    drops = [f"unavailable: {e}"]
+                out["breakup"] = {"D": D, "pinch_offs": len(peaks), "L_b_over_D": [v / D for v in peaks], "detached_drops_d_e_over_D": drops,
                                   "L_b_over_D_mean": (sum(peaks) / len(peaks) / D) if peaks else None, "t_star_end": done * pr["inlet_u"][2] / D,
                                   "case": args.case, "Re_We_Fr": inputs.JET_TABLE6[args.case]}
             pre = [r for r in series if r["outlet_phi_max"] < 0.01]
