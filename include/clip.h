@@ -104,7 +104,8 @@ int clip_init(clip_t* h, const void* d_phi0, const void* d_u0);
  * on the other lattices with even nx, the generic k_phi + k_step otherwise (and on the planes next to an INLET / OUTLET face).
  * All paths compute the same step; they agree to round-off, and each is deterministic: clip_step(a); clip_step(b) equals
  * clip_step(a + b) bit for bit.  clip_params.path / tile_ty / tile_chunks / runtime_nx override the choice (tests, tuning); the
- * library reads nothing from the environment. */
+ * library reads nothing from the environment.  On lattices of up to 4 M nodes (launch-bound), n >= 32 and a stream that can be captured
+ * (not the legacy default stream), the steps are replayed 16 at a time from a CUDA graph the handle captures once. */
 int clip_step(clip_t* h, int n);
 
 /* phase_only mode: prescribe the velocity field u [3][nz][ny][nx] (device) that the following collisions use; the
@@ -167,6 +168,9 @@ const char* clip_last_error(const clip_t* h);
 
 /* Number of kernel launches the handle has enqueued so far (instrumentation for bench.py's gpu_launches). */
 long long clip_launch_count(const clip_t* h);
+
+/* Number of time steps the handle has run by replaying its CUDA graph (instrumentation; see clip_step). */
+long long clip_graph_steps(const clip_t* h);
 
 /* Instrumentation for bench.py's roofline: like clip_step(h, n), but every kernel launch is bracketed by CUDA
  * events on the handle's stream; after synchronising the stream (this call is host-synchronous) the elapsed

@@ -82,6 +82,8 @@ def lib():
         L.clip_last_error.argtypes = [C.c_void_p]
         L.clip_launch_count.restype = C.c_longlong
         L.clip_launch_count.argtypes = [C.c_void_p]
+        L.clip_graph_steps.restype = C.c_longlong
+        L.clip_graph_steps.argtypes = [C.c_void_p]
         L.clip_step_profiled.restype = C.c_int
         L.clip_step_profiled.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.clip_kernel_kinds.restype = C.c_int
@@ -142,6 +144,10 @@ def clip_last_error(h=None) -> str:
 
 def clip_launch_count(h) -> int:
     return int(lib().clip_launch_count(h))
+
+
+def clip_graph_steps(h) -> int:
+    return int(lib().clip_graph_steps(h))
 
 
 def clip_halo_bytes(h) -> int:
@@ -304,6 +310,10 @@ class Clip:
     @property
     def launches(self) -> int:
         return clip_launch_count(self._h)
+
+    @property
+    def graph_steps(self) -> int:
+        return clip_graph_steps(self._h)
 
     def close(self):
         if getattr(self, "_h", None):

@@ -212,6 +212,10 @@ struct clip_handle {
   cudaEvent_t ev_start, ev_bnd, ev_halo;
   bool overlap_open;         // between clip_step_halo_begin and clip_step_halo_end
   bool split_done;           // the last do_step packed the records itself (split launch)
+  cudaGraphExec_t gexec;     // GRAPH_STEPS time steps of a small lattice captured as one CUDA graph (step_graphed); nullptr: none
+  bool graph_tried;
+  long long graph_launches;  // kernel launches inside one replay
+  long long graph_steps;     // time steps run by graph replays so far (instrumentation)
   FusedPlan fplan;
   bool inited;
   int mode;            // clip_params.path: 0 = automatic (k_fused + k_fix on wide lattices, else k_phi2 + k_step2), 1 = generic kernels
@@ -596,6 +600,49 @@ k_halo_unpack(const __grid_constant__ clip::KP<T> P, const T* recv_lo, const T* 
   if (side ? add_hi : add_lo) phi_next[ib] += recv[11 * P.nxy + c];
 }
 
+// Small lattices are launch-bound (64^3: two launches of ~5 and ~10 us per step): clip_step(n) replays GRAPH_STEPS steps as ONE CUDA
+// graph (SURVEY.md:121).  The A/B buffers return to the same roles after an even number of steps, so one graph captured at parity 0
+// serves every replay; kernel parameters (device pointers into the caller's workspace, sizes) are frozen in it.  Only on a stream that
+// can be captured (not the legacy default stream, not a stream the caller is capturing), without HALO faces, up to 4 M nodes.
+constexpr int GRAPH_STEPS = 16;
+bool graph_eligible(const clip_handle* h) {
+  if ((long long)h->nx * h->ny * h->nz > (1LL << 22)) return false;
+  if (h->p.bc[4] == CLIP_BC_HALO || h->p.bc[5] == CLIP_BC_HALO) return false;
+  if (h->stream == nullptr || h->stream == cudaStreamLegacy || h->stream == cudaStreamPerThread) return false;
+  cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(h->stream, &st) != cudaSuccess) { cudaGetLastError(); return false; }
+  return st == cudaStreamCaptureStatusNone;
+}
+template <typename T> int step_graphed(clip_handle* h, int n) {
+  if (n < 2 * GRAPH_STEPS || (h->graph_tried && !h->gexec) || !graph_eligible(h)) return do_step<T>(h, n);
+  // reach the state the graph is (to be) captured in: buffer parity 0 and, on the k_fused path, phi(t+1) in place
+  while (n > 0 && (h->cur != 0 || (use_fused(h) && !h->phi_ahead))) {
+    const int rc = do_step<T>(h, 1);
+    if (rc != CLIP_OK) return rc;
+    --n;
+  }
+  if (!h->gexec && n >= GRAPH_STEPS) {
+    h->graph_tried = true;
+    const long long t0 = h->t, l0 = h->launches;
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+      const int rc = do_step<T>(h, GRAPH_STEPS);     // recorded, not run: the host-side counters are put back below
+      const cudaError_t e = cudaStreamEndCapture(h->stream, &graph);
+      h->graph_launches = h->launches - l0;
+      h->t = t0; h->launches = l0;                   // cur / phi_cur are back at parity 0 after an even number of steps
+      if (rc == CLIP_OK && e == cudaSuccess && graph && cudaGraphInstantiate(&h->gexec, graph, 0) != cudaSuccess) h->gexec = nullptr;
+      if (graph) cudaGraphDestroy(graph);
+    }
+    cudaGetLastError();  // a failed capture is not an error of the step: plain launches follow
+  }
+  while (h->gexec && n >= GRAPH_STEPS) {
+    if (cudaGraphLaunch(h->gexec, h->stream) != cudaSuccess) { set_err(h->err, "clip_step: graph launch: %s", cudaGetErrorString(cudaGetLastError())); return CLIP_ECUDA; }
+    h->t += GRAPH_STEPS; h->launches += h->graph_launches; h->graph_steps += GRAPH_STEPS;
+    n -= GRAPH_STEPS;
+  }
+  return do_step<T>(h, n);
+}
+
 }  // namespace
 
 extern "C" {
@@ -716,6 +763,7 @@ int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params,
   h->stream = (cudaStream_t)cuda_stream; h->cur = 0; h->phi_cur = 0; h->phi_ahead = false; h->inited = false;
   h->phi_partial[0] = h->phi_partial[1] = false;
   h->halo_stream = nullptr; h->ev_start = h->ev_bnd = h->ev_halo = nullptr; h->overlap_open = false; h->split_done = false;
+  h->gexec = nullptr; h->graph_tried = false; h->graph_launches = 0; h->graph_steps = 0;
   h->zlo = params->bc[4] == CLIP_BC_HALO ? 1 : 0; h->zhi = nz - (params->bc[5] == CLIP_BC_HALO ? 1 : 0);
   h->fplan = fused_plan(nx, ny, nz, params);
   h->mode = params->path;
@@ -770,7 +818,7 @@ int clip_step(clip_t* h, int n) {
   if (!h->inited) { set_err(h->err, "clip_step: clip_init has not been called"); return CLIP_ESTATE; }
   if (n < 0) { set_err(h->err, "clip_step: n must be >= 0"); return CLIP_EINVAL; }
   if (h->overlap_open) { set_err(h->err, "clip_step: an overlapped step is open (clip_step_halo_end missing)"); return CLIP_ESTATE; }
-  return h->p.precision == 32 ? do_step<float>(h, n) : do_step<double>(h, n);
+  return h->p.precision == 32 ? step_graphed<float>(h, n) : step_graphed<double>(h, n);
 }
 
 int clip_step_profiled(clip_t* h, int n, double* ms, long long* count) {
@@ -808,6 +856,7 @@ int clip_destroy(clip_t* h) {
   if (!h) return CLIP_EINVAL;
   if (!h->mask_host.empty()) cudaStreamSynchronize(h->stream);  // the mask upload reads host memory we own
   if (h->ev_start) { cudaEventDestroy(h->ev_start); cudaEventDestroy(h->ev_bnd); cudaEventDestroy(h->ev_halo); }
+  if (h->gexec) cudaGraphExecDestroy(h->gexec);
   delete h;
   return CLIP_OK;
 }
@@ -815,5 +864,6 @@ int clip_destroy(clip_t* h) {
 const char* clip_last_error(const clip_t* h) { return h ? h->err : g_create_error; }
 
 long long clip_launch_count(const clip_t* h) { return h ? h->launches : 0; }
+long long clip_graph_steps(const clip_t* h) { return h ? h->graph_steps : 0; }
 
 }  // extern "C"

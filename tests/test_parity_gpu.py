@@ -461,6 +461,32 @@ def test_fused_tma_path(precision):
                 assert np.abs(a - b).max() <= tol * max(1.0, np.abs(a).max()), (case["name"], over)
 
 
+@pytest.mark.parametrize("precision", [64, 32])
+def test_graph_replay_of_small_lattices_is_exact(precision):
+    """clip_step(n) on a launch-bound lattice and a capturable stream replays 16 steps at a time from a CUDA graph (clip.h): the fields
+    must equal the plain launches (legacy default stream: no graph) bit for bit, also across several clip_step calls and with an
+    odd number of leading steps; pair kernels, k_fused (phi one step ahead), jet replica (generic planes, outlet lambda kernel)."""
+    import torch
+    from paper_2505_12205_b200 import clip
+    cases = [(inputs.sweep_drops(n=32, ndrops=3, rmin=3, rmax=6), {}), (inputs.sweep_drops(shape=(64, 16, 12), ndrops=4, rmin=3, rmax=5), {"path": 3}),
+             (inputs.jet(nxy=24, nz=32, r_nozzle=4.0), {}), (inputs.sweep_drops(shape=(21, 12, 10), ndrops=3, rmin=3, rmax=4), {})]
+    for case, over in cases:
+        c = dict(case, params=dict(case["params"], **over))
+        ref = _gpu(c, 150, precision)
+        params = dict(c["params"], precision=precision)
+        side = torch.cuda.Stream()
+        sim = clip.Clip(c["nx"], c["ny"], c["nz"], params, stream=side)
+        sim.init(torch.as_tensor(c["phi0"]), torch.as_tensor(c["u0"]))
+        sim.step(3); sim.step(100); sim.step(5); sim.step(42)
+        out = sim.get()
+        side.synchronize()
+        got = [t.double().cpu().numpy() for t in out]
+        assert sim.graph_steps >= 112, (case["name"], sim.graph_steps)      # 96 of the 100 and 32 of the 42, or the like
+        sim.close()
+        for a, b in zip(ref, got):
+            assert np.array_equal(a, b), case["name"]
+
+
 def test_fused_path_is_deterministic_at_full_size():
     """k_fused keeps phi's partial sums in a shared-memory ring that warps of a block fill and flush at different times
     (one barrier per plane, warp-edge sends through side arrays) and hands tile halos over through `part`: any race would
