@@ -590,7 +590,8 @@ def test_phase_only_prescribed_velocity(precision):
     sim.close()
 
 
-def test_capillary_wave_against_prosperetti():
+@pytest.mark.parametrize("lattice", [0, 1], ids=["d3q19_nz1", "d2q9"])
+def test_capillary_wave_against_prosperetti(lattice):
     """SURVEY 8(f) NEXT-4, the paper's Sec. 5.1 validation ON THE PRODUCT at the paper's own resolution (256 x 512, D3Q19
     with nz = 1; free-slip sides, no-slip top / bottom; nu = 0.005, sigma = 1e-4, xi = 4, M = 0.02, eta0 = 0.02 L0;
     PAPER.md:559-595): two periods (343 000 steps) of the interface amplitude eta(t) (Eq. 43: linear interpolation of the
@@ -603,6 +604,7 @@ def test_capillary_wave_against_prosperetti():
     from paper_2505_12205_b200 import clip
     L0, nu = 256, 0.005
     case = inputs.capillary_wave(L0=L0, nu=nu)
+    case["params"]["lattice"] = lattice        # 1: the paper's own lattice for this test (D2Q9)
     pr = case["params"]
     k = 2 * np.pi / L0
     w0 = np.sqrt(pr["sigma"] * k ** 3 / (pr["rho_h"] + pr["rho_l"]))
@@ -627,7 +629,7 @@ def test_capillary_wave_against_prosperetti():
     ts, num = np.array(ts), np.array(eta) / eta[0]
     ref = cf.prosperetti_capillary_wave(ts, nu, k, pr["sigma"], pr["rho_h"], pr["rho_l"])
     err, rms = np.abs(num - ref).max(), np.sqrt(((num - ref) ** 2).mean())
-    print(f"capillary wave 256x512, nu = {nu}: max |eta* - Prosperetti| = {err:.3f}, rms = {rms:.3f}; first trough {num.min():.3f} vs {ref.min():.3f}")
+    print(f"capillary wave 256x512 ({'D2Q9' if lattice else 'D3Q19 nz = 1'}), nu = {nu}: max |eta* - Prosperetti| = {err:.3f}, rms = {rms:.3f}; first trough {num.min():.3f} vs {ref.min():.3f}")
     assert err < 0.15 and rms < 0.09                     # measured 0.098 / 0.060 (a ~3 % phase lag accumulates over two periods)
     assert abs(num.min() - ref.min()) < 0.05             # depth of the first trough (damping): measured -0.662 vs -0.681
     zc = lambda v: next(ts[i] + (ts[i + 1] - ts[i]) * v[i] / (v[i] - v[i + 1]) for i in range(len(v) - 1) if v[i] > 0 >= v[i + 1])
