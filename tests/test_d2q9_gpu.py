@@ -176,3 +176,35 @@ def test_shear_interface_table4_on_the_gpu():
     mass = float(phi.sum() / phi0.sum() - 1.0)
     print(f"shear interface on the GPU (D2Q9, 200^2, 10 000 steps): Eq. 50 error {err:.6e} (oracle {err_gold:.6e}); phi = 1 outside: {err * np.sqrt(s_in / s_out):.3e} (paper 8.58e-3); mass drift {mass:.1e}")
     assert abs(err / err_gold - 1) < 1e-6 and abs(mass) < 1e-11
+
+
+@pytest.mark.parametrize("rho_ratio", [10.0, 1000.0])
+def test_poiseuille_paper_cases_on_the_gpu(rho_ratio):
+    """The paper's own two-phase Poiseuille cases (Sec. 5.3, Fig. 11a / 11b: 2-D, 64 nodes across, rho* = 10 and 1000,
+    mu* = 100, F_b = rho g) ON THE PRODUCT (D2Q9, fp64) to steady state, against the quadrature of Eq. 45 with the smoothed rho(y), mu(y)
+    of the run (the paper compares with a finite-difference solution of the same equation, :655-660).  rho* = 1000 is beyond what the
+    oracle pins (rho* = 10): reported and gated at 3 %."""
+    import os
+    import sys
+    import torch
+    sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+    import closed_forms as cf
+    from paper_2505_12205_b200 import clip
+    tau_b = 0.5                                        # the light fluid (PAPER.md Fig. 11c: tau_L = 0.5)
+    tau_a = tau_b * 100.0 / rho_ratio                  # mu* = rho* tau_A / tau_B = 100
+    case = inputs.poiseuille2d(nx=4, ny=64, tau_a=tau_a, tau_b=tau_b, rho_a=rho_ratio, rho_b=1.0, gx=1e-7 / rho_ratio * 10.0)
+    sim = clip.Clip.from_case(case, precision=64)
+    du, steps = 1.0, 0
+    while steps < 600000 and du > 1e-13:
+        sim.step(1999); prev = sim.get()[2].clone(); sim.step(1); steps += 2000
+        du = float((sim.get()[2] - prev).abs().max())
+    phi, p, u = (t.cpu().numpy() for t in sim.get())
+    torch.cuda.synchronize()
+    sim.close()
+    pr = case["params"]
+    rho_of = lambda f: pr["rho_l"] + f * (pr["rho_h"] - pr["rho_l"])                    # noqa: E731
+    mu_of = lambda f: rho_of(f) * (pr["tau_l"] + f * (pr["tau_h"] - pr["tau_l"])) / 3     # noqa: E731
+    ref = cf.poiseuille_quadrature(phi[0].mean(axis=1), rho_of, mu_of, pr["g"][0])
+    err = cf.l2_rel(u[0, 0].mean(axis=1), ref)
+    print(f"D2Q9 Poiseuille rho* = {rho_ratio:g}, mu* = 100 on the GPU: L2 (Eq. 47) = {err:.2e} after {steps} steps (du {du:.1e}), u_max {u[0].max():.2e}")
+    assert np.isfinite(u).all() and du <= 1e-13 and err < 0.03

@@ -697,3 +697,32 @@ def test_laplace_table3_on_the_gpu():
     for (R, sigma), e in errs.items():
         assert e < 3.0, (R, sigma, e)                              # Laplace's law within 3 % at the paper's resolution
         assert abs(e - gold[R][sigma]) < 2.5, (R, sigma, e)        # percentage points from the printed value
+
+
+def test_poiseuille_config2_to_steady_state_on_the_gpu():
+    """BASELINE configs[1] proper ON THE PRODUCT: 4 x 128 x 4, y walls, tau_A = 1.0, tau_B = 0.1, density ratio 1, g_x = 1e-6, fp64, 147 000
+    steps (where the oracle's stored run stopped at |du| < 1e-10): the profile must equal the oracle's stored one
+    (tests/golden/poiseuille_config2.txt, written by oracle/ alone) to 1e-10 and meet the north_star gate against Eq. 45."""
+    import os
+    import sys
+    import torch
+    sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+    import closed_forms as cf
+    from paper_2505_12205_b200 import clip
+    d = np.loadtxt(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "poiseuille_config2.txt"))
+    case = inputs.poiseuille(nx=4, ny=128, nz=4, tau_a=1.0, tau_b=0.1)
+    sim = clip.Clip.from_case(case, precision=64)
+    sim.step(146999)
+    u_prev = sim.get()[2].cpu().numpy()
+    sim.step(1)
+    phi, p, u = (t.cpu().numpy() for t in sim.get())
+    torch.cuda.synchronize()
+    sim.close()
+    assert np.abs(u - u_prev).max() < 1e-10                                        # steady
+    ux, ph = u[0].mean(axis=(0, 2)), phi.mean(axis=(0, 2))
+    assert np.ptp(u[0], axis=(0, 2)).max() < 1e-14 and np.abs(u[1:]).max() < 1e-12  # one-dimensional
+    assert np.abs(ux - d[:, 2]).max() < 1e-10 and np.abs(ph - d[:, 1]).max() < 1e-10
+    ref = cf.poiseuille_quadrature(ph, lambda f: np.ones_like(f), lambda f: (0.1 + f * 0.9) / 3.0, 1e-6)
+    err = cf.l2_rel(ux, ref)
+    print(f"Poiseuille configs[1] on the GPU, 147 000 steps: L2 (Eq. 47) vs Eq. 45 = {err:.2e}, max |u_x - oracle| = {np.abs(ux - d[:, 2]).max():.1e}")
+    assert err < 0.01
