@@ -535,7 +535,7 @@ def main():
     ap.add_argument("--plumbing-only", action="store_true",
                     help="no GPU work: start the ranks, rendezvous (gloo), reduce dummy timings and print the line's skeleton (CPU test of --gpus N)")
     ap.add_argument("--nz", type=int, default=0, help="jet workload only: planes along the jet (default 6 n = 1536; shorter for profiling runs)")
-    ap.add_argument("--path", type=int, default=0, choices=[0, 1, 2, 3, 4],
+    ap.add_argument("--path", type=int, default=0, choices=[0, 1, 2, 3, 4, 5],
                     help="clip_params.path: 0 automatic (default), 1 generic kernels, 2 pair kernels (k_phi2 + k_step2), 3 k_fused wherever admitted")
     ap.add_argument("--case", default="l", help="--long-run jetpaper: row of the paper's Table 6 (a .. l)")
     ap.add_argument("--tile-ty", type=int, default=0, help="clip_params.tile_ty (k_fused rows per tile: 0 automatic, 4, 8, 16)")

@@ -72,7 +72,8 @@ typedef struct clip_params {
   int path;                /* kernel path of clip_step (not part of the method; all paths compute the same step): 0 = automatic
                               (see clip_step), 1 = generic kernels only, 2 = never k_fused (pair kernels where the lattice admits
                               them), 3 = k_fused wherever the lattice admits it, 4 = k_fused_tma (k_fused fed by bulk-async copies through
-                              shared memory; x / y faces PERIODIC) where admitted, else as 3.  The slabs of one lattice must agree on whether
+                              shared memory; x / y faces PERIODIC) where admitted, else as 3; 5 = the same with only the g populations staged (experiments,
+                              profiles/r02_experiments.md).  The slabs of one lattice must agree on whether
                               phi(t+1) is kept in a second buffer */
   int tile_ty, tile_chunks; /* k_fused tiling (tests / tuning; 0 = automatic): lattice rows per tile (4, 8 or 16, must divide ny) and
                               number of equal chunks along z (1 .. min(nz, 256)); they enter clip_workspace_bytes */

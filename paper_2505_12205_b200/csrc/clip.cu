@@ -37,7 +37,7 @@ struct Layout {
 // Tiling of the single-pass kernel k_fused (clip_fused.cuh): tiles of `ty` rows x one z chunk; the number of tiles is
 // chosen close to (and not above) a whole number of waves of resident blocks on the 148 SMs of a B200.
 struct FusedPlan {
-  bool ok, fills_gpu, pays, tma;  // tma: path 4, k_fused_tma (bulk-async feed) admitted
+  bool ok, fills_gpu, pays, tma, tma_g;  // tma: path 4, k_fused_tma (bulk-async feed) admitted
   int ty, ytiles, nchunks, tzmax, threads, blocks_per_sm;
   int zc[clip::FUSED_MAX_CHUNKS + 1];  // chunk boundaries along z
   size_t part_words, smem_bytes;
@@ -63,12 +63,16 @@ FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   const int nwarps = f.threads / 32;
   f.smem_bytes = (size_t)clip::FUSED_SLOTS * (f.ty + 2) * (nx + 2 * nwarps) * word;
   int bps = clip::fused_threads_per_sm(p->precision, f.threads) / f.threads;
-  if (p->path == 4) {  // k_fused_tma: two stages of 38 rows behind the ring; periodic x / y faces only
+  if (p->path == 4 || p->path == 5) {  // k_fused_tma: two stages of 38 (path 5, hybrid: 19) rows behind the ring; periodic x / y faces only
     bool periodic_xy = true;
     for (int k = 0; k < 4; ++k) periodic_xy = periodic_xy && p->bc[k] == CLIP_BC_PERIODIC;
     periodic_xy = periodic_xy && p->bc[4] != CLIP_BC_WALL && p->bc[5] != CLIP_BC_WALL;   // a z wall needs the wall body
-    const size_t need = (f.smem_bytes + 127) / 128 * 128 + (size_t)clip::TMA_STAGES * 38 * nx * word + 64;
-    if (periodic_xy && need + 1024 <= 227 * 1024) { f.tma = true; f.smem_bytes = need; bps = (int)((227 * 1024) / (need + 1024)); }
+    const size_t need = (f.smem_bytes + 127) / 128 * 128 + (size_t)clip::TMA_STAGES * (p->path == 5 ? 19 : 38) * nx * word + 64;
+    if (periodic_xy && need + 1024 <= 227 * 1024) {
+      f.tma = true; f.tma_g = p->path == 5; f.smem_bytes = need;
+      const int by_smem = (int)((227 * 1024) / (need + 1024));
+      bps = f.tma_g ? (bps < by_smem ? bps : by_smem) : by_smem;
+    }
   }
   if (bps > 32) bps = 32;
   if (bps < 1) bps = 1;
@@ -182,7 +186,7 @@ const char* validate(int nx, int ny, int nz, const clip_params* p) {
   if (p->outlet_clamp != 0 && p->outlet_clamp != 1) return "outlet_clamp must be 0 (B.25 as printed) or 1 (lambda = max(0, U))";
   if (p->outlet_u_time != 0 && p->outlet_u_time != 1) return "outlet_u_time must be 0 (stored u(t)) or 1 (post-stream moment at t+dt)";
   if (p->outlet_u_time == 1 && p->phase_only) return "outlet_u_time = 1 needs the hydrodynamic populations (not phase_only)";
-  if (p->path < 0 || p->path > 4) return "path must be 0 (automatic), 1 (generic), 2 (no k_fused), 3 (k_fused where admitted) or 4 (k_fused_tma where admitted)";
+  if (p->path < 0 || p->path > 5) return "path must be 0 (automatic), 1 (generic), 2 (no k_fused), 3 (k_fused where admitted), 4 (k_fused_tma) or 5 (k_fused_tma, g only)";
   if (p->tile_ty != 0 && p->tile_ty != 4 && p->tile_ty != 8 && p->tile_ty != 16) return "tile_ty must be 0 (automatic), 4, 8 or 16";
   if (p->tile_chunks < 0) return "tile_chunks must be >= 0";
   if (p->runtime_nx != 0 && p->runtime_nx != 1) return "runtime_nx must be 0 or 1";
@@ -327,7 +331,7 @@ struct Prof {  // optional per-launch event timing (clip_step_profiled)
   void end(int k) { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, stream); ev.push_back(e); kind.push_back(k); }
 };
 
-bool use_fused(const clip_handle* h) { return fast_ok(h) && h->fplan.ok && (h->mode == 3 || h->mode == 4 || (h->mode == 0 && h->fplan.pays)); }
+bool use_fused(const clip_handle* h) { return fast_ok(h) && h->fplan.ok && (h->mode >= 3 || (h->mode == 0 && h->fplan.pays)); }
 
 // lambda of B.25 for the step about to run (k_outlet_lam; the plane-wide schemes of B.22 add a one-block reduction)
 template <typename T> void outlet_lambda(clip_handle* h, const clip::KP<T>& P, Prof* prof) {
@@ -437,7 +441,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
         cudaStreamWaitEvent(h->stream, h->ev_bnd, 0);
       } else {
         U.c_mode = 0;
-        if (fp.tma) fe = clip::launch_fused_tma<T>(h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+        if (fp.tma) fe = clip::launch_fused_tma<T>(h->nx_special, fp.tma_g, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
         else fe = clip::launch_fused<T>(faces, h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
       }
       if (fe != cudaSuccess) { set_err(h->err, "k_fused: %s", cudaGetErrorString(fe)); return CLIP_ECUDA; }

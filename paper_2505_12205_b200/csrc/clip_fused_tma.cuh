@@ -72,6 +72,38 @@ template <typename T> struct StagePull {
   }
 };
 
+// Hybrid (experiment): f, u and phi from global memory as in k_fused (first load round, in registers), only the 19 g segments -- the
+// SECOND load round of step_pair -- through a shared-memory stage [19][nx].
+template <typename T> struct StagePullG {
+  static constexpr bool F_FIRST = true;
+  const T* stage;  // [19][nx]: the g segments
+  unsigned long long* bar;
+  unsigned parity;
+  template <typename T2, int HL, int NX, int SET, int WALLS>
+  __device__ __forceinline__ void run(const KP<T2>& P, const Geo& geo, P2<T2> (&v)[Q]) const {
+    if (SET == 0) { Pull2All<T2, HL, NX, 0, WALLS>::run(P.p_src, P.nx, geo, v); return; }
+    mbar_wait(bar, parity);
+    StagePull<T2>::template All<T2, HL, NX, 0, WALLS>::run(stage, NX ? NX : P.nx, geo, v);   // slot a of the g stage
+  }
+  template <typename T2, int HL> __device__ __forceinline__ void load_u(const KP<T2>& P, const Geo& geo, P2<T2>& ux, P2<T2>& uy, P2<T2>& uz) const {
+    GlobalPull().template load_u<T2, HL>(P, geo, ux, uy, uz);
+  }
+  template <typename T2, int HP> __device__ __forceinline__ void stencil(const KP<T2>& P, const Geo& geo, P2<T2>& phi, P2<T2> (&G)[3], P2<T2>& L) const {
+    GlobalPull().template stencil<T2, HP>(P, geo, phi, G, L);
+  }
+};
+template <typename T, int NX, int a = 0> struct IssueRowG {
+  static __device__ __forceinline__ void run(const KP<T>& P, const Geo& g0, T* stage, unsigned long long* bar) {
+    const int nx = NX ? NX : P.nx;
+    const T* src = pop_row<T, -cy(a), -cz(a)>(P.p_src, g0) + (Q + a) * nx;
+    bulk_g2s(stage + a * nx, src, (unsigned)(nx * sizeof(T)), bar);
+    IssueRowG<T, NX, a + 1>::run(P, g0, stage, bar);
+  }
+};
+template <typename T, int NX> struct IssueRowG<T, NX, Q> {
+  static __device__ __forceinline__ void run(const KP<T>&, const Geo&, T*, unsigned long long*) {}
+};
+
 // one thread: issue the 38 segment copies of lattice row (y, z) into `stage`
 template <typename T, int NX, int c = 0> struct IssueRow {
   static __device__ __forceinline__ void run(const KP<T>& P, const Geo& g0, T* stage, unsigned long long* bar) {
@@ -87,8 +119,10 @@ template <typename T, int NX> struct IssueRow<T, NX, NC> {
 };
 
 // grid = (ytiles, nchunks) as k_fused; dynamic shared memory = ring + edges | stages (128-byte aligned) | mbarriers
-template <typename T, int NX, int MAXT, int MINB>
+// GONLY: the hybrid form (StagePullG): stages of 19 g segments, everything else as k_fused
+template <typename T, int NX, int MAXT, int MINB, bool GONLY = false>
 __global__ void __launch_bounds__(MAXT, MINB) k_fused_tma(const __grid_constant__ FP<T> FPp, const FusedP<T> U) {
+  constexpr int NSEG = GONLY ? Q : NC;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const KP<T>& P = FPp.k;
   const int nx = NX ? NX : P.nx;
@@ -100,13 +134,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused_tma(const __grid_constant_
   T* edge_m = edge_p + nslots * rows * nwarps;
   const size_t ring_bytes = ((size_t)nslots * rows * (nx + 2 * nwarps) * sizeof(T) + 127) / 128 * 128;
   T* stages = reinterpret_cast<T*>(smem_raw + ring_bytes);
-  unsigned long long* full = reinterpret_cast<unsigned long long*>(smem_raw + ring_bytes + (size_t)TMA_STAGES * NC * nx * sizeof(T));
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(smem_raw + ring_bytes + (size_t)TMA_STAGES * NSEG * nx * sizeof(T));
   const int x0 = 2 * threadIdx.x;
   const int iy = blockIdx.x;
   const int c = U.c_mode == 0 ? (int)blockIdx.y : (U.c_mode == 1 ? (blockIdx.y ? U.nchunks - 1 : 0) : (int)blockIdx.y + 1);
   const int y0 = iy * U.ty, z0 = U.zc[c], z1 = U.zc[c + 1];
   const int tz = z1 - z0;
-  const unsigned row_bytes = (unsigned)(NC * nx * sizeof(T));
+  const unsigned row_bytes = (unsigned)(NSEG * nx * sizeof(T));
   if (threadIdx.x == 0) {
     for (int s = 0; s < TMA_STAGES; ++s) mbar_init(full + s, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -118,7 +152,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused_tma(const __grid_constant_
     const Geo g0 = make_geo<T, 0>(P, 0, y0 + ly, z0 + lz);
     unsigned long long* bar = full + (r % TMA_STAGES);
     mbar_expect_tx(bar, row_bytes);
-    IssueRow<T, NX>::run(P, g0, stages + (size_t)(r % TMA_STAGES) * NC * nx, bar);
+    if (GONLY) IssueRowG<T, NX>::run(P, g0, stages + (size_t)(r % TMA_STAGES) * NSEG * nx, bar);
+    else IssueRow<T, NX>::run(P, g0, stages + (size_t)(r % TMA_STAGES) * NSEG * nx, bar);
   };
   const int nrows = tz * U.ty;
   if (threadIdx.x == 0) issue(0);
@@ -142,7 +177,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused_tma(const __grid_constant_
   };
   int r = 0;
   StagePull<T> pl, nxt;
-  pl.prefetch(P, make_geo<T, 0>(P, x0, y0, z0));
+  StagePullG<T> pg;
+  if (!GONLY) pl.prefetch(P, make_geo<T, 0>(P, x0, y0, z0));
 #pragma unroll 1
   for (int lz = 0; lz < tz; ++lz) {
     const int z = z0 + lz;
@@ -152,15 +188,21 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused_tma(const __grid_constant_
       sc.j = ly + 1;
       // the other stage was read for the last time in the previous iteration (barrier below): refill it with the next row
       if (threadIdx.x == 0 && r + 1 < nrows) issue(r + 1);
-      pl.stage = stages + (size_t)(r % TMA_STAGES) * NC * nx;
-      pl.bar = full + (r % TMA_STAGES);
-      pl.parity = (unsigned)((r / TMA_STAGES) & 1);
-      if (r + 1 < nrows) {  // u and phi of the next row: in flight during this row's arithmetic
-        const int ly1 = ly + 1 < U.ty ? ly + 1 : 0, lz1 = ly + 1 < U.ty ? lz : lz + 1;
-        nxt.prefetch(P, make_geo<T, 0>(P, x0, y0 + ly1, z0 + lz1));
+      T* const st = stages + (size_t)(r % TMA_STAGES) * NSEG * nx;
+      if (GONLY) {
+        pg.stage = st; pg.bar = full + (r % TMA_STAGES); pg.parity = (unsigned)((r / TMA_STAGES) & 1);
+        step_pair<T, LD_NC, LD_NC, ST_WB, NX, 0, NoWait, Scatter<T, 0>, false, StagePullG<T>>(FPp, x0, y0 + ly, z, NoWait(), sc, pg);
+      } else {
+        pl.stage = st;
+        pl.bar = full + (r % TMA_STAGES);
+        pl.parity = (unsigned)((r / TMA_STAGES) & 1);
+        if (r + 1 < nrows) {  // u and phi of the next row: in flight during this row's arithmetic
+          const int ly1 = ly + 1 < U.ty ? ly + 1 : 0, lz1 = ly + 1 < U.ty ? lz : lz + 1;
+          nxt.prefetch(P, make_geo<T, 0>(P, x0, y0 + ly1, z0 + lz1));
+        }
+        step_pair<T, LD_NC, LD_NC, ST_WB, NX, 0, NoWait, Scatter<T, 0>, false, StagePull<T>>(FPp, x0, y0 + ly, z, NoWait(), sc, pl);
+        pl.raw = nxt.raw; pl.u0 = nxt.u0; pl.u1 = nxt.u1; pl.u2 = nxt.u2;
       }
-      step_pair<T, LD_NC, LD_NC, ST_WB, NX, 0, NoWait, Scatter<T, 0>, false, StagePull<T>>(FPp, x0, y0 + ly, z, NoWait(), sc, pl);
-      pl.raw = nxt.raw; pl.u0 = nxt.u0; pl.u1 = nxt.u1; pl.u2 = nxt.u2;
       __syncthreads();  // every thread has taken its values out of this stage (and, at a plane's end, finished the plane's scatter)
     }
     flush(lz - 1);

@@ -24,7 +24,7 @@ template <typename T> void launch_step2(int faces, bool xwalls, int nx, dim3 g, 
 // returns the CUDA error of the shared-memory opt-in (cudaFuncSetAttribute, once per device and instantiation) or of nothing
 template <typename T> cudaError_t launch_fused(int faces, int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
 // k_fused_tma (bulk-async feed; periodic x / y faces): same grid and FusedP as k_fused, more shared memory
-template <typename T> cudaError_t launch_fused_tma(int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
+template <typename T> cudaError_t launch_fused_tma(int nx, bool gonly, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
 template <typename T> void launch_fix(dim3 g, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
 
 }  // namespace clip

@@ -89,9 +89,10 @@ template <typename T> cudaError_t launch_fused(int faces, int nx, dim3 g, dim3 b
   if (faces == 2) return nx == 192 ? launch_fused_nx<T, 192, 2>(g, b, smem, st, F, U) : launch_fused_nx<T, 0, 2>(g, b, smem, st, F, U);  // as launch_step2
   return faces ? launch_fused_w<T, 1>(nx, g, b, smem, st, F, U) : launch_fused_w<T, 0>(nx, g, b, smem, st, F, U);
 }
-template <typename T, int NX> cudaError_t launch_fused_tma_nx(dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
+template <typename T, int NX, bool GONLY> cudaError_t launch_fused_tma_nx(dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
   constexpr int MAXT = NX ? NX / 2 : 256;
-  auto kern = k_fused_tma<T, NX, MAXT, 1>;
+  constexpr int MINB = (GONLY && sizeof(T) == 4 && 384 / MAXT > 0) ? 384 / MAXT : 1;   // hybrid: k_fused's occupancy
+  auto kern = k_fused_tma<T, NX, MAXT, MINB, GONLY>;
   static bool attr_done[MAX_DEVICES] = {};
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
@@ -104,13 +105,20 @@ template <typename T, int NX> cudaError_t launch_fused_tma_nx(dim3 g, dim3 b, si
   kern<<<g, b, smem, st>>>(F, U);
   return cudaSuccess;
 }
-template <typename T> cudaError_t launch_fused_tma(int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
+template <typename T> cudaError_t launch_fused_tma(int nx, bool gonly, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
+  if (gonly) {
+    switch (nx) {
+      case 256: return launch_fused_tma_nx<T, 256, true>(g, b, smem, st, F, U);
+      case 512: return launch_fused_tma_nx<T, 512, true>(g, b, smem, st, F, U);
+      default: return launch_fused_tma_nx<T, 0, true>(g, b, smem, st, F, U);
+    }
+  }
   switch (nx) {
-    case 128: return launch_fused_tma_nx<T, 128>(g, b, smem, st, F, U);
-    case 256: return launch_fused_tma_nx<T, 256>(g, b, smem, st, F, U);
-    case 384: return launch_fused_tma_nx<T, 384>(g, b, smem, st, F, U);
-    case 512: return launch_fused_tma_nx<T, 512>(g, b, smem, st, F, U);
-    default: return launch_fused_tma_nx<T, 0>(g, b, smem, st, F, U);
+    case 128: return launch_fused_tma_nx<T, 128, false>(g, b, smem, st, F, U);
+    case 256: return launch_fused_tma_nx<T, 256, false>(g, b, smem, st, F, U);
+    case 384: return launch_fused_tma_nx<T, 384, false>(g, b, smem, st, F, U);
+    case 512: return launch_fused_tma_nx<T, 512, false>(g, b, smem, st, F, U);
+    default: return launch_fused_tma_nx<T, 0, false>(g, b, smem, st, F, U);
   }
 }
 template <typename T> void launch_fix(dim3 g, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {

@@ -66,7 +66,7 @@ def test_validation_without_gpu():
         (dict(M=-0.2), "tau_phi"),
         (dict(outlet_u_mode=3), "outlet_u_mode"),
         (dict(visc_interp=7), "visc_interp"),
-        (dict(path=5), "path"),
+        (dict(path=6), "path"),
         (dict(outlet_clamp=2), "outlet_clamp"),
         (dict(outlet_u_time=2), "outlet_u_time"),
         (dict(outlet_u_time=1, phase_only=1), "outlet_u_time"),

@@ -435,8 +435,9 @@ def test_fused_single_pass_path(name, precision):
             assert np.abs(a - b).max() <= tol * max(1.0, np.abs(a).max()), (name, env)
 
 
+@pytest.mark.parametrize("path", [4, 5])
 @pytest.mark.parametrize("precision", [64, 32])
-def test_fused_tma_path(precision):
+def test_fused_tma_path(precision, path):
     """k_fused_tma (path 4: the 38 population rows of a lattice row arrive in shared memory by bulk-async copies, one row ahead;
     x / y faces PERIODIC) against k_phi2 + k_step2: round-off only; several tilings; periodic z, walled z and an inlet / outlet pair."""
     import torch
@@ -450,7 +451,7 @@ def test_fused_tma_path(precision):
     for case in cases:
         ref = _gpu_p(case, 25, precision, path=2)
         for over in ({}, {"tile_chunks": 1}, {"tile_chunks": case["nz"]}):
-            c = dict(case, params=dict(case["params"], path=4, **over))
+            c = dict(case, params=dict(case["params"], path=path, **over))
             sim = clip.Clip.from_case(c, precision=precision)
             sim.step(25)
             out = [t.double().cpu().numpy() for t in sim.get()]
