@@ -181,6 +181,28 @@ int clip_step_profiled(clip_t* h, int n, double* ms, long long* count);
 int clip_kernel_kinds(void);
 const char* clip_kernel_name(int kind);
 
+/* ---- no-allocation entry point --------------------------------------------------------------------------------------------------
+ * For callers that may not allocate device memory at all (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc) and therefore cannot provide a workspace: lambda of the convective outlet for the step t -> t+1 (App. B.5: B.22 with
+ * the three schemes U_local / U_ave / U_max; lambda = U dt / dx of B.25; U from the stored velocity of
+ * the previous time step, i.e. outlet_u_time = 0; outlet_clamp as in clip_params, reading R12) -- what
+ * k_outlet_lam + k_outlet_reduce compute inside clip_step for a lattice with an OUTLET on +z, with the same reduction order.
+ *   d_u       device, [3][nz][ny][nx] words of `precision` (the layout clip_get writes): u(t); only u_z of layer nz-2 is read
+ *   d_lambda  device, [ny][nx] words: receives lambda (uniform over the plane for outlet_u_mode 1 and 2)
+ * Both aligned to the word size and owned by the caller; the two kernels are enqueued on `cuda_stream` (cudaStream_t as void*, NULL =
+ * the default stream) of the CURRENT device, no host synchronisation.
+ * The per-column scratch of the reduction lives in a static device array inside the library (2 MiB per GPU that loads the library,
+ * held until exit), hence the limit nx * ny <= CLIP_STATIC_MAX_PLANE_NODES; larger planes are refused with CLIP_EINVAL.  Every call on
+ * a device shares that array: calls that may overlap on the GPU (different streams without an ordering between them) race and must
+ * be serialised by the caller; calls on one stream, or on different devices, are safe.  The array needs no clearing: each call
+ * writes every entry it later reads.  Calls no cudaMalloc / cudaFree or other allocating routine.
+ * Returns CLIP_OK, CLIP_EINVAL (sizes, modes, pointers) or CLIP_ECUDA; text via clip_static_last_error() (per host thread,
+ * library-owned, valid until that thread's next call of clip_outlet_lambda_static). */
+#define CLIP_STATIC_MAX_PLANE_NODES 262144
+int clip_outlet_lambda_static(const void* d_u, int nx, int ny, int nz, int precision, int outlet_u_mode, int outlet_clamp,
+                              void* d_lambda, void* cuda_stream);
+const char* clip_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -101,6 +101,10 @@ def lib():
         L.clip_step_halo_end.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.clip_kernel_name.restype = C.c_char_p
         L.clip_kernel_name.argtypes = [C.c_int]
+        L.clip_outlet_lambda_static.restype = C.c_int
+        L.clip_outlet_lambda_static.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        L.clip_static_last_error.restype = C.c_char_p
+        L.clip_static_last_error.argtypes = []
         _lib = L
     return _lib
 
@@ -181,6 +185,20 @@ def clip_step_profiled(h, n: int):
     cnt = (C.c_longlong * k)()
     rc = lib().clip_step_profiled(h, int(n), ms, cnt)
     return rc, {lib().clip_kernel_name(i).decode(): (ms[i], cnt[i]) for i in range(k)}
+
+
+CLIP_STATIC_MAX_PLANE_NODES = 262144
+
+
+def clip_outlet_lambda_static(d_u: int, nx, ny, nz, precision, outlet_u_mode, outlet_clamp, d_lambda: int, cuda_stream: int) -> int:
+    """No-allocation entry point (include/clip.h): lambda of the convective outlet from u(t), scratch in a static device array."""
+    return lib().clip_outlet_lambda_static(C.c_void_p(d_u), int(nx), int(ny), int(nz), int(precision), int(outlet_u_mode),
+                                           int(outlet_clamp), C.c_void_p(d_lambda), C.c_void_p(cuda_stream))
+
+
+def clip_static_last_error() -> str:
+    s = lib().clip_static_last_error()
+    return s.decode() if s else ""
 
 
 class ClipError(RuntimeError):
