@@ -293,7 +293,7 @@ def run_ours(args):
 
 def run_slab(args):
     """`--decomp slab`: ONE periodic lattice n x n x (n * N) cut into N z slabs, one per GPU (weak scaling: n^3 owned nodes per
-    GPU), halo exchange of two planes per cut after every step (paper_2505_12205_b200/slab.py).  With N = 1
+    GPU), exchange of one 12-word record per face node and cut side after every step (paper_2505_12205_b200/slab.py).  With N = 1
     the slab is its own neighbour: the line then shows what packing, copying and unpacking the halos costs on one GPU."""
     import torch
     import torch.distributed as dist

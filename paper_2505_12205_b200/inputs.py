@@ -248,3 +248,43 @@ def sweep2d(nx=128, ny=96, seed=2505, ndrops=8, rmin=5.0, rmax=12.0, W=4.0, u_am
     case["params"].update(lattice=1, bc=tuple(bc))
     case["name"] = f"sweep2d_{nx}x{ny}"
     return case
+
+
+RANDOM_LATTICE_SEEDS = range(96)   # the seeds tests/test_fuzz_gpu.py runs
+
+
+def random_lattice(seed, nx_choices=(8, 12, 20, 34, 64, 128, 192, 66, 40, 256), ny_choices=(4, 7, 8, 10, 12, 16, 20),
+                   nz_choices=(4, 5, 8, 9, 12, 17, 33)):
+    """Seeded random small lattice for the path fuzz (tests/test_fuzz_gpu.py): sizes, faces (every combination the ABI admits in x / y;
+    PERIODIC, WALL, FREESLIP, INLET + OUTLET, WALL + OUTLET, INLET + WALL in z), material parameters, collision operator, viscosity
+    interpolation, gravity, outlet scheme / clamp / time level, three seeded drops (minimum-image distance across PERIODIC faces) and an
+    i.i.d. uniform u0.  An inlet gets the liquid stub of jet() in front of its disc and a density ratio <= 50: a bare phi = 1 disc
+    next to gas under a random velocity field is not a start the method runs from (oracle and kernels alike diverge within ten
+    steps), and neither is a drop cut off sharply at a periodic seam."""
+    rng = np.random.Generator(np.random.PCG64([2505, int(seed)]))
+    pick = lambda a: a[int(rng.integers(len(a)))]   # noqa: E731
+    nx, ny, nz = pick(nx_choices), pick(ny_choices), pick(nz_choices)
+    xf = pick([(PERIODIC, PERIODIC), (WALL, WALL), (FREESLIP, FREESLIP), (FREESLIP, WALL), (WALL, FREESLIP)])
+    yf = pick([(PERIODIC, PERIODIC), (WALL, WALL), (FREESLIP, FREESLIP), (FREESLIP, WALL), (WALL, FREESLIP)])
+    zf = pick([(PERIODIC, PERIODIC), (WALL, WALL), (INLET, OUTLET), (WALL, OUTLET), (INLET, WALL), (FREESLIP, FREESLIP), (INLET, OUTLET)])
+    inlet = zf[0] == INLET
+    W = 3.0
+    p = default_params(
+        rho_l=pick([0.02, 0.1, 1.0] if inlet else [1.0e-3, 0.1, 1.0]), tau_l=pick([0.8, 0.3, 0.1]), tau_h=pick([0.8, 0.6]),
+        visc_interp=pick([0, 1, 2]), collision=pick([0, 0, 1]), g=pick([(0.0, 0.0, 0.0), (1.0e-5, -2.0e-5, 3.0e-5)]),
+        rho_ref=pick([0.0, 1.0]), sigma=pick([0.01, 0.002]), M=pick([0.1, 0.05]), W=W,
+        inlet_u=(0.0, 0.0, 0.03), inlet_c=(nx / 2 - 0.5, ny / 2 - 0.5), inlet_r=min(nx, ny) / 4,
+        outlet_clamp=pick([0, 1]), outlet_u_mode=pick([0, 1, 2]), outlet_u_time=pick([0, 1]), bc=xf + yf + zf)
+    x, y, z = _grid(nx, ny, nz)
+    phi0 = np.zeros((nz, ny, nx))
+    for _ in range(3):
+        c = rng.uniform(0.0, 1.0, 3) * np.array([nx, ny, nz], dtype=np.float64)
+        R = rng.uniform(2.0, max(2.5, min(nx, ny, nz) / 3))
+        d = [np.abs(q - c[k]) for k, q in enumerate((x, y, z))]
+        d = [np.minimum(dk, n - dk) if f[0] == PERIODIC else dk for dk, n, f in zip(d, (nx, ny, nz), (xf, yf, zf))]
+        phi0 = np.maximum(phi0, 0.5 + 0.5 * np.tanh(2.0 * (R - np.sqrt(d[0] ** 2 + d[1] ** 2 + d[2] ** 2)) / W))
+    if inlet:
+        rxy = np.sqrt((x - p["inlet_c"][0]) ** 2 + (y - p["inlet_c"][1]) ** 2)
+        phi0 = np.maximum(phi0, 0.5 + 0.5 * np.tanh(2.0 * np.minimum(p["inlet_r"] - rxy, p["inlet_r"] - z) / W))
+    u0 = rng.uniform(-0.01, 0.01, size=(3, nz, ny, nx))
+    return _case(nx, ny, nz, p, phi0, u0, f"random{seed}_{nx}x{ny}x{nz}")

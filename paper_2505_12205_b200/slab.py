@@ -1,6 +1,6 @@
 """z-slab decomposition of one lattice over several GPUs (include/clip.h, clip_halo_pack).
 
-One process per GPU owns `nz / world` consecutive z planes plus ONE ghost plane beyond each interior cut (face type CLIP_BC_HALO:
+One process per GPU owns about `nz / world` consecutive z planes (slab_range) plus ONE ghost plane beyond each interior cut (face type CLIP_BC_HALO:
 libclip steps the owned planes only).  After every step each side of a cut sends one record of 12 words per face node -- the ten
 populations of its boundary plane that move towards the neighbour (Eq. 13 / 33 streaming; Alg. 2 :432-459) and
 two partial sums of phi(t+1) = sum_a g_a (Eq. 38), from which both sides complete phi on the two planes of the cut (the stencils of
@@ -18,15 +18,15 @@ _HALO_BC = 5  # CLIP_BC_HALO
 
 
 def slab_range(nz: int, rank: int, world: int):
-    """Owned planes [z0, z1) of `rank`: equal slabs (every rank must pick the same kernel path, clip.h)."""
+    """Owned planes [z0, z1) of `rank`: consecutive slabs of nz // world planes, the first nz % world slabs one plane more (the halo
+    record does not depend on the kernel path a slab's lattice admits, so the slabs need not be equal)."""
     if world < 1 or not 0 <= rank < world:
         raise ValueError("bad rank / world")
-    if nz % world != 0:
-        raise ValueError(f"nz = {nz} is not a multiple of the {world} slabs")
-    own = nz // world
-    if own < 2:
-        raise ValueError(f"a slab must own at least 2 planes (got {own}): its two halo records must not depend on each other")
-    return rank * own, (rank + 1) * own
+    base, rem = divmod(nz, world)
+    if base < 2:
+        raise ValueError(f"a slab must own at least 2 planes (got {base}): its two halo records must not depend on each other")
+    z0 = rank * base + min(rank, rem)
+    return z0, z0 + base + (1 if rank < rem else 0)
 
 
 def slab_ghosts(rank: int, world: int, z_periodic: bool):

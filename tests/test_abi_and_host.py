@@ -103,6 +103,24 @@ def test_elongated_lattices_do_not_overflow_the_tiling_tables():
             assert n < 86 * 4 * nodes + (1 << 20), (shape, over, n / nodes)
 
 
+def test_random_lattices_of_the_path_fuzz_are_valid_inputs():
+    """inputs.random_lattice (tests/test_fuzz_gpu.py): every seed the fuzz uses passes the library's validation for every path, is
+    reproducible, and the seeds together reach every face type and both collision operators."""
+    import numpy as np
+    faces, colls = set(), set()
+    for seed in inputs.RANDOM_LATTICE_SEEDS:
+        case = inputs.random_lattice(seed)
+        again = inputs.random_lattice(seed)
+        assert np.array_equal(case["phi0"], again["phi0"]) and np.array_equal(case["u0"], again["u0"]) and case["params"] == again["params"]
+        assert case["phi0"].min() >= 0.0 and case["phi0"].max() <= 1.0
+        for path in (0, 1, 2, 3):
+            for prec in (32, 64):
+                p = dict(case["params"], path=path, precision=prec)
+                assert clip.clip_workspace_bytes(case["nx"], case["ny"], case["nz"], clip.make_params(p)) > 0, (seed, clip.clip_last_error(None))
+        faces.update(case["params"]["bc"]); colls.add(case["params"]["collision"])
+    assert faces == {inputs.PERIODIC, inputs.WALL, inputs.INLET, inputs.OUTLET, inputs.FREESLIP} and colls == {0, 1}
+
+
 def test_no_cpu_fallback(tmp_path, monkeypatch):
     """A missing libclip.so is a hard error; the product never imports the oracle."""
     monkeypatch.setattr(clip, "_lib", None)

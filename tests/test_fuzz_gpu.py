@@ -1,0 +1,78 @@
+"""Path fuzz: every kernel path of clip_step (clip_params.path 0 automatic, 1 generic, 2 pair kernels, 3 k_fused; each falls back to
+the generic kernels for the planes / lattices it does not admit) against the ORACLE on seeded random small lattices -- sizes with ragged
+tails and thin z, every face combination the ABI admits, both collision operators, the three viscosity interpolations, gravity, the
+outlet schemes / clamp / time levels (inputs.random_lattice).  20 steps; tolerances of test_parity_gpu.py (north_star)."""
+import numpy as np
+import pytest
+
+from paper_2505_12205_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FP64_ABS = 1e-10
+FP32_PHI, FP32_U = 1e-4, 1e-3
+STEPS = 20
+_ref = {}
+
+
+def _run(case, precision, path):
+    import torch
+    from paper_2505_12205_b200 import clip
+    params = dict(case["params"], precision=precision, path=path)
+    sim = clip.Clip(case["nx"], case["ny"], case["nz"], params)
+    sim.init(torch.as_tensor(case["phi0"]), torch.as_tensor(case["u0"]))
+    sim.step(STEPS)
+    out = tuple(t.double().cpu().numpy() for t in sim.get())
+    ran = [k for k, (ms, cnt) in sim.step_profiled(1).items() if cnt]
+    sim.close()
+    return out, ran
+
+
+@pytest.mark.parametrize("seed", list(inputs.RANDOM_LATTICE_SEEDS))
+def test_every_path_against_the_oracle_on_a_random_lattice(seed):
+    from oracle.clip_oracle import Oracle
+    case = inputs.random_lattice(seed)
+    o = Oracle.from_case(case)
+    o.step(STEPS)
+    rphi, rp, ru = o.get()
+    assert np.isfinite(rphi).all() and np.isfinite(ru).all(), "the generator is meant to avoid starts the method itself cannot run"
+    seen = set()
+    for path in (1, 0, 2, 3):
+        (phi, p, u), ran = _run(case, 64, path)
+        seen.update(ran)
+        e = [np.abs(a - b).max() for a, b in ((phi, rphi), (p, rp), (u, ru))]
+        assert all(np.isfinite(v) and v <= FP64_ABS for v in e), (case["name"], case["params"]["bc"], path, ran, e)
+    (phi, p, u), ran = _run(case, 32, 0)
+    ephi = np.abs(phi - rphi).max() / np.abs(rphi).max()
+    eu = np.abs(u - ru).max() / max(np.abs(ru).max(), 1e-30)
+    print(f"{case['name']} bc {case['params']['bc']}: kernels {sorted(seen)}; fp32 phi {ephi:.1e} u {eu:.1e}")
+    assert ephi <= FP32_PHI and eu <= FP32_U, (case["name"], ran, ephi, eu)
+
+
+@pytest.mark.parametrize("seed", [s for s in inputs.RANDOM_LATTICE_SEEDS if s % 2 == 0])
+def test_slabs_of_a_random_lattice_against_the_oracle(seed):
+    """The same lattices cut into two or three z slabs, unequal where nz is no multiple (clip_halo_pack / clip_halo_unpack through paper_2505_12205_b200/slab.py, all
+    slabs in this process, stepped one after the other): owned planes against the oracle, fp64, automatic path."""
+    import torch
+    from oracle.clip_oracle import Oracle
+    from paper_2505_12205_b200 import slab
+    case = inputs.random_lattice(seed)
+    world = 2 + (seed // 2) % 2
+    if case["nz"] // world < 2:
+        pytest.skip("too thin to cut: a slab owns at least two planes")
+    o = Oracle.from_case(case)
+    o.step(STEPS)
+    ref = o.get()
+    phi0, u0 = torch.as_tensor(case["phi0"]), torch.as_tensor(case["u0"])
+    params = dict(case["params"], precision=64)
+    group = [slab.SlabClip(case["nx"], case["ny"], case["nz"], params, r, world, overlap=bool(seed % 4 == 0)) for r in range(world)]
+    for s in group:
+        s.init(phi0, u0)
+    slab.step_group(group, STEPS)
+    parts = [s.get() for s in group]
+    torch.cuda.synchronize()
+    out = (torch.cat([p[0] for p in parts], 0), torch.cat([p[1] for p in parts], 0), torch.cat([p[2] for p in parts], 1))
+    for s in group:
+        s.close()
+    e = [np.abs(a.double().cpu().numpy() - b).max() for a, b in zip(out, ref)]
+    assert all(np.isfinite(v) and v <= FP64_ABS for v in e), (case["name"], case["params"]["bc"], world, e)

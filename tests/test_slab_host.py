@@ -17,7 +17,7 @@ from paper_2505_12205_b200 import slab
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-@pytest.mark.parametrize("nz,world,periodic", [(8, 1, True), (8, 2, True), (12, 3, True), (8, 2, False), (16, 4, False), (6, 3, True)])
+@pytest.mark.parametrize("nz,world,periodic", [(8, 1, True), (8, 2, True), (12, 3, True), (8, 2, False), (16, 4, False), (6, 3, True), (10, 3, True), (33, 2, False), (17, 4, False)])
 def test_partition_covers_the_lattice(nz, world, periodic):
     owned = []
     for r in range(world):
@@ -42,8 +42,7 @@ def test_partition_covers_the_lattice(nz, world, periodic):
 
 
 def test_partition_rejects_bad_splits():
-    with pytest.raises(ValueError):
-        slab.slab_range(10, 0, 3)       # not a multiple
+    assert [slab.slab_range(10, r, 3) for r in range(3)] == [(0, 4), (4, 7), (7, 10)]   # unequal slabs are fine
     with pytest.raises(ValueError):
         slab.slab_range(4, 0, 4)        # a slab must own two planes
     with pytest.raises(ValueError):
