@@ -288,3 +288,29 @@ def random_lattice(seed, nx_choices=(8, 12, 20, 34, 64, 128, 192, 66, 40, 256), 
         phi0 = np.maximum(phi0, 0.5 + 0.5 * np.tanh(2.0 * np.minimum(p["inlet_r"] - rxy, p["inlet_r"] - z) / W))
     u0 = rng.uniform(-0.01, 0.01, size=(3, nz, ny, nx))
     return _case(nx, ny, nz, p, phi0, u0, f"random{seed}_{nx}x{ny}x{nz}")
+
+
+def random_lattice2d(seed):
+    """random_lattice on the D2Q9 lattice (nz = 1, z faces PERIODIC): x / y faces PERIODIC, WALL, FREESLIP and the mixed pairs, seeded
+    discs, in-plane u0."""
+    rng = np.random.Generator(np.random.PCG64([2509, int(seed)]))
+    pick = lambda a: a[int(rng.integers(len(a)))]   # noqa: E731
+    nx, ny = pick((8, 12, 20, 34, 64, 66, 128, 250, 256, 21)), pick((4, 7, 8, 16, 33, 64))
+    faces = [(PERIODIC, PERIODIC), (WALL, WALL), (FREESLIP, FREESLIP), (FREESLIP, WALL), (WALL, FREESLIP)]
+    xf, yf = pick(faces), pick(faces)
+    W = 3.0
+    p = default_params(
+        rho_l=pick([1.0e-3, 0.1, 1.0]), tau_l=pick([0.8, 0.3, 0.1]), tau_h=pick([0.8, 0.6]), visc_interp=pick([0, 1, 2]),
+        collision=pick([0, 0, 1]), g=pick([(0.0, 0.0, 0.0), (1.0e-5, -2.0e-5, 0.0)]), rho_ref=pick([0.0, 1.0]),
+        sigma=pick([0.01, 0.002]), M=pick([0.1, 0.05]), W=W, bc=xf + yf + (PERIODIC, PERIODIC), lattice=1)
+    x, y, _ = _grid(nx, ny, 1)
+    phi0 = np.zeros((1, ny, nx))
+    for _k in range(3):
+        c = rng.uniform(0.0, 1.0, 2) * np.array([nx, ny], dtype=np.float64)
+        R = rng.uniform(2.0, max(2.5, min(nx, ny) / 3))
+        d = [np.abs(q - c[k]) for k, q in enumerate((x, y))]
+        d = [np.minimum(dk, n - dk) if f[0] == PERIODIC else dk for dk, n, f in zip(d, (nx, ny), (xf, yf))]
+        phi0 = np.maximum(phi0, 0.5 + 0.5 * np.tanh(2.0 * (R - np.sqrt(d[0] ** 2 + d[1] ** 2)) / W))
+    u0 = rng.uniform(-0.01, 0.01, size=(3, 1, ny, nx))
+    u0[2] = 0.0
+    return _case(nx, ny, 1, p, phi0, u0, f"random2d_{seed}_{nx}x{ny}")

@@ -76,3 +76,24 @@ def test_slabs_of_a_random_lattice_against_the_oracle(seed):
         s.close()
     e = [np.abs(a.double().cpu().numpy() - b).max() for a, b in zip(out, ref)]
     assert all(np.isfinite(v) and v <= FP64_ABS for v in e), (case["name"], case["params"]["bc"], world, e)
+
+
+@pytest.mark.parametrize("seed", range(64))
+def test_d2q9_paths_against_the_oracle_on_a_random_lattice(seed):
+    """The D2Q9 lattice (clip_params.lattice = 1): automatic path (pair kernels where nx is even) and the thread-per-node kernels
+    (path = 1) against the D2Q9 build of the oracle, fp64; the automatic path in fp32."""
+    from oracle.clip_oracle import Oracle
+    case = inputs.random_lattice2d(seed)
+    o = Oracle.from_case(case)
+    assert o.Q == 9
+    o.step(STEPS)
+    rphi, rp, ru = o.get()
+    assert np.isfinite(rphi).all() and np.isfinite(ru).all()
+    for path in (1, 0):
+        (phi, p, u), ran = _run(case, 64, path)
+        e = [np.abs(a - b).max() for a, b in ((phi, rphi), (p, rp), (u, ru))]
+        assert all(np.isfinite(v) and v <= FP64_ABS for v in e), (case["name"], case["params"]["bc"], path, ran, e)
+    (phi, p, u), ran = _run(case, 32, 0)
+    ephi = np.abs(phi - rphi).max() / np.abs(rphi).max()
+    eu = np.abs(u - ru).max() / max(np.abs(ru).max(), 1e-30)
+    assert ephi <= FP32_PHI and eu <= FP32_U, (case["name"], ran, ephi, eu)
