@@ -106,7 +106,13 @@ int clip_init(clip_t* h, const void* d_phi0, const void* d_u0);
  * All paths compute the same step; they agree to round-off, and each is deterministic: clip_step(a); clip_step(b) equals
  * clip_step(a + b) bit for bit.  clip_params.path / tile_ty / tile_chunks / runtime_nx override the choice (tests, tuning); the
  * library reads nothing from the environment.  On lattices of up to 4 M nodes (launch-bound), n >= 32 and a stream that can be captured
- * (not the legacy default stream), the steps are replayed 16 at a time from a CUDA graph the handle captures once. */
+ * (not the legacy default stream), the steps are replayed 16 at a time from a CUDA graph the handle captures once.
+ * Capture by the CALLER: called while the handle's stream is being captured, clip_step records its launches into the caller's graph
+ * and starts no capture of its own.  Such a graph may be replayed any number of times if it holds an EVEN number of steps (the two
+ * population buffers and, on the k_fused path, the two phi buffers swap roles every step) and the handle took at least one step
+ * outside the capture since clip_init (the k_fused path's one-off phi pre-pass is then behind it); no other call on the handle
+ * goes into the same graph, phase_only lattices (clip_set_u between steps) excepted from this use.  The handle's counters
+ * (clip_launch_count) advance at capture, not at replay. */
 int clip_step(clip_t* h, int n);
 
 /* phase_only mode: prescribe the velocity field u [3][nz][ny][nx] (device) that the following collisions use; the

@@ -488,6 +488,42 @@ def test_graph_replay_of_small_lattices_is_exact(precision):
             assert np.array_equal(a, b), case["name"]
 
 
+@pytest.mark.parametrize("precision", [64, 32])
+def test_the_caller_may_capture_clip_step_in_a_cuda_graph(precision):
+    """include/clip.h, clip_step: called while the handle's stream is being captured, clip_step records its launches into the CALLER's
+    graph (and starts no capture of its own).  An even number of steps, captured after one plain step, can be replayed any number of
+    times: the fields equal the plain launches bit for bit -- pair kernels, k_fused (two phi buffers), jet replica (generic planes and
+    the outlet kernels in the same graph), generic kernels."""
+    import torch
+    from paper_2505_12205_b200 import clip
+    cases = [(inputs.sweep_drops(n=32, ndrops=3, rmin=3, rmax=6), {}), (inputs.sweep_drops(shape=(64, 16, 12), ndrops=4, rmin=3, rmax=5), {"path": 3}),
+             (inputs.jet(nxy=24, nz=32, r_nozzle=4.0), {}), (inputs.sweep_drops(shape=(21, 12, 10), ndrops=3, rmin=3, rmax=4), {})]
+    for case, over in cases:
+        c = dict(case, params=dict(case["params"], **over))
+        ref = _gpu(c, 1 + 4 * 5 + 3, precision)
+        side = torch.cuda.Stream()
+        sim = clip.Clip(c["nx"], c["ny"], c["nz"], dict(c["params"], precision=precision), stream=side)
+        sim.init(torch.as_tensor(c["phi0"]), torch.as_tensor(c["u0"]))
+        sim.step(1)
+        side.synchronize()
+        l0 = sim.launches
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            sim.step(4)
+        per_replay = sim.launches - l0
+        assert per_replay >= 8 and sim.graph_steps == 0      # recorded into the caller's graph, not replayed from the handle's own
+        with torch.cuda.stream(side):
+            for _ in range(5):
+                g.replay()
+        sim.step(3)
+        out = sim.get()
+        side.synchronize()
+        got = [t.double().cpu().numpy() for t in out]
+        sim.close()
+        for a, b in zip(ref, got):
+            assert np.array_equal(a, b), case["name"]
+
+
 def test_fused_path_is_deterministic_at_full_size():
     """k_fused keeps phi's partial sums in a shared-memory ring that warps of a block fill and flush at different times
     (one barrier per plane, warp-edge sends through side arrays) and hands tile halos over through `part`: any race would
