@@ -424,7 +424,7 @@ def run_long(args):
         case = inputs.rayleigh_taylor(L=args.n // 2, precision=prec)
         total = args.steps if args.steps_given else 20000
     elif args.long_run == "jetpaper":   # the paper's own set-up (Sec. 6.1, Table 6 row --case): 6 D x 6 D x 20 D, free-slip sides, gravity
-        case = inputs.jet_paper(case=args.case, D=args.n // 8, precision=prec)
+        case = inputs.jet_paper(case=args.case, D=args.n // 8, precision=prec, W=args.width, M=args.mobility, U=args.uj)
         total = args.steps if args.steps_given else 40000
     else:
         case = inputs.jet(nxy=3 * args.n // 4, nz=6 * args.n, r_nozzle=12.0 * args.n / 256, We=args.we, precision=prec)
@@ -542,6 +542,9 @@ def main():
     ap.add_argument("--tile-chunks", type=int, default=0, help="clip_params.tile_chunks (k_fused: number of equal z chunks, 0 automatic)")
     ap.add_argument("--long-run", default=None, choices=["rt", "jet", "jetpaper"],
                     help="run BASELINE configs[2] (rt, 20000 steps) or configs[3] (jet, 50000 steps) at full length with diagnostics; one JSON line")
+    ap.add_argument("--width", type=float, default=4.0, help="--long-run jetpaper: interface width W (the paper does not state it for the jets)")
+    ap.add_argument("--mobility", type=float, default=0.1, help="--long-run jetpaper: Allen-Cahn mobility M (not stated by the paper either)")
+    ap.add_argument("--uj", type=float, default=0.05, help="--long-run jetpaper: inlet velocity in lattice units (the paper: 0.05, PAPER.md:849)")
     ap.add_argument("--we", type=float, default=2.2, help="Weber number of the jet (--long-run jet)")
     args = ap.parse_args()
     args.steps_given = any(a == "--steps" or a.startswith("--steps=") for a in sys.argv[1:])

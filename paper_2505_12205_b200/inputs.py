@@ -134,14 +134,14 @@ JET_TABLE6 = {"a": (151, 0.44, 2.60), "b": (211, 0.88, 3.65), "c": (228, 1.03, 3
               "k": (423, 3.52, 7.31), "l": (454, 4.05, 7.84)}
 
 
-def jet_paper(case="l", D=32, W=4.0, precision=32, nz=None):
+def jet_paper(case="l", D=32, W=4.0, precision=32, nz=None, M=0.1, U=0.05):
     """The paper's own jet set-up (Sec. 6.1, Fig. 18; Eq. 58-59; Table 6): domain 6 D x 6 D x 20 D, circular inlet of
     diameter D with uniform velocity u_j = 0.05 and rho_j = 1 (:849), FREE-SLIP side walls, convective outlet, gravity along the jet
     with F_g = (rho - rho_L) g (Eq. 58: rho_ref = rho_l), rho* = 814, mu* = 55, and (Re, We, Fr) of the named row of Table 6
     (Eq. 59: sigma = rho_j u_j^2 D / We, nu_j = u_j D / Re, g = u_j^2 / (Fr^2 D)).  The jet runs along +z here (the paper's y).
-    D = 32 gives 192 x 192 x 640; D = 4 the parity replica 24 x 24 x 80."""
+    D = 32 gives 192 x 192 x 640; D = 4 the parity replica 24 x 24 x 80.  The paper states neither the interface width nor the mobility of
+    these runs: W and M are free here; U = u_j is the paper's 0.05 unless a run needs a smaller lattice velocity (same Re, We, Fr)."""
     Re, We, Fr = JET_TABLE6[case]
-    U = 0.05
     nxy, nz = 6 * D, (20 * D if nz is None else nz)
     x, y, z = _grid(nxy, nxy, nz)
     c = 0.5 * (nxy - 1)
@@ -152,7 +152,7 @@ def jet_paper(case="l", D=32, W=4.0, precision=32, nz=None):
     rho_h, rho_l = 1.0, 1.0 / 814.0
     nu_h = U * D / Re
     nu_l = nu_h * 814.0 / 55.0                                                    # mu* = 55
-    p = default_params(precision=precision, rho_h=rho_h, rho_l=rho_l, tau_h=3 * nu_h, tau_l=3 * nu_l, sigma=rho_h * U * U * D / We, W=W, M=0.1,
+    p = default_params(precision=precision, rho_h=rho_h, rho_l=rho_l, tau_h=3 * nu_h, tau_l=3 * nu_l, sigma=rho_h * U * U * D / We, W=W, M=M,
                        g=(0.0, 0.0, U * U / (Fr * Fr * D)), rho_ref=rho_l,
                        bc=(FREESLIP,) * 4 + (INLET, OUTLET), inlet_u=(0.0, 0.0, U), inlet_phi=1.0, inlet_c=(c, c), inlet_r=r_n, outlet_clamp=1)
     return _case(nxy, nxy, nz, p, phi0, u0, f"jet_paper_{case}_D{D}")
