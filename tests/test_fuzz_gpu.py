@@ -7,7 +7,10 @@ Why 20 steps and not 100: run for 100 steps, 153 of the 160 lattices below still
 seven, four are starts from which the ORACLE itself goes non-finite (seeds 54, 57; 2-D 8, 18), and on three 2-D lattices at density
 ratio 1000 (2-D seeds 5, 29, 37) the difference is 1.4e-10 .. 7.9e-9 in phi -- exactly what two runs of the oracle differ by when
 the input of one is perturbed by 1e-15 relative (4.2e-9, 5.0e-10, 1.4e-10): round-off amplified on the phi plateau, DESIGN.md
-reading G21, not a property of a kernel path."""
+reading G21, not a property of a kernel path.
+
+The seeds 100 .. 699 of both generators went through the same checks once (2026-11-05, one B200, two minutes): no difference beyond the
+tolerances, no start the oracle cannot run."""
 import numpy as np
 import pytest
 
