@@ -81,6 +81,11 @@ typedef struct clip_params {
   int lattice;             /* velocity set: 0 (default) = D3Q19, Eq. 14-15 (:169-176); 1 = D2Q9, the lattice of the paper's 2-D benchmarks
                               (:568): nz must be 1, the z faces PERIODIC, the x / y faces PERIODIC, WALL or FREESLIP; u_z is returned as
                               given to clip_init (0).  Thread-per-node kernels (k_phi9 + k_step9) */
+  int cluster_y;           /* k_fused, tuning / tests: y-adjacent tiles per thread-block cluster, whose shared tile surfaces are completed
+                              through distributed shared memory instead of the partial-sum buffer.  0 = automatic (fp32: 4 at nx = 128,
+                              2 at nx = 192, the lattices with 64- / 96-thread blocks, where it is measured to pay; else none),
+                              1 = none, 2, 4 or 8 = that many where the number of y tiles is a multiple (else none).  Same results bit
+                              for bit */
 } clip_params;
 
 typedef struct clip_handle clip_t;

@@ -31,6 +31,7 @@ class clip_params(C.Structure):
         ("outlet_clamp", C.c_int), ("outlet_u_time", C.c_int),
         ("path", C.c_int), ("tile_ty", C.c_int), ("tile_chunks", C.c_int), ("runtime_nx", C.c_int),
         ("lattice", C.c_int),
+        ("cluster_y", C.c_int),
     ]
 
 
@@ -47,7 +48,7 @@ def make_params(p: dict) -> clip_params:
     s.visc_interp = int(p["visc_interp"])
     s.collision = int(p.get("collision", 0))
     s.phase_only = int(p.get("phase_only", 0))
-    for k in ("outlet_clamp", "outlet_u_time", "path", "tile_ty", "tile_chunks", "runtime_nx", "lattice"):
+    for k in ("outlet_clamp", "outlet_u_time", "path", "tile_ty", "tile_chunks", "runtime_nx", "lattice", "cluster_y"):
         setattr(s, k, int(p.get(k, 0)))
     return s
 

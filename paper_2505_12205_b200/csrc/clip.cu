@@ -39,6 +39,7 @@ struct Layout {
 struct FusedPlan {
   bool ok, fills_gpu, pays, tma, tma_g;  // tma: path 4, k_fused_tma (bulk-async feed) admitted
   int ty, ytiles, nchunks, tzmax, threads, blocks_per_sm;
+  int cs;  // y-adjacent tiles per thread-block cluster (1: none): k_fused<..., CL = true>
   int zc[clip::FUSED_MAX_CHUNKS + 1];  // chunk boundaries along z
   size_t part_words, smem_bytes;
 };
@@ -125,6 +126,13 @@ FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   f.tzmax = 1;
   for (int c = 0; c < nchunks; ++c) f.tzmax = f.zc[c + 1] - f.zc[c] > f.tzmax ? f.zc[c + 1] - f.zc[c] : f.tzmax;
   f.part_words = (size_t)f.ytiles * nchunks * (2 * f.tzmax + 2 * (f.ty + 2)) * nx;
+  // Clusters of y-adjacent tiles (clip_fused.cuh, flush_slot_cl): measured to pay with the small blocks of nx = 128 (RT 128 x 512 x 128
+  // fp32: +2.4 % with 4 tiles) and nx = 192 (the jets, fp32: +1 .. 2 % with 2); slower at nx >= 256 and in fp64 (the per-plane
+  // barrier of the cluster couples the blocks; profiles/r02_experiments.md 4e)
+  f.cs = p->cluster_y;
+  if (f.cs == 0)   // ... and only with several waves of tiles (128^3 with k_fused forced: 0.166 against 0.139 ms)
+    f.cs = (p->precision == 32 && !f.tma && (long long)f.ytiles * max_chunks >= 4 * cap) ? (nx == 128 ? 4 : (nx == 192 ? 2 : 1)) : 1;
+  if (f.cs < 1 || f.tma || f.ytiles % f.cs != 0) f.cs = 1;
   f.ok = true;
   return f;
 }
@@ -190,6 +198,7 @@ const char* validate(int nx, int ny, int nz, const clip_params* p) {
   if (p->tile_ty != 0 && p->tile_ty != 4 && p->tile_ty != 8 && p->tile_ty != 16) return "tile_ty must be 0 (automatic), 4, 8 or 16";
   if (p->tile_chunks < 0) return "tile_chunks must be >= 0";
   if (p->runtime_nx != 0 && p->runtime_nx != 1) return "runtime_nx must be 0 or 1";
+  if (p->cluster_y != 0 && p->cluster_y != 1 && p->cluster_y != 2 && p->cluster_y != 4 && p->cluster_y != 8) return "cluster_y must be 0 (automatic), 1, 2, 4 or 8";
   if (p->lattice != 0 && p->lattice != 1) return "lattice must be 0 (D3Q19) or 1 (D2Q9)";
   if (p->lattice == 1) {
     if (nz != 1 || p->bc[4] != CLIP_BC_PERIODIC || p->bc[5] != CLIP_BC_PERIODIC) return "D2Q9 needs nz = 1 and PERIODIC z faces";
@@ -419,6 +428,7 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       U.ty = fp.ty; U.ytiles = fp.ytiles; U.nchunks = fp.nchunks; U.tzmax = fp.tzmax;
       for (int c = 0; c <= fp.nchunks; ++c) U.zc[c] = fp.zc[c];
       U.tile_stride = (long long)(2 * fp.tzmax + 2 * (fp.ty + 2)) * h->nx;
+      U.cs = 1;
       if (prof) prof->begin();
       cudaError_t fe;
       if (split && !fp.tma && fp.nchunks >= 3 && fp.zc[1] - fp.zc[0] >= 2 && fp.zc[fp.nchunks] - fp.zc[fp.nchunks - 1] >= 2) {
@@ -439,6 +449,9 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
           h->launches += 1;
         }
         cudaStreamWaitEvent(h->stream, h->ev_bnd, 0);
+      } else if (fp.cs > 1) {   // thread-block clusters of fp.cs y-adjacent tiles; k_fix (same U) skips the surfaces they share
+        U.c_mode = 0; U.cs = fp.cs;
+        fe = clip::launch_fused_cl<T>(faces, h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
       } else {
         U.c_mode = 0;
         if (fp.tma) fe = clip::launch_fused_tma<T>(h->nx_special, fp.tma_g, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);

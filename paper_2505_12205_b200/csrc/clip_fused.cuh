@@ -19,6 +19,7 @@
 // sending node as the opposite population, i.e. its g+ lands on the sender's own row and column.
 #pragma once
 #include "clip_fast.cuh"
+#include <cooperative_groups.h>
 
 namespace clip {
 
@@ -33,6 +34,7 @@ template <typename T> struct FusedP {
   int zc[FUSED_MAX_CHUNKS + 1];  // chunk c covers the planes zc[c] .. zc[c+1]-1 (sizes <= tzmax; clip.cu: fused_plan)
   long long tile_stride;  // elements of `part` per tile
   int z_wrap;             // the z faces are PERIODIC: the first and the last chunk are neighbours (k_fix)
+  int cs;                 // tiles per thread-block cluster along y (k_fused<..., CL = true>; k_fix then skips their shared surfaces); <= 1: none
   int c_mode;             // which chunks a k_fused launch covers: 0 all (c = blockIdx.y), 1 the first and the last one, 2 all others
 };
 // rows of a tile's slab in `part`
@@ -157,9 +159,37 @@ __device__ __forceinline__ void flush_slot(T* ring, T* edge_p, T* edge_m, int nx
   }
 }
 
+// Cluster form (k_fused<..., CL = true>): the tiles of a thread-block cluster are neighbours in y.  A halo row that belongs to a tile of
+// the same cluster is not written to `part`: the owner of the lattice row adds it -- read from the neighbour's ring through distributed
+// shared memory, and zeroed there -- to its own sum before the row goes to phi_dst.  lo_* / hi_*: ring and edge arrays of the lower /
+// upper neighbour in the cluster (nullptr: none, that surface goes through `part` as without clusters).
+template <typename T, typename D>
+__device__ __forceinline__ void flush_slot_cl(T* ring, T* edge_p, T* edge_m, int nx, int rows, int nwarps, int warp, int lane, int x0, int s, D dst_row,
+                                              T* lo_ring, T* lo_ep, T* lo_em, T* hi_ring, T* hi_ep, T* hi_em) {
+  typedef P2<T> V;
+  typedef typename PairOf<T>::type U;
+  const int wl = warp == 0 ? nwarps - 1 : warp - 1, wr = warp == nwarps - 1 ? 0 : warp + 1;
+  auto take = [&](T* rg, T* ep, T* em, int row) -> V {   // read and zero one row's column pair (+ the warp-edge sends) of a ring
+    U* p = reinterpret_cast<U*>(rg + (size_t)row * nx + x0);
+    V v = V(*p);
+    *p = V(T(0)).v;
+    if (lane == 0) { T& e = ep[row * nwarps + wl]; v = v + V(e, T(0)); e = T(0); }
+    if (lane == 31) { T& e = em[row * nwarps + wr]; v = v + V(T(0), e); e = T(0); }
+    return v;
+  };
+  for (int j = 0; j < rows; ++j) {
+    if ((j == 0 && lo_ring) || (j == rows - 1 && hi_ring)) continue;   // the neighbour takes (and zeroes) this row
+    V v = take(ring, edge_p, edge_m, s * rows + j);
+    if (j == 1 && lo_ring) v = v + take(lo_ring, lo_ep, lo_em, s * rows + rows - 1);
+    if (j == rows - 2 && hi_ring) v = v + take(hi_ring, hi_ep, hi_em, s * rows);
+    T* d = dst_row(j);
+    if (d) st_pair<T>(d + x0, v);
+  }
+}
+
 // grid = (ytiles, nchunks); block = nx/2 threads (nx % 64 == 0); dynamic shared memory = ring + edges.
 // WALLS (kernel level): 0 = periodic lattice, 1 = lattice with WALL faces, 2 = lattice with FREESLIP (and maybe WALL) faces in x / y
-template <typename T, int NX, int WALLS, int MAXT, int MINB>
+template <typename T, int NX, int WALLS, int MAXT, int MINB, bool CL = false>
 __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP<T> FPp, const FusedP<T> U) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const KP<T>& P = FPp.k;
@@ -176,7 +206,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP
   const int y0 = iy * U.ty, z0 = U.zc[c], z1 = U.zc[c + 1];
   const int tz = z1 - z0;
   for (int i = threadIdx.x; i < nslots * rows * (nx + 2 * nwarps); i += blockDim.x) ring[i] = T(0);
-  __syncthreads();
+  T *lo_ring = nullptr, *lo_ep = nullptr, *lo_em = nullptr, *hi_ring = nullptr, *hi_ep = nullptr, *hi_em = nullptr;
+  if constexpr (CL) {   // cluster (cs, 1, 1): rank = blockIdx.x % cs, the tiles iy - 1 / iy + 1 of the same chunk
+    namespace cg = cooperative_groups;
+    cg::cluster_group cl = cg::this_cluster();
+    const unsigned rk = cl.block_rank(), cs = cl.num_blocks();
+    if (rk > 0) { lo_ring = cl.map_shared_rank(ring, rk - 1); lo_ep = cl.map_shared_rank(edge_p, rk - 1); lo_em = cl.map_shared_rank(edge_m, rk - 1); }
+    if (rk + 1 < cs) { hi_ring = cl.map_shared_rank(ring, rk + 1); hi_ep = cl.map_shared_rank(edge_p, rk + 1); hi_em = cl.map_shared_rank(edge_m, rk + 1); }
+    cl.sync();
+  } else {
+    __syncthreads();
+  }
   T* const slab = U.part + (long long)(c * U.ytiles + iy) * U.tile_stride;
   Scatter<T, WALLS == 2 ? 3 : (WALLS ? 1 : 0)> sc;
   sc.ring = ring; sc.edge_p = edge_p; sc.edge_m = edge_m; sc.nx = nx; sc.rows = rows; sc.nwarps = nwarps; sc.warp = warp; sc.lane = lane;
@@ -189,11 +229,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP
       });
     } else {
       T* const plane = U.phi_dst + ((long long)(z0 + k) * P.ny + y0) * nx;
-      flush_slot<T>(ring, edge_p, edge_m, nx, rows, nwarps, warp, lane, x0, s, [&](int j) -> T* {
+      auto dst = [&](int j) -> T* {
         if (j == 0) return slab + (long long)slot_ym(k) * nx;
         if (j == rows - 1) return slab + (long long)slot_yp(k, U.tzmax) * nx;
         return plane + (long long)(j - 1) * nx;
-      });
+      };
+      if constexpr (CL) flush_slot_cl<T>(ring, edge_p, edge_m, nx, rows, nwarps, warp, lane, x0, s, dst, lo_ring, lo_ep, lo_em, hi_ring, hi_ep, hi_em);
+      else flush_slot<T>(ring, edge_p, edge_m, nx, rows, nwarps, warp, lane, x0, s, dst);
     }
   };
   // FOUR ring slots for three live planes: the slot flushed after plane lz (plane lz-1) is not touched while plane lz+1
@@ -227,11 +269,14 @@ __global__ void __launch_bounds__(MAXT, MINB) k_fused(const __grid_constant__ FP
         step_pair<T, LD_NC, LD_NC, ST_WB, NX, 0>(FPp, x0, y, z, NoWait(), sp);
       }
     }
-    __syncthreads();  // also keeps the block's warps on the same plane: without it the kernel is 4 % slower (L1 reuse)
+    // also keeps the block's warps on the same plane: without it the kernel is 4 % slower (L1 reuse).  Cluster form: the neighbours'
+    // sums of plane lz - 1 are complete, and what they took from this ring during their last flush is zeroed
+    if constexpr (CL) cooperative_groups::this_cluster().sync(); else __syncthreads();
     flush(lz - 1);
   }
   flush(tz - 1);
   flush(tz);
+  if constexpr (CL) cooperative_groups::this_cluster().sync();   // no block leaves while a neighbour may still read its ring
 }
 
 // phi(t+1) of the rows on a tile surface: own sum + the neighbour tiles' partials, fixed order.
@@ -283,14 +328,16 @@ template <typename T> __global__ void __launch_bounds__(FIX_THREADS) k_fix(const
     const bool zlo = lz == 0 && (U.z_wrap || c > 0), zhi = lz == tz - 1 && (U.z_wrap || c < U.nchunks - 1);
     const T* src[8];
     int ns = 0;
-    if (ylo) src[ns++] = slab(c, iym, slot_yp(lz, U.tzmax));
-    if (yhi) src[ns++] = slab(c, iyp, slot_ym(lz));
+    // (cluster form of k_fused: the surfaces between the tiles of a cluster are already complete)
+    if (ylo && (U.cs <= 1 || iy % U.cs == 0)) src[ns++] = slab(c, iym, slot_yp(lz, U.tzmax));
+    if (yhi && (U.cs <= 1 || iy % U.cs == U.cs - 1)) src[ns++] = slab(c, iyp, slot_ym(lz));
     if (zlo) src[ns++] = slab(cm, iy, slot_zp(ly + 1, U.tzmax, U.ty));
     if (zhi) src[ns++] = slab(cp, iy, slot_zm(ly + 1, U.tzmax));
     if (ylo && zlo) src[ns++] = slab(cm, iym, slot_zp(U.ty + 1, U.tzmax, U.ty));
     if (ylo && zhi) src[ns++] = slab(cp, iym, slot_zm(U.ty + 1, U.tzmax));
     if (yhi && zlo) src[ns++] = slab(cm, iyp, slot_zp(0, U.tzmax, U.ty));
     if (yhi && zhi) src[ns++] = slab(cp, iyp, slot_zm(0, U.tzmax));
+    if (ns == 0) continue;
     T* const row = U.phi_dst + ((long long)(z0 + lz) * P.ny + y) * nx;
     for (int v = v0; v < vpr; v += tv) {
       W a = __ldca(reinterpret_cast<const W*>(row) + v);

@@ -23,6 +23,8 @@ template <typename T> void launch_phi2(int faces, int nx, dim3 g, dim3 b, cudaSt
 template <typename T> void launch_step2(int faces, bool xwalls, int nx, dim3 g, dim3 b, cudaStream_t st, const FP<T>& F);
 // returns the CUDA error of the shared-memory opt-in (cudaFuncSetAttribute, once per device and instantiation) or of nothing
 template <typename T> cudaError_t launch_fused(int faces, int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
+// cluster form of k_fused (U.cs tiles per thread-block cluster along y; g.x % U.cs == 0)
+template <typename T> cudaError_t launch_fused_cl(int faces, int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
 // k_fused_tma (bulk-async feed; periodic x / y faces): same grid and FusedP as k_fused, more shared memory
 template <typename T> cudaError_t launch_fused_tma(int nx, bool gonly, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);
 template <typename T> void launch_fix(dim3 g, cudaStream_t st, const FP<T>& F, const FusedP<T>& U);

@@ -89,6 +89,35 @@ template <typename T> cudaError_t launch_fused(int faces, int nx, dim3 g, dim3 b
   if (faces == 2) return nx == 192 ? launch_fused_nx<T, 192, 2>(g, b, smem, st, F, U) : launch_fused_nx<T, 0, 2>(g, b, smem, st, F, U);  // as launch_step2
   return faces ? launch_fused_w<T, 1>(nx, g, b, smem, st, F, U) : launch_fused_w<T, 0>(nx, g, b, smem, st, F, U);
 }
+template <typename T, int NX, int W> cudaError_t launch_fused_cl_nx(dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
+  constexpr int MAXT = NX ? NX / 2 : 256;
+  constexpr int TPSM = fused_threads_per_sm(sizeof(T) == 4 ? 32 : 64, MAXT);
+  constexpr int MINB = TPSM / MAXT > 0 ? TPSM / MAXT : 1;
+  auto kern = k_fused<T, NX, W, MAXT, MINB, true>;
+  static bool attr_done[MAX_DEVICES] = {};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= MAX_DEVICES || !attr_done[dev]) {
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024);
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < MAX_DEVICES) attr_done[dev] = true;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = g; cfg.blockDim = b; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = (unsigned)U.cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, F, U);
+}
+// Cluster form: own instantiations for the widths where clusters are the default (nx = 128, 192); every other width takes the
+// runtime-nx kernel (clip_params.cluster_y forced: tests, tuning).
+template <typename T> cudaError_t launch_fused_cl(int faces, int nx, dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
+  if (faces == 2) return nx == 192 ? launch_fused_cl_nx<T, 192, 2>(g, b, smem, st, F, U) : launch_fused_cl_nx<T, 0, 2>(g, b, smem, st, F, U);
+  if (faces) return nx == 128 ? launch_fused_cl_nx<T, 128, 1>(g, b, smem, st, F, U) : (nx == 192 ? launch_fused_cl_nx<T, 192, 1>(g, b, smem, st, F, U) : launch_fused_cl_nx<T, 0, 1>(g, b, smem, st, F, U));
+  return nx == 128 ? launch_fused_cl_nx<T, 128, 0>(g, b, smem, st, F, U) : (nx == 192 ? launch_fused_cl_nx<T, 192, 0>(g, b, smem, st, F, U) : launch_fused_cl_nx<T, 0, 0>(g, b, smem, st, F, U));
+}
 template <typename T, int NX, bool GONLY> cudaError_t launch_fused_tma_nx(dim3 g, dim3 b, size_t smem, cudaStream_t st, const FP<T>& F, const FusedP<T>& U) {
   constexpr int MAXT = NX ? NX / 2 : 256;
   constexpr int MINB = (GONLY && sizeof(T) == 4 && 384 / MAXT > 0) ? 384 / MAXT : 1;   // hybrid: k_fused's occupancy

@@ -34,7 +34,7 @@ def default_params(**kw) -> dict:
         outlet_u_mode=0, visc_interp=0, collision=0, phase_only=0,
         outlet_clamp=0, outlet_u_time=0,
         lattice=0,  # 0 = D3Q19; 1 = D2Q9 (nz = 1, z faces PERIODIC): the lattice of the paper's 2-D benchmarks
-        path=0, tile_ty=0, tile_chunks=0, runtime_nx=0,  # libclip only: kernel path / tiling (include/clip.h); the oracle ignores them
+        path=0, tile_ty=0, tile_chunks=0, runtime_nx=0, cluster_y=0,  # libclip only: kernel path / tiling (include/clip.h); the oracle ignores them
     )
     p.update(kw)
     return p

@@ -435,6 +435,31 @@ def test_fused_single_pass_path(name, precision):
             assert np.abs(a - b).max() <= tol * max(1.0, np.abs(a).max()), (name, env)
 
 
+CLUSTER_LATTICES = dict(FUSED_LATTICES)
+CLUSTER_LATTICES.update({
+    "periodic_128x32x12": lambda: inputs.sweep_drops(shape=(128, 32, 12), ndrops=6, rmin=3, rmax=6),      # 8 y tiles: clusters of 2, 4, 8
+    "rt_wide_128x64x16": lambda: _with(inputs.sweep_drops(shape=(128, 64, 16), ndrops=8, rmin=3, rmax=7), bc=(inputs.PERIODIC, inputs.PERIODIC, inputs.WALL, inputs.WALL, inputs.PERIODIC, inputs.PERIODIC), rho_l=0.1, g=(0.0, -1e-5, 0.0)),
+    "walled_192x16x8": lambda: inputs.walled_box(nx=192, ny=16, nz=8),                                      # the jet's width, 4 y tiles
+})
+
+
+@pytest.mark.parametrize("name", list(CLUSTER_LATTICES))
+@pytest.mark.parametrize("precision", [64, 32])
+def test_fused_thread_block_clusters(name, precision):
+    """k_fused with thread-block clusters of y-adjacent tiles (clip_params.cluster_y; the tile surfaces inside a cluster are completed
+    through distributed shared memory, k_fix skips them) against k_fused without: the additions keep their order, so the fields are
+    equal BIT FOR BIT -- clusters of 2, 4, 8 tiles (where the tile count allows; else the request falls back to none), default and
+    forced tilings, the runtime-nx form, walls, free-slip, open z faces."""
+    case = CLUSTER_LATTICES[name]()
+    steps = 30
+    for tiling in ({}, {"tile_chunks": 1}, {"tile_chunks": 3, "runtime_nx": 1}):
+        ref = _gpu_p(case, steps, precision, path=3, cluster_y=1, **tiling)
+        for cs in (2, 4, 8, 0):
+            out = _gpu_p(case, steps, precision, path=3, cluster_y=cs, **tiling)
+            for a, b in zip(ref, out):
+                assert np.array_equal(a, b), (name, cs, tiling)
+
+
 @pytest.mark.parametrize("path", [4, 5])
 @pytest.mark.parametrize("precision", [64, 32])
 def test_fused_tma_path(precision, path):
