@@ -495,6 +495,7 @@ def test_graph_replay_of_small_lattices_is_exact(precision):
     import torch
     from paper_2505_12205_b200 import clip
     cases = [(inputs.sweep_drops(n=32, ndrops=3, rmin=3, rmax=6), {}), (inputs.sweep_drops(shape=(64, 16, 12), ndrops=4, rmin=3, rmax=5), {"path": 3}),
+             (inputs.sweep_drops(shape=(64, 16, 12), ndrops=4, rmin=3, rmax=5), {"path": 3, "cluster_y": 2}),   # cluster launches inside a graph
              (inputs.jet(nxy=24, nz=32, r_nozzle=4.0), {}), (inputs.sweep_drops(shape=(21, 12, 10), ndrops=3, rmin=3, rmax=4), {})]
     for case, over in cases:
         c = dict(case, params=dict(case["params"], **over))
@@ -522,6 +523,7 @@ def test_the_caller_may_capture_clip_step_in_a_cuda_graph(precision):
     import torch
     from paper_2505_12205_b200 import clip
     cases = [(inputs.sweep_drops(n=32, ndrops=3, rmin=3, rmax=6), {}), (inputs.sweep_drops(shape=(64, 16, 12), ndrops=4, rmin=3, rmax=5), {"path": 3}),
+             (inputs.sweep_drops(shape=(64, 16, 12), ndrops=4, rmin=3, rmax=5), {"path": 3, "cluster_y": 2}),   # cluster launches inside a graph
              (inputs.jet(nxy=24, nz=32, r_nozzle=4.0), {}), (inputs.sweep_drops(shape=(21, 12, 10), ndrops=3, rmin=3, rmax=4), {})]
     for case, over in cases:
         c = dict(case, params=dict(case["params"], **over))
