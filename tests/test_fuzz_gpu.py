@@ -114,7 +114,7 @@ _fused_seen = []
 @pytest.mark.parametrize("seed", range(24))
 def test_k_fused_with_random_tilings_on_a_random_wide_lattice(seed):
     """Wider lattices (nx 64 .. 320, ny 8 .. 32, nz 8 .. 33) with `path = 3` (k_fused wherever the lattice admits it) and seeded tile
-    heights, chunk counts and the runtime-nx form: the single-pass kernel's tile / chunk / halo logic against the oracle, fp64 and
+    heights, chunk counts, cluster sizes and the runtime-nx form: the single-pass kernel's tile / chunk / halo logic against the oracle, fp64 and
     fp32; where the lattice is thick enough also cut into slabs that take the overlapped step (clip_step_halo_begin / _end)."""
     import torch
     from oracle.clip_oracle import Oracle
@@ -126,7 +126,8 @@ def test_k_fused_with_random_tilings_on_a_random_wide_lattice(seed):
     ref = o.get()
     assert all(np.isfinite(a).all() for a in ref)
     for precision in (64, 32):
-        over = dict(path=3, tile_ty=int(rng.choice([0, 4, 8])), tile_chunks=int(rng.choice([0, 0, 1, 2, 3, 5])), runtime_nx=int(rng.choice([0, 0, 1])))
+        over = dict(path=3, tile_ty=int(rng.choice([0, 4, 8])), tile_chunks=int(rng.choice([0, 0, 1, 2, 3, 5])), runtime_nx=int(rng.choice([0, 0, 1])),
+                    cluster_y=int(rng.choice([0, 1, 2, 4])))
         sim = clip.Clip(case["nx"], case["ny"], case["nz"], dict(case["params"], precision=precision, **over))
         sim.init(torch.as_tensor(case["phi0"]), torch.as_tensor(case["u0"]))
         sim.step(STEPS)
@@ -143,7 +144,7 @@ def test_k_fused_with_random_tilings_on_a_random_wide_lattice(seed):
     if case["nz"] // 3 >= 4:
         world = 2 + seed % 2
         phi0, u0 = torch.as_tensor(case["phi0"]), torch.as_tensor(case["u0"])
-        group = [slab.SlabClip(case["nx"], case["ny"], case["nz"], dict(case["params"], precision=64, path=3), r, world, overlap=True) for r in range(world)]
+        group = [slab.SlabClip(case["nx"], case["ny"], case["nz"], dict(case["params"], precision=64, path=3, cluster_y=2 * (seed % 2)), r, world, overlap=True) for r in range(world)]
         for s in group:
             s.init(phi0, u0)
         slab.step_group(group, STEPS)
