@@ -251,7 +251,7 @@ template <typename T> clip::KP<T> make_kp(const clip_handle* h) {
   P.nxy = (long long)h->nx * h->ny;
   P.any_nonperiodic = 0;
   for (int k = 0; k < 6; ++k) { P.bc[k] = p.bc[k]; if (p.bc[k] != CLIP_BC_PERIODIC) P.any_nonperiodic = 1; }
-  P.z_lo = h->zlo; P.z_cnt = h->zhi - h->zlo;
+  P.z_lo = h->zlo; P.z_cnt = h->zhi - h->zlo; P.z_skip_at = 0; P.z_skip = 0;
   P.has_inlet = p.bc[4] == CLIP_BC_INLET;
   P.has_outlet = p.bc[5] == CLIP_BC_OUTLET;
   P.visc_interp = p.visc_interp;
@@ -360,15 +360,13 @@ template <typename T> void fused_open_planes(clip_handle* h, Prof* prof) {
   clip::KP<T> P = make_kp<T>(h);
   P.phi = (T*)(h->ws + (h->phi_cur ? h->L.off_phi : h->L.off_phi2));
   if (P.has_outlet) outlet_lambda<T>(h, P, prof);
-  for (int side = 0; side < 2; ++side) {
-    if (!(side ? ghi : glo)) continue;
-    clip::KP<T> Q = P;
-    Q.z_lo = side ? h->nz - 2 : 0; Q.z_cnt = 2;
-    if (prof) prof->begin();
-    clip::k_phi<T><<<grid_for(2 * P.nxy, 256), 256, 0, h->stream>>>(Q);
-    if (prof) prof->end(KIND_PHI);
-    h->launches += 1;
-  }
+  clip::KP<T> Q = P;   // planes 0, 1 and / or nz-2, nz-1 in one launch
+  Q.z_lo = glo ? 0 : h->nz - 2; Q.z_cnt = 2 * (glo + ghi);
+  if (glo && ghi) { Q.z_skip_at = 2; Q.z_skip = h->nz - 4; }
+  if (prof) prof->begin();
+  clip::k_phi<T><<<grid_for(Q.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(Q);
+  if (prof) prof->end(KIND_PHI);
+  h->launches += 1;
 }
 
 // k_fused path, once after clip_init: phi(t+1) = sum_a g+_a(x - e_a, t) into the second phi buffer (one k_phi2 launch, plus the
@@ -412,14 +410,17 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       T* const phi_next = (T*)(h->ws + (h->phi_cur ? h->L.off_phi : h->L.off_phi2));
       F.k.phi = phi_next;
       fused_prepass<T>(h, prof);
-      for (int side = 0; side < 2; ++side) {  // the INLET / OUTLET plane: generic kernel, phi(t+1) and lambda are in place
-        if (!(side ? h->p.bc[5] == CLIP_BC_OUTLET : h->p.bc[4] == CLIP_BC_INLET)) continue;
-        clip::KP<T> Q = F.k;
-        Q.z_lo = side ? h->nz - 1 : 0; Q.z_cnt = 1;
-        if (prof) prof->begin();
-        clip::k_step<T, true><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Q);   // the k_fused path is WMRT, two-phase
-        if (prof) prof->end(KIND_STEP);
-        h->launches += 1;
+      {  // the INLET / OUTLET planes (one launch for both): generic kernel, phi(t+1) and lambda are in place
+        const int olo = h->p.bc[4] == CLIP_BC_INLET ? 1 : 0, ohi = h->p.bc[5] == CLIP_BC_OUTLET ? 1 : 0;
+        if (olo + ohi) {
+          clip::KP<T> Q = F.k;
+          Q.z_lo = olo ? 0 : h->nz - 1; Q.z_cnt = olo + ohi;
+          if (olo && ohi) { Q.z_skip_at = 1; Q.z_skip = h->nz - 2; }
+          if (prof) prof->begin();
+          clip::k_step<T, true><<<grid_for(Q.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(Q);   // the k_fused path is WMRT, two-phase
+          if (prof) prof->end(KIND_STEP);
+          h->launches += 1;
+        }
       }
       clip::FusedP<T> U;
       U.z_wrap = h->p.bc[4] == CLIP_BC_PERIODIC ? 1 : 0;
@@ -472,8 +473,9 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
     }
     // planes next to an INLET / OUTLET face: generic kernels; all other planes: pair kernels (when the lattice allows)
     const int glo = (fast && h->p.bc[4] == CLIP_BC_INLET) ? 1 : 0, ghi = (fast && h->p.bc[5] == CLIP_BC_OUTLET) ? 1 : 0;
-    clip::KP<T> Plo = P, Phi = P;
-    Plo.z_lo = 0; Plo.z_cnt = glo; Phi.z_lo = h->nz - ghi; Phi.z_cnt = ghi;
+    clip::KP<T> Pface = P;   // the planes z = 0 and / or nz-1, one launch
+    Pface.z_lo = glo ? 0 : h->nz - 1; Pface.z_cnt = glo + ghi;
+    if (glo && ghi) { Pface.z_skip_at = 1; Pface.z_skip = h->nz - 2; }
     clip::FP<T> F;
     if (fast) { F = make_fp<T>(P); F.k.z_lo = h->zlo + glo; F.k.z_cnt = h->zhi - ghi - F.k.z_lo; fg.z = (unsigned)F.k.z_cnt; }
     if (P.has_outlet) outlet_lambda<T>(h, P, prof);  // lambda of B.25 for this step, before anything of the step reads it
@@ -496,13 +498,12 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
         if (prof) prof->end(pass == 0 ? KIND_PHI : KIND_STEP);
         continue;
       }
-      for (int side = 0; side < 2; ++side) {
-        if (!(side ? ghi : glo)) continue;
-        const clip::KP<T>& Q = side ? Phi : Plo;
+      if (glo + ghi) {
+        const clip::KP<T>& Q = Pface;
         if (prof) prof->begin();
-        if (pass == 0) clip::k_phi<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Q);
-        else if (plain) clip::k_step<T, true><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Q);
-        else clip::k_step<T><<<grid_for(P.nxy, 256), 256, 0, h->stream>>>(Q);
+        if (pass == 0) clip::k_phi<T><<<grid_for(Q.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(Q);
+        else if (plain) clip::k_step<T, true><<<grid_for(Q.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(Q);
+        else clip::k_step<T><<<grid_for(Q.z_cnt * P.nxy, 256), 256, 0, h->stream>>>(Q);
         h->launches += 1;
         if (prof) prof->end(pass == 0 ? KIND_PHI : KIND_STEP);
       }

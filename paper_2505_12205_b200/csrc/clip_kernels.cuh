@@ -53,6 +53,8 @@ template <typename T> struct KP {
   int bc[6];
   int has_inlet, has_outlet, any_nonperiodic, visc_interp, collision, phase_only, outlet_u_mode, outlet_clamp, outlet_u_time;
   int z_lo, z_cnt;  // planes [z_lo, z_lo + z_cnt) a k_phi* / k_step* launch covers (whole lattice: 0, nz)
+  int z_skip_at, z_skip;  // generic k_phi / k_step: the launch's planes number z_skip_at and up lie z_skip planes further on (the planes next
+                          // to an INLET and an OUTLET face in ONE launch); none: z_skip = 0
   T rho_h, rho_l, drho;
   T tau_h, tau_l, itau_h, itau_l, rt_h, rt_l;  // rt = rho tau = 3 mu (Eq. 23, 25)
   T beta4, kappa, inv_W, om_phi;
@@ -446,7 +448,7 @@ template <typename T> __global__ void __launch_bounds__(1024) k_outlet_reduce(co
 template <typename T> __global__ void __launch_bounds__(256) k_phi(const __grid_constant__ KP<T> P) {
   const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= P.z_cnt * P.nxy) return;
-  const long long i = j + P.z_lo * P.nxy;
+  const long long i = j + (P.z_lo + (P.z_skip && j >= P.z_skip_at * P.nxy ? P.z_skip : 0)) * P.nxy;
   const int x = (int)(i % P.nx);
   const long long r = i / P.nx;
   const int y = (int)(r % P.ny), z = (int)(r / P.ny);
@@ -462,7 +464,7 @@ template <typename T> __global__ void __launch_bounds__(256) k_phi(const __grid_
 template <typename T, bool PLAIN = false> __global__ void __launch_bounds__(256) k_step(const __grid_constant__ KP<T> P) {
   const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= P.z_cnt * P.nxy) return;
-  const long long i = j + P.z_lo * P.nxy;
+  const long long i = j + (P.z_lo + (P.z_skip && j >= P.z_skip_at * P.nxy ? P.z_skip : 0)) * P.nxy;
   const int x = (int)(i % P.nx);
   const long long r = i / P.nx;
   const int y = (int)(r % P.ny), z = (int)(r / P.ny);
