@@ -453,6 +453,11 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
       } else if (fp.cs > 1) {   // thread-block clusters of fp.cs y-adjacent tiles; k_fix (same U) skips the surfaces they share
         U.c_mode = 0; U.cs = fp.cs;
         fe = clip::launch_fused_cl<T>(faces, h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+        if (fe != cudaSuccess) {  // a device / partition that cannot place the cluster: the plain kernel from now on (same results)
+          cudaGetLastError();
+          h->fplan.cs = 1; U.cs = 1;
+          fe = clip::launch_fused<T>(faces, h->nx_special, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
+        }
       } else {
         U.c_mode = 0;
         if (fp.tma) fe = clip::launch_fused_tma<T>(h->nx_special, fp.tma_g, dim3(fp.ytiles, fp.nchunks), dim3(fp.threads), fp.smem_bytes, h->stream, F, U);
