@@ -192,6 +192,7 @@ def run_ours(args):
         case = inputs.sweep_drops(n=n, seed=rank_seed(rank), precision=prec)
     case["params"]["path"] = args.path
     case["params"]["tile_ty"], case["params"]["tile_chunks"] = args.tile_ty, args.tile_chunks
+    case["params"]["cluster_y"] = args.cluster_y
     nxl, nyl, nzl = case["nx"], case["ny"], case["nz"]
     nodes = nxl * nyl * nzl
     # a stream of its own (not the legacy default stream): clip_step can then replay small lattices from a CUDA graph (clip.h)
@@ -539,6 +540,7 @@ def main():
                     help="clip_params.path: 0 automatic (default), 1 generic kernels, 2 pair kernels (k_phi2 + k_step2), 3 k_fused wherever admitted")
     ap.add_argument("--case", default="l", help="--long-run jetpaper: row of the paper's Table 6 (a .. l)")
     ap.add_argument("--tile-ty", type=int, default=0, help="clip_params.tile_ty (k_fused rows per tile: 0 automatic, 4, 8, 16)")
+    ap.add_argument("--cluster-y", type=int, default=0, choices=[0, 1, 2, 4, 8], help="clip_params.cluster_y (k_fused: y tiles per thread-block cluster; 0 automatic, 1 none)")
     ap.add_argument("--tile-chunks", type=int, default=0, help="clip_params.tile_chunks (k_fused: number of equal z chunks, 0 automatic)")
     ap.add_argument("--long-run", default=None, choices=["rt", "jet", "jetpaper"],
                     help="run BASELINE configs[2] (rt, 20000 steps) or configs[3] (jet, 50000 steps) at full length with diagnostics; one JSON line")
