@@ -137,6 +137,39 @@ FusedPlan fused_plan(int nx, int ny, int nz, const clip_params* p) {
   return f;
 }
 
+// Single-pass path of the D2Q9 lattice (clip_d2q9.cuh, k_fused9 + k_fix9): chunks of whole rows, one block each; as many chunks as
+// fill a whole number of waves of resident blocks with at most 16 rows each.
+struct Fused9Plan {
+  bool ok, pays;
+  int nchunks, threads;
+  size_t smem_bytes, part_words;
+};
+Fused9Plan fused9_plan(int nx, int ny, const clip_params* p) {
+  Fused9Plan f{};
+  if (p->lattice != 1 || p->phase_only || nx % 64 != 0 || ny < 4 || p->path < 3) return f;   // built (and given its two buffers) on request only
+  const size_t word = p->precision == 32 ? 4 : 8;
+  f.smem_bytes = 4 * ((size_t)nx + 2 * (size_t)(nx / 64)) * word;
+  if (f.smem_bytes + 1024 > 227 * 1024) return f;
+  f.threads = nx / 2 < 256 ? nx / 2 : 256;
+  int bps = (int)((227 * 1024) / (f.smem_bytes + 1024));
+  const int by_regs = p->precision == 32 ? 2048 / 4 / f.threads : 256 / f.threads;   // <= 128 registers (fp32) / 255 (fp64) per thread
+  if (bps > by_regs) bps = by_regs;
+  if (bps < 1) bps = 1;
+  const long long cap = (long long)B200_SMS * bps;
+  long long n = cap;
+  while (ny / n > 16 && n + cap <= clip::d2q9::FUSED9_MAX_CHUNKS) n += cap;   // more waves rather than chunks of more than 16 rows
+  if (n > ny / 2) n = ny / 2 > 0 ? ny / 2 : 1;                                 // at least two rows per chunk
+  if (p->tile_chunks >= 1) n = p->tile_chunks < ny ? p->tile_chunks : ny;
+  if (n > clip::d2q9::FUSED9_MAX_CHUNKS) n = clip::d2q9::FUSED9_MAX_CHUNKS;
+  f.nchunks = (int)n;
+  f.part_words = (size_t)f.nchunks * 2 * nx;
+  // measured (profiles/r02_experiments.md 4f): correct, 1.036 x the algorithmic DRAM traffic, but issue-bound at two 256-thread blocks per
+  // SM: 4096^2 fp32 0.559 ms against 0.524 for k_phi9p + k_step9p, fp64 1.062 against 1.001 -- an option (path = 3), never the default
+  f.pays = false;
+  f.ok = true;
+  return f;
+}
+
 Layout make_layout(int nx, int ny, int nz, const clip_params* p) {
   Layout L{};
   L.word = p->precision == 32 ? 4 : 8;
@@ -153,8 +186,9 @@ Layout make_layout(int nx, int ny, int nz, const clip_params* p) {
   L.off_lam = take(outlet ? nxy * L.word : 0);
   L.off_mask = take(inlet ? nxy : 0);
   const FusedPlan fp = fused_plan(nx, ny, nz, p);                // k_fused: second phi buffer + tile-halo partial sums
-  L.off_phi2 = take(fp.ok ? n * L.word : 0);
-  L.off_part = take(fp.ok ? fp.part_words * L.word : 0);
+  const Fused9Plan f9 = fused9_plan(nx, ny, p);                   // the D2Q9 single-pass path: the same two buffers
+  L.off_phi2 = take((fp.ok || f9.ok) ? n * L.word : 0);
+  L.off_part = take(fp.ok ? fp.part_words * L.word : (f9.ok ? f9.part_words * L.word : 0));
   L.total = o;
   return L;
 }
@@ -230,6 +264,7 @@ struct clip_handle {
   long long graph_launches;  // kernel launches inside one replay
   long long graph_steps;     // time steps run by graph replays so far (instrumentation)
   FusedPlan fplan;
+  Fused9Plan f9;
   bool inited;
   int mode;            // clip_params.path: 0 = automatic (k_fused + k_fix on wide lattices, else k_phi2 + k_step2), 1 = generic kernels
                        // only, 2 = k_phi2 + k_step2, 3 = k_fused wherever the lattice allows
@@ -341,6 +376,7 @@ struct Prof {  // optional per-launch event timing (clip_step_profiled)
 };
 
 bool use_fused(const clip_handle* h) { return fast_ok(h) && h->fplan.ok && (h->mode >= 3 || (h->mode == 0 && h->fplan.pays)); }
+bool use_fused9(const clip_handle* h) { return h->p.lattice == 1 && h->f9.ok && (h->mode >= 3 || (h->mode == 0 && h->f9.pays)); }
 
 // lambda of B.25 for the step about to run (k_outlet_lam; the plane-wide schemes of B.22 add a one-block reduction)
 template <typename T> void outlet_lambda(clip_handle* h, const clip::KP<T>& P, Prof* prof) {
@@ -401,6 +437,45 @@ template <typename T> int do_step(clip_handle* h, int nsteps, Prof* prof = nullp
   const bool plain = h->p.collision == CLIP_COLL_WMRT && !h->p.phase_only;   // k_step<T, true>: no mode tests in the direction loop
   for (int s = 0; s < nsteps; ++s) {
     clip::KP<T> P = make_kp<T>(h);
+    if (use_fused9(h)) {  // D2Q9, one pass over f and g (clip_d2q9.cuh): the state is that of the k_fused path below
+      const Fused9Plan& f9 = h->f9;
+      T* const phi_now = (T*)(h->ws + (h->phi_cur ? h->L.off_phi2 : h->L.off_phi));
+      T* const phi_next = (T*)(h->ws + (h->phi_cur ? h->L.off_phi : h->L.off_phi2));
+      const dim3 g9((h->nx / 2 + 127) / 128, h->ny);
+      if (!h->phi_ahead) {   // once after clip_init: phi(t+1) = sum_a g+_a(x - e_a, t)
+        clip::KP<T> Q = P;
+        Q.phi = phi_next;
+        if (prof) prof->begin();
+        clip::d2q9::k_phi9p<T><<<g9, 128, 0, h->stream>>>(Q);
+        if (prof) prof->end(KIND_PHI2);
+        h->launches += 1;
+        h->phi_ahead = true;
+      }
+      clip::KP<T> Q = P;
+      Q.phi = phi_next;
+      clip::d2q9::Fused9P<T> U9;
+      U9.phi_dst = phi_now; U9.part = (T*)(h->ws + h->L.off_part); U9.nchunks = f9.nchunks;
+      auto kern = clip::d2q9::k_fused9<T>;
+      constexpr int DEV_MAX = 64;
+      static bool attr9[DEV_MAX] = {};   // the shared-memory opt-in is per device (and per T: do_step<T>)
+      int dev = 0;
+      cudaGetDevice(&dev);
+      if (dev < 0 || dev >= DEV_MAX || !attr9[dev]) {
+        const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024);
+        if (e != cudaSuccess) { set_err(h->err, "k_fused9: %s", cudaGetErrorString(e)); return CLIP_ECUDA; }
+        if (dev >= 0 && dev < DEV_MAX) attr9[dev] = true;
+      }
+      if (prof) prof->begin();
+      kern<<<f9.nchunks, f9.threads, f9.smem_bytes, h->stream>>>(Q, U9);
+      if (prof) { prof->end(KIND_FUSED); prof->begin(); }
+      clip::d2q9::k_fix9<T><<<dim3(f9.nchunks, (h->nx / 2 + 127) / 128), 128, 0, h->stream>>>(Q, U9);
+      if (prof) prof->end(KIND_FIX);
+      h->launches += 2;
+      h->cur ^= 1;
+      h->phi_cur ^= 1;
+      h->t += 1;
+      continue;
+    }
     if (fused) {  // one pass over f and g (clip_fused.cuh) + the tile-surface fix-up of phi(t+2)
       // State between fused steps: populations f+(t), g+(t); phi buffer `phi_cur` = phi(t) (what clip_get returns), the
       // other buffer = phi(t+1) = sum_a g+_a(x - e_a, t), which the collision at t+1 needs (first step: one k_phi2).
@@ -639,7 +714,7 @@ bool graph_eligible(const clip_handle* h) {
 template <typename T> int step_graphed(clip_handle* h, int n) {
   if (n < 2 * GRAPH_STEPS || (h->graph_tried && !h->gexec) || !graph_eligible(h)) return do_step<T>(h, n);
   // reach the state the graph is (to be) captured in: buffer parity 0 and, on the k_fused path, phi(t+1) in place
-  while (n > 0 && (h->cur != 0 || (use_fused(h) && !h->phi_ahead))) {
+  while (n > 0 && (h->cur != 0 || ((use_fused(h) || use_fused9(h)) && !h->phi_ahead))) {
     const int rc = do_step<T>(h, 1);
     if (rc != CLIP_OK) return rc;
     --n;
@@ -789,6 +864,7 @@ int clip_create(clip_t** out, int nx, int ny, int nz, const clip_params* params,
   h->gexec = nullptr; h->graph_tried = false; h->graph_launches = 0; h->graph_steps = 0;
   h->zlo = params->bc[4] == CLIP_BC_HALO ? 1 : 0; h->zhi = nz - (params->bc[5] == CLIP_BC_HALO ? 1 : 0);
   h->fplan = fused_plan(nx, ny, nz, params);
+  h->f9 = fused9_plan(nx, ny, params);
   h->mode = params->path;
   h->fast_threads = 128;  // measured: fp64 8.2 vs 7.6 GLUPS, fp32 (with 3 blocks per SM) +2 % against 256-thread blocks
   h->nx_special = params->runtime_nx ? 0 : nx;

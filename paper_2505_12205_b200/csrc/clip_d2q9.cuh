@@ -11,6 +11,8 @@
 // FREESLIP in x and y; nz = 1.  State: pop [ny][18][nx] (A/B), phi [ny][nx], u [3][ny][nx] (u_z == 0, never touched by a step).
 #pragma once
 #include "clip_kernels.cuh"
+#include "clip_fused.cuh"
+#include <type_traits>
 
 namespace clip {
 namespace d2q9 {
@@ -251,11 +253,16 @@ template <typename T> __device__ __forceinline__ Geo9 make_geo9(const KP<T>& P, 
   g.cxp = g.wp ? (P.bc[1] == BC_PERIODIC ? 2 - P.nx : 1) : 2;
   return g;
 }
-template <typename T, int a, int SET> __device__ __forceinline__ P2<T> pull9p(const T* __restrict__ src, const Geo9& g) {
+// LEAN: the pair is away from every face and from the row ends (no wrap, bounce or reflection to select): plain shifted loads
+template <typename T, int a, int SET, bool LEAN = false> __device__ __forceinline__ P2<T> pull9p(const T* __restrict__ src, const Geo9& g) {
   const int nx = g.nx;
   const long long rs = ey(a) == 1 ? g.rm : (ey(a) == -1 ? g.rp : g.r0);   // the row the population comes from
   const T* __restrict__ rp = src + rs + (SET * Q9 + a) * nx + g.x0;
   if (a == 0) return ld_pair<T>(rp);
+  if (LEAN) {
+    if (ex(a) == 0) return ld_pair<T>(rp);
+    return ex(a) == 1 ? P2<T>(ld_one<T>(rp - 1), ld_one<T>(rp)) : P2<T>(ld_one<T>(rp + 1), ld_one<T>(rp + 2));
+  }
   const T* __restrict__ own = src + g.r0 + (SET * Q9 + opp9(a)) * nx + g.x0;
   const bool rb = (ey(a) == 1 && g.bym) || (ey(a) == -1 && g.byp);
   const bool ry = (ey(a) == 1 && g.sym) || (ey(a) == -1 && g.syp);
@@ -279,26 +286,26 @@ template <typename T, int a, int SET> __device__ __forceinline__ P2<T> pull9p(co
   if (rb) { plo = own; phi = own + 1; }
   return P2<T>(ld_one<T>(plo), ld_one<T>(phi));
 }
-template <typename T, int SET, int a = 0> struct Pull9p {
+template <typename T, int SET, bool LEAN = false, int a = 0> struct Pull9p {
   static __device__ __forceinline__ void run(const T* __restrict__ src, const Geo9& g, P2<T> (&v)[Q9]) {
-    v[a] = pull9p<T, a, SET>(src, g);
-    Pull9p<T, SET, a + 1>::run(src, g, v);
+    v[a] = pull9p<T, a, SET, LEAN>(src, g);
+    Pull9p<T, SET, LEAN, a + 1>::run(src, g, v);
   }
 };
-template <typename T, int SET> struct Pull9p<T, SET, Q9> { static __device__ __forceinline__ void run(const T* __restrict__, const Geo9&, P2<T> (&)[Q9]) {} };
+template <typename T, int SET, bool LEAN> struct Pull9p<T, SET, LEAN, Q9> { static __device__ __forceinline__ void run(const T* __restrict__, const Geo9&, P2<T> (&)[Q9]) {} };
 
 template <typename T> struct Row3p { P2<T> L, C, R; };
-template <typename T> __device__ __forceinline__ Row3p<T> ld_row3p(const T* __restrict__ phi, int row, const Geo9& g) {
+template <typename T, bool LEAN = false> __device__ __forceinline__ Row3p<T> ld_row3p(const T* __restrict__ phi, int row, const Geo9& g) {
   Row3p<T> r;
   r.C = ld_pair<T>(phi + row + g.x0);
-  const T m = ld_one<T>(phi + row + g.x0 + g.cxm), p = ld_one<T>(phi + row + g.x0 + g.cxp);
+  const T m = ld_one<T>(phi + row + g.x0 + (LEAN ? -1 : g.cxm)), p = ld_one<T>(phi + row + g.x0 + (LEAN ? 2 : g.cxp));
   r.L = P2<T>(m, r.C.lo());
   r.R = P2<T>(r.C.hi(), p);
   return r;
 }
-template <typename T> __device__ __forceinline__ void stencil9p(const T* __restrict__ phi, const Geo9& g, P2<T>& pc, P2<T> (&G)[2], P2<T>& L) {
+template <typename T, bool LEAN = false> __device__ __forceinline__ void stencil9p(const T* __restrict__ phi, const Geo9& g, P2<T>& pc, P2<T> (&G)[2], P2<T>& L) {
   typedef P2<T> V;
-  const Row3p<T> c = ld_row3p<T>(phi, g.p0, g), yp = ld_row3p<T>(phi, g.pp, g), ym = ld_row3p<T>(phi, g.pm, g);
+  const Row3p<T> c = ld_row3p<T, LEAN>(phi, g.p0, g), yp = ld_row3p<T, LEAN>(phi, g.pp, g), ym = ld_row3p<T, LEAN>(phi, g.pm, g);
   pc = c.C;
   const V d1 = c.R - pc, d2 = c.L - pc, d3 = yp.C - pc, d4 = ym.C - pc;
   const V d5 = yp.R - pc, d6 = ym.L - pc, d7 = ym.R - pc, d8 = yp.L - pc;
@@ -395,18 +402,16 @@ template <typename T> __global__ void __launch_bounds__(128) k_phi9p(const __gri
   Pull9p<T, 1>::run(P.p_src, g, v);
   st_pair<T>(P.phi + g.p0 + x0, (v[0] + ((v[1] + v[2]) + (v[3] + v[4]))) + ((v[5] + v[6]) + (v[7] + v[8])));
 }
-template <typename T> __global__ void __launch_bounds__(128) k_step9p(const __grid_constant__ KP<T> P) {
+// One node pair of row y: stream -> BC -> macros -> both collisions -> store; g holds the post-collision g+ on return.
+template <typename T, bool LEAN = false> __device__ __forceinline__ void step9p_pair(const KP<T>& P, const Geo9& geo, int x0, P2<T> (&g)[Q9]) {
   typedef P2<T> V;
-  int x0, y;
-  if (!pair9_coords(P, x0, y)) return;
-  const Geo9 geo = make_geo9(P, x0, y);
-  V f[Q9], g[Q9];
-  Pull9p<T, 0>::run(P.p_src, geo, f);
-  Pull9p<T, 1>::run(P.p_src, geo, g);
+  V f[Q9];
+  Pull9p<T, 0, LEAN>::run(P.p_src, geo, f);
+  Pull9p<T, 1, LEAN>::run(P.p_src, geo, g);
   const int i = geo.p0 + x0;
   V ux = ld_pair<T>(P.u + i), uy = ld_pair<T>(P.u + P.n + i);
   V phi, G[2], L;
-  stencil9p<T>(P.phi, geo, phi, G, L);
+  stencil9p<T, LEAN>(P.phi, geo, phi, G, L);
   const Mat9p<T> mat = materials9p<T>(P, phi, L);
   const Mom9p<T> m = moments9p<T>(f);
   if (!P.phase_only) {  // macros, Alg. 3 (lagged u, R13), then Eq. 31b
@@ -420,6 +425,153 @@ template <typename T> __global__ void __launch_bounds__(128) k_step9p(const __gr
   T* const rd = P.p_dst + geo.r0 + x0;
 #pragma unroll
   for (int a = 0; a < Q9; ++a) { st_pair<T>(rd + a * P.nx, f[a]); st_pair<T>(rd + (Q9 + a) * P.nx, g[a]); }
+}
+template <typename T> __global__ void __launch_bounds__(128) k_step9p(const __grid_constant__ KP<T> P) {
+  int x0, y;
+  if (!pair9_coords(P, x0, y)) return;
+  const Geo9 geo = make_geo9(P, x0, y);
+  P2<T> g[Q9];
+  step9p_pair<T>(P, geo, x0, g);
+}
+
+// ------------------------------------------------------------------------------------------------ single pass (k_fused9 + k_fix9)
+// The 2-D analogue of k_fused (clip_fused.cuh): ONE pass over f and g per step.  A block owns a chunk of whole lattice rows
+// [yc[c], yc[c+1]) and walks it row by row, 2 * blockDim.x nodes at a time; phi(t+2) = sum_a g+_a(x - e_a, t+1) is accumulated on chip
+// from the g+ just computed, in a shared-memory ring of four rows (y-1, y, y+1 and the one being flushed): the three x-directions of
+// a target row are combined by warp shuffles, every thread adds only into its own column pair, what crosses a warp's 64-node column
+// group goes through the edge arrays (periodic wrap in x included).  Finished rows are flushed to phi_dst, the two rows just outside
+// the chunk to `part` [chunk][2][nx]; k_fix9 adds them to the first / last row of the neighbouring chunks (fixed order, deterministic).
+// WALL / FREESLIP faces: where a population lands -- a link through a wall returns to the sender (B.10-B.11), a link through a
+// free-slip face keeps its tangential displacement (B.8-B.9), a wall crossing anywhere wins (R11).
+constexpr int FUSED9_MAX_CHUNKS = 2048;
+template <typename T> struct Fused9P {
+  T* phi_dst;   // phi(t+2)                                   [ny][nx]
+  T* part;      // the two halo rows of every chunk            [nchunks][2][nx]
+  int nchunks;  // chunk c covers the rows c * ny / nchunks .. (c + 1) * ny / nchunks - 1
+};
+template <typename T> struct Tri9 { P2<T> v0, vp, vm; };
+
+template <typename T>
+__global__ void __launch_bounds__(256, sizeof(T) == 4 ? 2 : 1) k_fused9(const __grid_constant__ KP<T> P, const Fused9P<T> U) {
+  typedef P2<T> V;
+  typedef typename PairOf<T>::type W2;
+  extern __shared__ __align__(16) unsigned char smem9[];
+  const int nx = P.nx, nwc = nx >> 6;                 // 64-node column groups (one warp each)
+  T* const ring = reinterpret_cast<T*>(smem9);        // [4][nx]
+  T* const edge_p = ring + 4 * nx;                    // [4][nwc]: lane 31's +x sends (land in the next group's first column)
+  T* const edge_m = edge_p + 4 * nwc;                 // [4][nwc]: lane 0's -x sends (land in the previous group's last column)
+  const int lane = threadIdx.x & 31;
+  const int c = blockIdx.x;
+  const int y0 = (int)((long long)c * P.ny / U.nchunks), y1 = (int)((long long)(c + 1) * P.ny / U.nchunks), rows = y1 - y0;
+  for (int i = threadIdx.x; i < 4 * (nx + 2 * nwc); i += blockDim.x) ring[i] = T(0);
+  __syncthreads();
+  T* const slab = U.part + (long long)c * 2 * nx;
+  // flush of the chunk's row k (-1 .. rows), held in ring slot (k + 1) % 4; the slot is left zeroed
+  auto flush = [&](int k) {
+    const int s = (k + 1) & 3;
+    T* const dst = k < 0 ? slab : (k >= rows ? slab + nx : U.phi_dst + (long long)(y0 + k) * nx);
+    for (int x0 = 2 * threadIdx.x; x0 < nx; x0 += 2 * blockDim.x) {
+      const int wc = x0 >> 6, wl = wc == 0 ? nwc - 1 : wc - 1, wr = wc == nwc - 1 ? 0 : wc + 1;
+      W2* p = reinterpret_cast<W2*>(ring + s * nx + x0);
+      V v = V(*p);
+      *p = V(T(0)).v;
+      if (lane == 0) { T& e = edge_p[s * nwc + wl]; v = v + V(e, T(0)); e = T(0); }
+      if (lane == 31) { T& e = edge_m[s * nwc + wr]; v = v + V(T(0), e); e = T(0); }
+      st_pair<T>(dst + x0, v);
+    }
+  };
+  // one node pair: the step, then where its nine g+ land.  LEAN: no face and no row end next to the pair (warp-uniform choice)
+  auto pair = [&](auto lean_tag, const Geo9& geo, int x0, int sm, int sc, int sp) {
+    constexpr bool LEAN = decltype(lean_tag)::value;
+    V g[Q9];
+    step9p_pair<T, LEAN>(P, geo, x0, g);
+    V own(T(0));
+    Tri9<T> up = {g[dir9(0, 1)], g[dir9(1, 1)], g[dir9(-1, 1)]}, dn = {g[dir9(0, -1)], g[dir9(1, -1)], g[dir9(-1, -1)]};
+    Tri9<T> me = {g[0], g[dir9(1, 0)], g[dir9(-1, 0)]};
+    if (!LEAN) {
+      if (geo.byp) { own = own + ((up.v0 + up.vp) + up.vm); up.v0 = V(T(0)); up.vp = V(T(0)); up.vm = V(T(0)); }
+      if (geo.bym) { own = own + ((dn.v0 + dn.vp) + dn.vm); dn.v0 = V(T(0)); dn.vp = V(T(0)); dn.vm = V(T(0)); }
+      if (geo.syp) { me.v0 = me.v0 + up.v0; me.vp = me.vp + up.vp; me.vm = me.vm + up.vm; up.v0 = V(T(0)); up.vp = V(T(0)); up.vm = V(T(0)); }
+      if (geo.sym) { me.v0 = me.v0 + dn.v0; me.vp = me.vp + dn.vp; me.vm = me.vm + dn.vm; dn.v0 = V(T(0)); dn.vp = V(T(0)); dn.vm = V(T(0)); }
+    }
+    V cc[3];
+    T ep[3], em[3];
+    auto finish = [&](Tri9<T> t, V& cv, T& e_p, T& e_m) {
+      if (!LEAN) {
+        if (geo.bxp) { own = own + V(T(0), t.vp.hi()); t.vp = V(t.vp.lo(), T(0)); }
+        if (geo.bxm) { own = own + V(t.vm.lo(), T(0)); t.vm = V(T(0), t.vm.hi()); }
+        if (geo.sxp) { t.v0 = t.v0 + V(T(0), t.vp.hi()); t.vp = V(t.vp.lo(), T(0)); }
+        if (geo.sxm) { t.v0 = t.v0 + V(t.vm.lo(), T(0)); t.vm = V(T(0), t.vm.hi()); }
+      }
+      T a = shfl_up1(t.vp.hi()), b = shfl_dn1(t.vm.lo());
+      if (lane == 0) a = T(0);
+      if (lane == 31) b = T(0);
+      cv = (t.v0 + V(a, t.vp.lo())) + V(t.vm.hi(), b);
+      e_p = t.vp.hi(); e_m = t.vm.lo();
+    };
+    finish(up, cc[0], ep[0], em[0]);
+    finish(dn, cc[1], ep[1], em[1]);
+    finish(me, cc[2], ep[2], em[2]);   // own row last: it also collects what bounced back
+    cc[2] = cc[2] + own;
+    const int sl[3] = {sp, sm, sc};
+    W2* q[3];
+    W2 o[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { q[k] = reinterpret_cast<W2*>(ring + sl[k] * nx + x0); o[k] = *q[k]; }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) *q[k] = (V(o[k]) + cc[k]).v;
+    if (lane == 0 || lane == 31) {
+      T* const e = (lane ? edge_p : edge_m) + (x0 >> 6);
+#pragma unroll
+      for (int k = 0; k < 3; ++k) e[sl[k] * nwc] += lane ? ep[k] : em[k];
+    }
+  };
+#pragma unroll 1
+  for (int ly = 0; ly < rows; ++ly) {
+    const int y = y0 + ly;
+    const int sm = ly & 3, sc = (ly + 1) & 3, sp = (ly + 2) & 3;   // slots of the rows y-1, y, y+1
+    const bool yface = (y == 0 && P.bc[2] != BC_PERIODIC) || (y == P.ny - 1 && P.bc[3] != BC_PERIODIC);
+    Geo9 lg{};   // the row's part of the lean geometry (rows wrap in y; no face flags)
+    {
+      const int ym = y > 0 ? y - 1 : P.ny - 1, yp = y < P.ny - 1 ? y + 1 : 0;
+      lg.nx = nx;
+      lg.r0 = (long long)y * NC9 * nx; lg.rm = (long long)ym * NC9 * nx; lg.rp = (long long)yp * NC9 * nx;
+      lg.p0 = y * nx; lg.pm = ym * nx; lg.pp = yp * nx;
+    }
+#pragma unroll 1
+    for (int x0 = 2 * threadIdx.x; x0 < nx; x0 += 2 * blockDim.x) {
+      const int wc = x0 >> 6;
+      if (yface || wc == 0 || wc == nwc - 1) {
+        pair(std::false_type(), make_geo9(P, x0, y), x0, sm, sc, sp);
+      } else {
+        Geo9 geo = lg;
+        geo.x0 = x0;
+        pair(std::true_type(), geo, x0, sm, sc, sp);
+      }
+    }
+    __syncthreads();
+    flush(ly - 1);
+  }
+  flush(rows - 1);
+  flush(rows);
+}
+
+// phi(t+2) of the first and the last row of every chunk: + what the neighbouring chunks sent.  grid = (nchunks, ceil(nx / 4 / 128))
+template <typename T> __global__ void __launch_bounds__(128) k_fix9(const __grid_constant__ KP<T> P, const Fused9P<T> U) {
+  const int c = blockIdx.x, nx = P.nx;
+  const int x0 = 2 * (blockIdx.y * blockDim.x + threadIdx.x);
+  if (x0 >= nx) return;
+  const int y0 = (int)((long long)c * P.ny / U.nchunks), y1 = (int)((long long)(c + 1) * P.ny / U.nchunks);
+  const bool wrap = P.bc[2] == BC_PERIODIC;
+  const int cm = c == 0 ? U.nchunks - 1 : c - 1, cp = c == U.nchunks - 1 ? 0 : c + 1;
+  if (c > 0 || wrap) {   // the row below sent its +y populations here: halo row 1 (yp) of the chunk below
+    T* const r = U.phi_dst + (long long)y0 * nx + x0;
+    st_pair<T>(r, ld_pair<T>(r) + ld_pair<T>(U.part + ((long long)cm * 2 + 1) * nx + x0));
+  }
+  if (c < U.nchunks - 1 || wrap) {
+    T* const r = U.phi_dst + (long long)(y1 - 1) * nx + x0;
+    st_pair<T>(r, ld_pair<T>(r) + ld_pair<T>(U.part + ((long long)cp * 2) * nx + x0));
+  }
 }
 
 }  // namespace d2q9

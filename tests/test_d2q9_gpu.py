@@ -208,3 +208,37 @@ def test_poiseuille_paper_cases_on_the_gpu(rho_ratio):
     err = cf.l2_rel(u[0, 0].mean(axis=1), ref)
     print(f"D2Q9 Poiseuille rho* = {rho_ratio:g}, mu* = 100 on the GPU: L2 (Eq. 47) = {err:.2e} after {steps} steps (du {du:.1e}), u_max {u[0].max():.2e}")
     assert np.isfinite(u).all() and du <= 1e-13 and err < 0.03
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_single_pass_d2q9_against_the_pair_kernels(precision):
+    """k_fused9 + k_fix9 (path = 3: one pass over f and g, phi(t+2) scattered on chip in a ring of four rows, chunk halos through partial
+    rows) against k_phi9p + k_step9p: the same arithmetic up to the association of phi's nine-term sum -> round-off only; periodic,
+    walled, mixed free-slip / wall faces, BGK; the default chunking, one chunk, one row per chunk, five chunks."""
+    import torch
+    from paper_2505_12205_b200 import clip
+
+    def run(case, **over):
+        sim = clip.Clip(case["nx"], case["ny"], case["nz"], dict(case["params"], precision=precision, **over))
+        sim.init(torch.as_tensor(case["phi0"]), torch.as_tensor(case["u0"]))
+        sim.step(30)
+        out = [t.double().cpu().numpy() for t in sim.get()]
+        ran = {k for k, (ms, cnt) in sim.step_profiled(1).items() if cnt}
+        sim.close()
+        return out, ran
+
+    cases = [_with(inputs.sweep2d(nx=128, ny=96), rho_l=0.01),
+             _with(inputs.sweep2d(nx=64, ny=50, ndrops=4), bc=(WL,) * 4 + (P_, P_), rho_l=0.05, g=(1e-5, -2e-5, 0.0)),
+             _with(inputs.sweep2d(nx=64, ny=36, ndrops=3, rmin=4, rmax=6), bc=(FS, WL, FS, FS, P_, P_), rho_l=0.1),
+             _with(inputs.sweep2d(nx=192, ny=40, ndrops=3, rmin=4, rmax=6), bc=(WL, FS, WL, FS, P_, P_), rho_l=0.1, collision=1, tau_l=0.3),
+             _with(inputs.sweep2d(nx=512, ny=24, ndrops=4, rmin=4, rmax=6), rho_l=0.1)]      # two sweeps of 256 threads per row
+    tol = 1e-12 if precision == 64 else 3e-5
+    for case in cases:
+        ref, r0 = run(case, path=2)
+        assert "k_fused" not in r0
+        for over in ({}, {"tile_chunks": 1}, {"tile_chunks": case["ny"]}, {"tile_chunks": 5}):
+            out, ran = run(case, path=3, **over)
+            assert "k_fused" in ran and "k_fix" in ran
+            for a, b in zip(ref, out):
+                assert np.isfinite(b).all()
+                assert np.abs(a - b).max() <= tol * max(1.0, np.abs(a).max()), (case["name"], over)

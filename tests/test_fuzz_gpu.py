@@ -89,8 +89,8 @@ def test_slabs_of_a_random_lattice_against_the_oracle(seed):
 
 @pytest.mark.parametrize("seed", range(64))
 def test_d2q9_paths_against_the_oracle_on_a_random_lattice(seed):
-    """The D2Q9 lattice (clip_params.lattice = 1): automatic path (pair kernels where nx is even) and the thread-per-node kernels
-    (path = 1) against the D2Q9 build of the oracle, fp64; the automatic path in fp32."""
+    """The D2Q9 lattice (clip_params.lattice = 1): automatic path (pair kernels where nx is even), the thread-per-node kernels
+    (path = 1) and the single-pass kernels (path = 3) against the D2Q9 build of the oracle, fp64; fp32 on the automatic or the single-pass path."""
     from oracle.clip_oracle import Oracle
     case = inputs.random_lattice2d(seed)
     o = Oracle.from_case(case)
@@ -98,11 +98,13 @@ def test_d2q9_paths_against_the_oracle_on_a_random_lattice(seed):
     o.step(STEPS)
     rphi, rp, ru = o.get()
     assert np.isfinite(rphi).all() and np.isfinite(ru).all()
-    for path in (1, 0):
+    for path in (1, 0, 3):     # 3: the single-pass kernels k_fused9 + k_fix9 where nx is a multiple of 64, else as 0
         (phi, p, u), ran = _run(case, 64, path)
         e = [np.abs(a - b).max() for a, b in ((phi, rphi), (p, rp), (u, ru))]
         assert all(np.isfinite(v) and v <= FP64_ABS for v in e), (case["name"], case["params"]["bc"], path, ran, e)
-    (phi, p, u), ran = _run(case, 32, 0)
+        if path == 3 and case["nx"] % 64 == 0 and case["ny"] >= 4:
+            assert "k_fused" in ran, (case["name"], ran)
+    (phi, p, u), ran = _run(case, 32, 3 if seed % 2 else 0)
     ephi = np.abs(phi - rphi).max() / np.abs(rphi).max()
     eu = np.abs(u - ru).max() / max(np.abs(ru).max(), 1e-30)
     assert ephi <= FP32_PHI and eu <= FP32_U, (case["name"], ran, ephi, eu)
