@@ -80,7 +80,9 @@ typedef struct clip_params {
   int runtime_nx;          /* 1 = take the runtime-nx instantiation of the pair kernels even where nx has its own (tests) */
   int lattice;             /* velocity set: 0 (default) = D3Q19, Eq. 14-15 (:169-176); 1 = D2Q9, the lattice of the paper's 2-D benchmarks
                               (:568): nz must be 1, the z faces PERIODIC, the x / y faces PERIODIC, WALL or FREESLIP; u_z is returned as
-                              given to clip_init (0).  Thread-per-node kernels (k_phi9 + k_step9) */
+                              given to clip_init (0).  Pair-per-thread kernels k_phi9p + k_step9p where nx is even, else the thread-per-node
+                              kernels k_phi9 + k_step9; path = 3 takes the single-pass kernels k_fused9 + k_fix9 where nx % 64 == 0 (an option:
+                              measured slower than the pair kernels, profiles/r02_experiments.md 4f) */
   int cluster_y;           /* k_fused, tuning / tests: y-adjacent tiles per thread-block cluster, whose shared tile surfaces are completed
                               through distributed shared memory instead of the partial-sum buffer.  0 = automatic (fp32: 4 at nx = 128,
                               2 at nx = 192, the lattices with 64- / 96-thread blocks, where it is measured to pay; else none),
